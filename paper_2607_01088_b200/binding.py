@@ -1,0 +1,221 @@
+"""ctypes binding of librosa.so — same names as include/rosa.h, argument marshalling only.
+
+PyTorch is used by callers for device memory and streams; this module only reads
+``tensor.data_ptr()``.  Every step of the path runs inside the library's CUDA kernels.
+There is no fallback: a missing library raises ImportError-like ``RosaError`` at load time.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Dict, Optional, Sequence
+
+import numpy as np
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "librosa.so")
+
+ROSA_OK, ROSA_ERR_INVALID_ARG, ROSA_ERR_UNBOUND_ROBOT = 0, -1, -2
+ROSA_ERR_CAPACITY, ROSA_ERR_CUDA, ROSA_ERR_UNSUPPORTED = -3, -4, -5
+ROSA_F32, ROSA_BF16 = 0, 1
+
+EXPORTS = ("rosa_expert_create", "rosa_expert_destroy", "rosa_prefix_kv_bind", "rosa_prefix_kv_unbind",
+           "rosa_denoise_batch", "rosa_denoise_batch_ex", "rosa_denoise_batch_host",
+           "rosa_last_launch_count", "rosa_kernel_family", "rosa_debug_gemm", "rosa_last_error",
+           "rosa_version")
+
+
+class RosaError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"librosa status {status}: {msg}")
+        self.status = status
+
+
+class rosa_expert_config_t(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in ("layers", "d_model", "n_q_heads", "n_kv_heads", "head_dim", "ffn",
+                                         "horizon", "action_dim", "max_robots", "max_batch",
+                                         "max_prefix_len", "max_steps")] + \
+               [(n, C.c_float) for n in ("rope_base", "rms_eps", "time_min_period", "time_max_period")]
+
+
+_GLOBAL = ("w_in", "b_in", "w_t1", "b_t1", "w_t2", "b_t2", "w_out", "b_out", "g_final")
+_LAYER = ("g_attn", "wq", "wk", "wv", "wo", "g_mlp", "w_gate", "w_up", "w_down")
+
+
+class rosa_weights_t(C.Structure):
+    _fields_ = [("dtype", C.c_int), ("on_device", C.c_int32)] + [(n, C.c_void_p) for n in _GLOBAL] + \
+               [(n, C.POINTER(C.c_void_p)) for n in _LAYER]
+
+
+_lib = None
+
+
+def load():
+    """dlopen librosa.so (built in-tree by ``build.py``); loud failure if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RosaError(ROSA_ERR_CUDA, f"{LIB_PATH} not built: run `python -m paper_2607_01088_b200.build` "
+                                       "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    vp, i32, i64 = C.c_void_p, C.c_int32, C.c_int64
+    lib.rosa_expert_create.argtypes = [C.POINTER(rosa_expert_config_t), C.POINTER(rosa_weights_t), C.POINTER(vp)]
+    lib.rosa_expert_destroy.argtypes = [vp]
+    lib.rosa_prefix_kv_bind.argtypes = [vp, i32, C.POINTER(vp), C.POINTER(vp), i32, C.c_int]
+    lib.rosa_prefix_kv_unbind.argtypes = [vp, i32]
+    lib.rosa_denoise_batch.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp]
+    lib.rosa_denoise_batch_ex.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.rosa_denoise_batch_host.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp]
+    lib.rosa_last_launch_count.argtypes = [vp, C.POINTER(i64)]
+    lib.rosa_kernel_family.argtypes = [vp, C.POINTER(i32)]
+    lib.rosa_debug_gemm.argtypes = [i32, i32, i32, i32, vp, vp, vp, vp]
+    lib.rosa_last_error.restype = C.c_char_p
+    lib.rosa_version.restype = i32
+    for n in EXPORTS:
+        if n not in ("rosa_last_error", "rosa_version"):
+            getattr(lib, n).restype = C.c_int
+    _lib = lib
+    return lib
+
+
+def _check(st: int):
+    if st != ROSA_OK:
+        raise RosaError(st, load().rosa_last_error().decode())
+
+
+def _ptr(t) -> int:
+    """Address of a torch tensor / numpy array / int (None -> NULL)."""
+    if t is None:
+        return 0
+    if isinstance(t, int):
+        return t
+    if isinstance(t, np.ndarray):
+        assert t.flags["C_CONTIGUOUS"]
+        return t.ctypes.data
+    assert t.is_contiguous()
+    return t.data_ptr()
+
+
+def _host(a, dtype) -> Optional[np.ndarray]:
+    return None if a is None else np.ascontiguousarray(a, dtype=dtype)
+
+
+def _stream_handle(stream) -> int:
+    if stream is None:
+        return 0
+    return stream if isinstance(stream, int) else stream.cuda_stream
+
+
+class Expert:
+    """Opaque ``rosa_expert_t*`` plus the Python references that keep borrowed buffers alive."""
+
+    def __init__(self, handle: int, cfg: rosa_expert_config_t):
+        self.handle = handle
+        self.cfg = cfg
+        self._keep: Dict[int, tuple] = {}
+
+    def __del__(self):
+        try:
+            if self.handle:
+                rosa_expert_destroy(self)
+        except Exception:
+            pass
+
+
+def rosa_expert_create(cfg: dict, weights: Dict[str, object], *, max_robots: int, max_batch: int,
+                       max_prefix_len: int, max_steps: int = 16) -> Expert:
+    """``cfg``: ExpertConfig fields; ``weights``: name -> float32 numpy array (or list per layer).
+    Host float32 pointers are handed to the library, which converts and repacks them itself."""
+    lib = load()
+    c = rosa_expert_config_t()
+    for k in ("layers", "d_model", "n_q_heads", "n_kv_heads", "head_dim", "ffn", "horizon", "action_dim"):
+        setattr(c, k, int(cfg[k]))
+    c.max_robots, c.max_batch, c.max_prefix_len, c.max_steps = max_robots, max_batch, max_prefix_len, max_steps
+    c.rope_base, c.rms_eps = float(cfg["rope_base"]), float(cfg["rms_eps"])
+    c.time_min_period, c.time_max_period = float(cfg["time_min_period"]), float(cfg["time_max_period"])
+    w = rosa_weights_t()
+    w.dtype, w.on_device = ROSA_F32, 0
+    keep = []
+    for n in _GLOBAL:
+        a = np.ascontiguousarray(weights[n], dtype=np.float32)
+        keep.append(a)
+        setattr(w, n, a.ctypes.data)
+    for n in _LAYER:
+        arrs = [np.ascontiguousarray(a, dtype=np.float32) for a in weights[n]]
+        keep.append(arrs)
+        pa = (C.c_void_p * len(arrs))(*[a.ctypes.data for a in arrs])
+        keep.append(pa)
+        setattr(w, n, pa)
+    out = C.c_void_p()
+    _check(lib.rosa_expert_create(C.byref(c), C.byref(w), C.byref(out)))
+    return Expert(out.value, c)
+
+
+def rosa_expert_destroy(e: Expert):
+    h, e.handle = e.handle, 0
+    e._keep.clear()
+    if h:
+        _check(load().rosa_expert_destroy(h))
+
+
+def rosa_prefix_kv_bind(e: Expert, robot: int, k_layers: Sequence, v_layers: Sequence, length: int,
+                        dtype: int = ROSA_BF16):
+    """k_layers/v_layers: per-layer device tensors (or raw device addresses) [len, n_kv, hd]."""
+    n = e.cfg.layers
+    ka = (C.c_void_p * n)(*[_ptr(t) for t in k_layers]) if length > 0 else None
+    va = (C.c_void_p * n)(*[_ptr(t) for t in v_layers]) if length > 0 else None
+    _check(load().rosa_prefix_kv_bind(e.handle, robot, ka, va, length, dtype))
+    e._keep[robot] = (list(k_layers), list(v_layers))
+
+
+def rosa_prefix_kv_unbind(e: Expert, robot: int):
+    _check(load().rosa_prefix_kv_unbind(e.handle, robot))
+    e._keep.pop(robot, None)
+
+
+def rosa_denoise_batch(e: Expert, robot_ids, noise, t_start, n_steps, out_actions, stream=None):
+    ids = _host(robot_ids, np.int32)
+    t0, ns = _host(t_start, np.float32), _host(n_steps, np.int32)
+    _check(load().rosa_denoise_batch(e.handle, len(ids), _ptr(ids), _ptr(noise), _ptr(t0), _ptr(ns),
+                                     _ptr(out_actions), _stream_handle(stream)))
+
+
+def rosa_denoise_batch_ex(e: Expert, robot_ids, noise, t_start, dt, n_steps, out_actions,
+                          out_velocity=None, stream=None):
+    ids = _host(robot_ids, np.int32)
+    t0, d, ns = _host(t_start, np.float32), _host(dt, np.float32), _host(n_steps, np.int32)
+    _check(load().rosa_denoise_batch_ex(e.handle, len(ids), _ptr(ids), _ptr(noise), _ptr(t0), _ptr(d), _ptr(ns),
+                                        _ptr(out_actions), _ptr(out_velocity), _stream_handle(stream)))
+
+
+def rosa_denoise_batch_host(e: Expert, robot_ids, noise_host, t_start, dt, n_steps, out_actions_host, stream=None):
+    """noise_host / out_actions_host: host float32 buffers (numpy arrays or pinned torch CPU tensors)."""
+    ids = _host(robot_ids, np.int32)
+    t0, d, ns = _host(t_start, np.float32), _host(dt, np.float32), _host(n_steps, np.int32)
+    _check(load().rosa_denoise_batch_host(e.handle, len(ids), _ptr(ids), _ptr(noise_host), _ptr(t0), _ptr(d),
+                                          _ptr(ns), _ptr(out_actions_host), _stream_handle(stream)))
+
+
+def rosa_last_launch_count(e: Expert) -> int:
+    n = C.c_int64()
+    _check(load().rosa_last_launch_count(e.handle, C.byref(n)))
+    return n.value
+
+
+def rosa_kernel_family(e: Expert) -> int:
+    n = C.c_int32()
+    _check(load().rosa_kernel_family(e.handle, C.byref(n)))
+    return n.value
+
+
+def rosa_debug_gemm(family: int, M: int, N: int, K: int, A_bf16, W_bf16, C_f32, stream=None):
+    _check(load().rosa_debug_gemm(family, M, N, K, _ptr(A_bf16), _ptr(W_bf16), _ptr(C_f32), _stream_handle(stream)))
+
+
+def rosa_last_error() -> str:
+    return load().rosa_last_error().decode()
+
+
+def rosa_version() -> int:
+    return load().rosa_version()

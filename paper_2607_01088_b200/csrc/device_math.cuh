@@ -1,0 +1,27 @@
+// Scalar device math shared by every kernel of librosa (readings R3, R6).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace rosa {
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ float warp_max(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+// swish(z) = z / (1 + e^-z)
+__device__ __forceinline__ float swish_f(float z) { return z / (1.f + __expf(-z)); }
+// GELU, tanh form (R6): 0.5 z (1 + tanh(sqrt(2/pi) (z + 0.044715 z^3)))
+// tanh(u) = 1 - 2/(1 + e^{2u}) keeps full fp32 accuracy for the range that matters.
+__device__ __forceinline__ float gelu_tanh_f(float z) {
+  const float u = 0.7978845608028654f * fmaf(0.044715f * z * z, z, z);
+  const float t = 1.f - 2.f / (1.f + __expf(2.f * u));
+  return 0.5f * z * (1.f + t);
+}
+
+}  // namespace rosa

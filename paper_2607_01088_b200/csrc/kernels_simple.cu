@@ -1,0 +1,343 @@
+// Shape-generic CUDA-core kernels: the elementwise steps of the hot path (used by both kernel
+// families) and the simple GEMM / attention family (cfg0-sized shapes, debugging, and the
+// on-device reference the tcgen05 kernels are unit-tested against).
+// Steps follow DESIGN.md section 1 (a1..a10 of SURVEY.md section 8(a)).
+#include "device_math.cuh"
+#include "rosa_internal.h"
+
+namespace rosa {
+
+// ------------------------------------------------------------------ x gather / scatter
+__global__ void k_gather_x(float* __restrict__ x, const CallPtrs* __restrict__ cp, Tables tb, int HA) {
+  int p = blockIdx.x;
+  const float* s = cp->noise + (size_t)tb.src[p] * HA;
+  for (int i = threadIdx.x; i < HA; i += blockDim.x) x[(size_t)p * HA + i] = s[i];
+}
+__global__ void k_scatter_x(const CallPtrs* __restrict__ cp, const float* __restrict__ x, Tables tb, int HA) {
+  int p = blockIdx.x;
+  float* d = cp->out + (size_t)tb.src[p] * HA;
+  for (int i = threadIdx.x; i < HA; i += blockDim.x) d[i] = x[(size_t)p * HA + i];
+}
+void launch_gather_x(float* x, const CallPtrs* cp, const Tables& tb, int HA, cudaStream_t s) {
+  k_gather_x<<<tb.batch, 128, 0, s>>>(x, cp, tb, HA);
+}
+void launch_scatter_x(const CallPtrs* cp, const float* x, const Tables& tb, int HA, cudaStream_t s) {
+  k_scatter_x<<<tb.batch, 128, 0, s>>>(cp, x, tb, HA);
+}
+
+// ------------------------------------------------------------------ a1 (time half), hoisted
+// tvec[k][p][n] = b_t1[n] + sum_c W_t1[n][c] * tau_c(t0_p + k dt_p), c < d   (readings R2, R3).
+// The time half of W_1 u is per robot, not per token, and t_k is known at call time, so it is
+// computed once per call for every iteration.  sin/cos in fp64: angles reach ~1571 rad.
+__global__ void k_timevec(float* __restrict__ tvec, const bf16* __restrict__ w_t1,
+                          const float* __restrict__ b_t1, Dims dm, Tables tb, int max_batch) {
+  extern __shared__ float tau[];  // [d]
+  const int p = blockIdx.x, k = blockIdx.y, d = dm.d, half = d / 2;
+  if (k >= tb.nsteps[p]) return;
+  const double t = (double)tb.t0[p] + (double)k * (double)tb.dt[p];
+  for (int j = threadIdx.x; j < half; j += blockDim.x) {
+    double frac = (double)j / (double)(half > 1 ? half - 1 : 1);
+    double period = (double)dm.pmin * pow((double)dm.pmax / (double)dm.pmin, frac);
+    double sn, cs;
+    sincos(6.283185307179586476925286766559 * t / period, &sn, &cs);
+    tau[j] = (float)sn;
+    tau[half + j] = (float)cs;
+  }
+  __syncthreads();
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+  float* out = tvec + ((size_t)k * max_batch + p) * d;
+  for (int n = warp; n < d; n += nw) {
+    const bf16* wr = w_t1 + (size_t)n * 2 * d;
+    float acc = 0.f;
+    for (int c = lane; c < d; c += 32) acc = fmaf(__bfloat162float(wr[c]), tau[c], acc);
+    acc = warp_sum(acc);
+    if (lane == 0) out[n] = acc + b_t1[n];
+  }
+}
+void launch_timevec(float* tvec, const bf16* w_t1, const float* b_t1, const Dims& dm,
+                    const Tables& tb, int nsteps_max, int max_batch, cudaStream_t s) {
+  dim3 grid(tb.batch, nsteps_max);
+  k_timevec<<<grid, 256, dm.d * sizeof(float), s>>>(tvec, w_t1, b_t1, dm, tb, max_batch);
+}
+
+// ------------------------------------------------------------------ a1 (action half)
+// a[m][n] = bf16( b_in[n] + sum_c x[m][c] W_in[n][c] ), x in fp32 (R11).
+__global__ void k_inproj(bf16* __restrict__ a, const float* __restrict__ x,
+                         const bf16* __restrict__ w_in, const float* __restrict__ b_in, int d, int A,
+                         const int* __restrict__ m_active) {
+  __shared__ float xs[64];
+  const int m = blockIdx.x;
+  if (m >= *m_active) return;
+  if (threadIdx.x < A) xs[threadIdx.x] = x[(size_t)m * A + threadIdx.x];
+  __syncthreads();
+  for (int n = threadIdx.x; n < d; n += blockDim.x) {
+    float acc = b_in[n];
+    for (int c = 0; c < A; ++c) acc = fmaf(xs[c], __bfloat162float(w_in[(size_t)n * A + c]), acc);
+    a[(size_t)m * d + n] = __float2bfloat16(acc);
+  }
+}
+void launch_inproj(bf16* a, const float* x, const bf16* w_in, const float* b_in, const Dims& dm,
+                   const Tables& tb, int k_iter, int M, cudaStream_t s) {
+  k_inproj<<<M, 128, 0, s>>>(a, x, w_in, b_in, dm.d, dm.A, tb.m_active + k_iter);
+}
+
+// ------------------------------------------------------------------ a2 RMSNorm (R5)
+// out = bf16( h * rsqrt(mean(h^2) + eps) * g ); one warp per token row; statistics in fp32.
+__global__ void k_rmsnorm(bf16* __restrict__ out, const float* __restrict__ h,
+                          const float* __restrict__ g, int d, float eps,
+                          const int* __restrict__ m_active) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int m = blockIdx.x * (blockDim.x >> 5) + warp;
+  if (m >= *m_active) return;
+  const float* row = h + (size_t)m * d;
+  float ss = 0.f;
+  for (int c = lane * 4; c < d; c += 128) {
+    float4 v = *reinterpret_cast<const float4*>(row + c);
+    ss += v.x * v.x + v.y * v.y + v.z * v.z + v.w * v.w;
+  }
+  ss = warp_sum(ss);
+  const float r = rsqrtf(ss / (float)d + eps);
+  for (int c = lane * 4; c < d; c += 128) {
+    float4 v = *reinterpret_cast<const float4*>(row + c);
+    float4 gg = *reinterpret_cast<const float4*>(g + c);
+    __nv_bfloat162 lo = __floats2bfloat162_rn(v.x * r * gg.x, v.y * r * gg.y);
+    __nv_bfloat162 hi = __floats2bfloat162_rn(v.z * r * gg.z, v.w * r * gg.w);
+    uint2 pk;
+    pk.x = *reinterpret_cast<uint32_t*>(&lo);
+    pk.y = *reinterpret_cast<uint32_t*>(&hi);
+    *reinterpret_cast<uint2*>(out + (size_t)m * d + c) = pk;
+  }
+}
+void launch_rmsnorm(bf16* out, const float* h, const float* g, const Dims& dm, const Tables& tb,
+                    int k_iter, int M, cudaStream_t s) {
+  const int wpb = 8;
+  k_rmsnorm<<<(M + wpb - 1) / wpb, wpb * 32, 0, s>>>(out, h, g, dm.d, dm.eps, tb.m_active + k_iter);
+}
+
+// ------------------------------------------------------------------ a9 + a10 (+ a11 bookkeeping)
+// v = RMSNorm(h; g_f) W_out^T + b_out ; x <- x + dt_p v.  One warp per token row.  The
+// normalised row stays in fp32 (no bf16 rounding of this operand).  Optional velocity export in
+// the caller's robot order.
+__global__ void k_final(float* __restrict__ x, const CallPtrs* __restrict__ cp,
+                        const float* __restrict__ h, const float* __restrict__ g,
+                        const bf16* __restrict__ w_out, const float* __restrict__ b_out, int d, int A,
+                        int H, float eps, Tables tb, int k_iter) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int m = blockIdx.x * (blockDim.x >> 5) + warp;
+  if (m >= tb.m_active[k_iter]) return;
+  float* vel_out = cp->vel;
+  const int batch_ext = cp->batch_ext;
+  const int p = m / H, j = m - p * H;
+  const float* row = h + (size_t)m * d;
+  float ss = 0.f;
+  for (int c = lane; c < d; c += 32) ss = fmaf(row[c], row[c], ss);
+  ss = warp_sum(ss);
+  const float r = rsqrtf(ss / (float)d + eps);
+  const float dt = tb.dt[p];
+  for (int a = 0; a < A; ++a) {
+    const bf16* wr = w_out + (size_t)a * d;
+    float acc = 0.f;
+    for (int c = lane; c < d; c += 32) acc = fmaf(row[c] * r * g[c], __bfloat162float(wr[c]), acc);
+    acc = warp_sum(acc);
+    if (lane == 0) {
+      const float v = acc + b_out[a];
+      float* xp = x + (size_t)m * A + a;
+      *xp = fmaf(dt, v, *xp);
+      if (vel_out) vel_out[(((size_t)k_iter * batch_ext + tb.src[p]) * H + j) * A + a] = v;
+    }
+  }
+}
+void launch_final(float* x, const CallPtrs* cp, const float* h, const float* g, const bf16* w_out,
+                  const float* b_out, const Dims& dm, const Tables& tb, int k_iter, int M,
+                  cudaStream_t s) {
+  const int wpb = 4;
+  k_final<<<(M + wpb - 1) / wpb, wpb * 32, 0, s>>>(x, cp, h, g, w_out, b_out, dm.d, dm.A, dm.H,
+                                                  dm.eps, tb, k_iter);
+}
+
+__global__ void k_f32_to_bf16(bf16* __restrict__ dst, const float* __restrict__ src, size_t n) {
+  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (; i < n; i += stride) dst[i] = __float2bfloat16(src[i]);
+}
+void launch_f32_to_bf16(bf16* dst, const float* src, size_t n, cudaStream_t s) {
+  if (n == 0) return;
+  int blocks = (int)((n + 255) / 256);
+  if (blocks > 4096) blocks = 4096;
+  k_f32_to_bf16<<<blocks, 256, 0, s>>>(dst, src, n);
+}
+
+// ------------------------------------------------------------------ CUDA-core GEMM (family 0)
+// C[M,N] fp32 = A[M,K] * W[N,K]^T, bf16 operands, fp32 accumulate.  64x64 tile, 16x16 threads,
+// 4x4 micro-tile.  Not a fast kernel: it is the shape-generic family and the on-device reference.
+constexpr int GN_T = 64, GN_K = 32;
+__global__ void __launch_bounds__(256) k_gemm_naive(const bf16* __restrict__ A, const bf16* __restrict__ W,
+                                                    float* __restrict__ C, int M, int N, int K,
+                                                    const int* __restrict__ m_active) {
+  __shared__ float As[GN_K][GN_T + 4];
+  __shared__ float Ws[GN_K][GN_T + 4];
+  const int m_lim = m_active ? min(M, *m_active) : M;
+  const int m0 = blockIdx.y * GN_T, n0 = blockIdx.x * GN_T;
+  if (m0 >= m_lim) return;
+  const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+  float acc[4][4] = {};
+  for (int k0 = 0; k0 < K; k0 += GN_K) {
+    for (int i = threadIdx.x; i < GN_T * GN_K; i += 256) {
+      int r = i / GN_K, c = i % GN_K;
+      int gm = m0 + r, gn = n0 + r, gk = k0 + c;
+      As[c][r] = (gm < m_lim && gk < K) ? __bfloat162float(A[(size_t)gm * K + gk]) : 0.f;
+      Ws[c][r] = (gn < N && gk < K) ? __bfloat162float(W[(size_t)gn * K + gk]) : 0.f;
+    }
+    __syncthreads();
+#pragma unroll 8
+    for (int kk = 0; kk < GN_K; ++kk) {
+      float a[4], b[4];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) a[i] = As[kk][ty * 4 + i];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) b[j] = Ws[kk][tx * 4 + j];
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j] = fmaf(a[i], b[j], acc[i][j]);
+    }
+    __syncthreads();
+  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    int gm = m0 + ty * 4 + i;
+    if (gm >= m_lim) continue;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      int gn = n0 + tx * 4 + j;
+      if (gn < N) C[(size_t)gm * N + gn] = acc[i][j];
+    }
+  }
+}
+void launch_gemm_naive(const bf16* A, const bf16* W, float* C, int M, int N, int K,
+                       const int* m_active, cudaStream_t s) {
+  dim3 grid((N + GN_T - 1) / GN_T, (M + GN_T - 1) / GN_T);
+  k_gemm_naive<<<grid, 256, 0, s>>>(A, W, C, M, N, K, m_active);
+}
+
+// ------------------------------------------------------------------ epilogues over the fp32 scratch
+__global__ void k_epilogue(int epi, const float* __restrict__ C, int M, int N, EpiArgs a) {
+  const int m_lim = a.m_active ? min(M, *a.m_active) : M;
+  const size_t total = (size_t)m_lim * N;
+  for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
+       idx += (size_t)gridDim.x * blockDim.x) {
+    const int m = (int)(idx / N), n = (int)(idx % N);
+    const float acc = C[idx];
+    switch (epi) {
+      case EPI_STORE_F32: a.out_f32[(size_t)m * a.ld_out + n] = acc; break;
+      case EPI_SWISH_ROWBIAS:
+        a.out_bf16[(size_t)m * a.ld_out + n] = __float2bfloat16(swish_f(acc + a.rowbias[(size_t)(m / a.H) * N + n]));
+        break;
+      case EPI_BIAS_F32: a.out_f32[(size_t)m * a.ld_out + n] = acc + a.bias[n]; break;
+      case EPI_RESID: a.out_f32[(size_t)m * a.ld_out + n] += acc; break;
+      case EPI_ROPE: {
+        float r = acc;
+        if (n < a.rope_cols) {
+          const int half = a.hd / 2, c = n % a.hd, p = m / a.H, j = m - p * a.H;
+          const int pos = a.rlen[a.ids[p]] + j;
+          const int cc = c < half ? c : c - half;
+          const float2 cs = a.rope_tab[(size_t)pos * half + cc];
+          const float other = C[(size_t)m * N + (c < half ? n + half : n - half)];
+          r = c < half ? acc * cs.x - other * cs.y : acc * cs.x + other * cs.y;
+        }
+        a.out_bf16[(size_t)m * a.ld_out + n] = __float2bfloat16(r);
+      } break;
+      case EPI_GEGLU: {
+        const int g = a.gu_blk, blk = n / (2 * g), r = n % (2 * g);
+        if (r < g) {
+          const float up = C[idx + g];
+          a.out_bf16[(size_t)m * a.ld_out + blk * g + r] = __float2bfloat16(gelu_tanh_f(acc) * up);
+        }
+      } break;
+    }
+  }
+}
+void launch_epilogue(Epi epi, const float* C, int M, int N, const EpiArgs& a, cudaStream_t s) {
+  size_t total = (size_t)M * N;
+  int blocks = (int)((total + 255) / 256);
+  if (blocks > 148 * 16) blocks = 148 * 16;
+  if (blocks < 1) blocks = 1;
+  k_epilogue<<<blocks, 256, 0, s>>>((int)epi, C, M, N, a);
+}
+
+// ------------------------------------------------------------------ a5 attention (family 0)
+// One block per (robot p, action token j): all n_q heads of that token against
+// [prefix K/V of the robot ; the block's own k/v] (R8: full visibility, scale 1/sqrt(hd)).
+// Thread-per-key scores into shared memory, block softmax, thread-per-channel P V.
+__global__ void __launch_bounds__(256) k_attn_simple(Dims dm, Tables tb, int layer,
+                                                     const bf16* __restrict__ qkv, bf16* __restrict__ o,
+                                                     int k_iter) {
+  extern __shared__ float sm[];
+  const int p = blockIdx.x / dm.H, j = blockIdx.x % dm.H;
+  const int m = p * dm.H + j;
+  if (m >= tb.m_active[k_iter]) return;
+  const int robot = tb.ids[p], L = tb.rlen[robot], T = L + dm.H, hd = dm.hd, nq = dm.nq;
+  const int group = dm.nq / dm.nkv;
+  const bf16* pk = tb.rk[(size_t)robot * dm.layers + layer];
+  const bf16* pv = tb.rv[(size_t)robot * dm.layers + layer];
+  float* qs = sm;                 // [nq*hd]
+  float* sc = sm + nq * hd;       // [nq][T]
+  float* red = sc + (size_t)nq * T;  // [nq] row max, then [nq] row sum
+  const bf16* qrow = qkv + (size_t)m * dm.qkv_n;
+  for (int i = threadIdx.x; i < nq * hd; i += blockDim.x) qs[i] = __bfloat162float(qrow[i]);
+  __syncthreads();
+  const float scale = rsqrtf((float)hd);
+  for (int s = threadIdx.x; s < T; s += blockDim.x) {
+    for (int g = 0; g < dm.nkv; ++g) {
+      const bf16* kr = s < L ? pk + ((size_t)s * dm.nkv + g) * hd
+                             : qkv + (size_t)(p * dm.H + (s - L)) * dm.qkv_n + dm.q_n + g * hd;
+      for (int a = g * group; a < (g + 1) * group; ++a) {
+        float acc = 0.f;
+        for (int c = 0; c < hd; c += 2) {
+          float2 kv = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(kr + c));
+          acc = fmaf(qs[a * hd + c], kv.x, acc);
+          acc = fmaf(qs[a * hd + c + 1], kv.y, acc);
+        }
+        sc[(size_t)a * T + s] = acc * scale;
+      }
+    }
+  }
+  __syncthreads();
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+  for (int a = warp; a < nq; a += nw) {
+    float mx = -INFINITY;
+    for (int s = lane; s < T; s += 32) mx = fmaxf(mx, sc[(size_t)a * T + s]);
+    mx = warp_max(mx);
+    float sum = 0.f;
+    for (int s = lane; s < T; s += 32) {
+      float e = __expf(sc[(size_t)a * T + s] - mx);
+      sc[(size_t)a * T + s] = e;
+      sum += e;
+    }
+    sum = warp_sum(sum);
+    if (lane == 0) red[a] = 1.f / sum;
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < nq * hd; i += blockDim.x) {
+    const int a = i / hd, c = i % hd, g = a / group;
+    float acc = 0.f;
+    for (int s = 0; s < T; ++s) {
+      const bf16* vr = s < L ? pv + ((size_t)s * dm.nkv + g) * hd
+                             : qkv + (size_t)(p * dm.H + (s - L)) * dm.qkv_n + dm.q_n + dm.nkv * hd + g * hd;
+      acc = fmaf(sc[(size_t)a * T + s], __bfloat162float(vr[c]), acc);
+    }
+    o[(size_t)m * dm.q_n + i] = __float2bfloat16(acc * red[a]);
+  }
+}
+void launch_attn_simple(const Dims& dm, const Tables& tb, int layer, const bf16* qkv, bf16* o,
+                        int k_iter, int max_len, cudaStream_t s) {
+  size_t smem = ((size_t)dm.nq * dm.hd + (size_t)dm.nq * (max_len + dm.H) + dm.nq) * sizeof(float);
+  static size_t configured = 0;
+  if (smem > configured) {
+    cudaFuncSetAttribute(k_attn_simple, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    configured = smem;
+  }
+  k_attn_simple<<<tb.batch * dm.H, 256, smem, s>>>(dm, tb, layer, qkv, o, k_iter);
+}
+
+}  // namespace rosa

@@ -1,0 +1,576 @@
+// C-ABI entry points of librosa (include/rosa.h) and the host runtime that sequences the hot
+// path: per-call device tables, the N-step loop, CUDA-graph capture/replay.
+#include <algorithm>
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <map>
+#include <numeric>
+#include <tuple>
+
+#include "rosa_internal.h"
+
+namespace rosa {
+
+static thread_local std::string g_err = "";
+void set_error(const std::string& msg) { g_err = msg; }
+
+#define CK(call)                                                                      \
+  do {                                                                                \
+    cudaError_t _e = (call);                                                          \
+    if (_e != cudaSuccess) {                                                          \
+      set_error(std::string(#call) + ": " + cudaGetErrorString(_e));                  \
+      return ROSA_ERR_CUDA;                                                           \
+    }                                                                                 \
+  } while (0)
+
+static inline uint16_t f2bf(float f) {  // round-to-nearest-even, host side
+  uint32_t u;
+  memcpy(&u, &f, 4);
+  if ((u & 0x7fffffffu) > 0x7f800000u) return (uint16_t)((u >> 16) | 0x40);
+  u += 0x7fffu + ((u >> 16) & 1u);
+  return (uint16_t)(u >> 16);
+}
+static inline float bf2f(uint16_t b) {
+  uint32_t u = (uint32_t)b << 16;
+  float f;
+  memcpy(&f, &u, 4);
+  return f;
+}
+
+constexpr int kStageRing = 4;
+
+struct GraphKey {
+  int batch, nmax, vel;
+  bool operator<(const GraphKey& o) const {
+    return std::tie(batch, nmax, vel) < std::tie(o.batch, o.nmax, o.vel);
+  }
+};
+
+}  // namespace rosa
+
+using namespace rosa;
+
+struct rosa_expert {
+  rosa_expert_config_t cfg;
+  Dims dm;
+  int family = 0;     // 0 simple, 1 tcgen05
+  bool use_graph = true;
+  int max_pos = 0;
+  // weights
+  bf16 *w_in = nullptr, *w_t1 = nullptr, *w_t1a = nullptr, *w_t2 = nullptr, *w_out = nullptr;
+  float *b_in = nullptr, *b_t1 = nullptr, *b_t2 = nullptr, *b_out = nullptr, *g_final = nullptr;
+  std::vector<LayerWeights> lw;
+  float2* rope_tab = nullptr;
+  // workspaces
+  float *x = nullptr, *h = nullptr, *tvec = nullptr, *scratch = nullptr;
+  bf16 *abuf = nullptr, *zbuf = nullptr, *nrm = nullptr, *qkv = nullptr, *obuf = nullptr, *mact = nullptr;
+  // robot table (device) + host mirror
+  const bf16** d_rk = nullptr;
+  const bf16** d_rv = nullptr;
+  int* d_rlen = nullptr;
+  std::vector<int> h_rlen;         // -1 = unbound
+  std::vector<std::vector<bf16*>> owned;  // per robot: library-owned K/V buffers (fp32 binds)
+  int max_len_bound = 0;
+  // per-call tables
+  char* d_call = nullptr;          // fixed device block
+  char* h_stage[kStageRing] = {};  // pinned ring
+  cudaEvent_t stage_ev[kStageRing] = {};
+  int stage_next = 0;
+  size_t call_bytes = 0;
+  size_t off_ids, off_src, off_t0, off_dt, off_ns, off_mact, off_ptrs;
+  std::map<GraphKey, cudaGraphExec_t> graphs;
+  std::map<GraphKey, int64_t> graph_launches;
+  cudaStream_t cap_stream = nullptr;
+  int64_t last_launches = 0;
+  float* e2e_dev = nullptr;  // staging for rosa_denoise_batch_host
+  std::vector<void*> allocs;
+};
+
+namespace rosa {
+
+static rosa_status_t dev_alloc(rosa_expert* e, void** p, size_t bytes) {
+  CK(cudaMalloc(p, bytes ? bytes : 16));
+  e->allocs.push_back(*p);
+  return ROSA_OK;
+}
+
+// Bring a caller tensor to host float32 (weights are repacked on the host once, at create).
+static rosa_status_t fetch_f32(const void* src, size_t n, rosa_dtype_t dt, int on_device,
+                               std::vector<float>& out) {
+  out.resize(n);
+  const size_t esz = dt == ROSA_F32 ? 4 : 2;
+  std::vector<char> raw;
+  const void* hp = src;
+  if (on_device) {
+    raw.resize(n * esz);
+    CK(cudaMemcpy(raw.data(), src, n * esz, cudaMemcpyDeviceToHost));
+    hp = raw.data();
+  }
+  if (dt == ROSA_F32) {
+    memcpy(out.data(), hp, n * 4);
+  } else {
+    const uint16_t* b = (const uint16_t*)hp;
+    for (size_t i = 0; i < n; ++i) out[i] = bf2f(b[i]);
+  }
+  return ROSA_OK;
+}
+static rosa_status_t upload_bf16(rosa_expert* e, const std::vector<float>& v, bf16** out) {
+  std::vector<uint16_t> b(v.size());
+  for (size_t i = 0; i < v.size(); ++i) b[i] = f2bf(v[i]);
+  rosa_status_t st = dev_alloc(e, (void**)out, b.size() * 2);
+  if (st != ROSA_OK) return st;
+  CK(cudaMemcpy(*out, b.data(), b.size() * 2, cudaMemcpyHostToDevice));
+  return ROSA_OK;
+}
+static rosa_status_t upload_f32(rosa_expert* e, const std::vector<float>& v, float** out) {
+  rosa_status_t st = dev_alloc(e, (void**)out, v.size() * 4);
+  if (st != ROSA_OK) return st;
+  CK(cudaMemcpy(*out, v.data(), v.size() * 4, cudaMemcpyHostToDevice));
+  return ROSA_OK;
+}
+
+static Tables make_tables(const rosa_expert* e, int batch) {
+  Tables tb;
+  tb.ids = (const int*)(e->d_call + e->off_ids);
+  tb.src = (const int*)(e->d_call + e->off_src);
+  tb.t0 = (const float*)(e->d_call + e->off_t0);
+  tb.dt = (const float*)(e->d_call + e->off_dt);
+  tb.nsteps = (const int*)(e->d_call + e->off_ns);
+  tb.m_active = (const int*)(e->d_call + e->off_mact);
+  tb.rk = e->d_rk;
+  tb.rv = e->d_rv;
+  tb.rlen = e->d_rlen;
+  tb.batch = batch;
+  return tb;
+}
+
+static void destroy_impl(rosa_expert* e) {
+  if (!e) return;
+  cudaDeviceSynchronize();
+  for (auto& kv : e->graphs) cudaGraphExecDestroy(kv.second);
+  for (void* p : e->allocs) cudaFree(p);
+  for (auto& v : e->owned)
+    for (bf16* p : v) cudaFree(p);
+  for (int i = 0; i < kStageRing; ++i) {
+    if (e->h_stage[i]) cudaFreeHost(e->h_stage[i]);
+    if (e->stage_ev[i]) cudaEventDestroy(e->stage_ev[i]);
+  }
+  if (e->cap_stream) cudaStreamDestroy(e->cap_stream);
+  delete e;
+}
+
+static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weights_t* w, rosa_expert* e) {
+  Dims& dm = e->dm;
+  dm.layers = c->layers; dm.d = c->d_model; dm.nq = c->n_q_heads; dm.nkv = c->n_kv_heads;
+  dm.hd = c->head_dim; dm.F = c->ffn; dm.H = c->horizon; dm.A = c->action_dim;
+  dm.qkv_n = (dm.nq + 2 * dm.nkv) * dm.hd;
+  dm.q_n = dm.nq * dm.hd;
+  dm.gu_blk = 64;
+  dm.rope_base = c->rope_base; dm.eps = c->rms_eps; dm.pmin = c->time_min_period; dm.pmax = c->time_max_period;
+  const int d = dm.d, F = dm.F, A = dm.A;
+  const rosa_dtype_t dt = w->dtype;
+  const int od = w->on_device;
+  std::vector<float> t, u;
+  rosa_status_t st;
+#define FETCH(ptr, n) if ((st = fetch_f32(ptr, (size_t)(n), dt, od, t)) != ROSA_OK) return st
+#define UPB(dst) if ((st = upload_bf16(e, t, &(dst))) != ROSA_OK) return st
+#define UPF(dst) if ((st = upload_f32(e, t, &(dst))) != ROSA_OK) return st
+  FETCH(w->w_in, (size_t)d * A); UPB(e->w_in);
+  FETCH(w->b_in, d); UPF(e->b_in);
+  FETCH(w->w_t1, (size_t)d * 2 * d); UPB(e->w_t1);
+  u.resize((size_t)d * d);  // action half of W_1 (columns d..2d-1, R2) as its own [d,d] matrix
+  for (int n = 0; n < d; ++n) memcpy(&u[(size_t)n * d], &t[(size_t)n * 2 * d + d], (size_t)d * 4);
+  t.swap(u); UPB(e->w_t1a);
+  FETCH(w->b_t1, d); UPF(e->b_t1);
+  FETCH(w->w_t2, (size_t)d * d); UPB(e->w_t2);
+  FETCH(w->b_t2, d); UPF(e->b_t2);
+  FETCH(w->w_out, (size_t)A * d); UPB(e->w_out);
+  FETCH(w->b_out, A); UPF(e->b_out);
+  FETCH(w->g_final, d); UPF(e->g_final);
+  e->lw.resize(dm.layers);
+  for (int l = 0; l < dm.layers; ++l) {
+    LayerWeights& L = e->lw[l];
+    FETCH(w->g_attn[l], d); UPF(L.g_attn);
+    FETCH(w->g_mlp[l], d); UPF(L.g_mlp);
+    // packed [wq ; wk ; wv]  -> one QKV GEMM (step a3)
+    std::vector<float> pk((size_t)dm.qkv_n * d);
+    FETCH(w->wq[l], (size_t)dm.q_n * d); memcpy(pk.data(), t.data(), t.size() * 4);
+    FETCH(w->wk[l], (size_t)dm.nkv * dm.hd * d); memcpy(pk.data() + (size_t)dm.q_n * d, t.data(), t.size() * 4);
+    FETCH(w->wv[l], (size_t)dm.nkv * dm.hd * d);
+    memcpy(pk.data() + (size_t)(dm.q_n + dm.nkv * dm.hd) * d, t.data(), t.size() * 4);
+    t.swap(pk); UPB(L.wqkv);
+    FETCH(w->wo[l], (size_t)d * dm.q_n); UPB(L.wo);
+    // gate/up interleaved in blocks of gu_blk rows -> one GEMM + GeGLU epilogue (step a7)
+    std::vector<float> gu((size_t)2 * F * d);
+    const int g = dm.gu_blk;
+    FETCH(w->w_gate[l], (size_t)F * d);
+    for (int f = 0; f < F; ++f)
+      memcpy(&gu[((size_t)(f / g) * 2 * g + f % g) * d], &t[(size_t)f * d], (size_t)d * 4);
+    FETCH(w->w_up[l], (size_t)F * d);
+    for (int f = 0; f < F; ++f)
+      memcpy(&gu[((size_t)(f / g) * 2 * g + g + f % g) * d], &t[(size_t)f * d], (size_t)d * 4);
+    t.swap(gu); UPB(L.wgu);
+    FETCH(w->w_down[l], (size_t)d * F); UPB(L.wdown);
+  }
+#undef FETCH
+#undef UPB
+#undef UPF
+  // RoPE table in fp64 (R7): pos in [0, max_prefix_len + H), c < hd/2 -> (cos, sin)(pos * base^(-2c/hd))
+  e->max_pos = c->max_prefix_len + dm.H;
+  {
+    const int half = dm.hd / 2;
+    std::vector<float2> tab((size_t)e->max_pos * half);
+    for (int cidx = 0; cidx < half; ++cidx) {
+      const double theta = std::pow((double)dm.rope_base, -2.0 * cidx / dm.hd);
+      for (int pos = 0; pos < e->max_pos; ++pos) {
+        const double phi = pos * theta;
+        tab[(size_t)pos * half + cidx] = make_float2((float)std::cos(phi), (float)std::sin(phi));
+      }
+    }
+    if ((st = dev_alloc(e, (void**)&e->rope_tab, tab.size() * sizeof(float2))) != ROSA_OK) return st;
+    CK(cudaMemcpy(e->rope_tab, tab.data(), tab.size() * sizeof(float2), cudaMemcpyHostToDevice));
+  }
+  // workspaces (rows padded to a multiple of 128 for the tile kernels)
+  const size_t Mmax = ((size_t)c->max_batch * dm.H + 127) / 128 * 128;
+  const size_t HA = (size_t)dm.H * A;
+#define WS(ptr, bytes) if ((st = dev_alloc(e, (void**)&(ptr), (bytes))) != ROSA_OK) return st
+  WS(e->x, (size_t)c->max_batch * HA * 4);
+  WS(e->h, Mmax * d * 4);
+  WS(e->tvec, (size_t)c->max_steps * c->max_batch * d * 4);
+  WS(e->abuf, Mmax * d * 2);
+  WS(e->zbuf, Mmax * d * 2);
+  WS(e->nrm, Mmax * d * 2);
+  WS(e->qkv, Mmax * dm.qkv_n * 2);
+  WS(e->obuf, Mmax * dm.q_n * 2);
+  WS(e->mact, Mmax * F * 2);
+  WS(e->scratch, Mmax * (size_t)std::max(2 * F, dm.qkv_n) * 4);
+  WS(e->e2e_dev, (size_t)c->max_batch * HA * 4);
+  CK(cudaMemset(e->abuf, 0, Mmax * d * 2));
+  CK(cudaMemset(e->zbuf, 0, Mmax * d * 2));
+  CK(cudaMemset(e->nrm, 0, Mmax * d * 2));
+  CK(cudaMemset(e->qkv, 0, Mmax * dm.qkv_n * 2));
+  CK(cudaMemset(e->obuf, 0, Mmax * dm.q_n * 2));
+  CK(cudaMemset(e->mact, 0, Mmax * F * 2));
+  // robot table
+  WS(e->d_rk, (size_t)c->max_robots * dm.layers * sizeof(void*));
+  WS(e->d_rv, (size_t)c->max_robots * dm.layers * sizeof(void*));
+  WS(e->d_rlen, (size_t)c->max_robots * 4);
+  CK(cudaMemset(e->d_rk, 0, (size_t)c->max_robots * dm.layers * sizeof(void*)));
+  CK(cudaMemset(e->d_rv, 0, (size_t)c->max_robots * dm.layers * sizeof(void*)));
+  CK(cudaMemset(e->d_rlen, 0, (size_t)c->max_robots * 4));
+  e->h_rlen.assign(c->max_robots, -1);
+  e->owned.resize(c->max_robots);
+  // per-call table block
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off += (bytes + 15) / 16 * 16; return o; };
+  e->off_ids = take((size_t)c->max_batch * 4);
+  e->off_src = take((size_t)c->max_batch * 4);
+  e->off_t0 = take((size_t)c->max_batch * 4);
+  e->off_dt = take((size_t)c->max_batch * 4);
+  e->off_ns = take((size_t)c->max_batch * 4);
+  e->off_mact = take((size_t)c->max_steps * 4);
+  e->off_ptrs = take(sizeof(CallPtrs));
+  e->call_bytes = off;
+  WS(e->d_call, e->call_bytes);
+#undef WS
+  for (int i = 0; i < kStageRing; ++i) {
+    CK(cudaMallocHost((void**)&e->h_stage[i], e->call_bytes));
+    CK(cudaEventCreateWithFlags(&e->stage_ev[i], cudaEventDisableTiming));
+  }
+  CK(cudaStreamCreateWithFlags(&e->cap_stream, cudaStreamNonBlocking));
+  return ROSA_OK;
+}
+
+// One GEMM + epilogue of the path, in whichever kernel family the expert runs.
+static cudaError_t gemm(rosa_expert* e, Epi epi, const bf16* A, const bf16* W, int M, int N, int K,
+                        const EpiArgs& a, cudaStream_t s) {
+  if (e->family == 1 && tc_gemm_supported(N, K)) {
+    e->last_launches += 1;
+    return launch_gemm_tc(epi, A, W, M, N, K, a, s);
+  }
+  launch_gemm_naive(A, W, e->scratch, M, N, K, a.m_active, s);
+  launch_epilogue(epi, e->scratch, M, N, a, s);
+  e->last_launches += 2;
+  return cudaGetLastError();
+}
+
+// Enqueue the whole call (steps a1..a11) on `s`.  Everything that changes from call to call is
+// read from the device tables, so the same sequence can be captured once per (batch, nmax).
+static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, cudaStream_t s) {
+  const Dims& dm = e->dm;
+  const Tables tb = make_tables(e, batch);
+  const CallPtrs* cp = (const CallPtrs*)(e->d_call + e->off_ptrs);
+  const int M = batch * dm.H, d = dm.d;
+  cudaError_t err;
+  e->last_launches = 0;
+  launch_gather_x(e->x, cp, tb, dm.H * dm.A, s);
+  launch_timevec(e->tvec, e->w_t1, e->b_t1, dm, tb, nmax, e->cfg.max_batch, s);
+  e->last_launches += 2;
+  for (int k = 0; k < nmax; ++k) {
+    EpiArgs ea{};
+    ea.m_active = tb.m_active + k;
+    ea.H = dm.H; ea.hd = dm.hd; ea.gu_blk = dm.gu_blk;
+    // a1: h0 = W2 swish(W1 [tau ; W_in x + b_in] + b1) + b2
+    launch_inproj(e->abuf, e->x, e->w_in, e->b_in, dm, tb, k, M, s);
+    e->last_launches += 1;
+    ea.out_bf16 = e->zbuf; ea.ld_out = d;
+    ea.rowbias = e->tvec + (size_t)k * e->cfg.max_batch * d;
+    if ((err = gemm(e, EPI_SWISH_ROWBIAS, e->abuf, e->w_t1a, M, d, d, ea, s)) != cudaSuccess) return err;
+    ea.out_f32 = e->h; ea.bias = e->b_t2;
+    if ((err = gemm(e, EPI_BIAS_F32, e->zbuf, e->w_t2, M, d, d, ea, s)) != cudaSuccess) return err;
+    for (int l = 0; l < dm.layers; ++l) {
+      const LayerWeights& L = e->lw[l];
+      launch_rmsnorm(e->nrm, e->h, L.g_attn, dm, tb, k, M, s);                       // a2
+      ea.out_bf16 = e->qkv; ea.ld_out = dm.qkv_n;
+      ea.rope_tab = e->rope_tab; ea.ids = tb.ids; ea.rlen = tb.rlen;
+      ea.rope_cols = dm.q_n + dm.nkv * dm.hd;
+      if ((err = gemm(e, EPI_ROPE, e->nrm, L.wqkv, M, dm.qkv_n, d, ea, s)) != cudaSuccess) return err;  // a3+a4
+      launch_attn_simple(dm, tb, l, e->qkv, e->obuf, k, e->cfg.max_prefix_len, s);   // a5
+      ea.out_f32 = e->h; ea.ld_out = d;
+      if ((err = gemm(e, EPI_RESID, e->obuf, L.wo, M, d, dm.q_n, ea, s)) != cudaSuccess) return err;    // a6
+      launch_rmsnorm(e->nrm, e->h, L.g_mlp, dm, tb, k, M, s);                        // a2
+      ea.out_bf16 = e->mact; ea.ld_out = dm.F;
+      if ((err = gemm(e, EPI_GEGLU, e->nrm, L.wgu, M, 2 * dm.F, d, ea, s)) != cudaSuccess) return err;  // a7
+      ea.out_f32 = e->h; ea.ld_out = d;
+      if ((err = gemm(e, EPI_RESID, e->mact, L.wdown, M, d, dm.F, ea, s)) != cudaSuccess) return err;   // a8
+      e->last_launches += 3;
+    }
+    launch_final(e->x, cp, e->h, e->g_final, e->w_out, e->b_out, dm, tb, k, M, s);    // a9 + a10
+    e->last_launches += 1;
+  }
+  launch_scatter_x(cp, e->x, tb, dm.H * dm.A, s);
+  e->last_launches += 1;
+  return cudaGetLastError();
+}
+
+static rosa_status_t denoise_impl(rosa_expert* e, int batch, const int32_t* ids, const float* noise,
+                                  const float* t_start, const float* dt, const int32_t* n_steps,
+                                  float* out, float* out_vel, cudaStream_t stream) {
+  if (!e || !ids || !noise || !n_steps || !out) { set_error("NULL argument"); return ROSA_ERR_INVALID_ARG; }
+  if (batch < 1) { set_error("batch < 1"); return ROSA_ERR_INVALID_ARG; }
+  if (batch > e->cfg.max_batch) { set_error("batch > max_batch"); return ROSA_ERR_CAPACITY; }
+  const Dims& dm = e->dm;
+  int nmax = 0;
+  std::vector<char> seen(e->cfg.max_robots, 0);
+  for (int i = 0; i < batch; ++i) {
+    if (ids[i] < 0 || ids[i] >= e->cfg.max_robots) { set_error("robot id out of range"); return ROSA_ERR_INVALID_ARG; }
+    if (seen[ids[i]]) { set_error("duplicate robot id in batch"); return ROSA_ERR_INVALID_ARG; }
+    seen[ids[i]] = 1;
+    if (e->h_rlen[ids[i]] < 0) { set_error("robot has no prefix K/V bound"); return ROSA_ERR_UNBOUND_ROBOT; }
+    if (n_steps[i] < 1) { set_error("n_steps < 1"); return ROSA_ERR_INVALID_ARG; }
+    if (n_steps[i] > e->cfg.max_steps) { set_error("n_steps > max_steps"); return ROSA_ERR_CAPACITY; }
+    nmax = std::max(nmax, (int)n_steps[i]);
+  }
+  // internal order: n_steps descending (stable) -> the active set of iteration k is a row prefix
+  std::vector<int> order(batch);
+  std::iota(order.begin(), order.end(), 0);
+  std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return n_steps[a] > n_steps[b]; });
+  const int slot = e->stage_next;
+  e->stage_next = (slot + 1) % kStageRing;
+  CK(cudaEventSynchronize(e->stage_ev[slot]));  // the copy that last used this slot has completed
+  char* hs = e->h_stage[slot];
+  int* h_ids = (int*)(hs + e->off_ids); int* h_src = (int*)(hs + e->off_src);
+  float* h_t0 = (float*)(hs + e->off_t0); float* h_dt = (float*)(hs + e->off_dt);
+  int* h_ns = (int*)(hs + e->off_ns); int* h_ma = (int*)(hs + e->off_mact);
+  for (int p = 0; p < batch; ++p) {
+    const int i = order[p];
+    h_ids[p] = ids[i]; h_src[p] = i;
+    h_t0[p] = t_start ? t_start[i] : 1.0f;
+    h_dt[p] = dt ? dt[i] : -h_t0[p] / (float)n_steps[i];
+    h_ns[p] = n_steps[i];
+  }
+  for (int k = 0; k < e->cfg.max_steps; ++k) {
+    int act = 0;
+    for (int p = 0; p < batch; ++p) act += h_ns[p] > k;
+    h_ma[k] = act * dm.H;
+  }
+  CallPtrs* h_cp = (CallPtrs*)(hs + e->off_ptrs);
+  h_cp->noise = noise; h_cp->out = out; h_cp->vel = out_vel; h_cp->batch_ext = batch;
+  CK(cudaMemcpyAsync(e->d_call, hs, e->call_bytes, cudaMemcpyHostToDevice, stream));
+  CK(cudaEventRecord(e->stage_ev[slot], stream));
+  if (out_vel) CK(cudaMemsetAsync(out_vel, 0, (size_t)nmax * batch * dm.H * dm.A * 4, stream));
+  if (!e->use_graph) {
+    CK(enqueue_call(e, batch, nmax, stream));
+    return ROSA_OK;
+  }
+  const GraphKey key{batch, nmax, 0};
+  auto it = e->graphs.find(key);
+  if (it == e->graphs.end()) {
+    cudaGraph_t g = nullptr;
+    CK(cudaStreamBeginCapture(e->cap_stream, cudaStreamCaptureModeThreadLocal));
+    cudaError_t err = enqueue_call(e, batch, nmax, e->cap_stream);
+    cudaError_t err2 = cudaStreamEndCapture(e->cap_stream, &g);
+    if (err != cudaSuccess || err2 != cudaSuccess) {
+      if (g) cudaGraphDestroy(g);
+      set_error(std::string("graph capture failed: ") + cudaGetErrorString(err != cudaSuccess ? err : err2));
+      return ROSA_ERR_CUDA;
+    }
+    cudaGraphExec_t ex = nullptr;
+    CK(cudaGraphInstantiate(&ex, g, 0));
+    cudaGraphDestroy(g);
+    it = e->graphs.emplace(key, ex).first;
+    e->graph_launches[key] = e->last_launches;
+  }
+  e->last_launches = e->graph_launches[key];
+  CK(cudaGraphLaunch(it->second, stream));
+  return ROSA_OK;
+}
+
+}  // namespace rosa
+
+// ===================================================================== C ABI
+extern "C" {
+
+rosa_status_t rosa_expert_create(const rosa_expert_config_t* c, const rosa_weights_t* w, rosa_expert_t** out) {
+  if (!c || !w || !out) { set_error("NULL argument"); return ROSA_ERR_INVALID_ARG; }
+  *out = nullptr;
+  if (c->layers < 1 || c->d_model < 1 || c->n_q_heads < 1 || c->n_kv_heads < 1 || c->head_dim < 2 ||
+      c->ffn < 1 || c->horizon < 1 || c->action_dim < 1 || c->max_robots < 1 || c->max_batch < 1 ||
+      c->max_prefix_len < 0 || c->max_steps < 1) {
+    set_error("non-positive dimension in config"); return ROSA_ERR_INVALID_ARG;
+  }
+  if (c->d_model % 64 || c->ffn % 64 || (c->n_q_heads * c->head_dim) % 64 || c->head_dim % 2 ||
+      c->head_dim > 256 || c->n_q_heads % c->n_kv_heads || c->action_dim > 64 || c->horizon > 64) {
+    set_error("unsupported shape (see rosa_expert_create in rosa.h)"); return ROSA_ERR_UNSUPPORTED;
+  }
+  if ((size_t)c->n_q_heads * (c->head_dim + c->max_prefix_len + c->horizon + 1) * 4 > 220 * 1024) {
+    set_error("max_prefix_len too large for the attention kernel's shared memory"); return ROSA_ERR_UNSUPPORTED;
+  }
+  const void* must[] = {w->w_in, w->b_in, w->w_t1, w->b_t1, w->w_t2, w->b_t2, w->w_out, w->b_out, w->g_final,
+                        w->g_attn, w->wq, w->wk, w->wv, w->wo, w->g_mlp, w->w_gate, w->w_up, w->w_down};
+  for (const void* p : must) if (!p) { set_error("NULL weight pointer"); return ROSA_ERR_INVALID_ARG; }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+    cudaGetLastError();
+    set_error("no CUDA device: librosa has no CPU fallback"); return ROSA_ERR_CUDA;
+  }
+  rosa_expert* e = new rosa_expert();
+  e->cfg = *c;
+  const char* fam = getenv("ROSA_KERNELS");
+  e->family = (fam && !strcmp(fam, "simple")) ? 0 : 1;
+  const char* gr = getenv("ROSA_GRAPH");
+  e->use_graph = !(gr && !strcmp(gr, "0"));
+  rosa_status_t st = create_impl(c, w, e);
+  if (st != ROSA_OK) { std::string keep = rosa_last_error(); destroy_impl(e); set_error(keep); return st; }
+  *out = e;
+  return ROSA_OK;
+}
+
+rosa_status_t rosa_expert_destroy(rosa_expert_t* e) {
+  if (!e) { set_error("NULL expert"); return ROSA_ERR_INVALID_ARG; }
+  destroy_impl(e);
+  return ROSA_OK;
+}
+
+rosa_status_t rosa_prefix_kv_unbind(rosa_expert_t* e, int32_t robot) {
+  if (!e) { set_error("NULL expert"); return ROSA_ERR_INVALID_ARG; }
+  if (robot < 0 || robot >= e->cfg.max_robots) { set_error("robot id out of range"); return ROSA_ERR_CAPACITY; }
+  if (!e->owned[robot].empty()) {
+    CK(cudaDeviceSynchronize());  // in-flight calls may still read the owned copies
+    for (bf16* p : e->owned[robot]) cudaFree(p);
+    e->owned[robot].clear();
+  }
+  e->h_rlen[robot] = -1;
+  return ROSA_OK;
+}
+
+rosa_status_t rosa_prefix_kv_bind(rosa_expert_t* e, int32_t robot, const void* const* k_layers,
+                                  const void* const* v_layers, int32_t len, rosa_dtype_t dtype) {
+  if (!e) { set_error("NULL expert"); return ROSA_ERR_INVALID_ARG; }
+  if (robot < 0 || robot >= e->cfg.max_robots) { set_error("robot id out of range"); return ROSA_ERR_CAPACITY; }
+  if (len < 0) { set_error("len < 0"); return ROSA_ERR_INVALID_ARG; }
+  if (len > e->cfg.max_prefix_len) { set_error("len > max_prefix_len"); return ROSA_ERR_CAPACITY; }
+  if (dtype != ROSA_F32 && dtype != ROSA_BF16) { set_error("bad dtype"); return ROSA_ERR_INVALID_ARG; }
+  const Dims& dm = e->dm;
+  if (len > 0) {
+    if (!k_layers || !v_layers) { set_error("NULL K/V pointer array"); return ROSA_ERR_INVALID_ARG; }
+    for (int l = 0; l < dm.layers; ++l) {
+      if (!k_layers[l] || !v_layers[l]) { set_error("NULL K/V layer pointer"); return ROSA_ERR_INVALID_ARG; }
+      if (((uintptr_t)k_layers[l] | (uintptr_t)v_layers[l]) & 15) { set_error("K/V pointer not 16-byte aligned"); return ROSA_ERR_INVALID_ARG; }
+    }
+  }
+  rosa_status_t st = rosa_prefix_kv_unbind(e, robot);
+  if (st != ROSA_OK) return st;
+  std::vector<const bf16*> hk(dm.layers, nullptr), hv(dm.layers, nullptr);
+  const size_t n = (size_t)len * dm.nkv * dm.hd;
+  if (len > 0 && dtype == ROSA_BF16) {
+    for (int l = 0; l < dm.layers; ++l) { hk[l] = (const bf16*)k_layers[l]; hv[l] = (const bf16*)v_layers[l]; }
+  } else if (len > 0) {
+    for (int l = 0; l < dm.layers; ++l) {
+      bf16 *ck = nullptr, *cv = nullptr;
+      CK(cudaMalloc((void**)&ck, n * 2)); e->owned[robot].push_back(ck);
+      CK(cudaMalloc((void**)&cv, n * 2)); e->owned[robot].push_back(cv);
+      launch_f32_to_bf16(ck, (const float*)k_layers[l], n, 0);
+      launch_f32_to_bf16(cv, (const float*)v_layers[l], n, 0);
+      hk[l] = ck; hv[l] = cv;
+    }
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(0));
+  }
+  CK(cudaMemcpy(e->d_rk + (size_t)robot * dm.layers, hk.data(), dm.layers * sizeof(void*), cudaMemcpyHostToDevice));
+  CK(cudaMemcpy(e->d_rv + (size_t)robot * dm.layers, hv.data(), dm.layers * sizeof(void*), cudaMemcpyHostToDevice));
+  CK(cudaMemcpy(e->d_rlen + robot, &len, 4, cudaMemcpyHostToDevice));
+  e->h_rlen[robot] = len;
+  return ROSA_OK;
+}
+
+rosa_status_t rosa_denoise_batch_ex(rosa_expert_t* e, int32_t batch, const int32_t* robot_ids, const float* noise,
+                                    const float* t_start, const float* dt, const int32_t* n_steps,
+                                    float* out_actions, float* out_velocity, void* stream) {
+  return denoise_impl(e, batch, robot_ids, noise, t_start, dt, n_steps, out_actions, out_velocity,
+                      (cudaStream_t)stream);
+}
+
+rosa_status_t rosa_denoise_batch(rosa_expert_t* e, int32_t batch, const int32_t* robot_ids, const float* noise,
+                                 const float* t_start, const int32_t* n_steps, float* out_actions, void* stream) {
+  return denoise_impl(e, batch, robot_ids, noise, t_start, nullptr, n_steps, out_actions, nullptr,
+                      (cudaStream_t)stream);
+}
+
+rosa_status_t rosa_denoise_batch_host(rosa_expert_t* e, int32_t batch, const int32_t* robot_ids,
+                                      const float* noise_host, const float* t_start, const float* dt,
+                                      const int32_t* n_steps, float* out_actions_host, void* stream) {
+  if (!e || !noise_host || !out_actions_host) { set_error("NULL argument"); return ROSA_ERR_INVALID_ARG; }
+  if (batch < 1 || batch > e->cfg.max_batch) { set_error("batch out of range"); return ROSA_ERR_CAPACITY; }
+  cudaStream_t s = (cudaStream_t)stream;
+  const size_t bytes = (size_t)batch * e->dm.H * e->dm.A * 4;
+  CK(cudaMemcpyAsync(e->e2e_dev, noise_host, bytes, cudaMemcpyHostToDevice, s));
+  rosa_status_t st = denoise_impl(e, batch, robot_ids, e->e2e_dev, t_start, dt, n_steps, e->e2e_dev, nullptr, s);
+  if (st != ROSA_OK) return st;
+  CK(cudaMemcpyAsync(out_actions_host, e->e2e_dev, bytes, cudaMemcpyDeviceToHost, s));
+  CK(cudaStreamSynchronize(s));
+  return ROSA_OK;
+}
+
+rosa_status_t rosa_last_launch_count(rosa_expert_t* e, int64_t* n) {
+  if (!e || !n) { set_error("NULL argument"); return ROSA_ERR_INVALID_ARG; }
+  *n = e->last_launches;
+  return ROSA_OK;
+}
+rosa_status_t rosa_kernel_family(rosa_expert_t* e, int32_t* family) {
+  if (!e || !family) { set_error("NULL argument"); return ROSA_ERR_INVALID_ARG; }
+  *family = e->family;
+  return ROSA_OK;
+}
+
+rosa_status_t rosa_debug_gemm(int32_t family, int32_t M, int32_t N, int32_t K, const void* A, const void* W,
+                              float* C, void* stream) {
+  if (!A || !W || !C || M < 1 || N < 1 || K < 1) { set_error("bad argument"); return ROSA_ERR_INVALID_ARG; }
+  cudaStream_t s = (cudaStream_t)stream;
+  if (family == 0) {
+    launch_gemm_naive((const bf16*)A, (const bf16*)W, C, M, N, K, nullptr, s);
+    CK(cudaGetLastError());
+    return ROSA_OK;
+  }
+  if (!tc_gemm_supported(N, K)) { set_error("shape not supported by the tcgen05 GEMM"); return ROSA_ERR_UNSUPPORTED; }
+  EpiArgs ea{};
+  ea.out_f32 = C; ea.ld_out = N;
+  CK(launch_gemm_tc(EPI_STORE_F32, (const bf16*)A, (const bf16*)W, M, N, K, ea, s));
+  return ROSA_OK;
+}
+
+const char* rosa_last_error(void) { return g_err.c_str(); }
+int32_t rosa_version(void) { return 1; }
+
+}  // extern "C"

@@ -1,0 +1,107 @@
+// Internal declarations of librosa (not part of the ABI).  sm_100a only.
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "rosa.h"
+
+typedef __nv_bfloat16 bf16;
+
+namespace rosa {
+
+// Model dimensions in the paper/BASELINE notation.
+struct Dims {
+  int layers, d, nq, nkv, hd, F, H, A;
+  int qkv_n;   // (nq + 2 nkv) * hd : packed [q heads | k heads | v heads]
+  int q_n;     // nq * hd
+  int gu_blk;  // gate/up interleave block: packed rows [b*2g, b*2g+g) = gate, next g = up
+  float rope_base, eps, pmin, pmax;
+};
+
+// Per-call device tables (internal batch order = robots sorted by n_steps, descending, so the
+// active set of iteration k is the prefix [0, m_active[k]) of the token rows).
+struct Tables {
+  const int* ids;       // [B] robot id of internal position p
+  const int* src;       // [B] index of p in the caller's noise/out arrays
+  const float* t0;      // [B]
+  const float* dt;      // [B]
+  const int* nsteps;    // [B]
+  const int* m_active;  // [max_steps] active token rows (= H * active robots) in iteration k
+  const bf16* const* rk;  // [max_robots * layers] prefix K pointer of (robot, layer)
+  const bf16* const* rv;  // [max_robots * layers]
+  const int* rlen;        // [max_robots]
+  int batch;
+};
+
+// Caller pointers of the current call live in device memory so that a captured graph can be
+// replayed for a different call (the kernels read them through this struct).
+struct CallPtrs {
+  const float* noise;  // [batch, H, A] caller order
+  float* out;          // [batch, H, A] caller order
+  float* vel;          // [nmax, batch, H, A] or null
+  int batch_ext;
+};
+
+struct LayerWeights {
+  bf16 *wqkv, *wo, *wgu, *wdown;  // [qkv_n,d] [d,q_n] [2F,d] (interleaved) [d,F]
+  float *g_attn, *g_mlp;          // [d]
+};
+
+// Epilogue selector shared by the CUDA-core path (separate elementwise kernels over an fp32
+// scratch) and the tcgen05 path (fused into the GEMM).
+enum Epi : int {
+  EPI_STORE_F32 = 0,     // C fp32 = acc                     (debug GEMM)
+  EPI_SWISH_ROWBIAS = 1, // out bf16 = swish(acc + tvec[m / H][n])
+  EPI_BIAS_F32 = 2,      // h fp32 = acc + bias[n]
+  EPI_ROPE = 3,          // qkv bf16 = rope(acc) on q and k heads at pos = len + j; v copied
+  EPI_RESID = 4,         // h fp32 += acc
+  EPI_GEGLU = 5          // out bf16 [M, N/2] = gelu_tanh(gate) * up (interleaved columns)
+};
+
+struct EpiArgs {
+  float* out_f32;         // EPI_STORE_F32 / BIAS_F32 / RESID
+  bf16* out_bf16;         // SWISH_ROWBIAS / ROPE / GEGLU
+  const float* bias;      // BIAS_F32: [N]
+  const float* rowbias;   // SWISH_ROWBIAS: [B, N] (already offset to iteration k)
+  const float2* rope_tab; // ROPE: [max_pos, hd/2] (cos, sin)
+  const int* ids;         // ROPE: Tables::ids
+  const int* rlen;        // ROPE: Tables::rlen
+  int H, hd, rope_cols;   // ROPE: columns [0, rope_cols) are rotated (q and k heads)
+  int gu_blk;             // GEGLU
+  int ld_out;             // leading dimension (elements) of the output
+  const int* m_active;    // device pointer to the active row count of this iteration (or null)
+};
+
+// ---- launchers (each checks nothing; callers validated shapes) -------------------------
+// simple CUDA-core family
+void launch_gemm_naive(const bf16* A, const bf16* W, float* C, int M, int N, int K,
+                       const int* m_active, cudaStream_t s);
+void launch_epilogue(Epi epi, const float* C, int M, int N, const EpiArgs& a, cudaStream_t s);
+void launch_attn_simple(const Dims& dm, const Tables& tb, int layer, const bf16* qkv, bf16* o,
+                        int k_iter, int max_len, cudaStream_t s);
+// common elementwise kernels
+void launch_gather_x(float* x, const CallPtrs* cp, const Tables& tb, int HA, cudaStream_t s);
+void launch_scatter_x(const CallPtrs* cp, const float* x, const Tables& tb, int HA, cudaStream_t s);
+void launch_timevec(float* tvec, const bf16* w_t1, const float* b_t1, const Dims& dm,
+                    const Tables& tb, int nsteps_max, int max_batch, cudaStream_t s);
+void launch_inproj(bf16* a, const float* x, const bf16* w_in, const float* b_in, const Dims& dm,
+                   const Tables& tb, int k_iter, int M, cudaStream_t s);
+void launch_rmsnorm(bf16* out, const float* h, const float* g, const Dims& dm, const Tables& tb,
+                    int k_iter, int M, cudaStream_t s);
+void launch_final(float* x, const CallPtrs* cp, const float* h, const float* g, const bf16* w_out,
+                  const float* b_out, const Dims& dm, const Tables& tb, int k_iter, int M,
+                  cudaStream_t s);
+void launch_f32_to_bf16(bf16* dst, const float* src, size_t n, cudaStream_t s);
+// tcgen05 family (gemm_tcgen05.cu)
+bool tc_gemm_supported(int N, int K);
+// A [M,K] bf16 row-major, W [N,K] bf16 row-major; returns cudaSuccess or an error
+cudaError_t launch_gemm_tc(Epi epi, const bf16* A, const bf16* W, int M, int N, int K,
+                           const EpiArgs& a, cudaStream_t s);
+
+void set_error(const std::string& msg);
+
+}  // namespace rosa
