@@ -1,6 +1,9 @@
 // Scalar device math shared by every kernel of librosa (readings R3, R6).
 #pragma once
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
+#include <stdint.h>
 
 namespace rosa {
 
@@ -13,6 +16,21 @@ __device__ __forceinline__ float warp_max(float v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
   return v;
+}
+// 16-bit GEMM operand conversions (fp16 or bf16 bits, warp-uniform selector)
+__device__ __forceinline__ uint16_t f2op(float v, int fp16) {
+  return fp16 ? __half_as_ushort(__float2half_rn(v)) : __bfloat16_as_ushort(__float2bfloat16_rn(v));
+}
+__device__ __forceinline__ float op2f(uint16_t b, int fp16) {
+  return fp16 ? __half2float(__ushort_as_half(b)) : __bfloat162float(__ushort_as_bfloat16(b));
+}
+__device__ __forceinline__ uint32_t pack_op2(float lo, float hi, int fp16) {
+  if (fp16) {
+    __half2 v = __floats2half2_rn(lo, hi);
+    return *reinterpret_cast<uint32_t*>(&v);
+  }
+  __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<uint32_t*>(&v);
 }
 // swish(z) = z / (1 + e^-z)
 __device__ __forceinline__ float swish_f(float z) { return z / (1.f + __expf(-z)); }

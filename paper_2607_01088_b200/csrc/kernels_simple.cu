@@ -62,9 +62,9 @@ void launch_timevec(float* tvec, const bf16* w_t1, const float* b_t1, const Dims
 
 // ------------------------------------------------------------------ a1 (action half)
 // a[m][n] = bf16( b_in[n] + sum_c x[m][c] W_in[n][c] ), x in fp32 (R11).
-__global__ void k_inproj(bf16* __restrict__ a, const float* __restrict__ x,
+__global__ void k_inproj(op16* __restrict__ a, const float* __restrict__ x,
                          const bf16* __restrict__ w_in, const float* __restrict__ b_in, int d, int A,
-                         const int* __restrict__ m_active) {
+                         int fp16, const int* __restrict__ m_active) {
   __shared__ float xs[64];
   const int m = blockIdx.x;
   if (m >= *m_active) return;
@@ -73,18 +73,18 @@ __global__ void k_inproj(bf16* __restrict__ a, const float* __restrict__ x,
   for (int n = threadIdx.x; n < d; n += blockDim.x) {
     float acc = b_in[n];
     for (int c = 0; c < A; ++c) acc = fmaf(xs[c], __bfloat162float(w_in[(size_t)n * A + c]), acc);
-    a[(size_t)m * d + n] = __float2bfloat16(acc);
+    a[(size_t)m * d + n] = f2op(acc, fp16);
   }
 }
-void launch_inproj(bf16* a, const float* x, const bf16* w_in, const float* b_in, const Dims& dm,
+void launch_inproj(op16* a, const float* x, const bf16* w_in, const float* b_in, const Dims& dm,
                    const Tables& tb, int k_iter, int M, cudaStream_t s) {
-  k_inproj<<<M, 128, 0, s>>>(a, x, w_in, b_in, dm.d, dm.A, tb.m_active + k_iter);
+  k_inproj<<<M, 128, 0, s>>>(a, x, w_in, b_in, dm.d, dm.A, dm.fp16, tb.m_active + k_iter);
 }
 
 // ------------------------------------------------------------------ a2 RMSNorm (R5)
 // out = bf16( h * rsqrt(mean(h^2) + eps) * g ); one warp per token row; statistics in fp32.
-__global__ void k_rmsnorm(bf16* __restrict__ out, const float* __restrict__ h,
-                          const float* __restrict__ g, int d, float eps,
+__global__ void k_rmsnorm(op16* __restrict__ out, const float* __restrict__ h,
+                          const float* __restrict__ g, int d, float eps, int fp16,
                           const int* __restrict__ m_active) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int m = blockIdx.x * (blockDim.x >> 5) + warp;
@@ -100,18 +100,16 @@ __global__ void k_rmsnorm(bf16* __restrict__ out, const float* __restrict__ h,
   for (int c = lane * 4; c < d; c += 128) {
     float4 v = *reinterpret_cast<const float4*>(row + c);
     float4 gg = *reinterpret_cast<const float4*>(g + c);
-    __nv_bfloat162 lo = __floats2bfloat162_rn(v.x * r * gg.x, v.y * r * gg.y);
-    __nv_bfloat162 hi = __floats2bfloat162_rn(v.z * r * gg.z, v.w * r * gg.w);
     uint2 pk;
-    pk.x = *reinterpret_cast<uint32_t*>(&lo);
-    pk.y = *reinterpret_cast<uint32_t*>(&hi);
+    pk.x = pack_op2(v.x * r * gg.x, v.y * r * gg.y, fp16);
+    pk.y = pack_op2(v.z * r * gg.z, v.w * r * gg.w, fp16);
     *reinterpret_cast<uint2*>(out + (size_t)m * d + c) = pk;
   }
 }
-void launch_rmsnorm(bf16* out, const float* h, const float* g, const Dims& dm, const Tables& tb,
+void launch_rmsnorm(op16* out, const float* h, const float* g, const Dims& dm, const Tables& tb,
                     int k_iter, int M, cudaStream_t s) {
   const int wpb = 8;
-  k_rmsnorm<<<(M + wpb - 1) / wpb, wpb * 32, 0, s>>>(out, h, g, dm.d, dm.eps, tb.m_active + k_iter);
+  k_rmsnorm<<<(M + wpb - 1) / wpb, wpb * 32, 0, s>>>(out, h, g, dm.d, dm.eps, dm.fp16, tb.m_active + k_iter);
 }
 
 // ------------------------------------------------------------------ a9 + a10 (+ a11 bookkeeping)
@@ -168,11 +166,11 @@ void launch_f32_to_bf16(bf16* dst, const float* src, size_t n, cudaStream_t s) {
 }
 
 // ------------------------------------------------------------------ CUDA-core GEMM (family 0)
-// C[M,N] fp32 = A[M,K] * W[N,K]^T, bf16 operands, fp32 accumulate.  64x64 tile, 16x16 threads,
+// C[M,N] fp32 = A[M,K] * W[N,K]^T, fp16 or bf16 operands, fp32 accumulate.  64x64 tile, 16x16 threads,
 // 4x4 micro-tile.  Not a fast kernel: it is the shape-generic family and the on-device reference.
 constexpr int GN_T = 64, GN_K = 32;
-__global__ void __launch_bounds__(256) k_gemm_naive(const bf16* __restrict__ A, const bf16* __restrict__ W,
-                                                    float* __restrict__ C, int M, int N, int K,
+__global__ void __launch_bounds__(256) k_gemm_naive(const op16* __restrict__ A, const op16* __restrict__ W,
+                                                    float* __restrict__ C, int M, int N, int K, int fp16,
                                                     const int* __restrict__ m_active) {
   __shared__ float As[GN_K][GN_T + 4];
   __shared__ float Ws[GN_K][GN_T + 4];
@@ -185,8 +183,8 @@ __global__ void __launch_bounds__(256) k_gemm_naive(const bf16* __restrict__ A, 
     for (int i = threadIdx.x; i < GN_T * GN_K; i += 256) {
       int r = i / GN_K, c = i % GN_K;
       int gm = m0 + r, gn = n0 + r, gk = k0 + c;
-      As[c][r] = (gm < m_lim && gk < K) ? __bfloat162float(A[(size_t)gm * K + gk]) : 0.f;
-      Ws[c][r] = (gn < N && gk < K) ? __bfloat162float(W[(size_t)gn * K + gk]) : 0.f;
+      As[c][r] = (gm < m_lim && gk < K) ? op2f(A[(size_t)gm * K + gk], fp16) : 0.f;
+      Ws[c][r] = (gn < N && gk < K) ? op2f(W[(size_t)gn * K + gk], fp16) : 0.f;
     }
     __syncthreads();
 #pragma unroll 8
@@ -214,10 +212,10 @@ __global__ void __launch_bounds__(256) k_gemm_naive(const bf16* __restrict__ A, 
     }
   }
 }
-void launch_gemm_naive(const bf16* A, const bf16* W, float* C, int M, int N, int K,
+void launch_gemm_naive(const op16* A, const op16* W, float* C, int M, int N, int K, int fp16,
                        const int* m_active, cudaStream_t s) {
   dim3 grid((N + GN_T - 1) / GN_T, (M + GN_T - 1) / GN_T);
-  k_gemm_naive<<<grid, 256, 0, s>>>(A, W, C, M, N, K, m_active);
+  k_gemm_naive<<<grid, 256, 0, s>>>(A, W, C, M, N, K, fp16, m_active);
 }
 
 // ------------------------------------------------------------------ epilogues over the fp32 scratch
@@ -231,7 +229,7 @@ __global__ void k_epilogue(int epi, const float* __restrict__ C, int M, int N, E
     switch (epi) {
       case EPI_STORE_F32: a.out_f32[(size_t)m * a.ld_out + n] = acc; break;
       case EPI_SWISH_ROWBIAS:
-        a.out_bf16[(size_t)m * a.ld_out + n] = __float2bfloat16(swish_f(acc + a.rowbias[(size_t)(m / a.H) * N + n]));
+        ((op16*)a.out16)[(size_t)m * a.ld_out + n] = f2op(swish_f(acc + a.rowbias[(size_t)(m / a.H) * N + n]), a.out_fp16);
         break;
       case EPI_BIAS_F32: a.out_f32[(size_t)m * a.ld_out + n] = acc + a.bias[n]; break;
       case EPI_RESID: a.out_f32[(size_t)m * a.ld_out + n] += acc; break;
@@ -245,13 +243,13 @@ __global__ void k_epilogue(int epi, const float* __restrict__ C, int M, int N, E
           const float other = C[(size_t)m * N + (c < half ? n + half : n - half)];
           r = c < half ? acc * cs.x - other * cs.y : acc * cs.x + other * cs.y;
         }
-        a.out_bf16[(size_t)m * a.ld_out + n] = __float2bfloat16(r);
+        ((bf16*)a.out16)[(size_t)m * a.ld_out + n] = __float2bfloat16(r);
       } break;
       case EPI_GEGLU: {
         const int g = a.gu_blk, blk = n / (2 * g), r = n % (2 * g);
         if (r < g) {
           const float up = C[idx + g];
-          a.out_bf16[(size_t)m * a.ld_out + blk * g + r] = __float2bfloat16(gelu_tanh_f(acc) * up);
+          ((op16*)a.out16)[(size_t)m * a.ld_out + blk * g + r] = f2op(gelu_tanh_f(acc) * up, a.out_fp16);
         }
       } break;
     }
@@ -270,7 +268,7 @@ void launch_epilogue(Epi epi, const float* C, int M, int N, const EpiArgs& a, cu
 // [prefix K/V of the robot ; the block's own k/v] (R8: full visibility, scale 1/sqrt(hd)).
 // Thread-per-key scores into shared memory, block softmax, thread-per-channel P V.
 __global__ void __launch_bounds__(256) k_attn_simple(Dims dm, Tables tb, int layer,
-                                                     const bf16* __restrict__ qkv, bf16* __restrict__ o,
+                                                     const bf16* __restrict__ qkv, op16* __restrict__ o,
                                                      int k_iter) {
   extern __shared__ float sm[];
   const int p = blockIdx.x / dm.H, j = blockIdx.x % dm.H;
@@ -326,10 +324,10 @@ __global__ void __launch_bounds__(256) k_attn_simple(Dims dm, Tables tb, int lay
                              : qkv + (size_t)(p * dm.H + (s - L)) * dm.qkv_n + dm.q_n + dm.nkv * hd + g * hd;
       acc = fmaf(sc[(size_t)a * T + s], __bfloat162float(vr[c]), acc);
     }
-    o[(size_t)m * dm.q_n + i] = __float2bfloat16(acc * red[a]);
+    o[(size_t)m * dm.q_n + i] = f2op(acc * red[a], dm.fp16);
   }
 }
-void launch_attn_simple(const Dims& dm, const Tables& tb, int layer, const bf16* qkv, bf16* o,
+void launch_attn_simple(const Dims& dm, const Tables& tb, int layer, const bf16* qkv, op16* o,
                         int k_iter, int max_len, cudaStream_t s) {
   size_t smem = ((size_t)dm.nq * dm.hd + (size_t)dm.nq * (max_len + dm.H) + dm.nq) * sizeof(float);
   static size_t configured = 0;

@@ -58,13 +58,15 @@ struct rosa_expert {
   bool use_graph = true;
   int max_pos = 0;
   // weights
-  bf16 *w_in = nullptr, *w_t1 = nullptr, *w_t1a = nullptr, *w_t2 = nullptr, *w_out = nullptr;
+  bf16 *w_in = nullptr, *w_t1 = nullptr, *w_out = nullptr;  // CUDA-core steps: bf16 as given
+  op16 *w_t1a = nullptr, *w_t2 = nullptr;                    // GEMM operands: fp16 or bf16 (dm.fp16)
   float *b_in = nullptr, *b_t1 = nullptr, *b_t2 = nullptr, *b_out = nullptr, *g_final = nullptr;
   std::vector<LayerWeights> lw;
   float2* rope_tab = nullptr;
   // workspaces
   float *x = nullptr, *h = nullptr, *tvec = nullptr, *scratch = nullptr;
-  bf16 *abuf = nullptr, *zbuf = nullptr, *nrm = nullptr, *qkv = nullptr, *obuf = nullptr, *mact = nullptr;
+  op16 *abuf = nullptr, *zbuf = nullptr, *nrm = nullptr, *obuf = nullptr, *mact = nullptr;
+  bf16* qkv = nullptr;  // q/k/v feed attention together with the bf16 prefix cache: always bf16
   // robot table (device) + host mirror
   const bf16** d_rk = nullptr;
   const bf16** d_rv = nullptr;
@@ -123,6 +125,20 @@ static rosa_status_t upload_bf16(rosa_expert* e, const std::vector<float>& v, bf
   CK(cudaMemcpy(*out, b.data(), b.size() * 2, cudaMemcpyHostToDevice));
   return ROSA_OK;
 }
+// GEMM operand upload: fp16 (RNE from the given values; bf16-valued inputs with |w| >= 6.1e-5
+// convert exactly) or bf16, per dm.fp16.
+static rosa_status_t upload_op16(rosa_expert* e, const std::vector<float>& v, op16** out) {
+  std::vector<uint16_t> b(v.size());
+  if (e->dm.fp16) {
+    for (size_t i = 0; i < v.size(); ++i) b[i] = __half_as_ushort(__float2half_rn(v[i]));
+  } else {
+    for (size_t i = 0; i < v.size(); ++i) b[i] = f2bf(v[i]);
+  }
+  rosa_status_t st = dev_alloc(e, (void**)out, b.size() * 2);
+  if (st != ROSA_OK) return st;
+  CK(cudaMemcpy(*out, b.data(), b.size() * 2, cudaMemcpyHostToDevice));
+  return ROSA_OK;
+}
 static rosa_status_t upload_f32(rosa_expert* e, const std::vector<float>& v, float** out) {
   rosa_status_t st = dev_alloc(e, (void**)out, v.size() * 4);
   if (st != ROSA_OK) return st;
@@ -167,6 +183,10 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
   dm.qkv_n = (dm.nq + 2 * dm.nkv) * dm.hd;
   dm.q_n = dm.nq * dm.hd;
   dm.gu_blk = 64;
+  {  // GEMM operand format: fp16 by default (reading R19), ROSA_GEMM_DTYPE=bf16 to compare
+    const char* gd = getenv("ROSA_GEMM_DTYPE");
+    dm.fp16 = (gd && !strcmp(gd, "bf16")) ? 0 : 1;
+  }
   dm.rope_base = c->rope_base; dm.eps = c->rms_eps; dm.pmin = c->time_min_period; dm.pmax = c->time_max_period;
   const int d = dm.d, F = dm.F, A = dm.A;
   const rosa_dtype_t dt = w->dtype;
@@ -175,15 +195,16 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
   rosa_status_t st;
 #define FETCH(ptr, n) if ((st = fetch_f32(ptr, (size_t)(n), dt, od, t)) != ROSA_OK) return st
 #define UPB(dst) if ((st = upload_bf16(e, t, &(dst))) != ROSA_OK) return st
+#define UPO(dst) if ((st = upload_op16(e, t, &(dst))) != ROSA_OK) return st
 #define UPF(dst) if ((st = upload_f32(e, t, &(dst))) != ROSA_OK) return st
   FETCH(w->w_in, (size_t)d * A); UPB(e->w_in);
   FETCH(w->b_in, d); UPF(e->b_in);
   FETCH(w->w_t1, (size_t)d * 2 * d); UPB(e->w_t1);
   u.resize((size_t)d * d);  // action half of W_1 (columns d..2d-1, R2) as its own [d,d] matrix
   for (int n = 0; n < d; ++n) memcpy(&u[(size_t)n * d], &t[(size_t)n * 2 * d + d], (size_t)d * 4);
-  t.swap(u); UPB(e->w_t1a);
+  t.swap(u); UPO(e->w_t1a);
   FETCH(w->b_t1, d); UPF(e->b_t1);
-  FETCH(w->w_t2, (size_t)d * d); UPB(e->w_t2);
+  FETCH(w->w_t2, (size_t)d * d); UPO(e->w_t2);
   FETCH(w->b_t2, d); UPF(e->b_t2);
   FETCH(w->w_out, (size_t)A * d); UPB(e->w_out);
   FETCH(w->b_out, A); UPF(e->b_out);
@@ -199,8 +220,8 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
     FETCH(w->wk[l], (size_t)dm.nkv * dm.hd * d); memcpy(pk.data() + (size_t)dm.q_n * d, t.data(), t.size() * 4);
     FETCH(w->wv[l], (size_t)dm.nkv * dm.hd * d);
     memcpy(pk.data() + (size_t)(dm.q_n + dm.nkv * dm.hd) * d, t.data(), t.size() * 4);
-    t.swap(pk); UPB(L.wqkv);
-    FETCH(w->wo[l], (size_t)d * dm.q_n); UPB(L.wo);
+    t.swap(pk); UPO(L.wqkv);
+    FETCH(w->wo[l], (size_t)d * dm.q_n); UPO(L.wo);
     // gate/up interleaved in blocks of gu_blk rows -> one GEMM + GeGLU epilogue (step a7)
     std::vector<float> gu((size_t)2 * F * d);
     const int g = dm.gu_blk;
@@ -210,11 +231,12 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
     FETCH(w->w_up[l], (size_t)F * d);
     for (int f = 0; f < F; ++f)
       memcpy(&gu[((size_t)(f / g) * 2 * g + g + f % g) * d], &t[(size_t)f * d], (size_t)d * 4);
-    t.swap(gu); UPB(L.wgu);
-    FETCH(w->w_down[l], (size_t)d * F); UPB(L.wdown);
+    t.swap(gu); UPO(L.wgu);
+    FETCH(w->w_down[l], (size_t)d * F); UPO(L.wdown);
   }
 #undef FETCH
 #undef UPB
+#undef UPO
 #undef UPF
   // RoPE table in fp64 (R7): pos in [0, max_prefix_len + H), c < hd/2 -> (cos, sin)(pos * base^(-2c/hd))
   e->max_pos = c->max_prefix_len + dm.H;
@@ -283,13 +305,13 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
 }
 
 // One GEMM + epilogue of the path, in whichever kernel family the expert runs.
-static cudaError_t gemm(rosa_expert* e, Epi epi, const bf16* A, const bf16* W, int M, int N, int K,
+static cudaError_t gemm(rosa_expert* e, Epi epi, const op16* A, const op16* W, int M, int N, int K,
                         const EpiArgs& a, cudaStream_t s) {
   if (e->family == 1 && tc_gemm_supported(N, K)) {
     e->last_launches += 1;
     return launch_gemm_tc(epi, A, W, M, N, K, a, s);
   }
-  launch_gemm_naive(A, W, e->scratch, M, N, K, a.m_active, s);
+  launch_gemm_naive(A, W, e->scratch, M, N, K, a.in_fp16, a.m_active, s);
   launch_epilogue(epi, e->scratch, M, N, a, s);
   e->last_launches += 2;
   return cudaGetLastError();
@@ -310,11 +332,11 @@ static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, cudaStream_
   for (int k = 0; k < nmax; ++k) {
     EpiArgs ea{};
     ea.m_active = tb.m_active + k;
-    ea.H = dm.H; ea.hd = dm.hd; ea.gu_blk = dm.gu_blk;
+    ea.H = dm.H; ea.hd = dm.hd; ea.gu_blk = dm.gu_blk; ea.in_fp16 = dm.fp16; ea.out_fp16 = dm.fp16;
     // a1: h0 = W2 swish(W1 [tau ; W_in x + b_in] + b1) + b2
     launch_inproj(e->abuf, e->x, e->w_in, e->b_in, dm, tb, k, M, s);
     e->last_launches += 1;
-    ea.out_bf16 = e->zbuf; ea.ld_out = d;
+    ea.out16 = e->zbuf; ea.ld_out = d;
     ea.rowbias = e->tvec + (size_t)k * e->cfg.max_batch * d;
     if ((err = gemm(e, EPI_SWISH_ROWBIAS, e->abuf, e->w_t1a, M, d, d, ea, s)) != cudaSuccess) return err;
     ea.out_f32 = e->h; ea.bias = e->b_t2;
@@ -322,7 +344,7 @@ static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, cudaStream_
     for (int l = 0; l < dm.layers; ++l) {
       const LayerWeights& L = e->lw[l];
       launch_rmsnorm(e->nrm, e->h, L.g_attn, dm, tb, k, M, s);                       // a2
-      ea.out_bf16 = e->qkv; ea.ld_out = dm.qkv_n;
+      ea.out16 = e->qkv; ea.ld_out = dm.qkv_n;
       ea.rope_tab = e->rope_tab; ea.ids = tb.ids; ea.rlen = tb.rlen;
       ea.rope_cols = dm.q_n + dm.nkv * dm.hd;
       if ((err = gemm(e, EPI_ROPE, e->nrm, L.wqkv, M, dm.qkv_n, d, ea, s)) != cudaSuccess) return err;  // a3+a4
@@ -330,7 +352,7 @@ static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, cudaStream_
       ea.out_f32 = e->h; ea.ld_out = d;
       if ((err = gemm(e, EPI_RESID, e->obuf, L.wo, M, d, dm.q_n, ea, s)) != cudaSuccess) return err;    // a6
       launch_rmsnorm(e->nrm, e->h, L.g_mlp, dm, tb, k, M, s);                        // a2
-      ea.out_bf16 = e->mact; ea.ld_out = dm.F;
+      ea.out16 = e->mact; ea.ld_out = dm.F;
       if ((err = gemm(e, EPI_GEGLU, e->nrm, L.wgu, M, 2 * dm.F, d, ea, s)) != cudaSuccess) return err;  // a7
       ea.out_f32 = e->h; ea.ld_out = d;
       if ((err = gemm(e, EPI_RESID, e->mact, L.wdown, M, d, dm.F, ea, s)) != cudaSuccess) return err;   // a8
@@ -448,7 +470,9 @@ rosa_status_t rosa_expert_create(const rosa_expert_config_t* c, const rosa_weigh
   rosa_expert* e = new rosa_expert();
   e->cfg = *c;
   const char* fam = getenv("ROSA_KERNELS");
-  e->family = (fam && !strcmp(fam, "simple")) ? 0 : 1;
+  // tcgen05 family needs head_dim == 256 (RoPE epilogue tile = one head) and 128/256-wide N tiles
+  const bool tc_shape = c->head_dim == 256 && c->d_model % 128 == 0 && (2 * c->ffn) % 256 == 0;
+  e->family = (fam && !strcmp(fam, "simple")) || !tc_shape ? 0 : 1;
   const char* gr = getenv("ROSA_GRAPH");
   e->use_graph = !(gr && !strcmp(gr, "0"));
   rosa_status_t st = create_impl(c, w, e);
@@ -559,14 +583,14 @@ rosa_status_t rosa_debug_gemm(int32_t family, int32_t M, int32_t N, int32_t K, c
   if (!A || !W || !C || M < 1 || N < 1 || K < 1) { set_error("bad argument"); return ROSA_ERR_INVALID_ARG; }
   cudaStream_t s = (cudaStream_t)stream;
   if (family == 0) {
-    launch_gemm_naive((const bf16*)A, (const bf16*)W, C, M, N, K, nullptr, s);
+    launch_gemm_naive((const op16*)A, (const op16*)W, C, M, N, K, 0, nullptr, s);
     CK(cudaGetLastError());
     return ROSA_OK;
   }
   if (!tc_gemm_supported(N, K)) { set_error("shape not supported by the tcgen05 GEMM"); return ROSA_ERR_UNSUPPORTED; }
   EpiArgs ea{};
   ea.out_f32 = C; ea.ld_out = N;
-  CK(launch_gemm_tc(EPI_STORE_F32, (const bf16*)A, (const bf16*)W, M, N, K, ea, s));
+  CK(launch_gemm_tc(EPI_STORE_F32, (const op16*)A, (const op16*)W, M, N, K, ea, s));
   return ROSA_OK;
 }
 

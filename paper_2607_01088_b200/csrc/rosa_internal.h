@@ -1,6 +1,7 @@
 // Internal declarations of librosa (not part of the ABI).  sm_100a only.
 #pragma once
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -10,6 +11,7 @@
 #include "rosa.h"
 
 typedef __nv_bfloat16 bf16;
+typedef uint16_t op16;  // 16-bit GEMM operand storage: fp16 or bf16 bits, chosen per expert (Dims::fp16)
 
 namespace rosa {
 
@@ -19,6 +21,7 @@ struct Dims {
   int qkv_n;   // (nq + 2 nkv) * hd : packed [q heads | k heads | v heads]
   int q_n;     // nq * hd
   int gu_blk;  // gate/up interleave block: packed rows [b*2g, b*2g+g) = gate, next g = up
+  int fp16;    // GEMM operands (weights + activations) held as fp16 (1) or bf16 (0); R19
   float rope_base, eps, pmin, pmax;
 };
 
@@ -47,7 +50,7 @@ struct CallPtrs {
 };
 
 struct LayerWeights {
-  bf16 *wqkv, *wo, *wgu, *wdown;  // [qkv_n,d] [d,q_n] [2F,d] (interleaved) [d,F]
+  op16 *wqkv, *wo, *wgu, *wdown;  // [qkv_n,d] [d,q_n] [2F,d] (interleaved) [d,F]
   float *g_attn, *g_mlp;          // [d]
 };
 
@@ -64,7 +67,9 @@ enum Epi : int {
 
 struct EpiArgs {
   float* out_f32;         // EPI_STORE_F32 / BIAS_F32 / RESID
-  bf16* out_bf16;         // SWISH_ROWBIAS / ROPE / GEGLU
+  void* out16;            // SWISH_ROWBIAS / GEGLU: op16 (fp16 or bf16 per out_fp16); ROPE: bf16
+  int out_fp16;           // 16-bit output format: 1 = fp16, 0 = bf16
+  int in_fp16;            // operand format of A and W
   const float* bias;      // BIAS_F32: [N]
   const float* rowbias;   // SWISH_ROWBIAS: [B, N] (already offset to iteration k)
   const float2* rope_tab; // ROPE: [max_pos, hd/2] (cos, sin)
@@ -78,19 +83,19 @@ struct EpiArgs {
 
 // ---- launchers (each checks nothing; callers validated shapes) -------------------------
 // simple CUDA-core family
-void launch_gemm_naive(const bf16* A, const bf16* W, float* C, int M, int N, int K,
+void launch_gemm_naive(const op16* A, const op16* W, float* C, int M, int N, int K, int fp16,
                        const int* m_active, cudaStream_t s);
 void launch_epilogue(Epi epi, const float* C, int M, int N, const EpiArgs& a, cudaStream_t s);
-void launch_attn_simple(const Dims& dm, const Tables& tb, int layer, const bf16* qkv, bf16* o,
+void launch_attn_simple(const Dims& dm, const Tables& tb, int layer, const bf16* qkv, op16* o,
                         int k_iter, int max_len, cudaStream_t s);
 // common elementwise kernels
 void launch_gather_x(float* x, const CallPtrs* cp, const Tables& tb, int HA, cudaStream_t s);
 void launch_scatter_x(const CallPtrs* cp, const float* x, const Tables& tb, int HA, cudaStream_t s);
 void launch_timevec(float* tvec, const bf16* w_t1, const float* b_t1, const Dims& dm,
                     const Tables& tb, int nsteps_max, int max_batch, cudaStream_t s);
-void launch_inproj(bf16* a, const float* x, const bf16* w_in, const float* b_in, const Dims& dm,
+void launch_inproj(op16* a, const float* x, const bf16* w_in, const float* b_in, const Dims& dm,
                    const Tables& tb, int k_iter, int M, cudaStream_t s);
-void launch_rmsnorm(bf16* out, const float* h, const float* g, const Dims& dm, const Tables& tb,
+void launch_rmsnorm(op16* out, const float* h, const float* g, const Dims& dm, const Tables& tb,
                     int k_iter, int M, cudaStream_t s);
 void launch_final(float* x, const CallPtrs* cp, const float* h, const float* g, const bf16* w_out,
                   const float* b_out, const Dims& dm, const Tables& tb, int k_iter, int M,
@@ -98,8 +103,8 @@ void launch_final(float* x, const CallPtrs* cp, const float* h, const float* g, 
 void launch_f32_to_bf16(bf16* dst, const float* src, size_t n, cudaStream_t s);
 // tcgen05 family (gemm_tcgen05.cu)
 bool tc_gemm_supported(int N, int K);
-// A [M,K] bf16 row-major, W [N,K] bf16 row-major; returns cudaSuccess or an error
-cudaError_t launch_gemm_tc(Epi epi, const bf16* A, const bf16* W, int M, int N, int K,
+// A [M,K] row-major, W [N,K] row-major, both fp16 or both bf16 (EpiArgs::in_fp16)
+cudaError_t launch_gemm_tc(Epi epi, const op16* A, const op16* W, int M, int N, int K,
                            const EpiArgs& a, cudaStream_t s);
 
 void set_error(const std::string& msg);
