@@ -288,7 +288,22 @@ bool make_tmap_2d(CUtensorMap* tm, const void* ptr, uint64_t rows, uint64_t K, u
   return r == CUDA_SUCCESS;
 }
 
-static int num_sms() {
+// Generic tiled map over 16-bit elements, SWIZZLE_128B (inner box = 64 elements = 128 B).
+// dims/box innermost first; strides_bytes has rank-1 entries (dims 1..rank-1).
+bool encode_tmap(CUtensorMap* tm, const void* ptr, int rank, const uint64_t* dims, const uint64_t* strides_bytes,
+                 const uint32_t* box) {
+  EncodeTiledFn enc = get_encode();
+  if (!enc) return false;
+  cuuint64_t d[5], st[4];
+  cuuint32_t b[5], es[5];
+  for (int i = 0; i < rank; ++i) { d[i] = dims[i]; b[i] = box[i]; es[i] = 1; }
+  for (int i = 0; i + 1 < rank; ++i) st[i] = strides_bytes[i];
+  return enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, (cuuint32_t)rank, const_cast<void*>(ptr), d, st, b, es,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+int num_sms() {
   static int n = 0;
   if (!n) {
     int dev = 0;

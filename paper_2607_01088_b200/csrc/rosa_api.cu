@@ -74,6 +74,8 @@ struct rosa_expert {
   std::vector<int> h_rlen;         // -1 = unbound
   std::vector<std::vector<bf16*>> owned;  // per robot: library-owned K/V buffers (fp32 binds)
   int max_len_bound = 0;
+  bool attn_tc = false;            // tcgen05 attention kernel in use
+  char* d_kv_maps = nullptr;       // [max_robots * layers * 2] CUtensorMap (prefix K, V per robot/layer)
   // per-call tables
   char* d_call = nullptr;          // fixed device block
   char* h_stage[kStageRing] = {};  // pinned ring
@@ -281,6 +283,15 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
   CK(cudaMemset(e->d_rk, 0, (size_t)c->max_robots * dm.layers * sizeof(void*)));
   CK(cudaMemset(e->d_rv, 0, (size_t)c->max_robots * dm.layers * sizeof(void*)));
   CK(cudaMemset(e->d_rlen, 0, (size_t)c->max_robots * 4));
+  {
+    const char* at = getenv("ROSA_ATTN");
+    e->attn_tc = e->family == 1 && tc_attn_supported(dm) && !(at && !strcmp(at, "simple"));
+    if (e->attn_tc) {
+      const size_t nb = (size_t)c->max_robots * dm.layers * 2 * tc_attn_map_bytes();
+      WS(e->d_kv_maps, nb);
+      CK(cudaMemset(e->d_kv_maps, 0, nb));
+    }
+  }
   e->h_rlen.assign(c->max_robots, -1);
   e->owned.resize(c->max_robots);
   // per-call table block
@@ -348,7 +359,11 @@ static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, cudaStream_
       ea.rope_tab = e->rope_tab; ea.ids = tb.ids; ea.rlen = tb.rlen;
       ea.rope_cols = dm.q_n + dm.nkv * dm.hd;
       if ((err = gemm(e, EPI_ROPE, e->nrm, L.wqkv, M, dm.qkv_n, d, ea, s)) != cudaSuccess) return err;  // a3+a4
-      launch_attn_simple(dm, tb, l, e->qkv, e->obuf, k, e->cfg.max_prefix_len, s);   // a5
+      if (e->attn_tc) {                                                              // a5
+        if ((err = launch_attn_tc(dm, tb, l, e->qkv, e->obuf, k, M, e->d_kv_maps, s)) != cudaSuccess) return err;
+      } else {
+        launch_attn_simple(dm, tb, l, e->qkv, e->obuf, k, e->cfg.max_prefix_len, s);
+      }
       ea.out_f32 = e->h; ea.ld_out = d;
       if ((err = gemm(e, EPI_RESID, e->obuf, L.wo, M, d, dm.q_n, ea, s)) != cudaSuccess) return err;    // a6
       launch_rmsnorm(e->nrm, e->h, L.g_mlp, dm, tb, k, M, s);                        // a2
@@ -534,6 +549,17 @@ rosa_status_t rosa_prefix_kv_bind(rosa_expert_t* e, int32_t robot, const void* c
   }
   CK(cudaMemcpy(e->d_rk + (size_t)robot * dm.layers, hk.data(), dm.layers * sizeof(void*), cudaMemcpyHostToDevice));
   CK(cudaMemcpy(e->d_rv + (size_t)robot * dm.layers, hv.data(), dm.layers * sizeof(void*), cudaMemcpyHostToDevice));
+  if (e->attn_tc && len > 0) {
+    const size_t mb = tc_attn_map_bytes();
+    std::vector<char> maps((size_t)dm.layers * 2 * mb + 64);
+    char* mp = (char*)(((uintptr_t)maps.data() + 63) & ~(uintptr_t)63);
+    for (int l = 0; l < dm.layers; ++l)
+      if (!tc_attn_make_prefix_maps(mp + (size_t)l * 2 * mb, hk[l], hv[l], len, dm)) {
+        set_error("cuTensorMapEncodeTiled failed for the prefix K/V"); return ROSA_ERR_CUDA;
+      }
+    CK(cudaMemcpy(e->d_kv_maps + (size_t)robot * dm.layers * 2 * mb, mp, (size_t)dm.layers * 2 * mb,
+                  cudaMemcpyHostToDevice));
+  }
   CK(cudaMemcpy(e->d_rlen + robot, &len, 4, cudaMemcpyHostToDevice));
   e->h_rlen[robot] = len;
   return ROSA_OK;

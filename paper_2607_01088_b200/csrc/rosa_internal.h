@@ -107,6 +107,13 @@ bool tc_gemm_supported(int N, int K);
 cudaError_t launch_gemm_tc(Epi epi, const op16* A, const op16* W, int M, int N, int K,
                            const EpiArgs& a, cudaStream_t s);
 
+// tcgen05 attention (attn_tcgen05.cu)
+bool tc_attn_supported(const Dims& dm);
+size_t tc_attn_map_bytes();  // sizeof(CUtensorMap)
+bool tc_attn_make_prefix_maps(void* out2_host, const bf16* k, const bf16* v, int len, const Dims& dm);
+cudaError_t launch_attn_tc(const Dims& dm, const Tables& tb, int layer, const bf16* qkv, op16* o, int k_iter,
+                           int M, const void* d_kv_maps, cudaStream_t s);
+
 void set_error(const std::string& msg);
 
 }  // namespace rosa

@@ -8,6 +8,11 @@
 #include <stdint.h>
 
 namespace rosa {
+// host helpers (gemm_tcgen05.cu)
+bool encode_tmap(CUtensorMap* tm, const void* ptr, int rank, const uint64_t* dims, const uint64_t* strides_bytes,
+                 const uint32_t* box);
+int num_sms();
+
 namespace tc {
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
