@@ -124,6 +124,33 @@ rosa_status_t rosa_denoise_batch_host(rosa_expert_t *e, int32_t batch, const int
 rosa_status_t rosa_last_launch_count(rosa_expert_t *e, int64_t *n_kernels);
 rosa_status_t rosa_kernel_family(rosa_expert_t *e, int32_t *family);
 
+/* Kernel classes of the hot path, for rosa_profile_batch. */
+typedef enum {
+  ROSA_KC_GATHER_SCATTER = 0, /* x gather at call start / scatter at call end */
+  ROSA_KC_TIMEVEC = 1,        /* a1, time half of W_1 (hoisted, once per call) */
+  ROSA_KC_INPROJ = 2,         /* a1, W_in x + b_in */
+  ROSA_KC_GEMM_EMBED = 3,     /* a1, the two d x d GEMMs of the time MLP */
+  ROSA_KC_RMSNORM = 4,        /* a2 */
+  ROSA_KC_GEMM_QKV = 5,       /* a3 + a4 */
+  ROSA_KC_ATTN = 6,           /* a5 */
+  ROSA_KC_GEMM_O = 7,         /* a6 */
+  ROSA_KC_GEMM_GATEUP = 8,    /* a7 */
+  ROSA_KC_GEMM_DOWN = 9,      /* a8 */
+  ROSA_KC_FINAL = 10,         /* a9 + a10 */
+  ROSA_KC_COUNT = 11
+} rosa_kernel_class_t;
+
+/* Measurement aid for bench.py (SURVEY 8(d) "evidence per kernel"): runs the same call as
+ * rosa_denoise_batch_ex, NOT through the CUDA graph, with a CUDA event recorded on `stream`
+ * between consecutive launches, synchronises, and returns per kernel class the summed device
+ * time in milliseconds (ms_out [host] float[ROSA_KC_COUNT]) and the number of launches
+ * (launches_out [host] int32[ROSA_KC_COUNT]).  Results are identical to the graphed call. */
+rosa_status_t rosa_profile_batch(rosa_expert_t *e, int32_t batch, const int32_t *robot_ids,
+                                 const float *noise, const float *t_start, const float *dt,
+                                 const int32_t *n_steps, float *out_actions, void *stream,
+                                 float *ms_out, int32_t *launches_out);
+const char *rosa_kernel_class_name(int32_t cls); /* "" if out of range */
+
 /* Kernel unit-test hook: C[M,N] (float32, [dev]) = A[M,K] * W[N,K]^T with bf16 [dev]
  * operands through the tcgen05/TMA GEMM (family 1) or the CUDA-core GEMM (family 0).
  * K % 64 == 0 and N % 64 == 0 required for family 1. */

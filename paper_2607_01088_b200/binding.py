@@ -21,8 +21,10 @@ ROSA_F32, ROSA_BF16 = 0, 1
 
 EXPORTS = ("rosa_expert_create", "rosa_expert_destroy", "rosa_prefix_kv_bind", "rosa_prefix_kv_unbind",
            "rosa_denoise_batch", "rosa_denoise_batch_ex", "rosa_denoise_batch_host",
+           "rosa_profile_batch", "rosa_kernel_class_name",
            "rosa_last_launch_count", "rosa_kernel_family", "rosa_debug_gemm", "rosa_last_error",
            "rosa_version")
+ROSA_KC_COUNT = 11
 
 
 class RosaError(RuntimeError):
@@ -70,10 +72,13 @@ def load():
     lib.rosa_last_launch_count.argtypes = [vp, C.POINTER(i64)]
     lib.rosa_kernel_family.argtypes = [vp, C.POINTER(i32)]
     lib.rosa_debug_gemm.argtypes = [i32, i32, i32, i32, vp, vp, vp, vp]
+    lib.rosa_profile_batch.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.rosa_kernel_class_name.argtypes = [i32]
+    lib.rosa_kernel_class_name.restype = C.c_char_p
     lib.rosa_last_error.restype = C.c_char_p
     lib.rosa_version.restype = i32
     for n in EXPORTS:
-        if n not in ("rosa_last_error", "rosa_version"):
+        if n not in ("rosa_last_error", "rosa_version", "rosa_kernel_class_name"):
             getattr(lib, n).restype = C.c_int
     _lib = lib
     return lib
@@ -195,6 +200,21 @@ def rosa_denoise_batch_host(e: Expert, robot_ids, noise_host, t_start, dt, n_ste
     t0, d, ns = _host(t_start, np.float32), _host(dt, np.float32), _host(n_steps, np.int32)
     _check(load().rosa_denoise_batch_host(e.handle, len(ids), _ptr(ids), _ptr(noise_host), _ptr(t0), _ptr(d),
                                           _ptr(ns), _ptr(out_actions_host), _stream_handle(stream)))
+
+
+def rosa_profile_batch(e: Expert, robot_ids, noise, t_start, dt, n_steps, out_actions, stream=None):
+    """Returns {kernel class name: (milliseconds, launches)} for one un-graphed, event-timed call."""
+    ids = _host(robot_ids, np.int32)
+    t0, d, ns = _host(t_start, np.float32), _host(dt, np.float32), _host(n_steps, np.int32)
+    ms = np.zeros(ROSA_KC_COUNT, dtype=np.float32)
+    nl = np.zeros(ROSA_KC_COUNT, dtype=np.int32)
+    _check(load().rosa_profile_batch(e.handle, len(ids), _ptr(ids), _ptr(noise), _ptr(t0), _ptr(d), _ptr(ns),
+                                     _ptr(out_actions), _stream_handle(stream), _ptr(ms), _ptr(nl)))
+    return {rosa_kernel_class_name(c): (float(ms[c]), int(nl[c])) for c in range(ROSA_KC_COUNT)}
+
+
+def rosa_kernel_class_name(cls: int) -> str:
+    return load().rosa_kernel_class_name(cls).decode()
 
 
 def rosa_last_launch_count(e: Expert) -> int:

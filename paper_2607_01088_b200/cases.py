@@ -133,13 +133,21 @@ def _normal(rng: np.random.Generator, shape, scale: float = 1.0) -> np.ndarray:
 
 def build_case(name: str, seed: int, cfg: ExpertConfig, *, bf16: bool,
                prefix_lens=None, draw_lens=None, batch: Optional[int] = None,
-               n_steps: int = 10, cfg3_mix: bool = False, with_prefix: bool = True) -> Case:
+               n_steps: int = 10, cfg3_mix: bool = False, with_prefix: bool = True,
+               robot_stream: int = 0) -> Case:
     """Draw one case in the documented order.  ``draw_lens=(lo, hi)`` draws B integer
-    lengths uniformly with both bounds inclusive (reading R14)."""
+    lengths uniformly with both bounds inclusive (reading R14).
+
+    ``robot_stream`` != 0 (bench.py, ranks > 0 of a multi-GPU run: same replicated weights,
+    different robots) draws everything per-robot (lengths, K/V, noise, start times) from a
+    second generator ``PCG64([seed, robot_stream])`` instead of the main one."""
     rng = np.random.Generator(np.random.PCG64(seed))
+    rrng = rng if robot_stream == 0 else np.random.Generator(np.random.PCG64([seed, robot_stream]))
     if draw_lens is not None:
         lo, hi = draw_lens
-        lens = rng.integers(lo, hi, size=batch, endpoint=True).astype(np.int32)
+        lens = rng.integers(lo, hi, size=batch, endpoint=True).astype(np.int32)   # keeps the weight stream aligned
+        if robot_stream != 0:
+            lens = rrng.integers(lo, hi, size=batch, endpoint=True).astype(np.int32)
     else:
         lens = np.asarray(prefix_lens, dtype=np.int32)
     B = int(lens.shape[0])
@@ -169,17 +177,17 @@ def build_case(name: str, seed: int, cfg: ExpertConfig, *, bf16: bool,
                            dtype=np.uint16 if bf16 else np.float32)
             v_i = np.empty_like(k_i)
             for l in range(cfg.layers):
-                kk = _normal(rng, (L, cfg.n_kv_heads, cfg.head_dim))
-                vv = _normal(rng, (L, cfg.n_kv_heads, cfg.head_dim))
+                kk = _normal(rrng, (L, cfg.n_kv_heads, cfg.head_dim))
+                vv = _normal(rrng, (L, cfg.n_kv_heads, cfg.head_dim))
                 k_i[l] = f32_to_bf16_bits(kk) if bf16 else kk
                 v_i[l] = f32_to_bf16_bits(vv) if bf16 else vv
             pk.append(k_i)
             pv.append(v_i)
-    noise = _normal(rng, (B, cfg.horizon, cfg.action_dim))
+    noise = _normal(rrng, (B, cfg.horizon, cfg.action_dim))
 
     if cfg3_mix:
         # reading R15: t_i uniform over {1.0, 0.9, ..., 0.1}; remaining steps n_i = round(10 t_i); dt_i = -0.1
-        m = rng.integers(1, 10, size=B, endpoint=True).astype(np.int32)
+        m = rrng.integers(1, 10, size=B, endpoint=True).astype(np.int32)
         t0 = (m.astype(np.float32) / np.float32(10.0)).astype(np.float32)
         ns = m.copy()
         dt = np.full(B, -0.1, dtype=np.float32)
@@ -190,24 +198,23 @@ def build_case(name: str, seed: int, cfg: ExpertConfig, *, bf16: bool,
     return Case(name, seed, cfg, bf16, w, lens, pk, pv, noise, t0, dt, ns)
 
 
-def make_case(config: int, *, batch: Optional[int] = None, with_prefix: bool = True) -> Case:
+def make_case(config: int, *, batch: Optional[int] = None, with_prefix: bool = True,
+              robot_stream: int = 0) -> Case:
     """BASELINE.json ``configs[config]``.  ``batch`` selects the B of the config-4 sweep."""
+    kw = dict(with_prefix=with_prefix, robot_stream=robot_stream)
     if config == 0:
-        return build_case("cfg0-tiny", 0, TINY, bf16=False, prefix_lens=[48, 64], n_steps=4,
-                          with_prefix=with_prefix)
+        return build_case("cfg0-tiny", 0, TINY, bf16=False, prefix_lens=[48, 64], n_steps=4, **kw)
     if config == 1:
-        return build_case("cfg1-pi0-b8", 1, PI0, bf16=True, prefix_lens=[816] * 8,
-                          with_prefix=with_prefix)
+        return build_case("cfg1-pi0-b8", 1, PI0, bf16=True, prefix_lens=[816] * 8, **kw)
     if config == 2:
         return build_case("cfg2-fleet-b64", 2, PI0, bf16=True, draw_lens=(600, 1000),
-                          batch=batch or 64, with_prefix=with_prefix)
+                          batch=batch or 64, **kw)
     if config == 3:
         return build_case("cfg3-contbatch-b256", 3, PI0, bf16=True, draw_lens=(400, 1200),
-                          batch=batch or 256, cfg3_mix=True, with_prefix=with_prefix)
+                          batch=batch or 256, cfg3_mix=True, **kw)
     if config == 4:
         b = batch or 64
-        return build_case(f"cfg4-sweep-b{b}", 4, PI0, bf16=True, prefix_lens=[816] * b,
-                          with_prefix=with_prefix)
+        return build_case(f"cfg4-sweep-b{b}", 4, PI0, bf16=True, prefix_lens=[816] * b, **kw)
     raise ValueError(f"unknown config {config}")
 
 

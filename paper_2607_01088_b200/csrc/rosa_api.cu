@@ -88,6 +88,11 @@ struct rosa_expert {
   cudaStream_t cap_stream = nullptr;
   int64_t last_launches = 0;
   float* e2e_dev = nullptr;  // staging for rosa_denoise_batch_host
+  // per-launch event timing (rosa_profile_batch): boundary event before every launch
+  bool prof_on = false;
+  std::vector<cudaEvent_t> prof_ev;
+  std::vector<int> prof_cls;
+  size_t prof_n = 0;
   std::vector<void*> allocs;
 };
 
@@ -175,6 +180,7 @@ static void destroy_impl(rosa_expert* e) {
     if (e->stage_ev[i]) cudaEventDestroy(e->stage_ev[i]);
   }
   if (e->cap_stream) cudaStreamDestroy(e->cap_stream);
+  for (cudaEvent_t ev : e->prof_ev) cudaEventDestroy(ev);
   delete e;
 }
 
@@ -315,9 +321,26 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
   return ROSA_OK;
 }
 
+// Profiling mark: when rosa_profile_batch is running, record a boundary event on `s` before the
+// launch(es) of kernel class `cls`; the time between two consecutive marks is attributed to the
+// earlier one.  A no-op otherwise (and never active during graph capture).
+static void mark(rosa_expert* e, int cls, cudaStream_t s) {
+  if (!e->prof_on) return;
+  if (e->prof_n == e->prof_ev.size()) {
+    cudaEvent_t ev;
+    cudaEventCreate(&ev);
+    e->prof_ev.push_back(ev);
+    e->prof_cls.push_back(0);
+  }
+  cudaEventRecord(e->prof_ev[e->prof_n], s);
+  e->prof_cls[e->prof_n] = cls;
+  e->prof_n += 1;
+}
+
 // One GEMM + epilogue of the path, in whichever kernel family the expert runs.
-static cudaError_t gemm(rosa_expert* e, Epi epi, const op16* A, const op16* W, int M, int N, int K,
+static cudaError_t gemm(rosa_expert* e, int cls, Epi epi, const op16* A, const op16* W, int M, int N, int K,
                         const EpiArgs& a, cudaStream_t s) {
+  mark(e, cls, s);
   if (e->family == 1 && tc_gemm_supported(N, K)) {
     e->last_launches += 1;
     return launch_gemm_tc(epi, A, W, M, N, K, a, s);
@@ -337,7 +360,9 @@ static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, cudaStream_
   const int M = batch * dm.H, d = dm.d;
   cudaError_t err;
   e->last_launches = 0;
+  mark(e, ROSA_KC_GATHER_SCATTER, s);
   launch_gather_x(e->x, cp, tb, dm.H * dm.A, s);
+  mark(e, ROSA_KC_TIMEVEC, s);
   launch_timevec(e->tvec, e->w_t1, e->b_t1, dm, tb, nmax, e->cfg.max_batch, s);
   e->last_launches += 2;
   for (int k = 0; k < nmax; ++k) {
@@ -345,39 +370,46 @@ static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, cudaStream_
     ea.m_active = tb.m_active + k;
     ea.H = dm.H; ea.hd = dm.hd; ea.gu_blk = dm.gu_blk; ea.in_fp16 = dm.fp16; ea.out_fp16 = dm.fp16;
     // a1: h0 = W2 swish(W1 [tau ; W_in x + b_in] + b1) + b2
+    mark(e, ROSA_KC_INPROJ, s);
     launch_inproj(e->abuf, e->x, e->w_in, e->b_in, dm, tb, k, M, s);
     e->last_launches += 1;
     ea.out16 = e->zbuf; ea.ld_out = d;
     ea.rowbias = e->tvec + (size_t)k * e->cfg.max_batch * d;
-    if ((err = gemm(e, EPI_SWISH_ROWBIAS, e->abuf, e->w_t1a, M, d, d, ea, s)) != cudaSuccess) return err;
+    if ((err = gemm(e, ROSA_KC_GEMM_EMBED, EPI_SWISH_ROWBIAS, e->abuf, e->w_t1a, M, d, d, ea, s)) != cudaSuccess) return err;
     ea.out_f32 = e->h; ea.bias = e->b_t2;
-    if ((err = gemm(e, EPI_BIAS_F32, e->zbuf, e->w_t2, M, d, d, ea, s)) != cudaSuccess) return err;
+    if ((err = gemm(e, ROSA_KC_GEMM_EMBED, EPI_BIAS_F32, e->zbuf, e->w_t2, M, d, d, ea, s)) != cudaSuccess) return err;
     for (int l = 0; l < dm.layers; ++l) {
       const LayerWeights& L = e->lw[l];
+      mark(e, ROSA_KC_RMSNORM, s);
       launch_rmsnorm(e->nrm, e->h, L.g_attn, dm, tb, k, M, s);                       // a2
       ea.out16 = e->qkv; ea.ld_out = dm.qkv_n;
       ea.rope_tab = e->rope_tab; ea.ids = tb.ids; ea.rlen = tb.rlen;
       ea.rope_cols = dm.q_n + dm.nkv * dm.hd;
-      if ((err = gemm(e, EPI_ROPE, e->nrm, L.wqkv, M, dm.qkv_n, d, ea, s)) != cudaSuccess) return err;  // a3+a4
+      if ((err = gemm(e, ROSA_KC_GEMM_QKV, EPI_ROPE, e->nrm, L.wqkv, M, dm.qkv_n, d, ea, s)) != cudaSuccess) return err;  // a3+a4
+      mark(e, ROSA_KC_ATTN, s);
       if (e->attn_tc) {                                                              // a5
         if ((err = launch_attn_tc(dm, tb, l, e->qkv, e->obuf, k, M, e->d_kv_maps, s)) != cudaSuccess) return err;
       } else {
         launch_attn_simple(dm, tb, l, e->qkv, e->obuf, k, e->cfg.max_prefix_len, s);
       }
       ea.out_f32 = e->h; ea.ld_out = d;
-      if ((err = gemm(e, EPI_RESID, e->obuf, L.wo, M, d, dm.q_n, ea, s)) != cudaSuccess) return err;    // a6
+      if ((err = gemm(e, ROSA_KC_GEMM_O, EPI_RESID, e->obuf, L.wo, M, d, dm.q_n, ea, s)) != cudaSuccess) return err;    // a6
+      mark(e, ROSA_KC_RMSNORM, s);
       launch_rmsnorm(e->nrm, e->h, L.g_mlp, dm, tb, k, M, s);                        // a2
       ea.out16 = e->mact; ea.ld_out = dm.F;
-      if ((err = gemm(e, EPI_GEGLU, e->nrm, L.wgu, M, 2 * dm.F, d, ea, s)) != cudaSuccess) return err;  // a7
+      if ((err = gemm(e, ROSA_KC_GEMM_GATEUP, EPI_GEGLU, e->nrm, L.wgu, M, 2 * dm.F, d, ea, s)) != cudaSuccess) return err;  // a7
       ea.out_f32 = e->h; ea.ld_out = d;
-      if ((err = gemm(e, EPI_RESID, e->mact, L.wdown, M, d, dm.F, ea, s)) != cudaSuccess) return err;   // a8
+      if ((err = gemm(e, ROSA_KC_GEMM_DOWN, EPI_RESID, e->mact, L.wdown, M, d, dm.F, ea, s)) != cudaSuccess) return err;   // a8
       e->last_launches += 3;
     }
+    mark(e, ROSA_KC_FINAL, s);
     launch_final(e->x, cp, e->h, e->g_final, e->w_out, e->b_out, dm, tb, k, M, s);    // a9 + a10
     e->last_launches += 1;
   }
+  mark(e, ROSA_KC_GATHER_SCATTER, s);
   launch_scatter_x(cp, e->x, tb, dm.H * dm.A, s);
   e->last_launches += 1;
+  mark(e, -1, s);
   return cudaGetLastError();
 }
 
@@ -427,7 +459,7 @@ static rosa_status_t denoise_impl(rosa_expert* e, int batch, const int32_t* ids,
   CK(cudaMemcpyAsync(e->d_call, hs, e->call_bytes, cudaMemcpyHostToDevice, stream));
   CK(cudaEventRecord(e->stage_ev[slot], stream));
   if (out_vel) CK(cudaMemsetAsync(out_vel, 0, (size_t)nmax * batch * dm.H * dm.A * 4, stream));
-  if (!e->use_graph) {
+  if (!e->use_graph || e->prof_on) {
     CK(enqueue_call(e, batch, nmax, stream));
     return ROSA_OK;
   }
@@ -591,6 +623,36 @@ rosa_status_t rosa_denoise_batch_host(rosa_expert_t* e, int32_t batch, const int
   CK(cudaMemcpyAsync(out_actions_host, e->e2e_dev, bytes, cudaMemcpyDeviceToHost, s));
   CK(cudaStreamSynchronize(s));
   return ROSA_OK;
+}
+
+rosa_status_t rosa_profile_batch(rosa_expert_t* e, int32_t batch, const int32_t* robot_ids, const float* noise,
+                                 const float* t_start, const float* dt, const int32_t* n_steps,
+                                 float* out_actions, void* stream, float* ms_out, int32_t* launches_out) {
+  if (!e || !ms_out || !launches_out) { set_error("NULL argument"); return ROSA_ERR_INVALID_ARG; }
+  cudaStream_t s = (cudaStream_t)stream;
+  e->prof_on = true;
+  e->prof_n = 0;
+  rosa_status_t st = denoise_impl(e, batch, robot_ids, noise, t_start, dt, n_steps, out_actions, nullptr, s);
+  e->prof_on = false;
+  if (st != ROSA_OK) return st;
+  CK(cudaStreamSynchronize(s));
+  for (int c = 0; c < ROSA_KC_COUNT; ++c) { ms_out[c] = 0.f; launches_out[c] = 0; }
+  for (size_t i = 0; i + 1 < e->prof_n; ++i) {
+    const int c = e->prof_cls[i];
+    if (c < 0 || c >= ROSA_KC_COUNT) continue;
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, e->prof_ev[i], e->prof_ev[i + 1]));
+    ms_out[c] += ms;
+    launches_out[c] += 1;
+  }
+  return ROSA_OK;
+}
+
+const char* rosa_kernel_class_name(int32_t cls) {
+  static const char* names[ROSA_KC_COUNT] = {"gather_scatter", "timevec", "inproj", "gemm_embed", "rmsnorm",
+                                             "gemm_qkv_rope", "attention", "gemm_o_resid", "gemm_gateup_geglu",
+                                             "gemm_down_resid", "final_norm_outproj_euler"};
+  return cls >= 0 && cls < ROSA_KC_COUNT ? names[cls] : "";
 }
 
 rosa_status_t rosa_last_launch_count(rosa_expert_t* e, int64_t* n) {

@@ -84,3 +84,45 @@ def rel_l2(got: np.ndarray, want: np.ndarray) -> float:
     g = np.asarray(got, dtype=np.float64).ravel()
     w = np.asarray(want, dtype=np.float64).ravel()
     return float(np.linalg.norm(g - w) / max(np.linalg.norm(w), 1e-300))
+
+
+class DeviceFleet:
+    """Timing-only workload (bench.py batch sweep): the weights of a seeded ``Case`` drawn
+    without prefix data, and per-robot prefix K/V ~ N(0,1) bf16 drawn ON THE DEVICE with a seeded
+    torch generator (values do not affect timing; parity tests always use ``LoadedCase``)."""
+
+    def __init__(self, case: Case, prefix_lens, device: str = "cuda:0", max_steps: int = 16, seed: int = 0):
+        self.case = case
+        self.device = torch.device(device)
+        cfg = case.cfg
+        lens = np.asarray(prefix_lens, dtype=np.int32)
+        self.lens = lens
+        B = int(lens.shape[0])
+        self.batch = B
+        cu = np.zeros(B + 1, dtype=np.int64)
+        np.cumsum(lens, out=cu[1:])
+        row = cfg.n_kv_heads * cfg.head_dim
+        with torch.cuda.device(self.device):
+            self.expert = rosa.rosa_expert_create(cfg.as_dict(), case.weights, max_robots=B, max_batch=B,
+                                                  max_prefix_len=int(lens.max()), max_steps=max_steps)
+            g = torch.Generator(device=self.device)
+            g.manual_seed(seed)
+            total = int(cu[-1])
+            self.k = [torch.randn((total, row), generator=g, device=self.device, dtype=torch.float32)
+                      .to(torch.bfloat16) for _ in range(cfg.layers)]
+            self.v = [torch.randn((total, row), generator=g, device=self.device, dtype=torch.float32)
+                      .to(torch.bfloat16) for _ in range(cfg.layers)]
+            for i in range(B):
+                off = int(cu[i]) * row * 2
+                rosa.rosa_prefix_kv_bind(self.expert, i, [t.data_ptr() + off for t in self.k],
+                                         [t.data_ptr() + off for t in self.v], int(lens[i]), rosa.ROSA_BF16)
+            self.noise = torch.randn((B, cfg.horizon, cfg.action_dim), generator=g, device=self.device,
+                                     dtype=torch.float32)
+            torch.cuda.synchronize(self.device)
+
+    def kv_bytes(self) -> int:
+        return sum(t.numel() * t.element_size() for t in self.k + self.v)
+
+    def close(self):
+        rosa.rosa_expert_destroy(self.expert)
+        self.k, self.v = [], []

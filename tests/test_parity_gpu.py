@@ -1,6 +1,12 @@
 """GPU parity: rosa_denoise_batch* (through the C ABI) against the CPU oracle, element by
 element on the same seeded inputs.  Tolerances are BASELINE.json north_star (3):
-final actions max-abs <= 2e-2 and rel-L2 <= 1e-2; per-step velocity rel-L2 <= 5e-3."""
+final actions max-abs <= 2e-2 and rel-L2 <= 1e-2; per-step velocity rel-L2 <= 5e-3
+(rel-L2 over the whole compared tensor, per Euler step for the velocity; reading R18).
+
+Full-size cases (cfg2 B=64, cfg3 B=256, sweep B up to 512) run the WHOLE batch on the GPU in
+the launch configuration bench.py times and compare a sample of robots with the oracle: robots
+are independent units (pin P2), so the oracle's single-robot result is the exact expectation
+for that robot's rows of the batched call."""
 import numpy as np
 import pytest
 import torch
@@ -9,11 +15,16 @@ from oracle import rosa_oracle as O
 from paper_2607_01088_b200 import binding as rosa
 from paper_2607_01088_b200 import build as rosa_build
 from paper_2607_01088_b200 import cases
-from paper_2607_01088_b200.runner import LoadedCase, rel_l2
+from paper_2607_01088_b200.runner import DeviceFleet, LoadedCase, rel_l2
 
 pytestmark = pytest.mark.gpu
 
 TOL_ACT_ABS, TOL_ACT_REL, TOL_VEL_REL = 2e-2, 1e-2, 5e-3
+
+# pi0 head geometry (8 q heads / 1 kv head / head_dim 256, H=50, A=32: the tcgen05 kernels) on a
+# narrow 2-layer model, so the oracle finishes edge-case batches in seconds
+MINI = cases.ExpertConfig(layers=2, d_model=256, n_q_heads=8, n_kv_heads=1, head_dim=256,
+                          ffn=512, horizon=50, action_dim=32)
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -22,24 +33,30 @@ def _built():
     rosa.load()
 
 
-def check_against_oracle(case, lc, robots, label):
-    """Run the listed robots as ONE batch on the GPU; oracle on the same robots."""
-    got_x, got_v = lc.run(robots=robots, want_velocity=True)
-    want_x, want_v = O.denoise_case(case, robots=robots, return_velocity=True)
+def compare(label, got_x, got_v, want_x, want_v):
     assert np.all(np.isfinite(got_x)), label
     err_abs = float(np.abs(got_x - want_x).max())
     err_rel = rel_l2(got_x, want_x)
-    vel_rel = [rel_l2(got_v[k], want_v[k]) for k in range(len(want_v))]
+    vel_rel = [rel_l2(got_v[k], want_v[k]) for k in range(len(want_v)) if np.any(want_v[k])]
     print(f"[{label}] actions max-abs {err_abs:.3e} rel-L2 {err_rel:.3e}; velocity rel-L2 max {max(vel_rel):.3e}")
     assert err_abs <= TOL_ACT_ABS, (label, err_abs)
     assert err_rel <= TOL_ACT_REL, (label, err_rel)
     assert max(vel_rel) <= TOL_VEL_REL, (label, vel_rel)
-    return got_x
+
+
+def check_against_oracle(case, lc, robots, label, sample=None):
+    """Run `robots` as ONE batch on the GPU; oracle on `sample` (positions in `robots`, default all)."""
+    got_x, got_v = lc.run(robots=robots, want_velocity=True)
+    pos = list(range(len(robots))) if sample is None else list(sample)
+    want_x, want_v = O.denoise_case(case, robots=[robots[p] for p in pos], return_velocity=True)
+    compare(label, got_x[pos], [v[pos] for v in got_v[:len(want_v)]], want_x, want_v)
+    return got_x, got_v
 
 
 def test_cfg0_tiny_fp32():
     case = cases.make_case(0)
     lc = LoadedCase(case)
+    assert rosa.rosa_kernel_family(lc.expert) == 0      # d=128 / head_dim 32: the shape-generic family
     check_against_oracle(case, lc, [0, 1], "cfg0")
     lc.close()
 
@@ -47,5 +64,234 @@ def test_cfg0_tiny_fp32():
 def test_cfg1_pi0_b8():
     case = cases.make_case(1)
     lc = LoadedCase(case)
+    assert rosa.rosa_kernel_family(lc.expert) == 1
     check_against_oracle(case, lc, list(range(8)), "cfg1")
     lc.close()
+
+
+def test_cfg2_fleet_b64_ragged_sampled():
+    case = cases.make_case(2)
+    assert case.batch == 64 and case.prefix_lens.min() >= 600 and case.prefix_lens.max() <= 1000
+    lc = LoadedCase(case)
+    # robot 2 (rows 100..149) and robot 5 (rows 250..299) straddle 128-row GEMM tile boundaries
+    check_against_oracle(case, lc, list(range(64)), "cfg2", sample=[0, 2, 5, 33, 63])
+    lc.close()
+
+
+def test_cfg3_continuous_batching_b256_sampled():
+    case = cases.make_case(3)
+    assert case.batch == 256
+    ns = case.n_steps
+    # one robot per remaining-step count that occurs, plus the first and last robots
+    sample = sorted({int(np.nonzero(ns == n)[0][0]) for n in np.unique(ns)} | {0, 255})
+    lc = LoadedCase(case)
+    got_x, got_v = check_against_oracle(case, lc, list(range(256)), "cfg3", sample=sample)
+    # R16: velocity rows of a robot are zero once it is inactive
+    for k in range(got_v.shape[0]):
+        inactive = ns <= k
+        assert not np.any(got_v[k][inactive])
+    lc.close()
+
+
+def test_cfg3_parity_variant_per_robot_dt():
+    """R15 parity-only variant: n_i drawn independently of t_i, so dt_i truly differs per robot."""
+    case = cases.build_case("cfg3-variant", 33, MINI, bf16=True, draw_lens=(40, 200), batch=12)
+    rng = np.random.default_rng(5)
+    case.n_steps = rng.integers(1, 7, size=12).astype(np.int32)
+    case.t_start = (rng.integers(1, 11, size=12) / 10.0).astype(np.float32)
+    case.dt = (-case.t_start / case.n_steps).astype(np.float32)
+    lc = LoadedCase(case)
+    check_against_oracle(case, lc, list(range(12)), "cfg3-variant")
+    lc.close()
+
+
+@pytest.mark.parametrize("B,sample", [(1, [0]), (3, [0, 2]), (128, [0, 127])])
+def test_cfg4_sweep_points(B, sample):
+    case = cases.make_case(4, batch=B)
+    lc = LoadedCase(case)
+    check_against_oracle(case, lc, list(range(B)), f"cfg4-B{B}", sample=sample)
+    lc.close()
+
+
+def test_cfg4_max_batch_512_property_and_sample():
+    """B=512 (largest sweep point): batch invariance on the GPU for three robots, and one robot
+    against the oracle (its prefix K/V is copied back from the seeded device generator)."""
+    base = cases.make_case(4, batch=1, with_prefix=False)
+    fl = DeviceFleet(base, [816] * 512, seed=4)
+    B, cfg = 512, base.cfg
+    ids = np.arange(B, dtype=np.int32)
+    t0 = np.ones(B, dtype=np.float32)
+    ns = np.full(B, 10, dtype=np.int32)
+    dt = (-t0 / 10).astype(np.float32)
+    out = torch.empty_like(fl.noise)
+    rosa.rosa_denoise_batch_ex(fl.expert, ids, fl.noise, t0, dt, ns, out, None, None)
+    torch.cuda.synchronize()
+    big = out.cpu().numpy()
+    pick = np.array([0, 255, 511], dtype=np.int32)
+    small_out = torch.empty((3,) + tuple(fl.noise.shape[1:]), dtype=torch.float32, device=fl.noise.device)
+    vel = torch.empty((10, 3) + tuple(fl.noise.shape[1:]), dtype=torch.float32, device=fl.noise.device)
+    rosa.rosa_denoise_batch_ex(fl.expert, pick, fl.noise[pick.tolist()].contiguous(), t0[:3], dt[:3], ns[:3],
+                               small_out, vel, None)
+    torch.cuda.synchronize()
+    small = small_out.cpu().numpy()
+    assert np.abs(big[pick] - small).max() <= 1e-3      # same kernels, different tile positions
+    # robot 511 against the oracle
+    row = cfg.n_kv_heads * cfg.head_dim
+    sl = slice(511 * 816, 512 * 816)
+    pk = np.stack([t[sl].float().cpu().numpy().reshape(816, cfg.n_kv_heads, cfg.head_dim) for t in fl.k])
+    pv = np.stack([t[sl].float().cpu().numpy().reshape(816, cfg.n_kv_heads, cfg.head_dim) for t in fl.v])
+    want_x, want_v = O.denoise_batch(cfg, base.weights, [pk], [pv], fl.noise[511:512].cpu().numpy(), t0[:1], dt[:1],
+                                     ns[:1], return_velocity=True)
+    compare("cfg4-B512-robot511", big[511:512], [vel[k, 2:3].cpu().numpy() for k in range(10)], want_x, want_v)
+    assert row == 256
+    fl.close()
+
+
+def edge_case(lens, seed=21, n_steps=3):
+    return cases.build_case("edge", seed, MINI, bf16=True, prefix_lens=list(lens), n_steps=n_steps)
+
+
+def test_edge_prefix_lengths():
+    """L = 0 (self-attention only, R8), 1, and lengths around the 64-key block boundary."""
+    case = edge_case([0, 1, 63, 64, 65, 127, 128, 129, 200])
+    lc = LoadedCase(case)
+    check_against_oracle(case, lc, list(range(case.batch)), "edge-lens")
+    lc.close()
+
+
+def test_edge_single_step_and_single_robot():
+    case = edge_case([100], n_steps=1)
+    lc = LoadedCase(case)
+    check_against_oracle(case, lc, [0], "edge-1x1")
+    lc.close()
+
+
+def test_p2_batch_invariance_p3_permutation_and_aliasing():
+    case = edge_case([70, 150, 33, 90, 64])
+    lc = LoadedCase(case)
+    full, _ = lc.run()
+    want, _ = O.denoise_case(case)
+    perm = [3, 0, 4, 2, 1]
+    got_perm, _ = lc.run(robots=perm)
+    assert np.abs(got_perm - full[perm]).max() <= 1e-3           # P3
+    solo, _ = lc.run(robots=[2])
+    assert np.abs(solo[0] - full[2]).max() <= 1e-3               # P2
+    assert rel_l2(got_perm, want[perm]) <= TOL_ACT_REL
+    # noise and out_actions may alias (rosa.h)
+    buf = torch.from_numpy(case.noise.copy()).cuda()
+    rosa.rosa_denoise_batch(lc.expert, np.arange(5, dtype=np.int32), buf, case.t_start, case.n_steps, buf)
+    torch.cuda.synchronize()
+    assert np.array_equal(buf.cpu().numpy(), full)               # P13 as well: bitwise equal to the first run
+    lc.close()
+
+
+def test_p13_determinism_bitwise():
+    case = edge_case([300, 10, 77])
+    lc = LoadedCase(case)
+    a, va = lc.run(want_velocity=True)
+    b, vb = lc.run(want_velocity=True)
+    assert np.array_equal(a, b) and np.array_equal(va, vb)
+    lc.close()
+
+
+def test_p12_softmax_stress_online_rescaling():
+    """Peaked softmax: three prefix keys per robot are scaled so that their logits have standard
+    deviation ~10, ~16 and ~26 (the N(0,1) bulk has ~0.64), placed in increasing order along the
+    key stream, so for many query rows the running maximum grows by more than 2^8 between key
+    blocks and the lazy O-rescale path of the attention kernel runs."""
+    case = edge_case([190, 260], seed=23, n_steps=2)
+    for i in range(case.batch):
+        k = cases.bf16_bits_to_f32(case.prefix_k[i]).copy()
+        L = k.shape[1]
+        for j, s in ((70, 15.0), (L // 2 + 40, 25.0), (L - 3, 40.0)):
+            k[:, j] *= s
+        case.prefix_k[i] = cases.f32_to_bf16_bits(k)
+    lc = LoadedCase(case)
+    check_against_oracle(case, lc, [0, 1], "p12-softmax-stress")
+    lc.close()
+
+
+def test_p4_zero_output_projection_and_p5_constant_velocity():
+    case = edge_case([50, 90])
+    case.weights["w_out"] = np.zeros_like(case.weights["w_out"])
+    case.weights["b_out"] = np.zeros_like(case.weights["b_out"])
+    lc = LoadedCase(case)
+    x, _ = lc.run()
+    assert np.array_equal(x, case.noise)                          # P4: exactly unchanged
+    lc.close()
+    c = cases.round_bf16(np.linspace(-1, 1, MINI.action_dim).astype(np.float32))
+    case.weights["b_out"] = c
+    case.t_start = np.array([1.0, 0.5], dtype=np.float32)
+    case.n_steps = np.array([4, 3], dtype=np.int32)
+    case.dt = (-case.t_start / case.n_steps).astype(np.float32)
+    lc = LoadedCase(case)
+    x, _ = lc.run()
+    want = case.noise - case.t_start[:, None, None] * c[None, None, :]   # x0 + n dt c = x0 - t0 c
+    assert np.abs(x - want).max() <= 1e-5
+    lc.close()
+
+
+def test_p6_step_composition_via_ex():
+    case = edge_case([120, 60], n_steps=10)
+    lc = LoadedCase(case)
+    full, _ = lc.run()
+    ids = np.arange(2, dtype=np.int32)
+    x = torch.from_numpy(case.noise).cuda()
+    dt = np.full(2, -0.1, dtype=np.float32)
+    rosa.rosa_denoise_batch_ex(lc.expert, ids, x, np.full(2, 1.0, np.float32), dt, np.full(2, 4, np.int32), x)
+    rosa.rosa_denoise_batch_ex(lc.expert, ids, x, np.full(2, 0.6, np.float32), dt, np.full(2, 6, np.int32), x)
+    torch.cuda.synchronize()
+    assert np.abs(x.cpu().numpy() - full).max() <= 1e-4
+    lc.close()
+
+
+def test_rebind_unbind_and_error_codes():
+    case = edge_case([40, 80, 120])
+    lc = LoadedCase(case)
+    e = lc.expert
+    noise = torch.from_numpy(case.noise).cuda()
+    out = torch.empty_like(noise)
+    ns = case.n_steps
+
+    def status(fn):
+        with pytest.raises(rosa.RosaError) as ei:
+            fn()
+        return ei.value.status
+
+    assert status(lambda: rosa.rosa_denoise_batch(e, [0, 0, 1], noise, None, ns, out)) == rosa.ROSA_ERR_INVALID_ARG
+    assert status(lambda: rosa.rosa_denoise_batch(e, [0, 1, 7], noise, None, ns, out)) == rosa.ROSA_ERR_INVALID_ARG
+    assert status(lambda: rosa.rosa_denoise_batch(e, [0, 1, 2], noise, None, [1, 0, 1], out)) == rosa.ROSA_ERR_INVALID_ARG
+    assert status(lambda: rosa.rosa_denoise_batch(e, [0, 1, 2], noise, None, [1, 99, 1], out)) == rosa.ROSA_ERR_CAPACITY
+    rosa.rosa_prefix_kv_unbind(e, 1)
+    assert status(lambda: rosa.rosa_denoise_batch(e, [0, 1, 2], noise, None, ns, out)) == rosa.ROSA_ERR_UNBOUND_ROBOT
+    k0 = [t for t in lc.kv_buffers[:MINI.layers]]
+    assert status(lambda: rosa.rosa_prefix_kv_bind(e, 1, k0, k0, 10 ** 6)) == rosa.ROSA_ERR_CAPACITY
+    # re-bind robot 1 to robot 0's prefix: its output must now equal robot 0's given the same noise
+    row = MINI.n_kv_heads * MINI.head_dim
+    kl, vl = lc.kv_buffers[:MINI.layers], lc.kv_buffers[MINI.layers:]
+    rosa.rosa_prefix_kv_bind(e, 1, [t.data_ptr() for t in kl], [t.data_ptr() for t in vl], 40)
+    n2 = torch.from_numpy(np.stack([case.noise[0], case.noise[0]])).cuda()
+    o2 = torch.empty_like(n2)
+    rosa.rosa_denoise_batch(e, [0, 1], n2, None, ns[:2], o2)
+    torch.cuda.synchronize()
+    o2 = o2.cpu().numpy()
+    assert np.abs(o2[0] - o2[1]).max() <= 1e-3
+    assert row == 256
+    lc.close()
+
+
+@pytest.mark.parametrize("M,N,K", [(1, 64, 64), (127, 128, 192), (129, 256, 1024), (400, 2560, 1024),
+                                   (3200, 1024, 4096), (333, 8192, 1024), (3200, 1024, 2048)])
+def test_tcgen05_gemm_unit(M, N, K):
+    """C = A W^T through the tcgen05/TMA kernel against numpy fp64 on the same bf16 operand values."""
+    rng = np.random.default_rng(M * 7 + N + K)
+    a = cases.round_bf16(rng.standard_normal((M, K), dtype=np.float32))
+    w = cases.round_bf16(rng.standard_normal((N, K), dtype=np.float32) * 0.05)
+    A = torch.from_numpy(cases.f32_to_bf16_bits(a).view(np.int16)).cuda()
+    W = torch.from_numpy(cases.f32_to_bf16_bits(w).view(np.int16)).cuda()
+    C = torch.zeros((M, N), dtype=torch.float32, device="cuda")
+    rosa.rosa_debug_gemm(1, M, N, K, A, W, C)
+    torch.cuda.synchronize()
+    want = a.astype(np.float64) @ w.astype(np.float64).T
+    got = C.cpu().numpy()
+    assert np.abs(got - want).max() <= 2e-5 * K ** 0.5 * 4 + 1e-6, np.abs(got - want).max()
