@@ -33,12 +33,12 @@ __device__ __forceinline__ uint32_t pack_op2(float lo, float hi, int fp16) {
   return *reinterpret_cast<uint32_t*>(&v);
 }
 // swish(z) = z / (1 + e^-z)
-__device__ __forceinline__ float swish_f(float z) { return z / (1.f + __expf(-z)); }
+__device__ __forceinline__ float swish_f(float z) { return __fdividef(z, 1.f + __expf(-z)); }
 // GELU, tanh form (R6): 0.5 z (1 + tanh(sqrt(2/pi) (z + 0.044715 z^3)))
 // tanh(u) = 1 - 2/(1 + e^{2u}) keeps full fp32 accuracy for the range that matters.
 __device__ __forceinline__ float gelu_tanh_f(float z) {
   const float u = 0.7978845608028654f * fmaf(0.044715f * z * z, z, z);
-  const float t = 1.f - 2.f / (1.f + __expf(2.f * u));
+  const float t = 1.f - __fdividef(2.f, 1.f + __expf(2.f * u));
   return 0.5f * z * (1.f + t);
 }
 

@@ -25,6 +25,7 @@ using namespace tc;
 
 constexpr int BM = 128, BK = 64;
 constexpr int kGemmThreads = 192;
+constexpr int kScrFloats = 32 * 66;  // per epilogue warp: 32 rows x up to 64 columns, padded
 
 template <int BN>
 struct GemmCfg {
@@ -32,7 +33,7 @@ struct GemmCfg {
   static constexpr int A_BYTES = BM * BK * 2;
   static constexpr int B_BYTES = BN * BK * 2;
   static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
-  static constexpr int SMEM = STAGES * STAGE_BYTES + 1024 /*align slack*/ + 256 /*barriers*/;
+  static constexpr int SMEM = STAGES * STAGE_BYTES + 1024 /*align slack*/ + 256 /*barriers*/ + 4 * kScrFloats * 4;
   static constexpr int TMEM_COLS = 2 * BN < 32 ? 32 : 2 * BN;
 };
 
@@ -55,6 +56,16 @@ __device__ __forceinline__ void ld_acc32(uint32_t taddr, float (&v)[32]) {
   tmem_ld_wait();
 #pragma unroll
   for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
+}
+
+// Fused RMSNorm (a2, R5): the A operand was the un-normalised residual h (16-bit copy) and the gain
+// is folded into W, so the accumulator row only needs the scale r = rsqrt(mean(h^2) + eps); the
+// producing GEMM left n_part partial sums of squares per row, added here in a fixed order.
+__device__ __forceinline__ float row_rscale(const EpiArgs& ea, int row) {
+  if (!ea.ssq_in) return 1.f;
+  float ss = 0.f;
+  for (int i = 0; i < ea.n_part; ++i) ss += ea.ssq_in[(size_t)row * ea.n_part + i];
+  return rsqrtf(ss * ea.inv_d + ea.eps);
 }
 
 template <int BN, int EPI>
@@ -133,10 +144,12 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
           tc_fence_after();
           const uint32_t a_addr = smem_base + s * Cfg::STAGE_BYTES;
           const uint32_t b_addr = a_addr + Cfg::A_BYTES;
+          if (!(ea.dbg & 2)) {
 #pragma unroll
-          for (int kk = 0; kk < BK / 16; ++kk) {
-            umma_bf16(d_tmem, make_sdesc_k128(a_addr + kk * 32), make_sdesc_k128(b_addr + kk * 32), idesc,
-                      (kb | kk) != 0);
+            for (int kk = 0; kk < BK / 16; ++kk) {
+              umma_bf16(d_tmem, make_sdesc_k128(a_addr + kk * 32), make_sdesc_k128(b_addr + kk * 32), idesc,
+                        (kb | kk) != 0);
+            }
           }
           umma_commit(empty_bar(s));
           if (++s == Cfg::STAGES) { s = 0; ph ^= 1; }
@@ -145,107 +158,182 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
       }
     }
   } else {  // ---------------- epilogue warps 2..5
+    // TMEM -> registers is thread = row (tcgen05.ld 32x32b); global memory wants lane = column.
+    // Each warp transposes through a private padded scratch in shared memory, so every global
+    // load/store below is one coalesced 64..512-byte row segment per instruction.
     const int q = warp & 3;  // TMEM lane quarter this warp may access
+    float* scr = reinterpret_cast<float*>(smem_raw + (bar_base + 256u - smem_u32(smem_raw))) + q * kScrFloats;
     int it = 0;
     for (int t = blockIdx.x; t < n_tiles; t += gridDim.x, ++it) {
       const int acc = it & 1;
       const uint32_t acc_ph = (it >> 1) & 1;
       const int m0 = (t % n_m) * BM, n0 = (t / n_m) * BN;
-      const int row = m0 + q * 32 + lane;
+      const int r0 = m0 + q * 32;            // first row of this warp
+      const int row = r0 + lane;             // row of this thread in the thread = row domain
       const bool ok = row < m_lim;
       mbar_wait(tfull_bar(acc), acc_ph);
       tc_fence_after();
       const uint32_t t_acc = tmem_base + ((uint32_t)(q * 32) << 16) + acc * BN;
+      if (ea.dbg & 1) {  // measurement aid: mainloop only
+        tc_fence_before();
+        mbar_arrive(tempty_bar(acc));
+        continue;
+      }
 
       if constexpr (EPI == EPI_STORE_F32 || EPI == EPI_BIAS_F32 || EPI == EPI_RESID) {
+        // h (fp32) = acc [+ h] [+ bias]; optionally also the 16-bit copy of the new h (A operand of
+        // the next GEMM) and this tile's partial sum of squares of each row (fused RMSNorm, a2)
+        float rowss[32];
+#pragma unroll
+        for (int rr = 0; rr < 32; ++rr) rowss[rr] = 0.f;
 #pragma unroll 1
         for (int c = 0; c < BN / 32; ++c) {
           float v[32];
           ld_acc32(t_acc + c * 32, v);
-          if (ok) {
-            float4* dst = reinterpret_cast<float4*>(ea.out_f32 + (size_t)row * ea.ld_out + n0 + c * 32);
+          if (c == BN / 32 - 1) {  // accumulator fully read: hand it back to the MMA warp
+            tc_fence_before();
+            mbar_arrive(tempty_bar(acc));
+          }
 #pragma unroll
-            for (int i = 0; i < 8; ++i) {
-              float4 o = make_float4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]);
-              if constexpr (EPI == EPI_RESID) {
-                const float4 h = dst[i];
-                o.x += h.x; o.y += h.y; o.z += h.z; o.w += h.w;
+          for (int i = 0; i < 32; ++i) scr[lane * 33 + i] = v[i];
+          __syncwarp();
+          const int col = n0 + c * 32 + lane;
+          float add = 0.f;
+          if constexpr (EPI == EPI_BIAS_F32) add = ea.bias[col];
+          float hold[32];
+          if constexpr (EPI == EPI_RESID) {
+#pragma unroll
+            for (int rr = 0; rr < 32; ++rr)
+              hold[rr] = (r0 + rr < m_lim) ? ea.out_f32[(size_t)(r0 + rr) * ea.ld_out + col] : 0.f;
+          }
+          // all shared-memory reads first: the compiler must assume scr aliases the global
+          // pointers, so a load placed after a store would wait for it
+          float o[32];
+#pragma unroll
+          for (int rr = 0; rr < 32; ++rr) o[rr] = scr[rr * 33 + lane] + add;
+#pragma unroll
+          for (int rr = 0; rr < 32; ++rr) {
+            if constexpr (EPI == EPI_RESID) o[rr] += hold[rr];
+            if (r0 + rr < m_lim) {
+              const size_t idx = (size_t)(r0 + rr) * ea.ld_out + col;
+              ea.out_f32[idx] = o[rr];
+              if constexpr (EPI != EPI_STORE_F32) {
+                if (ea.h16) ((uint16_t*)ea.h16)[idx] = f2op(o[rr], ea.out_fp16);
+                rowss[rr] = fmaf(o[rr], o[rr], rowss[rr]);
               }
-              if constexpr (EPI == EPI_BIAS_F32) {
-                const float4 b = *reinterpret_cast<const float4*>(ea.bias + n0 + c * 32 + 4 * i);
-                o.x += b.x; o.y += b.y; o.z += b.z; o.w += b.w;
-              }
-              dst[i] = o;
             }
           }
+          __syncwarp();
         }
-      } else if constexpr (EPI == EPI_SWISH_ROWBIAS) {
-        const float* rb = ea.rowbias + (size_t)((ok ? row : 0) / ea.H) * N + n0;
-#pragma unroll 1
-        for (int c = 0; c < BN / 32; ++c) {
-          float v[32];
-          ld_acc32(t_acc + c * 32, v);
-          if (ok) {
+        if constexpr (EPI != EPI_STORE_F32) {
+          if (ea.ssq_out) {
+            float mine = 0.f;
 #pragma unroll
-            for (int i = 0; i < 8; ++i) {
-              const float4 b = *reinterpret_cast<const float4*>(rb + c * 32 + 4 * i);
-              v[4 * i] = swish_f(v[4 * i] + b.x);
-              v[4 * i + 1] = swish_f(v[4 * i + 1] + b.y);
-              v[4 * i + 2] = swish_f(v[4 * i + 2] + b.z);
-              v[4 * i + 3] = swish_f(v[4 * i + 3] + b.w);
+            for (int rr = 0; rr < 32; ++rr) {
+              const float tot = warp_sum(rowss[rr]);
+              if (rr == lane) mine = tot;
             }
-            store_op16x32((uint16_t*)ea.out16 + (size_t)row * ea.ld_out + n0 + c * 32, v, ea.out_fp16);
+            if (ok) ea.ssq_out[(size_t)row * (N / BN) + n0 / BN] = mine;
           }
         }
       } else if constexpr (EPI == EPI_ROPE) {
         // BN == head_dim: the tile is exactly one head; pairs (c, c + hd/2) are both in TMEM.
         static_assert(EPI != EPI_ROPE || BN == 256, "RoPE epilogue assumes BN == head_dim == 256");
         const bool rot = n0 < ea.rope_cols;
-        int pos = 0;
+        const float rs = row_rscale(ea, ok ? row : 0);
+        int posr = 0;
         if (ok && rot) {
           const int p = row / ea.H;
-          pos = ea.rlen[ea.ids[p]] + (row - p * ea.H);
+          posr = ea.rlen[ea.ids[p]] + (row - p * ea.H);
         }
-        const float2* tab = ea.rope_tab + (size_t)pos * (BN / 2);
+        uint16_t* outp = (uint16_t*)ea.out16;
 #pragma unroll 1
-        for (int c = 0; c < BN / 64; ++c) {
-          float lo[32], hi[32];
-          ld_acc32(t_acc + c * 32, lo);
-          ld_acc32(t_acc + BN / 2 + c * 32, hi);
-          if (ok) {
-            if (rot) {
+        for (int c = 0; c < 2; ++c) {  // 64 low columns [64c, 64c+64) with their partners +128
+          float v[32];
+          float2 lo[32];
 #pragma unroll
-              for (int i = 0; i < 32; ++i) {
-                const float2 cs = tab[c * 32 + i];
-                const float a = lo[i], b = hi[i];
-                lo[i] = a * cs.x - b * cs.y;
-                hi[i] = b * cs.x + a * cs.y;
+          for (int hh = 0; hh < 2; ++hh) {
+            ld_acc32(t_acc + c * 64 + hh * 32, v);
+#pragma unroll
+            for (int i = 0; i < 32; i += 2)
+              *reinterpret_cast<float2*>(&scr[lane * 66 + hh * 32 + i]) = make_float2(v[i] * rs, v[i + 1] * rs);
+          }
+          __syncwarp();
+#pragma unroll
+          for (int rr = 0; rr < 32; ++rr) lo[rr] = *reinterpret_cast<const float2*>(&scr[rr * 66 + 2 * lane]);
+          __syncwarp();
+#pragma unroll
+          for (int hh = 0; hh < 2; ++hh) {
+            ld_acc32(t_acc + BN / 2 + c * 64 + hh * 32, v);
+#pragma unroll
+            for (int i = 0; i < 32; i += 2)
+              *reinterpret_cast<float2*>(&scr[lane * 66 + hh * 32 + i]) = make_float2(v[i] * rs, v[i + 1] * rs);
+          }
+          if (c == 1) {
+            tc_fence_before();
+            mbar_arrive(tempty_bar(acc));
+          }
+          __syncwarp();
+#pragma unroll
+          for (int half = 0; half < 2; ++half) {  // 16 rows at a time: loads, then math, then stores
+            float2 hi[16];
+            float4 cs[16];
+#pragma unroll
+            for (int r2 = 0; r2 < 16; ++r2) {
+              const int rr = half * 16 + r2;
+              hi[r2] = *reinterpret_cast<const float2*>(&scr[rr * 66 + 2 * lane]);
+              const int pos = __shfl_sync(0xffffffffu, posr, rr);
+              cs[r2] = rot ? *reinterpret_cast<const float4*>(ea.rope_tab + (size_t)pos * (BN / 2) + c * 64 + 2 * lane)
+                           : make_float4(1.f, 0.f, 1.f, 0.f);
+            }
+#pragma unroll
+            for (int r2 = 0; r2 < 16; ++r2) {
+              const int rr = half * 16 + r2;
+              const float a0 = lo[rr].x, b0 = hi[r2].x, a1 = lo[rr].y, b1 = hi[r2].y;
+              const float ax = a0 * cs[r2].x - b0 * cs[r2].y, bx = b0 * cs[r2].x + a0 * cs[r2].y;
+              const float ay = a1 * cs[r2].z - b1 * cs[r2].w, by = b1 * cs[r2].z + a1 * cs[r2].w;
+              if (r0 + rr < m_lim) {
+                uint16_t* dst = outp + (size_t)(r0 + rr) * ea.ld_out + n0 + c * 64 + 2 * lane;
+                *reinterpret_cast<uint32_t*>(dst) = pack_op2(ax, ay, 0);  // q/k/v feed attention: always bf16
+                *reinterpret_cast<uint32_t*>(dst + BN / 2) = pack_op2(bx, by, 0);
               }
             }
-            uint16_t* dst = (uint16_t*)ea.out16 + (size_t)row * ea.ld_out + n0 + c * 32;
-            store_op16x32(dst, lo, 0);  // q/k/v feed the attention kernel: always bf16
-            store_op16x32(dst + BN / 2, hi, 0);
           }
+          __syncwarp();
         }
       } else if constexpr (EPI == EPI_GEGLU) {
         // packed columns: [gate 64 | up 64] blocks (gu_blk = 64); output column = n/2 region
+        const float rs = row_rscale(ea, ok ? row : 0);
+        uint16_t* outp = (uint16_t*)ea.out16;
 #pragma unroll 1
         for (int blk = 0; blk < BN / 128; ++blk) {
-#pragma unroll 1
-          for (int c = 0; c < 2; ++c) {
-            float g[32], u[32];
-            ld_acc32(t_acc + blk * 128 + c * 32, g);
-            ld_acc32(t_acc + blk * 128 + 64 + c * 32, u);
-            if (ok) {
 #pragma unroll
-              for (int i = 0; i < 32; ++i) g[i] = gelu_tanh_f(g[i]) * u[i];
-              store_op16x32((uint16_t*)ea.out16 + (size_t)row * ea.ld_out + n0 / 2 + blk * 64 + c * 32, g, ea.out_fp16);
+          for (int hh = 0; hh < 2; ++hh) {
+            float g[32], u[32];
+            ld_acc32(t_acc + blk * 128 + hh * 32, g);
+            ld_acc32(t_acc + blk * 128 + 64 + hh * 32, u);
+            if (blk == BN / 128 - 1 && hh == 1) {
+              tc_fence_before();
+              mbar_arrive(tempty_bar(acc));
             }
+#pragma unroll
+            for (int i = 0; i < 32; i += 2)
+              *reinterpret_cast<float2*>(&scr[lane * 66 + hh * 32 + i]) =
+                  make_float2(gelu_tanh_f(g[i] * rs) * (u[i] * rs), gelu_tanh_f(g[i + 1] * rs) * (u[i + 1] * rs));
           }
+          __syncwarp();
+          float2 o[32];
+#pragma unroll
+          for (int rr = 0; rr < 32; ++rr) o[rr] = *reinterpret_cast<const float2*>(&scr[rr * 66 + 2 * lane]);
+#pragma unroll
+          for (int rr = 0; rr < 32; ++rr) {
+            if (r0 + rr < m_lim)
+              *reinterpret_cast<uint32_t*>(outp + (size_t)(r0 + rr) * ea.ld_out + n0 / 2 + blk * 64 + 2 * lane) =
+                  pack_op2(o[rr].x, o[rr].y, ea.out_fp16);
+          }
+          __syncwarp();
         }
       }
-      tc_fence_before();
-      mbar_arrive(tempty_bar(acc));
     }
   }
   tc_fence_before();
@@ -314,6 +402,8 @@ int num_sms() {
 }
 
 bool tc_gemm_supported(int N, int K) { return N % 64 == 0 && K % 64 == 0 && N >= 64; }
+// N tile of the EPI_BIAS_F32 / EPI_RESID launches (= columns per sum-of-squares partial)
+int tc_resid_bn(int N) { return N % 128 == 0 ? 128 : 64; }
 
 template <int BN, int EPI>
 static cudaError_t launch_one(const op16* A, const op16* W, int M, int N, int K, const EpiArgs& a, cudaStream_t s) {
@@ -338,12 +428,11 @@ cudaError_t launch_gemm_tc(Epi epi, const op16* A, const op16* W, int M, int N, 
                            cudaStream_t s) {
   switch (epi) {
     case EPI_STORE_F32:
+      if ((a.dbg >> 8) == 128 && N % 128 == 0) return launch_one<128, EPI_STORE_F32>(A, W, M, N, K, a, s);
+      if ((a.dbg >> 8) == 64) return launch_one<64, EPI_STORE_F32>(A, W, M, N, K, a, s);
       if (N % 256 == 0) return launch_one<256, EPI_STORE_F32>(A, W, M, N, K, a, s);
       if (N % 128 == 0) return launch_one<128, EPI_STORE_F32>(A, W, M, N, K, a, s);
       return launch_one<64, EPI_STORE_F32>(A, W, M, N, K, a, s);
-    case EPI_SWISH_ROWBIAS:
-      return N % 128 == 0 ? launch_one<128, EPI_SWISH_ROWBIAS>(A, W, M, N, K, a, s)
-                          : launch_one<64, EPI_SWISH_ROWBIAS>(A, W, M, N, K, a, s);
     case EPI_BIAS_F32:
       return N % 128 == 0 ? launch_one<128, EPI_BIAS_F32>(A, W, M, N, K, a, s)
                           : launch_one<64, EPI_BIAS_F32>(A, W, M, N, K, a, s);

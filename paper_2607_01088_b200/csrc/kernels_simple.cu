@@ -60,31 +60,53 @@ void launch_timevec(float* tvec, const bf16* w_t1, const float* b_t1, const Dims
   k_timevec<<<grid, 256, dm.d * sizeof(float), s>>>(tvec, w_t1, b_t1, dm, tb, max_batch);
 }
 
-// ------------------------------------------------------------------ a1 (action half)
-// a[m][n] = bf16( b_in[n] + sum_c x[m][c] W_in[n][c] ), x in fp32 (R11).
-__global__ void k_inproj(op16* __restrict__ a, const float* __restrict__ x,
-                         const bf16* __restrict__ w_in, const float* __restrict__ b_in, int d, int A,
-                         int fp16, const int* __restrict__ m_active) {
-  __shared__ float xs[64];
-  const int m = blockIdx.x;
-  if (m >= *m_active) return;
-  if (threadIdx.x < A) xs[threadIdx.x] = x[(size_t)m * A + threadIdx.x];
+// ------------------------------------------------------------------ a1 (action half + swish)
+// z[m][n] = swish( sum_c x[m][c] Wca[n][c] + bca[n] + tvec[p][n] ), with Wca = W_1[:, d:] W_in and
+// bca = W_1[:, d:] b_in folded at create (fp64 on the host): W_1 [tau ; W_in x + b_in] + b_1 is
+// linear in x, so the K = A contraction runs in fp32 on CUDA cores straight from x (R11: x fp32).
+// Block = EM_ROWS token rows; thread = output columns n, n + 256, ...
+constexpr int EM_ROWS = 16;
+__global__ void __launch_bounds__(256) k_embed1(op16* __restrict__ z, const float* __restrict__ x,
+                                                const float* __restrict__ wca, const float* __restrict__ bca,
+                                                const float* __restrict__ tvec, int d, int A, int H, int fp16,
+                                                const int* __restrict__ m_active) {
+  __shared__ float xs[EM_ROWS][64];
+  const int m0 = blockIdx.x * EM_ROWS, m_lim = *m_active;
+  if (m0 >= m_lim) return;
+  const int rows = min(EM_ROWS, m_lim - m0);
+  for (int i = threadIdx.x; i < EM_ROWS * A; i += blockDim.x) {
+    const int r = i / A, c = i - r * A;
+    xs[r][c] = r < rows ? x[(size_t)(m0 + r) * A + c] : 0.f;
+  }
   __syncthreads();
   for (int n = threadIdx.x; n < d; n += blockDim.x) {
-    float acc = b_in[n];
-    for (int c = 0; c < A; ++c) acc = fmaf(xs[c], __bfloat162float(w_in[(size_t)n * A + c]), acc);
-    a[(size_t)m * d + n] = f2op(acc, fp16);
+    float acc[EM_ROWS];
+    const float b = bca[n];
+#pragma unroll
+    for (int r = 0; r < EM_ROWS; ++r) acc[r] = b;
+    const float* wr = wca + (size_t)n * A;
+    for (int c = 0; c < A; ++c) {
+      const float w = wr[c];
+#pragma unroll
+      for (int r = 0; r < EM_ROWS; ++r) acc[r] = fmaf(xs[r][c], w, acc[r]);
+    }
+    for (int r = 0; r < rows; ++r) {
+      const int m = m0 + r;
+      z[(size_t)m * d + n] = f2op(swish_f(acc[r] + tvec[(size_t)(m / H) * d + n]), fp16);
+    }
   }
 }
-void launch_inproj(op16* a, const float* x, const bf16* w_in, const float* b_in, const Dims& dm,
-                   const Tables& tb, int k_iter, int M, cudaStream_t s) {
-  k_inproj<<<M, 128, 0, s>>>(a, x, w_in, b_in, dm.d, dm.A, dm.fp16, tb.m_active + k_iter);
+void launch_embed1(op16* z, const float* x, const float* wca, const float* bca, const float* tvec_k,
+                   const Dims& dm, const Tables& tb, int k_iter, int M, cudaStream_t s) {
+  k_embed1<<<(M + EM_ROWS - 1) / EM_ROWS, 256, 0, s>>>(z, x, wca, bca, tvec_k, dm.d, dm.A, dm.H, dm.fp16,
+                                                     tb.m_active + k_iter);
 }
 
 // ------------------------------------------------------------------ a2 RMSNorm (R5)
-// out = bf16( h * rsqrt(mean(h^2) + eps) * g ); one warp per token row; statistics in fp32.
-__global__ void k_rmsnorm(op16* __restrict__ out, const float* __restrict__ h,
-                          const float* __restrict__ g, int d, float eps, int fp16,
+// out = op16( h * rsqrt(mean(h^2) + eps) ); one warp per token row; statistics in fp32.  The gain g
+// is folded into the columns of the consuming weight matrix at create.  Family 0 only: the tcgen05
+// family fuses the norm into the neighbouring GEMM epilogues.
+__global__ void k_rmsnorm(op16* __restrict__ out, const float* __restrict__ h, int d, float eps, int fp16,
                           const int* __restrict__ m_active) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int m = blockIdx.x * (blockDim.x >> 5) + warp;
@@ -99,56 +121,80 @@ __global__ void k_rmsnorm(op16* __restrict__ out, const float* __restrict__ h,
   const float r = rsqrtf(ss / (float)d + eps);
   for (int c = lane * 4; c < d; c += 128) {
     float4 v = *reinterpret_cast<const float4*>(row + c);
-    float4 gg = *reinterpret_cast<const float4*>(g + c);
     uint2 pk;
-    pk.x = pack_op2(v.x * r * gg.x, v.y * r * gg.y, fp16);
-    pk.y = pack_op2(v.z * r * gg.z, v.w * r * gg.w, fp16);
+    pk.x = pack_op2(v.x * r, v.y * r, fp16);
+    pk.y = pack_op2(v.z * r, v.w * r, fp16);
     *reinterpret_cast<uint2*>(out + (size_t)m * d + c) = pk;
   }
 }
-void launch_rmsnorm(op16* out, const float* h, const float* g, const Dims& dm, const Tables& tb,
-                    int k_iter, int M, cudaStream_t s) {
+void launch_rmsnorm(op16* out, const float* h, const Dims& dm, const Tables& tb, int k_iter, int M,
+                    cudaStream_t s) {
   const int wpb = 8;
-  k_rmsnorm<<<(M + wpb - 1) / wpb, wpb * 32, 0, s>>>(out, h, g, dm.d, dm.eps, dm.fp16, tb.m_active + k_iter);
+  k_rmsnorm<<<(M + wpb - 1) / wpb, wpb * 32, 0, s>>>(out, h, dm.d, dm.eps, dm.fp16, tb.m_active + k_iter);
 }
 
 // ------------------------------------------------------------------ a9 + a10 (+ a11 bookkeeping)
 // v = RMSNorm(h; g_f) W_out^T + b_out ; x <- x + dt_p v.  One warp per token row.  The
 // normalised row stays in fp32 (no bf16 rounding of this operand).  Optional velocity export in
 // the caller's robot order.
-__global__ void k_final(float* __restrict__ x, const CallPtrs* __restrict__ cp,
-                        const float* __restrict__ h, const float* __restrict__ g,
-                        const bf16* __restrict__ w_out, const float* __restrict__ b_out, int d, int A,
-                        int H, float eps, Tables tb, int k_iter) {
+constexpr int FIN_AMAX = 64;  // action_dim <= 64 (rosa_expert_create)
+__global__ void __launch_bounds__(256) k_final(float* __restrict__ x, const CallPtrs* __restrict__ cp,
+                                               const float* __restrict__ h, const float* __restrict__ g,
+                                               const bf16* __restrict__ w_out, const float* __restrict__ b_out,
+                                               int d, int A, int H, float eps, Tables tb, int k_iter) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int m = blockIdx.x * (blockDim.x >> 5) + warp;
   if (m >= tb.m_active[k_iter]) return;
+  const float* row = h + (size_t)m * d;
+  float ss = 0.f;
+  for (int c = lane * 4; c < d; c += 128) {
+    const float4 v = *reinterpret_cast<const float4*>(row + c);
+    ss += v.x * v.x + v.y * v.y + v.z * v.z + v.w * v.w;
+  }
+  ss = warp_sum(ss);
+  const float r = rsqrtf(ss / (float)d + eps);
+  // lane-private partial dot products for every action dimension, 4 columns per lane per chunk
+  float acc[FIN_AMAX];
+#pragma unroll
+  for (int a = 0; a < FIN_AMAX; ++a) acc[a] = 0.f;
+  for (int c = lane * 4; c < d; c += 128) {
+    float4 v = *reinterpret_cast<const float4*>(row + c);
+    const float4 gg = *reinterpret_cast<const float4*>(g + c);
+    v.x *= r * gg.x; v.y *= r * gg.y; v.z *= r * gg.z; v.w *= r * gg.w;
+#pragma unroll
+    for (int a = 0; a < FIN_AMAX; ++a) {
+      if (a < A) {
+        const uint2 wb = *reinterpret_cast<const uint2*>(w_out + (size_t)a * d + c);
+        const float2 w01 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&wb.x));
+        const float2 w23 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&wb.y));
+        acc[a] = fmaf(v.x, w01.x, fmaf(v.y, w01.y, fmaf(v.z, w23.x, fmaf(v.w, w23.y, acc[a]))));
+      }
+    }
+  }
+  float mine = 0.f;  // lane a (and a + 32) keeps the reduced value of action dimension a
+  float mine_hi = 0.f;
+#pragma unroll
+  for (int a = 0; a < FIN_AMAX; ++a) {
+    if (a < A) {
+      const float v = warp_sum(acc[a]);
+      if ((a & 31) == lane) { if (a < 32) mine = v; else mine_hi = v; }
+    }
+  }
   float* vel_out = cp->vel;
   const int batch_ext = cp->batch_ext;
   const int p = m / H, j = m - p * H;
-  const float* row = h + (size_t)m * d;
-  float ss = 0.f;
-  for (int c = lane; c < d; c += 32) ss = fmaf(row[c], row[c], ss);
-  ss = warp_sum(ss);
-  const float r = rsqrtf(ss / (float)d + eps);
   const float dt = tb.dt[p];
-  for (int a = 0; a < A; ++a) {
-    const bf16* wr = w_out + (size_t)a * d;
-    float acc = 0.f;
-    for (int c = lane; c < d; c += 32) acc = fmaf(row[c] * r * g[c], __bfloat162float(wr[c]), acc);
-    acc = warp_sum(acc);
-    if (lane == 0) {
-      const float v = acc + b_out[a];
-      float* xp = x + (size_t)m * A + a;
-      *xp = fmaf(dt, v, *xp);
-      if (vel_out) vel_out[(((size_t)k_iter * batch_ext + tb.src[p]) * H + j) * A + a] = v;
-    }
+  for (int a = lane; a < A; a += 32) {
+    const float v = (a < 32 ? mine : mine_hi) + b_out[a];
+    float* xp = x + (size_t)m * A + a;
+    *xp = fmaf(dt, v, *xp);
+    if (vel_out) vel_out[(((size_t)k_iter * batch_ext + tb.src[p]) * H + j) * A + a] = v;
   }
 }
 void launch_final(float* x, const CallPtrs* cp, const float* h, const float* g, const bf16* w_out,
                   const float* b_out, const Dims& dm, const Tables& tb, int k_iter, int M,
                   cudaStream_t s) {
-  const int wpb = 4;
+  const int wpb = 8;
   k_final<<<(M + wpb - 1) / wpb, wpb * 32, 0, s>>>(x, cp, h, g, w_out, b_out, dm.d, dm.A, dm.H,
                                                   dm.eps, tb, k_iter);
 }
@@ -228,9 +274,6 @@ __global__ void k_epilogue(int epi, const float* __restrict__ C, int M, int N, E
     const float acc = C[idx];
     switch (epi) {
       case EPI_STORE_F32: a.out_f32[(size_t)m * a.ld_out + n] = acc; break;
-      case EPI_SWISH_ROWBIAS:
-        ((op16*)a.out16)[(size_t)m * a.ld_out + n] = f2op(swish_f(acc + a.rowbias[(size_t)(m / a.H) * N + n]), a.out_fp16);
-        break;
       case EPI_BIAS_F32: a.out_f32[(size_t)m * a.ld_out + n] = acc + a.bias[n]; break;
       case EPI_RESID: a.out_f32[(size_t)m * a.ld_out + n] += acc; break;
       case EPI_ROPE: {

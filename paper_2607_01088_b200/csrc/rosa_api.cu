@@ -58,14 +58,19 @@ struct rosa_expert {
   bool use_graph = true;
   int max_pos = 0;
   // weights
-  bf16 *w_in = nullptr, *w_t1 = nullptr, *w_out = nullptr;  // CUDA-core steps: bf16 as given
-  op16 *w_t1a = nullptr, *w_t2 = nullptr;                    // GEMM operands: fp16 or bf16 (dm.fp16)
-  float *b_in = nullptr, *b_t1 = nullptr, *b_t2 = nullptr, *b_out = nullptr, *g_final = nullptr;
+  bf16 *w_t1 = nullptr, *w_out = nullptr;  // CUDA-core steps: bf16 as given
+  float *wca = nullptr, *bca = nullptr;    // W_1[:, d:] W_in [d, A] and W_1[:, d:] b_in [d], folded in fp64
+  op16* w_t2 = nullptr;                    // GEMM operand: fp16 or bf16 (dm.fp16)
+  float *b_t1 = nullptr, *b_t2 = nullptr, *b_out = nullptr, *g_final = nullptr;
   std::vector<LayerWeights> lw;
   float2* rope_tab = nullptr;
   // workspaces
   float *x = nullptr, *h = nullptr, *tvec = nullptr, *scratch = nullptr;
-  op16 *abuf = nullptr, *zbuf = nullptr, *nrm = nullptr, *obuf = nullptr, *mact = nullptr;
+  // nrm: A operand of the QKV / gate-up GEMMs = normalised h (family 0) or the 16-bit copy of h
+  // itself (family 1, norm scale applied in the consumer's epilogue from the ssq partials)
+  op16 *zbuf = nullptr, *nrm = nullptr, *obuf = nullptr, *mact = nullptr;
+  float* ssq = nullptr;  // [Mmax, n_part] partial sums of squares of h rows (family 1)
+  int n_part = 1;
   bf16* qkv = nullptr;  // q/k/v feed attention together with the bf16 prefix cache: always bf16
   // robot table (device) + host mirror
   const bf16** d_rk = nullptr;
@@ -205,12 +210,29 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
 #define UPB(dst) if ((st = upload_bf16(e, t, &(dst))) != ROSA_OK) return st
 #define UPO(dst) if ((st = upload_op16(e, t, &(dst))) != ROSA_OK) return st
 #define UPF(dst) if ((st = upload_f32(e, t, &(dst))) != ROSA_OK) return st
-  FETCH(w->w_in, (size_t)d * A); UPB(e->w_in);
-  FETCH(w->b_in, d); UPF(e->b_in);
-  FETCH(w->w_t1, (size_t)d * 2 * d); UPB(e->w_t1);
-  u.resize((size_t)d * d);  // action half of W_1 (columns d..2d-1, R2) as its own [d,d] matrix
-  for (int n = 0; n < d; ++n) memcpy(&u[(size_t)n * d], &t[(size_t)n * 2 * d + d], (size_t)d * 4);
-  t.swap(u); UPO(e->w_t1a);
+  {  // a1 folding (exact algebra, fp64): Wca = W_1[:, d:] W_in, bca = W_1[:, d:] b_in
+    std::vector<float> win, bin;
+    if ((st = fetch_f32(w->w_in, (size_t)d * A, dt, od, win)) != ROSA_OK) return st;
+    if ((st = fetch_f32(w->b_in, (size_t)d, dt, od, bin)) != ROSA_OK) return st;
+    FETCH(w->w_t1, (size_t)d * 2 * d); UPB(e->w_t1);
+    std::vector<float> wca((size_t)d * A), bca(d);
+    std::vector<double> accr(A);
+    for (int n = 0; n < d; ++n) {
+      const float* w1a = &t[(size_t)n * 2 * d + d];
+      std::fill(accr.begin(), accr.end(), 0.0);
+      double accb = 0.0;
+      for (int j = 0; j < d; ++j) {
+        const double wj = w1a[j];
+        const float* wi = &win[(size_t)j * A];
+        for (int c = 0; c < A; ++c) accr[c] += wj * wi[c];
+        accb += wj * bin[j];
+      }
+      for (int c = 0; c < A; ++c) wca[(size_t)n * A + c] = (float)accr[c];
+      bca[n] = (float)accb;
+    }
+    if ((st = upload_f32(e, wca, &e->wca)) != ROSA_OK) return st;
+    if ((st = upload_f32(e, bca, &e->bca)) != ROSA_OK) return st;
+  }
   FETCH(w->b_t1, d); UPF(e->b_t1);
   FETCH(w->w_t2, (size_t)d * d); UPO(e->w_t2);
   FETCH(w->b_t2, d); UPF(e->b_t2);
@@ -220,14 +242,18 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
   e->lw.resize(dm.layers);
   for (int l = 0; l < dm.layers; ++l) {
     LayerWeights& L = e->lw[l];
-    FETCH(w->g_attn[l], d); UPF(L.g_attn);
-    FETCH(w->g_mlp[l], d); UPF(L.g_mlp);
+    // RMSNorm gains are folded into the columns of the consuming matrices: (h r g) W^T = r h (W g)^T
+    std::vector<float> g1, g2;
+    if ((st = fetch_f32(w->g_attn[l], (size_t)d, dt, od, g1)) != ROSA_OK) return st;
+    if ((st = fetch_f32(w->g_mlp[l], (size_t)d, dt, od, g2)) != ROSA_OK) return st;
     // packed [wq ; wk ; wv]  -> one QKV GEMM (step a3)
     std::vector<float> pk((size_t)dm.qkv_n * d);
     FETCH(w->wq[l], (size_t)dm.q_n * d); memcpy(pk.data(), t.data(), t.size() * 4);
     FETCH(w->wk[l], (size_t)dm.nkv * dm.hd * d); memcpy(pk.data() + (size_t)dm.q_n * d, t.data(), t.size() * 4);
     FETCH(w->wv[l], (size_t)dm.nkv * dm.hd * d);
     memcpy(pk.data() + (size_t)(dm.q_n + dm.nkv * dm.hd) * d, t.data(), t.size() * 4);
+    for (size_t n = 0; n < (size_t)dm.qkv_n; ++n)
+      for (int c = 0; c < d; ++c) pk[n * d + c] *= g1[c];
     t.swap(pk); UPO(L.wqkv);
     FETCH(w->wo[l], (size_t)d * dm.q_n); UPO(L.wo);
     // gate/up interleaved in blocks of gu_blk rows -> one GEMM + GeGLU epilogue (step a7)
@@ -239,6 +265,8 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
     FETCH(w->w_up[l], (size_t)F * d);
     for (int f = 0; f < F; ++f)
       memcpy(&gu[((size_t)(f / g) * 2 * g + g + f % g) * d], &t[(size_t)f * d], (size_t)d * 4);
+    for (size_t n = 0; n < (size_t)2 * F; ++n)
+      for (int c = 0; c < d; ++c) gu[n * d + c] *= g2[c];
     t.swap(gu); UPO(L.wgu);
     FETCH(w->w_down[l], (size_t)d * F); UPO(L.wdown);
   }
@@ -268,7 +296,6 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
   WS(e->x, (size_t)c->max_batch * HA * 4);
   WS(e->h, Mmax * d * 4);
   WS(e->tvec, (size_t)c->max_steps * c->max_batch * d * 4);
-  WS(e->abuf, Mmax * d * 2);
   WS(e->zbuf, Mmax * d * 2);
   WS(e->nrm, Mmax * d * 2);
   WS(e->qkv, Mmax * dm.qkv_n * 2);
@@ -276,7 +303,8 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
   WS(e->mact, Mmax * F * 2);
   WS(e->scratch, Mmax * (size_t)std::max(2 * F, dm.qkv_n) * 4);
   WS(e->e2e_dev, (size_t)c->max_batch * HA * 4);
-  CK(cudaMemset(e->abuf, 0, Mmax * d * 2));
+  e->n_part = d / tc_resid_bn(d);
+  WS(e->ssq, Mmax * e->n_part * 4);
   CK(cudaMemset(e->zbuf, 0, Mmax * d * 2));
   CK(cudaMemset(e->nrm, 0, Mmax * d * 2));
   CK(cudaMemset(e->qkv, 0, Mmax * dm.qkv_n * 2));
@@ -365,42 +393,48 @@ static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, cudaStream_
   mark(e, ROSA_KC_TIMEVEC, s);
   launch_timevec(e->tvec, e->w_t1, e->b_t1, dm, tb, nmax, e->cfg.max_batch, s);
   e->last_launches += 2;
+  const bool fused_norm = e->family == 1;  // RMSNorm fused into the GEMM epilogues (tcgen05 family)
   for (int k = 0; k < nmax; ++k) {
     EpiArgs ea{};
     ea.m_active = tb.m_active + k;
     ea.H = dm.H; ea.hd = dm.hd; ea.gu_blk = dm.gu_blk; ea.in_fp16 = dm.fp16; ea.out_fp16 = dm.fp16;
+    ea.inv_d = 1.f / (float)d; ea.eps = dm.eps; ea.n_part = e->n_part;
+    if (fused_norm) { ea.h16 = e->nrm; ea.ssq_out = e->ssq; ea.ssq_in = e->ssq; }
     // a1: h0 = W2 swish(W1 [tau ; W_in x + b_in] + b1) + b2
     mark(e, ROSA_KC_INPROJ, s);
-    launch_inproj(e->abuf, e->x, e->w_in, e->b_in, dm, tb, k, M, s);
+    launch_embed1(e->zbuf, e->x, e->wca, e->bca, e->tvec + (size_t)k * e->cfg.max_batch * d, dm, tb, k, M, s);
     e->last_launches += 1;
-    ea.out16 = e->zbuf; ea.ld_out = d;
-    ea.rowbias = e->tvec + (size_t)k * e->cfg.max_batch * d;
-    if ((err = gemm(e, ROSA_KC_GEMM_EMBED, EPI_SWISH_ROWBIAS, e->abuf, e->w_t1a, M, d, d, ea, s)) != cudaSuccess) return err;
-    ea.out_f32 = e->h; ea.bias = e->b_t2;
+    ea.out_f32 = e->h; ea.ld_out = d; ea.bias = e->b_t2;
     if ((err = gemm(e, ROSA_KC_GEMM_EMBED, EPI_BIAS_F32, e->zbuf, e->w_t2, M, d, d, ea, s)) != cudaSuccess) return err;
     for (int l = 0; l < dm.layers; ++l) {
       const LayerWeights& L = e->lw[l];
-      mark(e, ROSA_KC_RMSNORM, s);
-      launch_rmsnorm(e->nrm, e->h, L.g_attn, dm, tb, k, M, s);                       // a2
+      if (!fused_norm) {
+        mark(e, ROSA_KC_RMSNORM, s);
+        launch_rmsnorm(e->nrm, e->h, dm, tb, k, M, s);                               // a2
+        e->last_launches += 1;
+      }
       ea.out16 = e->qkv; ea.ld_out = dm.qkv_n;
       ea.rope_tab = e->rope_tab; ea.ids = tb.ids; ea.rlen = tb.rlen;
       ea.rope_cols = dm.q_n + dm.nkv * dm.hd;
-      if ((err = gemm(e, ROSA_KC_GEMM_QKV, EPI_ROPE, e->nrm, L.wqkv, M, dm.qkv_n, d, ea, s)) != cudaSuccess) return err;  // a3+a4
+      if ((err = gemm(e, ROSA_KC_GEMM_QKV, EPI_ROPE, e->nrm, L.wqkv, M, dm.qkv_n, d, ea, s)) != cudaSuccess) return err;  // a2+a3+a4
       mark(e, ROSA_KC_ATTN, s);
       if (e->attn_tc) {                                                              // a5
         if ((err = launch_attn_tc(dm, tb, l, e->qkv, e->obuf, k, M, e->d_kv_maps, s)) != cudaSuccess) return err;
       } else {
         launch_attn_simple(dm, tb, l, e->qkv, e->obuf, k, e->cfg.max_prefix_len, s);
       }
+      e->last_launches += 1;
       ea.out_f32 = e->h; ea.ld_out = d;
       if ((err = gemm(e, ROSA_KC_GEMM_O, EPI_RESID, e->obuf, L.wo, M, d, dm.q_n, ea, s)) != cudaSuccess) return err;    // a6
-      mark(e, ROSA_KC_RMSNORM, s);
-      launch_rmsnorm(e->nrm, e->h, L.g_mlp, dm, tb, k, M, s);                        // a2
+      if (!fused_norm) {
+        mark(e, ROSA_KC_RMSNORM, s);
+        launch_rmsnorm(e->nrm, e->h, dm, tb, k, M, s);                               // a2
+        e->last_launches += 1;
+      }
       ea.out16 = e->mact; ea.ld_out = dm.F;
-      if ((err = gemm(e, ROSA_KC_GEMM_GATEUP, EPI_GEGLU, e->nrm, L.wgu, M, 2 * dm.F, d, ea, s)) != cudaSuccess) return err;  // a7
+      if ((err = gemm(e, ROSA_KC_GEMM_GATEUP, EPI_GEGLU, e->nrm, L.wgu, M, 2 * dm.F, d, ea, s)) != cudaSuccess) return err;  // a2+a7
       ea.out_f32 = e->h; ea.ld_out = d;
       if ((err = gemm(e, ROSA_KC_GEMM_DOWN, EPI_RESID, e->mact, L.wdown, M, d, dm.F, ea, s)) != cudaSuccess) return err;   // a8
-      e->last_launches += 3;
     }
     mark(e, ROSA_KC_FINAL, s);
     launch_final(e->x, cp, e->h, e->g_final, e->w_out, e->b_out, dm, tb, k, M, s);    // a9 + a10
@@ -678,6 +712,7 @@ rosa_status_t rosa_debug_gemm(int32_t family, int32_t M, int32_t N, int32_t K, c
   if (!tc_gemm_supported(N, K)) { set_error("shape not supported by the tcgen05 GEMM"); return ROSA_ERR_UNSUPPORTED; }
   EpiArgs ea{};
   ea.out_f32 = C; ea.ld_out = N;
+  if (const char* dbg = getenv("ROSA_DBG")) ea.dbg = atoi(dbg);
   CK(launch_gemm_tc(EPI_STORE_F32, (const op16*)A, (const op16*)W, M, N, K, ea, s));
   return ROSA_OK;
 }

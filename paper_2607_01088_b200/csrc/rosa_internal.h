@@ -50,28 +50,31 @@ struct CallPtrs {
 };
 
 struct LayerWeights {
-  op16 *wqkv, *wo, *wgu, *wdown;  // [qkv_n,d] [d,q_n] [2F,d] (interleaved) [d,F]
-  float *g_attn, *g_mlp;          // [d]
+  op16 *wqkv, *wo, *wgu, *wdown;  // [qkv_n,d] [d,q_n] [2F,d] (interleaved) [d,F]; RMSNorm gains folded
+                                  // into the columns of wqkv and wgu
 };
 
 // Epilogue selector shared by the CUDA-core path (separate elementwise kernels over an fp32
 // scratch) and the tcgen05 path (fused into the GEMM).
 enum Epi : int {
   EPI_STORE_F32 = 0,     // C fp32 = acc                     (debug GEMM)
-  EPI_SWISH_ROWBIAS = 1, // out bf16 = swish(acc + tvec[m / H][n])
-  EPI_BIAS_F32 = 2,      // h fp32 = acc + bias[n]
-  EPI_ROPE = 3,          // qkv bf16 = rope(acc) on q and k heads at pos = len + j; v copied
-  EPI_RESID = 4,         // h fp32 += acc
-  EPI_GEGLU = 5          // out bf16 [M, N/2] = gelu_tanh(gate) * up (interleaved columns)
+  EPI_BIAS_F32 = 2,      // h fp32 = acc + bias[n]          (+ 16-bit copy and sum-of-squares partials)
+  EPI_ROPE = 3,          // qkv bf16 = rope(r * acc) on q and k heads at pos = len + j; v = r * acc
+  EPI_RESID = 4,         // h fp32 += acc                   (+ 16-bit copy and sum-of-squares partials)
+  EPI_GEGLU = 5          // out 16-bit [M, N/2] = gelu_tanh(r * gate) * (r * up) (interleaved columns)
 };
 
 struct EpiArgs {
   float* out_f32;         // EPI_STORE_F32 / BIAS_F32 / RESID
-  void* out16;            // SWISH_ROWBIAS / GEGLU: op16 (fp16 or bf16 per out_fp16); ROPE: bf16
+  void* out16;            // GEGLU: op16 (fp16 or bf16 per out_fp16); ROPE: bf16
+  void* h16;              // BIAS_F32 / RESID (tcgen05 family): op16 copy of the new h, or null
+  float* ssq_out;         // BIAS_F32 / RESID (tcgen05 family): [M, N / BN] partial sums of squares, or null
+  const float* ssq_in;    // ROPE / GEGLU (tcgen05 family): partials of the A operand's rows, or null
+  int n_part;             // partials per row in ssq_in
+  float inv_d, eps;       // 1 / d_model, rms_eps
   int out_fp16;           // 16-bit output format: 1 = fp16, 0 = bf16
   int in_fp16;            // operand format of A and W
   const float* bias;      // BIAS_F32: [N]
-  const float* rowbias;   // SWISH_ROWBIAS: [B, N] (already offset to iteration k)
   const float2* rope_tab; // ROPE: [max_pos, hd/2] (cos, sin)
   const int* ids;         // ROPE: Tables::ids
   const int* rlen;        // ROPE: Tables::rlen
@@ -79,6 +82,7 @@ struct EpiArgs {
   int gu_blk;             // GEGLU
   int ld_out;             // leading dimension (elements) of the output
   const int* m_active;    // device pointer to the active row count of this iteration (or null)
+  int dbg;                // measurement aid (ROSA_DBG): bit 0 skip the epilogue body, bit 1 skip the MMAs
 };
 
 // ---- launchers (each checks nothing; callers validated shapes) -------------------------
@@ -93,16 +97,17 @@ void launch_gather_x(float* x, const CallPtrs* cp, const Tables& tb, int HA, cud
 void launch_scatter_x(const CallPtrs* cp, const float* x, const Tables& tb, int HA, cudaStream_t s);
 void launch_timevec(float* tvec, const bf16* w_t1, const float* b_t1, const Dims& dm,
                     const Tables& tb, int nsteps_max, int max_batch, cudaStream_t s);
-void launch_inproj(op16* a, const float* x, const bf16* w_in, const float* b_in, const Dims& dm,
-                   const Tables& tb, int k_iter, int M, cudaStream_t s);
-void launch_rmsnorm(op16* out, const float* h, const float* g, const Dims& dm, const Tables& tb,
-                    int k_iter, int M, cudaStream_t s);
+void launch_embed1(op16* z, const float* x, const float* wca, const float* bca, const float* tvec_k,
+                   const Dims& dm, const Tables& tb, int k_iter, int M, cudaStream_t s);
+void launch_rmsnorm(op16* out, const float* h, const Dims& dm, const Tables& tb, int k_iter, int M,
+                    cudaStream_t s);
 void launch_final(float* x, const CallPtrs* cp, const float* h, const float* g, const bf16* w_out,
                   const float* b_out, const Dims& dm, const Tables& tb, int k_iter, int M,
                   cudaStream_t s);
 void launch_f32_to_bf16(bf16* dst, const float* src, size_t n, cudaStream_t s);
 // tcgen05 family (gemm_tcgen05.cu)
 bool tc_gemm_supported(int N, int K);
+int tc_resid_bn(int N);
 // A [M,K] row-major, W [N,K] row-major, both fp16 or both bf16 (EpiArgs::in_fp16)
 cudaError_t launch_gemm_tc(Epi epi, const op16* A, const op16* W, int M, int N, int K,
                            const EpiArgs& a, cudaStream_t s);
