@@ -68,6 +68,180 @@ __device__ __forceinline__ float row_rscale(const EpiArgs& ea, int row) {
   return rsqrtf(ss * ea.inv_d + ea.eps);
 }
 
+// Epilogue of one accumulator tile for one warp: its 32 rows (TMEM lanes) x BN columns.
+// `release()` is called once, as soon as the accumulator has been read completely.
+// TMEM -> registers is thread = row (tcgen05.ld 32x32b); global memory wants lane = column: the
+// warp transposes through its private padded scratch `scr` in shared memory, so every global
+// load/store is one coalesced 64..512-byte row segment per instruction.
+template <int BN, int EPI, typename Release>
+__device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, float* scr, uint32_t t_acc, int r0, int n0, int m_lim,
+                                              int N, int lane, Release release) {
+  const int row = r0 + lane;  // row of this thread in the thread = row domain
+  const bool ok = row < m_lim;
+  if constexpr (EPI == EPI_STORE_F32 || EPI == EPI_BIAS_F32 || EPI == EPI_RESID) {
+    // h (fp32) = acc [+ h] [+ bias]; optionally also the 16-bit copy of the new h (A operand of
+    // the next GEMM) and this tile's partial sum of squares of each row (fused RMSNorm, a2).
+    // Lane domain: 8 lanes x float4 cover the 32 columns of a chunk row; one instruction = 4 rows.
+    constexpr int P = 36;  // scratch pitch in floats: 16-byte aligned rows, conflict-free both ways
+    const int lr = lane >> 3, lc = (lane & 7) * 4;
+    float rowss[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) rowss[i] = 0.f;
+    const bool want_h16 = EPI != EPI_STORE_F32 && ea.h16 != nullptr;
+#pragma unroll 1
+    for (int c = 0; c < BN / 32; ++c) {
+      {
+        float v[32];
+        ld_acc32(t_acc + c * 32, v);
+        if (c == BN / 32 - 1) release();  // accumulator fully read: hand it back to the MMA warp
+#pragma unroll
+        for (int i = 0; i < 32; i += 4)
+          *reinterpret_cast<float4*>(&scr[lane * P + i]) = make_float4(v[i], v[i + 1], v[i + 2], v[i + 3]);
+      }
+      __syncwarp();
+      const int col = n0 + c * 32 + lc;
+      float4 add = make_float4(0.f, 0.f, 0.f, 0.f);
+      if constexpr (EPI == EPI_BIAS_F32) add = *reinterpret_cast<const float4*>(ea.bias + col);
+      float* gp = ea.out_f32 + (size_t)(r0 + lr) * ea.ld_out + col;
+      uint16_t* hp = (uint16_t*)ea.h16 + (size_t)(r0 + lr) * ea.ld_out + col;
+      const size_t step = (size_t)4 * ea.ld_out;
+      float4 o[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        o[i] = *reinterpret_cast<const float4*>(&scr[(i * 4 + lr) * P + lc]);
+        if constexpr (EPI == EPI_RESID) {
+          if (r0 + i * 4 + lr < m_lim) {
+            const float4 h = *reinterpret_cast<const float4*>(gp + i * step);
+            o[i].x += h.x; o[i].y += h.y; o[i].z += h.z; o[i].w += h.w;
+          }
+        }
+      }
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        o[i].x += add.x; o[i].y += add.y; o[i].z += add.z; o[i].w += add.w;
+        if (r0 + i * 4 + lr < m_lim) {
+          *reinterpret_cast<float4*>(gp + i * step) = o[i];
+          if constexpr (EPI != EPI_STORE_F32) {
+            if (want_h16)
+              *reinterpret_cast<uint2*>(hp + i * step) =
+                  make_uint2(pack_op2(o[i].x, o[i].y, ea.out_fp16), pack_op2(o[i].z, o[i].w, ea.out_fp16));
+            rowss[i] += o[i].x * o[i].x + o[i].y * o[i].y + o[i].z * o[i].z + o[i].w * o[i].w;
+          }
+        }
+      }
+      __syncwarp();
+    }
+    if constexpr (EPI != EPI_STORE_F32) {
+      if (ea.ssq_out) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+          float v = rowss[i];
+          v += __shfl_xor_sync(0xffffffffu, v, 1);
+          v += __shfl_xor_sync(0xffffffffu, v, 2);
+          v += __shfl_xor_sync(0xffffffffu, v, 4);
+          const int rw = r0 + i * 4 + lr;
+          if ((lane & 7) == 0 && rw < m_lim) ea.ssq_out[(size_t)rw * (N / BN) + n0 / BN] = v;
+        }
+      }
+    }
+  } else if constexpr (EPI == EPI_ROPE) {
+    // BN == head_dim: the tile is exactly one head; pairs (c, c + hd/2) are both in TMEM.
+    static_assert(EPI != EPI_ROPE || BN == 256, "RoPE epilogue assumes BN == head_dim == 256");
+    const bool rot = n0 < ea.rope_cols;
+    const float rs = row_rscale(ea, ok ? row : 0);
+    int posr = 0;
+    if (ok && rot) {
+      const int p = row / ea.H;
+      posr = ea.rlen[ea.ids[p]] + (row - p * ea.H);
+    }
+    uint16_t* outp = (uint16_t*)ea.out16;
+#pragma unroll 1
+    for (int c = 0; c < 2; ++c) {  // 64 low columns [64c, 64c+64) with their partners +128
+      float v[32];
+      float2 lo[32];
+#pragma unroll
+      for (int hh = 0; hh < 2; ++hh) {
+        ld_acc32(t_acc + c * 64 + hh * 32, v);
+#pragma unroll
+        for (int i = 0; i < 32; i += 2)
+          *reinterpret_cast<float2*>(&scr[lane * 66 + hh * 32 + i]) = make_float2(v[i] * rs, v[i + 1] * rs);
+      }
+      __syncwarp();
+#pragma unroll
+      for (int rr = 0; rr < 32; ++rr) lo[rr] = *reinterpret_cast<const float2*>(&scr[rr * 66 + 2 * lane]);
+      __syncwarp();
+#pragma unroll
+      for (int hh = 0; hh < 2; ++hh) {
+        ld_acc32(t_acc + BN / 2 + c * 64 + hh * 32, v);
+#pragma unroll
+        for (int i = 0; i < 32; i += 2)
+          *reinterpret_cast<float2*>(&scr[lane * 66 + hh * 32 + i]) = make_float2(v[i] * rs, v[i + 1] * rs);
+      }
+      if (c == 1) {
+        release();
+      }
+      __syncwarp();
+#pragma unroll
+      for (int half = 0; half < 2; ++half) {  // 16 rows at a time: loads, then math, then stores
+        float2 hi[16];
+        float4 cs[16];
+#pragma unroll
+        for (int r2 = 0; r2 < 16; ++r2) {
+          const int rr = half * 16 + r2;
+          hi[r2] = *reinterpret_cast<const float2*>(&scr[rr * 66 + 2 * lane]);
+          const int pos = __shfl_sync(0xffffffffu, posr, rr);
+          cs[r2] = rot ? *reinterpret_cast<const float4*>(ea.rope_tab + (size_t)pos * (BN / 2) + c * 64 + 2 * lane)
+                       : make_float4(1.f, 0.f, 1.f, 0.f);
+        }
+#pragma unroll
+        for (int r2 = 0; r2 < 16; ++r2) {
+          const int rr = half * 16 + r2;
+          const float a0 = lo[rr].x, b0 = hi[r2].x, a1 = lo[rr].y, b1 = hi[r2].y;
+          const float ax = a0 * cs[r2].x - b0 * cs[r2].y, bx = b0 * cs[r2].x + a0 * cs[r2].y;
+          const float ay = a1 * cs[r2].z - b1 * cs[r2].w, by = b1 * cs[r2].z + a1 * cs[r2].w;
+          if (r0 + rr < m_lim) {
+            uint16_t* dst = outp + (size_t)(r0 + rr) * ea.ld_out + n0 + c * 64 + 2 * lane;
+            *reinterpret_cast<uint32_t*>(dst) = pack_op2(ax, ay, 0);  // q/k/v feed attention: always bf16
+            *reinterpret_cast<uint32_t*>(dst + BN / 2) = pack_op2(bx, by, 0);
+          }
+        }
+      }
+      __syncwarp();
+    }
+  } else if constexpr (EPI == EPI_GEGLU) {
+    // packed columns: [gate 64 | up 64] blocks (gu_blk = 64); output column = n/2 region
+    const float rs = row_rscale(ea, ok ? row : 0);
+    uint16_t* outp = (uint16_t*)ea.out16;
+#pragma unroll 1
+    for (int blk = 0; blk < BN / 128; ++blk) {
+#pragma unroll
+      for (int hh = 0; hh < 2; ++hh) {
+        float g[32], u[32];
+        ld_acc32(t_acc + blk * 128 + hh * 32, g);
+        ld_acc32(t_acc + blk * 128 + 64 + hh * 32, u);
+        if (blk == BN / 128 - 1 && hh == 1) {
+          release();
+        }
+#pragma unroll
+        for (int i = 0; i < 32; i += 2)
+          *reinterpret_cast<float2*>(&scr[lane * 66 + hh * 32 + i]) =
+              make_float2(gelu_tanh_f(g[i] * rs) * (u[i] * rs), gelu_tanh_f(g[i + 1] * rs) * (u[i + 1] * rs));
+      }
+      __syncwarp();
+      float2 o[32];
+#pragma unroll
+      for (int rr = 0; rr < 32; ++rr) o[rr] = *reinterpret_cast<const float2*>(&scr[rr * 66 + 2 * lane]);
+#pragma unroll
+      for (int rr = 0; rr < 32; ++rr) {
+        if (r0 + rr < m_lim)
+          *reinterpret_cast<uint32_t*>(outp + (size_t)(r0 + rr) * ea.ld_out + n0 / 2 + blk * 64 + 2 * lane) =
+              pack_op2(o[rr].x, o[rr].y, ea.out_fp16);
+      }
+      __syncwarp();
+    }
+  }
+}
+
 template <int BN, int EPI>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, int M, int N, int K,
@@ -169,8 +343,6 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
       const uint32_t acc_ph = (it >> 1) & 1;
       const int m0 = (t % n_m) * BM, n0 = (t / n_m) * BN;
       const int r0 = m0 + q * 32;            // first row of this warp
-      const int row = r0 + lane;             // row of this thread in the thread = row domain
-      const bool ok = row < m_lim;
       mbar_wait(tfull_bar(acc), acc_ph);
       tc_fence_after();
       const uint32_t t_acc = tmem_base + ((uint32_t)(q * 32) << 16) + acc * BN;
@@ -180,160 +352,10 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         continue;
       }
 
-      if constexpr (EPI == EPI_STORE_F32 || EPI == EPI_BIAS_F32 || EPI == EPI_RESID) {
-        // h (fp32) = acc [+ h] [+ bias]; optionally also the 16-bit copy of the new h (A operand of
-        // the next GEMM) and this tile's partial sum of squares of each row (fused RMSNorm, a2)
-        float rowss[32];
-#pragma unroll
-        for (int rr = 0; rr < 32; ++rr) rowss[rr] = 0.f;
-#pragma unroll 1
-        for (int c = 0; c < BN / 32; ++c) {
-          float v[32];
-          ld_acc32(t_acc + c * 32, v);
-          if (c == BN / 32 - 1) {  // accumulator fully read: hand it back to the MMA warp
-            tc_fence_before();
-            mbar_arrive(tempty_bar(acc));
-          }
-#pragma unroll
-          for (int i = 0; i < 32; ++i) scr[lane * 33 + i] = v[i];
-          __syncwarp();
-          const int col = n0 + c * 32 + lane;
-          float add = 0.f;
-          if constexpr (EPI == EPI_BIAS_F32) add = ea.bias[col];
-          float hold[32];
-          if constexpr (EPI == EPI_RESID) {
-#pragma unroll
-            for (int rr = 0; rr < 32; ++rr)
-              hold[rr] = (r0 + rr < m_lim) ? ea.out_f32[(size_t)(r0 + rr) * ea.ld_out + col] : 0.f;
-          }
-          // all shared-memory reads first: the compiler must assume scr aliases the global
-          // pointers, so a load placed after a store would wait for it
-          float o[32];
-#pragma unroll
-          for (int rr = 0; rr < 32; ++rr) o[rr] = scr[rr * 33 + lane] + add;
-#pragma unroll
-          for (int rr = 0; rr < 32; ++rr) {
-            if constexpr (EPI == EPI_RESID) o[rr] += hold[rr];
-            if (r0 + rr < m_lim) {
-              const size_t idx = (size_t)(r0 + rr) * ea.ld_out + col;
-              ea.out_f32[idx] = o[rr];
-              if constexpr (EPI != EPI_STORE_F32) {
-                if (ea.h16) ((uint16_t*)ea.h16)[idx] = f2op(o[rr], ea.out_fp16);
-                rowss[rr] = fmaf(o[rr], o[rr], rowss[rr]);
-              }
-            }
-          }
-          __syncwarp();
-        }
-        if constexpr (EPI != EPI_STORE_F32) {
-          if (ea.ssq_out) {
-            float mine = 0.f;
-#pragma unroll
-            for (int rr = 0; rr < 32; ++rr) {
-              const float tot = warp_sum(rowss[rr]);
-              if (rr == lane) mine = tot;
-            }
-            if (ok) ea.ssq_out[(size_t)row * (N / BN) + n0 / BN] = mine;
-          }
-        }
-      } else if constexpr (EPI == EPI_ROPE) {
-        // BN == head_dim: the tile is exactly one head; pairs (c, c + hd/2) are both in TMEM.
-        static_assert(EPI != EPI_ROPE || BN == 256, "RoPE epilogue assumes BN == head_dim == 256");
-        const bool rot = n0 < ea.rope_cols;
-        const float rs = row_rscale(ea, ok ? row : 0);
-        int posr = 0;
-        if (ok && rot) {
-          const int p = row / ea.H;
-          posr = ea.rlen[ea.ids[p]] + (row - p * ea.H);
-        }
-        uint16_t* outp = (uint16_t*)ea.out16;
-#pragma unroll 1
-        for (int c = 0; c < 2; ++c) {  // 64 low columns [64c, 64c+64) with their partners +128
-          float v[32];
-          float2 lo[32];
-#pragma unroll
-          for (int hh = 0; hh < 2; ++hh) {
-            ld_acc32(t_acc + c * 64 + hh * 32, v);
-#pragma unroll
-            for (int i = 0; i < 32; i += 2)
-              *reinterpret_cast<float2*>(&scr[lane * 66 + hh * 32 + i]) = make_float2(v[i] * rs, v[i + 1] * rs);
-          }
-          __syncwarp();
-#pragma unroll
-          for (int rr = 0; rr < 32; ++rr) lo[rr] = *reinterpret_cast<const float2*>(&scr[rr * 66 + 2 * lane]);
-          __syncwarp();
-#pragma unroll
-          for (int hh = 0; hh < 2; ++hh) {
-            ld_acc32(t_acc + BN / 2 + c * 64 + hh * 32, v);
-#pragma unroll
-            for (int i = 0; i < 32; i += 2)
-              *reinterpret_cast<float2*>(&scr[lane * 66 + hh * 32 + i]) = make_float2(v[i] * rs, v[i + 1] * rs);
-          }
-          if (c == 1) {
-            tc_fence_before();
-            mbar_arrive(tempty_bar(acc));
-          }
-          __syncwarp();
-#pragma unroll
-          for (int half = 0; half < 2; ++half) {  // 16 rows at a time: loads, then math, then stores
-            float2 hi[16];
-            float4 cs[16];
-#pragma unroll
-            for (int r2 = 0; r2 < 16; ++r2) {
-              const int rr = half * 16 + r2;
-              hi[r2] = *reinterpret_cast<const float2*>(&scr[rr * 66 + 2 * lane]);
-              const int pos = __shfl_sync(0xffffffffu, posr, rr);
-              cs[r2] = rot ? *reinterpret_cast<const float4*>(ea.rope_tab + (size_t)pos * (BN / 2) + c * 64 + 2 * lane)
-                           : make_float4(1.f, 0.f, 1.f, 0.f);
-            }
-#pragma unroll
-            for (int r2 = 0; r2 < 16; ++r2) {
-              const int rr = half * 16 + r2;
-              const float a0 = lo[rr].x, b0 = hi[r2].x, a1 = lo[rr].y, b1 = hi[r2].y;
-              const float ax = a0 * cs[r2].x - b0 * cs[r2].y, bx = b0 * cs[r2].x + a0 * cs[r2].y;
-              const float ay = a1 * cs[r2].z - b1 * cs[r2].w, by = b1 * cs[r2].z + a1 * cs[r2].w;
-              if (r0 + rr < m_lim) {
-                uint16_t* dst = outp + (size_t)(r0 + rr) * ea.ld_out + n0 + c * 64 + 2 * lane;
-                *reinterpret_cast<uint32_t*>(dst) = pack_op2(ax, ay, 0);  // q/k/v feed attention: always bf16
-                *reinterpret_cast<uint32_t*>(dst + BN / 2) = pack_op2(bx, by, 0);
-              }
-            }
-          }
-          __syncwarp();
-        }
-      } else if constexpr (EPI == EPI_GEGLU) {
-        // packed columns: [gate 64 | up 64] blocks (gu_blk = 64); output column = n/2 region
-        const float rs = row_rscale(ea, ok ? row : 0);
-        uint16_t* outp = (uint16_t*)ea.out16;
-#pragma unroll 1
-        for (int blk = 0; blk < BN / 128; ++blk) {
-#pragma unroll
-          for (int hh = 0; hh < 2; ++hh) {
-            float g[32], u[32];
-            ld_acc32(t_acc + blk * 128 + hh * 32, g);
-            ld_acc32(t_acc + blk * 128 + 64 + hh * 32, u);
-            if (blk == BN / 128 - 1 && hh == 1) {
-              tc_fence_before();
-              mbar_arrive(tempty_bar(acc));
-            }
-#pragma unroll
-            for (int i = 0; i < 32; i += 2)
-              *reinterpret_cast<float2*>(&scr[lane * 66 + hh * 32 + i]) =
-                  make_float2(gelu_tanh_f(g[i] * rs) * (u[i] * rs), gelu_tanh_f(g[i + 1] * rs) * (u[i + 1] * rs));
-          }
-          __syncwarp();
-          float2 o[32];
-#pragma unroll
-          for (int rr = 0; rr < 32; ++rr) o[rr] = *reinterpret_cast<const float2*>(&scr[rr * 66 + 2 * lane]);
-#pragma unroll
-          for (int rr = 0; rr < 32; ++rr) {
-            if (r0 + rr < m_lim)
-              *reinterpret_cast<uint32_t*>(outp + (size_t)(r0 + rr) * ea.ld_out + n0 / 2 + blk * 64 + 2 * lane) =
-                  pack_op2(o[rr].x, o[rr].y, ea.out_fp16);
-          }
-          __syncwarp();
-        }
-      }
+      epilogue_tile<BN, EPI>(ea, scr, t_acc, r0, n0, m_lim, N, lane, [&] {
+        tc_fence_before();
+        mbar_arrive(tempty_bar(acc));
+      });
     }
   }
   tc_fence_before();
@@ -341,6 +363,148 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
   if (warp == 1) {
     tc_fence_after();
     tmem_dealloc(tmem_base, Cfg::TMEM_COLS);
+  }
+}
+
+// ------------------------------------------------------------------ CTA-pair variant (cta_group::2)
+// Pair tile 256 x BN: CTA r of the cluster holds A rows [m0 + 128 r, +128) and B rows
+// [n0 + (BN/2) r, +BN/2) of every k-block; ONE tcgen05.mma (M = 256) issued by the leader reads
+// both CTAs' shared memory and writes each CTA's 128 x BN half of D into that CTA's tensor memory.
+// Per CTA and k-block that is 16 KB + BN*64 B from L2 for 128 x BN x 64 MACs: a third less than
+// the single-CTA tile, which is what bounds the single-CTA kernel (profiles/r1_gemm_notes.md).
+template <int BN>
+struct Gemm2Cfg {
+  static constexpr int STAGES = BN == 256 ? 6 : 8;
+  static constexpr int A_BYTES = BM * BK * 2;
+  static constexpr int B_BYTES = (BN / 2) * BK * 2;
+  static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
+  static constexpr int SMEM = STAGES * STAGE_BYTES + 1024 + 256 + 4 * kScrFloats * 4;
+  static constexpr int TMEM_COLS = 2 * BN < 32 ? 32 : 2 * BN;
+};
+
+template <int BN, int EPI>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1)
+k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, int M, int N, int K,
+           EpiArgs ea) {
+  using Cfg = Gemm2Cfg<BN>;
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t bar_base = smem_base + Cfg::STAGES * Cfg::STAGE_BYTES;
+  auto full_bar = [&](int s) { return bar_base + 8u * s; };                        // used in the leader
+  auto empty_bar = [&](int s) { return bar_base + 8u * (Cfg::STAGES + s); };       // both CTAs
+  auto tfull_bar = [&](int a) { return bar_base + 8u * (2 * Cfg::STAGES + a); };   // both CTAs
+  auto tempty_bar = [&](int a) { return bar_base + 8u * (2 * Cfg::STAGES + 2 + a); };  // leader
+  const uint32_t tmem_slot = bar_base + 8u * (2 * Cfg::STAGES + 4);
+  volatile uint32_t* tmem_slot_ptr =
+      reinterpret_cast<volatile uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_ctarank();
+  const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
+  const int m_lim = ea.m_active ? min(M, *ea.m_active) : M;
+  const int n_m = (m_lim + 2 * BM - 1) / (2 * BM), n_n = N / BN;
+  const int n_tiles = n_m * n_n, n_kb = K / BK;
+
+  if (warp == 0 && lane == 0) {
+    prefetch_tensormap(&tmA);
+    prefetch_tensormap(&tmB);
+    for (int s = 0; s < Cfg::STAGES; ++s) {
+      mbar_init(full_bar(s), 2);   // one arrive.expect_tx per CTA of the pair
+      mbar_init(empty_bar(s), 1);  // tcgen05.commit (multicast)
+    }
+    for (int a = 0; a < 2; ++a) {
+      mbar_init(tfull_bar(a), 1);   // tcgen05.commit (multicast)
+      mbar_init(tempty_bar(a), 8);  // 4 epilogue warps x 2 CTAs
+    }
+    fence_barrier_init();
+  }
+  if (warp == 1) {
+    tmem_alloc_cg2(tmem_slot, Cfg::TMEM_COLS);
+    tmem_relinquish_cg2();
+  }
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync_all();  // the peer's barriers are initialised before anything is signalled on them
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot_ptr;
+
+  if (warp == 0) {
+    if (lane == 0) {  // ---------------- TMA producer (both CTAs; completion counted in the leader)
+      int s = 0;
+      uint32_t ph = 0;
+      for (int t = pair; t < n_tiles; t += n_pairs) {
+        const int m0 = (t % n_m) * (2 * BM) + (int)rank * BM, n0 = (t / n_m) * BN + (int)rank * (BN / 2);
+        for (int kb = 0; kb < n_kb; ++kb) {
+          mbar_wait(empty_bar(s), ph ^ 1);
+          const uint32_t lfull = mapa_shared(full_bar(s), 0);
+          mbar_expect_tx_cluster(lfull, Cfg::STAGE_BYTES);
+          const uint32_t a_dst = smem_base + s * Cfg::STAGE_BYTES;
+          tma_load_2d_cg2(a_dst, &tmA, lfull, kb * BK, m0);
+          tma_load_2d_cg2(a_dst + Cfg::A_BYTES, &tmB, lfull, kb * BK, n0);
+          if (++s == Cfg::STAGES) { s = 0; ph ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0 && rank == 0) {  // ---------------- MMA issuer (leader CTA only)
+      const uint32_t idesc =
+          ea.in_fp16 ? (make_idesc_bf16(2 * BM, BN) & ~((1u << 7) | (1u << 10))) : make_idesc_bf16(2 * BM, BN);
+      int s = 0, it = 0;
+      uint32_t ph = 0;
+      for (int t = pair; t < n_tiles; t += n_pairs, ++it) {
+        const int acc = it & 1;
+        const uint32_t acc_ph = (it >> 1) & 1;
+        mbar_wait(tempty_bar(acc), acc_ph ^ 1);
+        tc_fence_after();
+        const uint32_t d_tmem = tmem_base + acc * BN;
+        for (int kb = 0; kb < n_kb; ++kb) {
+          mbar_wait(full_bar(s), ph);
+          tc_fence_after();
+          const uint32_t a_addr = smem_base + s * Cfg::STAGE_BYTES;
+          const uint32_t b_addr = a_addr + Cfg::A_BYTES;
+          if (!(ea.dbg & 2)) {
+#pragma unroll
+            for (int kk = 0; kk < BK / 16; ++kk) {
+              umma_bf16_cg2(d_tmem, make_sdesc_k128(a_addr + kk * 32), make_sdesc_k128(b_addr + kk * 32), idesc,
+                            (kb | kk) != 0);
+            }
+          }
+          umma_commit_cg2(empty_bar(s));
+          if (++s == Cfg::STAGES) { s = 0; ph ^= 1; }
+        }
+        umma_commit_cg2(tfull_bar(acc));
+      }
+    }
+  } else {  // ---------------- epilogue warps 2..5 (both CTAs, each on its own 128 rows)
+    const int q = warp & 3;
+    float* scr = reinterpret_cast<float*>(smem_raw + (bar_base + 256u - smem_u32(smem_raw))) + q * kScrFloats;
+    int it = 0;
+    for (int t = pair; t < n_tiles; t += n_pairs, ++it) {
+      const int acc = it & 1;
+      const uint32_t acc_ph = (it >> 1) & 1;
+      const int m0 = (t % n_m) * (2 * BM) + (int)rank * BM, n0 = (t / n_m) * BN;
+      const int r0 = m0 + q * 32;
+      mbar_wait(tfull_bar(acc), acc_ph);
+      tc_fence_after();
+      const uint32_t t_acc = tmem_base + ((uint32_t)(q * 32) << 16) + acc * BN;
+      auto release = [&] {
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cluster(mapa_shared(tempty_bar(acc), 0));
+      };
+      if (ea.dbg & 1) {
+        release();
+        continue;
+      }
+      epilogue_tile<BN, EPI>(ea, scr, t_acc, r0, n0, m_lim, N, lane, release);
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync_all();  // the leader's MMAs read the peer's shared memory; nobody leaves early
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc_cg2(tmem_base, Cfg::TMEM_COLS);
   }
 }
 
@@ -402,8 +566,13 @@ int num_sms() {
 }
 
 bool tc_gemm_supported(int N, int K) { return N % 64 == 0 && K % 64 == 0 && N >= 64; }
+// CTA pairs (256-row tiles) once there is more than one 128-row tile of tokens
+static bool use_pair(int M) { return M > BM; }
 // N tile of the EPI_BIAS_F32 / EPI_RESID launches (= columns per sum-of-squares partial)
-int tc_resid_bn(int N) { return N % 128 == 0 ? 128 : 64; }
+int tc_resid_bn(int N, int M) {
+  if (use_pair(M) && N % 256 == 0) return 256;
+  return N % 128 == 0 ? 128 : 64;
+}
 
 template <int BN, int EPI>
 static cudaError_t launch_one(const op16* A, const op16* W, int M, int N, int K, const EpiArgs& a, cudaStream_t s) {
@@ -424,27 +593,53 @@ static cudaError_t launch_one(const op16* A, const op16* W, int M, int N, int K,
   return cudaGetLastError();
 }
 
+template <int BN, int EPI>
+static cudaError_t launch_two(const op16* A, const op16* W, int M, int N, int K, const EpiArgs& a, cudaStream_t s) {
+  using Cfg = Gemm2Cfg<BN>;
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(k_gemm_tc2<BN, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  CUtensorMap tmA, tmB;
+  if (!make_tmap_2d(&tmA, A, (uint64_t)M, (uint64_t)K, BM, a.in_fp16) ||
+      !make_tmap_2d(&tmB, W, (uint64_t)N, (uint64_t)K, BN / 2, a.in_fp16))
+    return cudaErrorInvalidValue;
+  const int tiles = ((M + 2 * BM - 1) / (2 * BM)) * (N / BN);
+  const int pairs = tiles < num_sms() / 2 ? tiles : num_sms() / 2;
+  k_gemm_tc2<BN, EPI><<<2 * pairs, kGemmThreads, Cfg::SMEM, s>>>(tmA, tmB, M, N, K, a);
+  return cudaGetLastError();
+}
+
+template <int EPI>
+static cudaError_t launch_by_n(const op16* A, const op16* W, int M, int N, int K, const EpiArgs& a, cudaStream_t s) {
+  const int forced = a.dbg >> 8;  // rosa_debug_gemm only: 1xx = single-CTA kernel, N tile xx0
+  const bool pair = forced ? forced / 1000 == 2 : use_pair(M);
+  const int bn = forced ? forced % 1000 : tc_resid_bn(N, M);
+  if (pair) {
+    if (bn == 256) return launch_two<256, EPI>(A, W, M, N, K, a, s);
+    if (bn == 128) return launch_two<128, EPI>(A, W, M, N, K, a, s);
+    return launch_two<64, EPI>(A, W, M, N, K, a, s);
+  }
+  if (bn == 256) return launch_one<256, EPI>(A, W, M, N, K, a, s);
+  if (bn == 128) return launch_one<128, EPI>(A, W, M, N, K, a, s);
+  return launch_one<64, EPI>(A, W, M, N, K, a, s);
+}
+
 cudaError_t launch_gemm_tc(Epi epi, const op16* A, const op16* W, int M, int N, int K, const EpiArgs& a,
                            cudaStream_t s) {
   switch (epi) {
-    case EPI_STORE_F32:
-      if ((a.dbg >> 8) == 128 && N % 128 == 0) return launch_one<128, EPI_STORE_F32>(A, W, M, N, K, a, s);
-      if ((a.dbg >> 8) == 64) return launch_one<64, EPI_STORE_F32>(A, W, M, N, K, a, s);
-      if (N % 256 == 0) return launch_one<256, EPI_STORE_F32>(A, W, M, N, K, a, s);
-      if (N % 128 == 0) return launch_one<128, EPI_STORE_F32>(A, W, M, N, K, a, s);
-      return launch_one<64, EPI_STORE_F32>(A, W, M, N, K, a, s);
-    case EPI_BIAS_F32:
-      return N % 128 == 0 ? launch_one<128, EPI_BIAS_F32>(A, W, M, N, K, a, s)
-                          : launch_one<64, EPI_BIAS_F32>(A, W, M, N, K, a, s);
-    case EPI_RESID:
-      return N % 128 == 0 ? launch_one<128, EPI_RESID>(A, W, M, N, K, a, s)
-                          : launch_one<64, EPI_RESID>(A, W, M, N, K, a, s);
+    case EPI_STORE_F32: return launch_by_n<EPI_STORE_F32>(A, W, M, N, K, a, s);
+    case EPI_BIAS_F32: return launch_by_n<EPI_BIAS_F32>(A, W, M, N, K, a, s);
+    case EPI_RESID: return launch_by_n<EPI_RESID>(A, W, M, N, K, a, s);
     case EPI_ROPE:
       if (a.hd != 256 || N % 256) return cudaErrorNotSupported;
-      return launch_one<256, EPI_ROPE>(A, W, M, N, K, a, s);
+      return use_pair(M) ? launch_two<256, EPI_ROPE>(A, W, M, N, K, a, s) : launch_one<256, EPI_ROPE>(A, W, M, N, K, a, s);
     case EPI_GEGLU:
       if (a.gu_blk != 64 || N % 256) return cudaErrorNotSupported;
-      return launch_one<256, EPI_GEGLU>(A, W, M, N, K, a, s);
+      return use_pair(M) ? launch_two<256, EPI_GEGLU>(A, W, M, N, K, a, s)
+                         : launch_one<256, EPI_GEGLU>(A, W, M, N, K, a, s);
   }
   return cudaErrorNotSupported;
 }

@@ -70,7 +70,6 @@ struct rosa_expert {
   // itself (family 1, norm scale applied in the consumer's epilogue from the ssq partials)
   op16 *zbuf = nullptr, *nrm = nullptr, *obuf = nullptr, *mact = nullptr;
   float* ssq = nullptr;  // [Mmax, n_part] partial sums of squares of h rows (family 1)
-  int n_part = 1;
   bf16* qkv = nullptr;  // q/k/v feed attention together with the bf16 prefix cache: always bf16
   // robot table (device) + host mirror
   const bf16** d_rk = nullptr;
@@ -303,8 +302,7 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
   WS(e->mact, Mmax * F * 2);
   WS(e->scratch, Mmax * (size_t)std::max(2 * F, dm.qkv_n) * 4);
   WS(e->e2e_dev, (size_t)c->max_batch * HA * 4);
-  e->n_part = d / tc_resid_bn(d);
-  WS(e->ssq, Mmax * e->n_part * 4);
+  WS(e->ssq, Mmax * (d / 64) * 4);
   CK(cudaMemset(e->zbuf, 0, Mmax * d * 2));
   CK(cudaMemset(e->nrm, 0, Mmax * d * 2));
   CK(cudaMemset(e->qkv, 0, Mmax * dm.qkv_n * 2));
@@ -398,7 +396,7 @@ static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, cudaStream_
     EpiArgs ea{};
     ea.m_active = tb.m_active + k;
     ea.H = dm.H; ea.hd = dm.hd; ea.gu_blk = dm.gu_blk; ea.in_fp16 = dm.fp16; ea.out_fp16 = dm.fp16;
-    ea.inv_d = 1.f / (float)d; ea.eps = dm.eps; ea.n_part = e->n_part;
+    ea.inv_d = 1.f / (float)d; ea.eps = dm.eps; ea.n_part = d / tc_resid_bn(d, M);
     if (fused_norm) { ea.h16 = e->nrm; ea.ssq_out = e->ssq; ea.ssq_in = e->ssq; }
     // a1: h0 = W2 swish(W1 [tau ; W_in x + b_in] + b1) + b2
     mark(e, ROSA_KC_INPROJ, s);
@@ -712,7 +710,7 @@ rosa_status_t rosa_debug_gemm(int32_t family, int32_t M, int32_t N, int32_t K, c
   if (!tc_gemm_supported(N, K)) { set_error("shape not supported by the tcgen05 GEMM"); return ROSA_ERR_UNSUPPORTED; }
   EpiArgs ea{};
   ea.out_f32 = C; ea.ld_out = N;
-  if (const char* dbg = getenv("ROSA_DBG")) ea.dbg = atoi(dbg);
+  if (const char* dbg = getenv("ROSA_DBG")) ea.dbg = atoi(dbg);  // bits 0-1 skip epilogue / MMA; >> 8: 1256 = single-CTA BN 256, 2128 = pair BN 128 ...
   CK(launch_gemm_tc(EPI_STORE_F32, (const op16*)A, (const op16*)W, M, N, K, ea, s));
   return ROSA_OK;
 }
