@@ -157,6 +157,11 @@ const char *rosa_kernel_class_name(int32_t cls); /* "" if out of range */
 rosa_status_t rosa_debug_gemm(int32_t family, int32_t M, int32_t N, int32_t K, const void *A_bf16,
                               const void *W_bf16, float *C, void *stream);
 
+/* Measurement aid: with the environment variable ROSA_DBG bit 4 set, the attention kernel records
+ * clock64() at its pipeline events for two CTAs; this copies [2][8 roles][32 key blocks] int64 values
+ * of the last launch to host_out and returns the count (0 if tracing is off). */
+int32_t rosa_debug_attn_trace(int64_t *host_out, int32_t n);
+
 const char *rosa_last_error(void); /* thread-local, never NULL */
 int32_t rosa_version(void);
 

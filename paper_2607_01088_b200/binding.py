@@ -21,7 +21,7 @@ ROSA_F32, ROSA_BF16 = 0, 1
 
 EXPORTS = ("rosa_expert_create", "rosa_expert_destroy", "rosa_prefix_kv_bind", "rosa_prefix_kv_unbind",
            "rosa_denoise_batch", "rosa_denoise_batch_ex", "rosa_denoise_batch_host",
-           "rosa_profile_batch", "rosa_kernel_class_name",
+           "rosa_profile_batch", "rosa_kernel_class_name", "rosa_debug_attn_trace",
            "rosa_last_launch_count", "rosa_kernel_family", "rosa_debug_gemm", "rosa_last_error",
            "rosa_version")
 ROSA_KC_COUNT = 11
@@ -75,10 +75,12 @@ def load():
     lib.rosa_profile_batch.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.rosa_kernel_class_name.argtypes = [i32]
     lib.rosa_kernel_class_name.restype = C.c_char_p
+    lib.rosa_debug_attn_trace.argtypes = [vp, i32]
+    lib.rosa_debug_attn_trace.restype = i32
     lib.rosa_last_error.restype = C.c_char_p
     lib.rosa_version.restype = i32
     for n in EXPORTS:
-        if n not in ("rosa_last_error", "rosa_version", "rosa_kernel_class_name"):
+        if n not in ("rosa_last_error", "rosa_version", "rosa_kernel_class_name", "rosa_debug_attn_trace"):
             getattr(lib, n).restype = C.c_int
     _lib = lib
     return lib
@@ -231,6 +233,12 @@ def rosa_kernel_family(e: Expert) -> int:
 
 def rosa_debug_gemm(family: int, M: int, N: int, K: int, A_bf16, W_bf16, C_f32, stream=None):
     _check(load().rosa_debug_gemm(family, M, N, K, _ptr(A_bf16), _ptr(W_bf16), _ptr(C_f32), _stream_handle(stream)))
+
+
+def rosa_debug_attn_trace() -> np.ndarray:
+    buf = np.zeros((2, 8, 32), dtype=np.int64)
+    load().rosa_debug_attn_trace(_ptr(buf), buf.size)
+    return buf
 
 
 def rosa_last_error() -> str:
