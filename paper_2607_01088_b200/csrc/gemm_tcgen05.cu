@@ -24,16 +24,17 @@ namespace rosa {
 using namespace tc;
 
 constexpr int BM = 128, BK = 64;
-constexpr int kGemmThreads = 192;
-constexpr int kScrFloats = 32 * 66;  // per epilogue warp: 32 rows x up to 64 columns, padded
+constexpr int kGemmThreads = 320;      // warp 0 TMA, warp 1 MMA, warps 2..9 epilogue (two per TMEM lane quarter)
+constexpr int kEpiWarps = 8;
+constexpr int kScrFloats = 32 * 36;    // per epilogue warp: a 32 x 32 fp32 chunk, pitch 36
 
 template <int BN>
 struct GemmCfg {
-  static constexpr int STAGES = BN == 256 ? 4 : (BN == 128 ? 6 : 8);
+  static constexpr int STAGES = BN == 256 ? 3 : (BN == 128 ? 5 : 7);
   static constexpr int A_BYTES = BM * BK * 2;
   static constexpr int B_BYTES = BN * BK * 2;
   static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
-  static constexpr int SMEM = STAGES * STAGE_BYTES + 1024 /*align slack*/ + 256 /*barriers*/ + 4 * kScrFloats * 4;
+  static constexpr int SMEM = STAGES * STAGE_BYTES + 1024 /*align slack*/ + 256 /*barriers*/ + kEpiWarps * kScrFloats * 4;
   static constexpr int TMEM_COLS = 2 * BN < 32 ? 32 : 2 * BN;
 };
 
@@ -68,35 +69,45 @@ __device__ __forceinline__ float row_rscale(const EpiArgs& ea, int row) {
   return rsqrtf(ss * ea.inv_d + ea.eps);
 }
 
-// Epilogue of one accumulator tile for one warp: its 32 rows (TMEM lanes) x BN columns.
-// `release()` is called once, as soon as the accumulator has been read completely.
-// TMEM -> registers is thread = row (tcgen05.ld 32x32b); global memory wants lane = column: the
-// warp transposes through its private padded scratch `scr` in shared memory, so every global
-// load/store is one coalesced 64..512-byte row segment per instruction.
+// Epilogue of one accumulator tile for one warp: its 32 rows (TMEM lane quarter) x ONE HALF of the
+// tile's BN columns (`half`: the 8 epilogue warps are two per lane quarter).  `release()` is called
+// once, as soon as this warp has read its part of the accumulator.
+// TMEM -> registers is thread = row (tcgen05.ld 32x32b); global memory wants lanes along columns:
+// the warp transposes 32 x 32 chunks through its private scratch `scr` (pitch 36 floats: 16-byte
+// rows, conflict-free both ways) and then works with 8 lanes x 4 columns per row, 4 rows per
+// instruction, so every global access is a coalesced 64..128-byte row segment.
 template <int BN, int EPI, typename Release>
 __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, float* scr, uint32_t t_acc, int r0, int n0, int m_lim,
-                                              int N, int lane, Release release) {
+                                              int N, int lane, int half, Release release) {
+  constexpr int P = 36;
+  const int lr = lane >> 3, lc = (lane & 7) * 4;
   const int row = r0 + lane;  // row of this thread in the thread = row domain
   const bool ok = row < m_lim;
+  auto to_scratch = [&](const float (&v)[32]) {
+#pragma unroll
+    for (int i = 0; i < 32; i += 4)
+      *reinterpret_cast<float4*>(&scr[lane * P + i]) = make_float4(v[i], v[i + 1], v[i + 2], v[i + 3]);
+  };
+  auto from_scratch = [&](float4 (&o)[8]) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) o[i] = *reinterpret_cast<const float4*>(&scr[(i * 4 + lr) * P + lc]);
+  };
   if constexpr (EPI == EPI_STORE_F32 || EPI == EPI_BIAS_F32 || EPI == EPI_RESID) {
     // h (fp32) = acc [+ h] [+ bias]; optionally also the 16-bit copy of the new h (A operand of
-    // the next GEMM) and this tile's partial sum of squares of each row (fused RMSNorm, a2).
-    // Lane domain: 8 lanes x float4 cover the 32 columns of a chunk row; one instruction = 4 rows.
-    constexpr int P = 36;  // scratch pitch in floats: 16-byte aligned rows, conflict-free both ways
-    const int lr = lane >> 3, lc = (lane & 7) * 4;
+    // the next GEMM) and this half-tile's partial sum of squares of each row (fused RMSNorm, a2)
+    constexpr int NC = BN / 64;  // 32-column chunks per half
     float rowss[8];
 #pragma unroll
     for (int i = 0; i < 8; ++i) rowss[i] = 0.f;
     const bool want_h16 = EPI != EPI_STORE_F32 && ea.h16 != nullptr;
 #pragma unroll 1
-    for (int c = 0; c < BN / 32; ++c) {
+    for (int cc = 0; cc < NC; ++cc) {
+      const int c = half * NC + cc;
       {
         float v[32];
         ld_acc32(t_acc + c * 32, v);
-        if (c == BN / 32 - 1) release();  // accumulator fully read: hand it back to the MMA warp
-#pragma unroll
-        for (int i = 0; i < 32; i += 4)
-          *reinterpret_cast<float4*>(&scr[lane * P + i]) = make_float4(v[i], v[i + 1], v[i + 2], v[i + 3]);
+        if (cc == NC - 1) release();
+        to_scratch(v);
       }
       __syncwarp();
       const int col = n0 + c * 32 + lc;
@@ -106,10 +117,10 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, float* scr, uin
       uint16_t* hp = (uint16_t*)ea.h16 + (size_t)(r0 + lr) * ea.ld_out + col;
       const size_t step = (size_t)4 * ea.ld_out;
       float4 o[8];
+      from_scratch(o);
+      if constexpr (EPI == EPI_RESID) {
 #pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        o[i] = *reinterpret_cast<const float4*>(&scr[(i * 4 + lr) * P + lc]);
-        if constexpr (EPI == EPI_RESID) {
+        for (int i = 0; i < 8; ++i) {
           if (r0 + i * 4 + lr < m_lim) {
             const float4 h = *reinterpret_cast<const float4*>(gp + i * step);
             o[i].x += h.x; o[i].y += h.y; o[i].z += h.z; o[i].w += h.w;
@@ -140,12 +151,13 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, float* scr, uin
           v += __shfl_xor_sync(0xffffffffu, v, 2);
           v += __shfl_xor_sync(0xffffffffu, v, 4);
           const int rw = r0 + i * 4 + lr;
-          if ((lane & 7) == 0 && rw < m_lim) ea.ssq_out[(size_t)rw * (N / BN) + n0 / BN] = v;
+          if ((lane & 7) == 0 && rw < m_lim) ea.ssq_out[(size_t)rw * (2 * N / BN) + 2 * (n0 / BN) + half] = v;
         }
       }
     }
   } else if constexpr (EPI == EPI_ROPE) {
-    // BN == head_dim: the tile is exactly one head; pairs (c, c + hd/2) are both in TMEM.
+    // BN == head_dim: the tile is exactly one head; pairs (c, c + hd/2) are both in TMEM.  This
+    // warp covers low columns [64 half, 64 half + 64) and their partners 128 further on.
     static_assert(EPI != EPI_ROPE || BN == 256, "RoPE epilogue assumes BN == head_dim == 256");
     const bool rot = n0 < ea.rope_cols;
     const float rs = row_rscale(ea, ok ? row : 0);
@@ -156,86 +168,83 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, float* scr, uin
     }
     uint16_t* outp = (uint16_t*)ea.out16;
 #pragma unroll 1
-    for (int c = 0; c < 2; ++c) {  // 64 low columns [64c, 64c+64) with their partners +128
-      float v[32];
-      float2 lo[32];
+    for (int cc = 0; cc < 2; ++cc) {
+      const int c = half * 2 + cc;  // 32-column chunk of the low half
+      float4 lo[8], hi[8];
+      {
+        float v[32];
+        ld_acc32(t_acc + c * 32, v);
 #pragma unroll
-      for (int hh = 0; hh < 2; ++hh) {
-        ld_acc32(t_acc + c * 64 + hh * 32, v);
+        for (int i = 0; i < 32; ++i) v[i] *= rs;
+        to_scratch(v);
+        __syncwarp();
+        from_scratch(lo);
+        __syncwarp();
+        ld_acc32(t_acc + BN / 2 + c * 32, v);
+        if (cc == 1) release();
 #pragma unroll
-        for (int i = 0; i < 32; i += 2)
-          *reinterpret_cast<float2*>(&scr[lane * 66 + hh * 32 + i]) = make_float2(v[i] * rs, v[i + 1] * rs);
+        for (int i = 0; i < 32; ++i) v[i] *= rs;
+        to_scratch(v);
+        __syncwarp();
+        from_scratch(hi);
       }
-      __syncwarp();
+      if (rot) {  // warp-uniform (one head per tile)
+        float4 cs0[8], cs1[8];  // (cos, sin) of columns lc, lc+1 | lc+2, lc+3
 #pragma unroll
-      for (int rr = 0; rr < 32; ++rr) lo[rr] = *reinterpret_cast<const float2*>(&scr[rr * 66 + 2 * lane]);
-      __syncwarp();
-#pragma unroll
-      for (int hh = 0; hh < 2; ++hh) {
-        ld_acc32(t_acc + BN / 2 + c * 64 + hh * 32, v);
-#pragma unroll
-        for (int i = 0; i < 32; i += 2)
-          *reinterpret_cast<float2*>(&scr[lane * 66 + hh * 32 + i]) = make_float2(v[i] * rs, v[i + 1] * rs);
-      }
-      if (c == 1) {
-        release();
-      }
-      __syncwarp();
-#pragma unroll
-      for (int half = 0; half < 2; ++half) {  // 16 rows at a time: loads, then math, then stores
-        float2 hi[16];
-        float4 cs[16];
-#pragma unroll
-        for (int r2 = 0; r2 < 16; ++r2) {
-          const int rr = half * 16 + r2;
-          hi[r2] = *reinterpret_cast<const float2*>(&scr[rr * 66 + 2 * lane]);
-          const int pos = __shfl_sync(0xffffffffu, posr, rr);
-          cs[r2] = rot ? *reinterpret_cast<const float4*>(ea.rope_tab + (size_t)pos * (BN / 2) + c * 64 + 2 * lane)
-                       : make_float4(1.f, 0.f, 1.f, 0.f);
+        for (int i = 0; i < 8; ++i) {
+          const int pos = __shfl_sync(0xffffffffu, posr, i * 4 + lr);
+          const float4* tp = reinterpret_cast<const float4*>(ea.rope_tab + (size_t)pos * (BN / 2) + c * 32 + lc);
+          cs0[i] = tp[0];
+          cs1[i] = tp[1];
         }
 #pragma unroll
-        for (int r2 = 0; r2 < 16; ++r2) {
-          const int rr = half * 16 + r2;
-          const float a0 = lo[rr].x, b0 = hi[r2].x, a1 = lo[rr].y, b1 = hi[r2].y;
-          const float ax = a0 * cs[r2].x - b0 * cs[r2].y, bx = b0 * cs[r2].x + a0 * cs[r2].y;
-          const float ay = a1 * cs[r2].z - b1 * cs[r2].w, by = b1 * cs[r2].z + a1 * cs[r2].w;
-          if (r0 + rr < m_lim) {
-            uint16_t* dst = outp + (size_t)(r0 + rr) * ea.ld_out + n0 + c * 64 + 2 * lane;
-            *reinterpret_cast<uint32_t*>(dst) = pack_op2(ax, ay, 0);  // q/k/v feed attention: always bf16
-            *reinterpret_cast<uint32_t*>(dst + BN / 2) = pack_op2(bx, by, 0);
-          }
+        for (int i = 0; i < 8; ++i) {
+          const float4 a = lo[i], b = hi[i];
+          lo[i].x = a.x * cs0[i].x - b.x * cs0[i].y; hi[i].x = b.x * cs0[i].x + a.x * cs0[i].y;
+          lo[i].y = a.y * cs0[i].z - b.y * cs0[i].w; hi[i].y = b.y * cs0[i].z + a.y * cs0[i].w;
+          lo[i].z = a.z * cs1[i].x - b.z * cs1[i].y; hi[i].z = b.z * cs1[i].x + a.z * cs1[i].y;
+          lo[i].w = a.w * cs1[i].z - b.w * cs1[i].w; hi[i].w = b.w * cs1[i].z + a.w * cs1[i].w;
+        }
+      }
+      uint16_t* dst = outp + (size_t)(r0 + lr) * ea.ld_out + n0 + c * 32 + lc;
+      const size_t step = (size_t)4 * ea.ld_out;
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        if (r0 + i * 4 + lr < m_lim) {  // q/k/v feed the attention kernel: always bf16
+          *reinterpret_cast<uint2*>(dst + i * step) = make_uint2(pack_op2(lo[i].x, lo[i].y, 0), pack_op2(lo[i].z, lo[i].w, 0));
+          *reinterpret_cast<uint2*>(dst + i * step + BN / 2) =
+              make_uint2(pack_op2(hi[i].x, hi[i].y, 0), pack_op2(hi[i].z, hi[i].w, 0));
         }
       }
       __syncwarp();
     }
   } else if constexpr (EPI == EPI_GEGLU) {
-    // packed columns: [gate 64 | up 64] blocks (gu_blk = 64); output column = n/2 region
+    // packed columns: [gate 64 | up 64] blocks (gu_blk = 64) -> 64 outputs; this warp takes block `half`
+    static_assert(EPI != EPI_GEGLU || BN == 256, "GeGLU epilogue assumes two 128-column blocks per tile");
     const float rs = row_rscale(ea, ok ? row : 0);
     uint16_t* outp = (uint16_t*)ea.out16;
+    const int blk = half;
 #pragma unroll 1
-    for (int blk = 0; blk < BN / 128; ++blk) {
-#pragma unroll
-      for (int hh = 0; hh < 2; ++hh) {
+    for (int hh = 0; hh < 2; ++hh) {
+      {
         float g[32], u[32];
         ld_acc32(t_acc + blk * 128 + hh * 32, g);
         ld_acc32(t_acc + blk * 128 + 64 + hh * 32, u);
-        if (blk == BN / 128 - 1 && hh == 1) {
-          release();
-        }
+        if (hh == 1) release();
 #pragma unroll
-        for (int i = 0; i < 32; i += 2)
-          *reinterpret_cast<float2*>(&scr[lane * 66 + hh * 32 + i]) =
-              make_float2(gelu_tanh_f(g[i] * rs) * (u[i] * rs), gelu_tanh_f(g[i + 1] * rs) * (u[i + 1] * rs));
+        for (int i = 0; i < 32; ++i) g[i] = gelu_tanh_f(g[i] * rs) * (u[i] * rs);
+        to_scratch(g);
       }
       __syncwarp();
-      float2 o[32];
+      float4 o[8];
+      from_scratch(o);
+      uint16_t* dst = outp + (size_t)(r0 + lr) * ea.ld_out + n0 / 2 + blk * 64 + hh * 32 + lc;
+      const size_t step = (size_t)4 * ea.ld_out;
 #pragma unroll
-      for (int rr = 0; rr < 32; ++rr) o[rr] = *reinterpret_cast<const float2*>(&scr[rr * 66 + 2 * lane]);
-#pragma unroll
-      for (int rr = 0; rr < 32; ++rr) {
-        if (r0 + rr < m_lim)
-          *reinterpret_cast<uint32_t*>(outp + (size_t)(r0 + rr) * ea.ld_out + n0 / 2 + blk * 64 + 2 * lane) =
-              pack_op2(o[rr].x, o[rr].y, ea.out_fp16);
+      for (int i = 0; i < 8; ++i) {
+        if (r0 + i * 4 + lr < m_lim)
+          *reinterpret_cast<uint2*>(dst + i * step) =
+              make_uint2(pack_op2(o[i].x, o[i].y, ea.out_fp16), pack_op2(o[i].z, o[i].w, ea.out_fp16));
       }
       __syncwarp();
     }
@@ -272,7 +281,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     }
     for (int a = 0; a < 2; ++a) {
       mbar_init(tfull_bar(a), 1);
-      mbar_init(tempty_bar(a), 128);
+      mbar_init(tempty_bar(a), kEpiWarps);
     }
     fence_barrier_init();
   }
@@ -285,37 +294,40 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
 
-  if (warp == 0) {
-    if (lane == 0) {  // ---------------- TMA producer
-      int s = 0;
-      uint32_t ph = 0;
-      for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
-        const int m0 = (t % n_m) * BM, n0 = (t / n_m) * BN;
-        for (int kb = 0; kb < n_kb; ++kb) {
-          mbar_wait(empty_bar(s), ph ^ 1);
+  // Role loops run with whole warps (warp-uniform state stays in uniform registers); only the
+  // TMA / tcgen05 issue is fenced to one elected lane.
+  if (warp == 0) {  // ---------------- TMA producer
+    int s = 0;
+    uint32_t ph = 0;
+    for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+      const int m0 = (t % n_m) * BM, n0 = (t / n_m) * BN;
+      for (int kb = 0; kb < n_kb; ++kb) {
+        mbar_wait(empty_bar(s), ph ^ 1);
+        if (elect_one()) {
           mbar_expect_tx(full_bar(s), Cfg::STAGE_BYTES);
           const uint32_t a_dst = smem_base + s * Cfg::STAGE_BYTES;
           tma_load_2d(a_dst, &tmA, full_bar(s), kb * BK, m0);
           tma_load_2d(a_dst + Cfg::A_BYTES, &tmB, full_bar(s), kb * BK, n0);
-          if (++s == Cfg::STAGES) { s = 0; ph ^= 1; }
         }
+        __syncwarp();
+        if (++s == Cfg::STAGES) { s = 0; ph ^= 1; }
       }
     }
-  } else if (warp == 1) {
-    if (lane == 0) {  // ---------------- MMA issuer
-      // fp16 operands: A/B format bits 0 instead of 1 (bf16)
-      const uint32_t idesc = ea.in_fp16 ? (make_idesc_bf16(BM, BN) & ~((1u << 7) | (1u << 10))) : make_idesc_bf16(BM, BN);
-      int s = 0, it = 0;
-      uint32_t ph = 0;
-      for (int t = blockIdx.x; t < n_tiles; t += gridDim.x, ++it) {
-        const int acc = it & 1;
-        const uint32_t acc_ph = (it >> 1) & 1;
-        mbar_wait(tempty_bar(acc), acc_ph ^ 1);
+  } else if (warp == 1) {  // ---------------- MMA issuer
+    // fp16 operands: A/B format bits 0 instead of 1 (bf16)
+    const uint32_t idesc = ea.in_fp16 ? (make_idesc_bf16(BM, BN) & ~((1u << 7) | (1u << 10))) : make_idesc_bf16(BM, BN);
+    int s = 0, it = 0;
+    uint32_t ph = 0;
+    for (int t = blockIdx.x; t < n_tiles; t += gridDim.x, ++it) {
+      const int acc = it & 1;
+      const uint32_t acc_ph = (it >> 1) & 1;
+      mbar_wait(tempty_bar(acc), acc_ph ^ 1);
+      tc_fence_after();
+      const uint32_t d_tmem = tmem_base + acc * BN;
+      for (int kb = 0; kb < n_kb; ++kb) {
+        mbar_wait(full_bar(s), ph);
         tc_fence_after();
-        const uint32_t d_tmem = tmem_base + acc * BN;
-        for (int kb = 0; kb < n_kb; ++kb) {
-          mbar_wait(full_bar(s), ph);
-          tc_fence_after();
+        if (elect_one()) {
           const uint32_t a_addr = smem_base + s * Cfg::STAGE_BYTES;
           const uint32_t b_addr = a_addr + Cfg::A_BYTES;
           if (!(ea.dbg & 2)) {
@@ -326,17 +338,16 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
             }
           }
           umma_commit(empty_bar(s));
-          if (++s == Cfg::STAGES) { s = 0; ph ^= 1; }
+          if (kb == n_kb - 1) umma_commit(tfull_bar(acc));
         }
-        umma_commit(tfull_bar(acc));
+        __syncwarp();
+        if (++s == Cfg::STAGES) { s = 0; ph ^= 1; }
       }
     }
-  } else {  // ---------------- epilogue warps 2..5
-    // TMEM -> registers is thread = row (tcgen05.ld 32x32b); global memory wants lane = column.
-    // Each warp transposes through a private padded scratch in shared memory, so every global
-    // load/store below is one coalesced 64..512-byte row segment per instruction.
-    const int q = warp & 3;  // TMEM lane quarter this warp may access
-    float* scr = reinterpret_cast<float*>(smem_raw + (bar_base + 256u - smem_u32(smem_raw))) + q * kScrFloats;
+  } else {  // ---------------- epilogue warps 2..9
+    const int q = warp & 3;            // TMEM lane quarter this warp may access
+    const int half = (warp - 2) >> 2;  // which half of the tile's columns
+    float* scr = reinterpret_cast<float*>(smem_raw + (bar_base + 256u - smem_u32(smem_raw))) + (warp - 2) * kScrFloats;
     int it = 0;
     for (int t = blockIdx.x; t < n_tiles; t += gridDim.x, ++it) {
       const int acc = it & 1;
@@ -346,16 +357,16 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
       mbar_wait(tfull_bar(acc), acc_ph);
       tc_fence_after();
       const uint32_t t_acc = tmem_base + ((uint32_t)(q * 32) << 16) + acc * BN;
-      if (ea.dbg & 1) {  // measurement aid: mainloop only
+      auto release = [&] {
         tc_fence_before();
-        mbar_arrive(tempty_bar(acc));
+        __syncwarp();
+        if (lane == 0) mbar_arrive(tempty_bar(acc));
+      };
+      if (ea.dbg & 1) {  // measurement aid: mainloop only
+        release();
         continue;
       }
-
-      epilogue_tile<BN, EPI>(ea, scr, t_acc, r0, n0, m_lim, N, lane, [&] {
-        tc_fence_before();
-        mbar_arrive(tempty_bar(acc));
-      });
+      epilogue_tile<BN, EPI>(ea, scr, t_acc, r0, n0, m_lim, N, lane, half, release);
     }
   }
   tc_fence_before();
@@ -374,11 +385,11 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
 // the single-CTA tile, which is what bounds the single-CTA kernel (profiles/r1_gemm_notes.md).
 template <int BN>
 struct Gemm2Cfg {
-  static constexpr int STAGES = BN == 256 ? 6 : 8;
+  static constexpr int STAGES = BN == 256 ? 5 : (BN == 128 ? 7 : 8);
   static constexpr int A_BYTES = BM * BK * 2;
   static constexpr int B_BYTES = (BN / 2) * BK * 2;
   static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
-  static constexpr int SMEM = STAGES * STAGE_BYTES + 1024 + 256 + 4 * kScrFloats * 4;
+  static constexpr int SMEM = STAGES * STAGE_BYTES + 1024 + 256 + kEpiWarps * kScrFloats * 4;
   static constexpr int TMEM_COLS = 2 * BN < 32 ? 32 : 2 * BN;
 };
 
@@ -414,7 +425,7 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
     }
     for (int a = 0; a < 2; ++a) {
       mbar_init(tfull_bar(a), 1);   // tcgen05.commit (multicast)
-      mbar_init(tempty_bar(a), 8);  // 4 epilogue warps x 2 CTAs
+      mbar_init(tempty_bar(a), 2 * kEpiWarps);  // epilogue warps of both CTAs
     }
     fence_barrier_init();
   }
@@ -428,25 +439,26 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
 
-  if (warp == 0) {
-    if (lane == 0) {  // ---------------- TMA producer (both CTAs; completion counted in the leader)
-      int s = 0;
-      uint32_t ph = 0;
-      for (int t = pair; t < n_tiles; t += n_pairs) {
-        const int m0 = (t % n_m) * (2 * BM) + (int)rank * BM, n0 = (t / n_m) * BN + (int)rank * (BN / 2);
-        for (int kb = 0; kb < n_kb; ++kb) {
-          mbar_wait(empty_bar(s), ph ^ 1);
+  if (warp == 0) {  // ---------------- TMA producer (both CTAs; completion counted in the leader)
+    int s = 0;
+    uint32_t ph = 0;
+    for (int t = pair; t < n_tiles; t += n_pairs) {
+      const int m0 = (t % n_m) * (2 * BM) + (int)rank * BM, n0 = (t / n_m) * BN + (int)rank * (BN / 2);
+      for (int kb = 0; kb < n_kb; ++kb) {
+        mbar_wait(empty_bar(s), ph ^ 1);
+        if (elect_one()) {
           const uint32_t lfull = mapa_shared(full_bar(s), 0);
           mbar_expect_tx_cluster(lfull, Cfg::STAGE_BYTES);
           const uint32_t a_dst = smem_base + s * Cfg::STAGE_BYTES;
           tma_load_2d_cg2(a_dst, &tmA, lfull, kb * BK, m0);
           tma_load_2d_cg2(a_dst + Cfg::A_BYTES, &tmB, lfull, kb * BK, n0);
-          if (++s == Cfg::STAGES) { s = 0; ph ^= 1; }
         }
+        __syncwarp();
+        if (++s == Cfg::STAGES) { s = 0; ph ^= 1; }
       }
     }
   } else if (warp == 1) {
-    if (lane == 0 && rank == 0) {  // ---------------- MMA issuer (leader CTA only)
+    if (rank == 0) {  // ---------------- MMA issuer (leader CTA only)
       const uint32_t idesc =
           ea.in_fp16 ? (make_idesc_bf16(2 * BM, BN) & ~((1u << 7) | (1u << 10))) : make_idesc_bf16(2 * BM, BN);
       int s = 0, it = 0;
@@ -460,24 +472,28 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
         for (int kb = 0; kb < n_kb; ++kb) {
           mbar_wait(full_bar(s), ph);
           tc_fence_after();
-          const uint32_t a_addr = smem_base + s * Cfg::STAGE_BYTES;
-          const uint32_t b_addr = a_addr + Cfg::A_BYTES;
-          if (!(ea.dbg & 2)) {
+          if (elect_one()) {
+            const uint32_t a_addr = smem_base + s * Cfg::STAGE_BYTES;
+            const uint32_t b_addr = a_addr + Cfg::A_BYTES;
+            if (!(ea.dbg & 2)) {
 #pragma unroll
-            for (int kk = 0; kk < BK / 16; ++kk) {
-              umma_bf16_cg2(d_tmem, make_sdesc_k128(a_addr + kk * 32), make_sdesc_k128(b_addr + kk * 32), idesc,
-                            (kb | kk) != 0);
+              for (int kk = 0; kk < BK / 16; ++kk) {
+                umma_bf16_cg2(d_tmem, make_sdesc_k128(a_addr + kk * 32), make_sdesc_k128(b_addr + kk * 32), idesc,
+                              (kb | kk) != 0);
+              }
             }
+            umma_commit_cg2(empty_bar(s));
+            if (kb == n_kb - 1) umma_commit_cg2(tfull_bar(acc));
           }
-          umma_commit_cg2(empty_bar(s));
+          __syncwarp();
           if (++s == Cfg::STAGES) { s = 0; ph ^= 1; }
         }
-        umma_commit_cg2(tfull_bar(acc));
       }
     }
-  } else {  // ---------------- epilogue warps 2..5 (both CTAs, each on its own 128 rows)
+  } else {  // ---------------- epilogue warps 2..9 (both CTAs, each on its own 128 rows)
     const int q = warp & 3;
-    float* scr = reinterpret_cast<float*>(smem_raw + (bar_base + 256u - smem_u32(smem_raw))) + q * kScrFloats;
+    const int half = (warp - 2) >> 2;
+    float* scr = reinterpret_cast<float*>(smem_raw + (bar_base + 256u - smem_u32(smem_raw))) + (warp - 2) * kScrFloats;
     int it = 0;
     for (int t = pair; t < n_tiles; t += n_pairs, ++it) {
       const int acc = it & 1;
@@ -496,7 +512,7 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
         release();
         continue;
       }
-      epilogue_tile<BN, EPI>(ea, scr, t_acc, r0, n0, m_lim, N, lane, release);
+      epilogue_tile<BN, EPI>(ea, scr, t_acc, r0, n0, m_lim, N, lane, half, release);
     }
   }
   tc_fence_before();
@@ -568,11 +584,13 @@ int num_sms() {
 bool tc_gemm_supported(int N, int K) { return N % 64 == 0 && K % 64 == 0 && N >= 64; }
 // CTA pairs (256-row tiles) once there is more than one 128-row tile of tokens
 static bool use_pair(int M) { return M > BM; }
-// N tile of the EPI_BIAS_F32 / EPI_RESID launches (= columns per sum-of-squares partial)
-int tc_resid_bn(int N, int M) {
+// N tile of the EPI_BIAS_F32 / EPI_RESID launches
+static int resid_bn(int N, int M) {
   if (use_pair(M) && N % 256 == 0) return 256;
   return N % 128 == 0 ? 128 : 64;
 }
+// columns per sum-of-squares partial written by those launches (half an N tile: two epilogue warps per row)
+int tc_ssq_cols(int N, int M) { return resid_bn(N, M) / 2; }
 
 template <int BN, int EPI>
 static cudaError_t launch_one(const op16* A, const op16* W, int M, int N, int K, const EpiArgs& a, cudaStream_t s) {
@@ -616,7 +634,7 @@ template <int EPI>
 static cudaError_t launch_by_n(const op16* A, const op16* W, int M, int N, int K, const EpiArgs& a, cudaStream_t s) {
   const int forced = a.dbg >> 8;  // rosa_debug_gemm only: 1xx = single-CTA kernel, N tile xx0
   const bool pair = forced ? forced / 1000 == 2 : use_pair(M);
-  const int bn = forced ? forced % 1000 : tc_resid_bn(N, M);
+  const int bn = forced ? forced % 1000 : resid_bn(N, M);
   if (pair) {
     if (bn == 256) return launch_two<256, EPI>(A, W, M, N, K, a, s);
     if (bn == 128) return launch_two<128, EPI>(A, W, M, N, K, a, s);

@@ -302,7 +302,7 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
   WS(e->mact, Mmax * F * 2);
   WS(e->scratch, Mmax * (size_t)std::max(2 * F, dm.qkv_n) * 4);
   WS(e->e2e_dev, (size_t)c->max_batch * HA * 4);
-  WS(e->ssq, Mmax * (d / 64) * 4);
+  WS(e->ssq, Mmax * (d / 32) * 4);
   CK(cudaMemset(e->zbuf, 0, Mmax * d * 2));
   CK(cudaMemset(e->nrm, 0, Mmax * d * 2));
   CK(cudaMemset(e->qkv, 0, Mmax * dm.qkv_n * 2));
@@ -396,7 +396,7 @@ static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, cudaStream_
     EpiArgs ea{};
     ea.m_active = tb.m_active + k;
     ea.H = dm.H; ea.hd = dm.hd; ea.gu_blk = dm.gu_blk; ea.in_fp16 = dm.fp16; ea.out_fp16 = dm.fp16;
-    ea.inv_d = 1.f / (float)d; ea.eps = dm.eps; ea.n_part = d / tc_resid_bn(d, M);
+    ea.inv_d = 1.f / (float)d; ea.eps = dm.eps; ea.n_part = d / tc_ssq_cols(d, M);
     if (fused_norm) { ea.h16 = e->nrm; ea.ssq_out = e->ssq; ea.ssq_in = e->ssq; }
     // a1: h0 = W2 swish(W1 [tau ; W_in x + b_in] + b1) + b2
     mark(e, ROSA_KC_INPROJ, s);
