@@ -158,7 +158,7 @@ rosa_status_t rosa_debug_gemm(int32_t family, int32_t M, int32_t N, int32_t K, c
                               const void *W_bf16, float *C, void *stream);
 
 /* Measurement aid: with the environment variable ROSA_DBG bit 4 set, the attention kernel records
- * clock64() at its pipeline events for two CTAs; this copies [2][8 roles][32 key blocks] int64 values
+ * clock64() at its pipeline events for two CTAs; this copies [2][16 roles][32 key blocks] int64 values
  * of the last launch to host_out and returns the count (0 if tracing is off). */
 int32_t rosa_debug_attn_trace(int64_t *host_out, int32_t n);
 

@@ -236,7 +236,7 @@ def rosa_debug_gemm(family: int, M: int, N: int, K: int, A_bf16, W_bf16, C_f32, 
 
 
 def rosa_debug_attn_trace() -> np.ndarray:
-    buf = np.zeros((2, 8, 32), dtype=np.int64)
+    buf = np.zeros((2, 16, 32), dtype=np.int64)
     load().rosa_debug_attn_trace(_ptr(buf), buf.size)
     return buf
 

@@ -32,10 +32,11 @@ constexpr int AT_KV = 64;         // keys per block
 constexpr int AT_KST = 4;         // K stages (K runs one block further ahead than V)
 constexpr int AT_ST = 3;          // V stages
 constexpr int AT_PF = 6;          // L2 prefetch distance in blocks
-constexpr int AT_THREADS = 192;   // warp 0 TMA, warp 1 MMA, warps 2..5 softmax/epilogue
+constexpr int AT_THREADS = 320;   // warp 0 TMA, warp 1 MMA, warps 2..9 softmax/epilogue (two per TMEM lane quarter)
 constexpr int AT_Q_BYTES = AT_ROWS * AT_HD * 2;     // 64 KB: 4 chunks [128 x 64] SW128
 constexpr int AT_KV_BYTES = AT_KV * AT_HD * 2;      // 32 KB: 4 chunks [64 x 64] SW128
-constexpr int AT_SMEM = (AT_KST + AT_ST) * AT_KV_BYTES + 1024 + 256;
+constexpr int AT_XCH_BYTES = 2 * 2 * AT_ROWS * 4;   // row-maximum / row-sum exchange between the two warps of a row
+constexpr int AT_SMEM = (AT_KST + AT_ST) * AT_KV_BYTES + 256 + AT_XCH_BYTES;
 constexpr float AT_RESCALE_THR = 8.0f;              // log2 units
 
 // exp2 on the SFU without the denormal-range fix-up sequence of exp2f (inputs here are <= 2^8)
@@ -43,36 +44,6 @@ __device__ __forceinline__ float ex2_approx(float x) {
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
-}
-
-// One 64-key block of one query row: running reference m_ref (log2 units, lazily raised), P = exp2(s c - m_ref)
-// as packed bf16 pairs, and the fp32 sum of the unrounded P.
-template <bool MASKED>
-__device__ __forceinline__ void softmax_block(float (&sc)[AT_KV], int n_valid, float c_log2, float& m_ref, float& factor,
-                                              float& psum, uint32_t (&pk)[AT_KV / 2]) {
-  if (MASKED) {
-#pragma unroll
-    for (int c = 0; c < AT_KV; ++c) sc[c] = c < n_valid ? sc[c] : -INFINITY;
-  }
-  float m_blk = sc[0];
-#pragma unroll
-  for (int c = 1; c < AT_KV; ++c) m_blk = fmaxf(m_blk, sc[c]);
-  m_blk *= c_log2;
-  if (m_blk > m_ref + AT_RESCALE_THR) {            // first block always lands here
-    factor = ex2_approx(m_ref - m_blk);            // 0 on the first block (m_ref = -inf)
-    m_ref = m_blk;
-  }
-  const float neg_m = -m_ref;
-  float s0 = 0.f, s1 = 0.f;
-#pragma unroll
-  for (int c = 0; c < AT_KV; c += 2) {
-    const float a = ex2_approx(fmaf(sc[c], c_log2, neg_m)), b = ex2_approx(fmaf(sc[c + 1], c_log2, neg_m));
-    s0 += a;
-    s1 += b;
-    __nv_bfloat162 v2 = __floats2bfloat162_rn(a, b);
-    pk[c >> 1] = *reinterpret_cast<uint32_t*>(&v2);
-  }
-  psum = s0 + s1;
 }
 
 struct AttnMaps {
@@ -83,14 +54,14 @@ struct AttnMaps {
 __global__ void __launch_bounds__(AT_THREADS, 1)
 k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__ kv_maps, Dims dm, Tables tb,
           int layer, op16* __restrict__ o, int k_iter, int tiles_per_robot, int dbg, long long* __restrict__ trace) {
-  extern __shared__ uint8_t smem_raw[];
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
   const int p = blockIdx.x / tiles_per_robot, tt = blockIdx.x % tiles_per_robot;
   if (p * dm.H >= tb.m_active[k_iter]) return;
   const int robot = tb.ids[p], L = tb.rlen[robot];
   const int nbp = (L + AT_KV - 1) / AT_KV, nb = nbp + 1;  // prefix blocks + one block of own tokens
 
-  const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  if ((dbg & 16) && threadIdx.x == 0 && (blockIdx.x == 0 || blockIdx.x == 200)) trace[((blockIdx.x == 0 ? 0 : 1) * 8 + 7) * 32] = clock64();
+  const uint32_t base = smem_u32(smem_raw);  // 1024-byte aligned (SWIZZLE_128B tiles)
+  if ((dbg & 16) && threadIdx.x == 0 && (blockIdx.x == 0 || blockIdx.x == 200)) trace[((blockIdx.x == 0 ? 0 : 1) * 16 + 7) * 32] = clock64();
   auto k_smem = [&](int s) { return base + (uint32_t)s * AT_KV_BYTES; };
   auto v_smem = [&](int s) { return base + (uint32_t)(AT_KST + s) * AT_KV_BYTES; };
   const uint32_t q_smem = k_smem(AT_KST - 2);  // Q passes through the last two K stages before block AT_KST-2 needs them
@@ -111,7 +82,7 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   // measurement aid (ROSA_DBG bit 4): clock64 at pipeline events of CTAs 0 and 200 -> trace[slot][role][block]
   const int tslot = (dbg & 16) ? (blockIdx.x == 0 ? 0 : (blockIdx.x == 200 ? 1 : -1)) : -1;
-#define AT_TRACE(role, blk) do { if (tslot >= 0 && (blk) < 32) trace[(tslot * 8 + (role)) * 32 + (blk)] = clock64(); } while (0)
+#define AT_TRACE(role, blk) do { if (tslot >= 0 && (blk) < 32) trace[(tslot * 16 + (role)) * 32 + (blk)] = clock64(); } while (0)
   const CUtensorMap* kmap = kv_maps + ((size_t)robot * dm.layers + layer) * 2;
   const CUtensorMap* vmap = kmap + 1;
 
@@ -121,10 +92,10 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
     for (int s = 0; s < AT_KST; ++s) { mbar_init(k_full(s), 1); mbar_init(k_empty(s), 1); }
     for (int s = 0; s < AT_ST; ++s) { mbar_init(v_full(s), 1); mbar_init(v_empty(s), 1); }
     mbar_init(s_full(0), 1); mbar_init(s_full(1), 1);
-    mbar_init(p_full(0), 128); mbar_init(p_full(1), 128);
+    mbar_init(p_full(0), 8); mbar_init(p_full(1), 8);  // one arrival per softmax warp
     mbar_init(pv_done, 1);
     mbar_init(q_full, 1);
-    mbar_init(q_done, 128);
+    mbar_init(q_done, 8);
     fence_barrier_init();
   }
   if (warp == 1) {
@@ -140,6 +111,8 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
   const uint32_t tmem_q = tmem_base + 384;      // columns [384, 512): Q, 256 bf16 per row
 
   const int tok0 = p * dm.H + tt * AT_TOK;      // first token row of this tile in the qkv buffer
+  pdl_wait();     // everything above overlapped the previous kernel's tail
+  pdl_trigger();
 
   if (warp == 0) {
     {  // ------------------------------------------------ TMA producer (whole warp; one lane issues)
@@ -152,10 +125,11 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
         if (i == AT_KST - 2) mbar_wait(q_done, 0);  // Q has left the last two K stages
         mbar_wait(k_empty(s), ((i / AT_KST) & 1) ^ 1);
         if (elect_one()) {
-          prefetch_blk(i + AT_PF);
           mbar_expect_tx(k_full(s), AT_KV_BYTES);
           if (i == nbp) tma_load_3d(k_smem(s), &maps.own, k_full(s), 0, p * dm.H, dm.q_n / 64);
           else tma_load_3d(k_smem(s), kmap, k_full(s), 0, i * AT_KV, 0);
+          if (i == 1) for (int j = 2; j < AT_PF; ++j) prefetch_blk(j);
+          if (i >= 1) prefetch_blk(i + AT_PF - 1);
           AT_TRACE(0, i);
         }
         __syncwarp();
@@ -163,10 +137,9 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
       if (elect_one()) {
         mbar_expect_tx(q_full, AT_Q_BYTES);
         for (int c = 0; c < 4; ++c) tma_load_3d(q_smem + c * (AT_ROWS * 128), &maps.q, q_full, c * 64, 0, tok0);
-        for (int i = 0; i < AT_PF; ++i) prefetch_blk(i);
       }
       __syncwarp();
-      load_k(0);
+      load_k(0);  // what the first MMAs need goes out before any prefetch
       for (int i = 0; i < nb; ++i) {  // K runs one block ahead of V: it is needed a whole softmax earlier
         if (i + 1 < nb) load_k(i + 1);
         const int s = i % AT_ST;
@@ -231,14 +204,18 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
       }
     }
   } else {
-    // ---------------------------------------------------------- softmax + epilogue warps
-    const int q = warp & 3;
+    // ---------------------------------------------------------- softmax + epilogue warps (2..9)
+    // Two warps per TMEM lane quarter: a query row's 64 scores of a block are split 32 / 32 between
+    // warp w (half 0) and warp w + 4 (half 1).  They exchange the row maximum through shared memory
+    // (so both take the same rescale decision) and keep separate partial row sums until the end.
+    const int q = warp & 3, half = (warp - 2) >> 2;
     const int r = q * 32 + lane;                       // query row of this thread
     const uint32_t lane_off = (uint32_t)(q * 32) << 16;
-    {  // Q: shared memory (SW128: 4 chunks of [128 rows x 128 B]) -> tensor memory, thread = row
+    float* xch = reinterpret_cast<float*>(smem_raw + ((AT_KST + AT_ST) * AT_KV_BYTES + 256));  // [2 buffers][2 halves][128]
+    {  // Q: shared memory (SW128: 4 chunks of [128 rows x 128 B]) -> tensor memory, thread = row, 2 chunks per half
       mbar_wait(q_full, 0);
 #pragma unroll 1
-      for (int cc = 0; cc < 4; ++cc) {
+      for (int cc = half * 2; cc < half * 2 + 2; ++cc) {
         uint32_t w[32];
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
@@ -250,42 +227,69 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
       }
       tmem_st_wait();
       tc_fence_before();
-      mbar_arrive(q_done);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(q_done);
     }
     const float c_log2 = rsqrtf((float)AT_HD) * 1.4426950408889634f;  // (1/sqrt(hd)) * log2(e)
-    float m_ref = -INFINITY, l_sum = 0.f;                             // m_ref in log2 units
+    float m_ref = -INFINITY, l_sum = 0.f;                             // m_ref in log2 units; l_sum: this half's part
     for (int i = 0; i < nb; ++i) {
       const int sb = i & 1;
-      const int n_valid = i == nbp ? dm.H : min(AT_KV, L - i * AT_KV);
+      const int n_valid = (i == nbp ? dm.H : min(AT_KV, L - i * AT_KV)) - half * 32;  // valid columns of this half
       mbar_wait(s_full(sb), (i >> 1) & 1);
       tc_fence_after();
       if (threadIdx.x == 64) AT_TRACE(4, i);
-      float sc[AT_KV];
+      float sc[32];
       {
-        uint32_t r0[32], r1[32];
-        tmem_ld32(tmem_s + lane_off + sb * AT_KV, r0);
-        tmem_ld32(tmem_s + lane_off + sb * AT_KV + 32, r1);
+        uint32_t r0[32];
+        tmem_ld32(tmem_s + lane_off + sb * AT_KV + half * 32, r0);
         tmem_ld_wait();
 #pragma unroll
-        for (int c = 0; c < 32; ++c) { sc[c] = __uint_as_float(r0[c]); sc[32 + c] = __uint_as_float(r1[c]); }
+        for (int c = 0; c < 32; ++c) sc[c] = __uint_as_float(r0[c]);
       }
-      float factor = 1.f, psum;
-      uint32_t pk[AT_KV / 2];
-      // two copies of the block arithmetic, so the 13-of-14 full blocks pay no per-element masking
-      if (dbg & 4) {  // measurement aid: no softmax arithmetic
-        psum = 1.f;
+      if (threadIdx.x == 64) AT_TRACE(8, i);
+      if (n_valid < 32) {  // warp-uniform; only the last prefix block and the own-token block
 #pragma unroll
-        for (int c = 0; c < AT_KV / 2; ++c) pk[c] = __float_as_uint(sc[2 * c]);
-      } else if (n_valid < AT_KV) softmax_block<true>(sc, n_valid, c_log2, m_ref, factor, psum, pk);
-      else softmax_block<false>(sc, n_valid, c_log2, m_ref, factor, psum, pk);
-      l_sum = l_sum * factor + psum;
+        for (int c = 0; c < 32; ++c) sc[c] = c < n_valid ? sc[c] : -INFINITY;
+      }
+      float m_blk = sc[0];
+#pragma unroll
+      for (int c = 1; c < 32; ++c) m_blk = fmaxf(m_blk, sc[c]);
+      xch[(sb * 2 + half) * AT_ROWS + r] = m_blk;
+      named_bar_sync(1 + q, 64);
+      m_blk = fmaxf(m_blk, xch[(sb * 2 + (half ^ 1)) * AT_ROWS + r]) * c_log2;
+      if (threadIdx.x == 64) AT_TRACE(9, i);
+      float factor = 1.f;
+      if (m_blk > m_ref + AT_RESCALE_THR) {            // first block always lands here
+        factor = ex2_approx(m_ref - m_blk);            // 0 on the first block (m_ref = -inf)
+        m_ref = m_blk;
+      }
+      uint32_t pk[16];
+      float s0 = 0.f, s1 = 0.f;
+      if (dbg & 4) {  // measurement aid: no softmax arithmetic
+        s0 = 1.f;
+#pragma unroll
+        for (int c = 0; c < 16; ++c) pk[c] = __float_as_uint(sc[2 * c]);
+      } else {
+        const float neg_m = -m_ref;
+#pragma unroll
+        for (int c = 0; c < 32; c += 2) {
+          const float a = ex2_approx(fmaf(sc[c], c_log2, neg_m)), b = ex2_approx(fmaf(sc[c + 1], c_log2, neg_m));
+          s0 += a;
+          s1 += b;
+          __nv_bfloat162 v2 = __floats2bfloat162_rn(a, b);
+          pk[c >> 1] = *reinterpret_cast<uint32_t*>(&v2);
+        }
+      }
+      l_sum = l_sum * factor + (s0 + s1);
+      if (threadIdx.x == 64) AT_TRACE(10, i);
       // Every block, not only when rescaling: a parity wait is only meaningful while the waiter is at
       // most one phase behind the barrier (PV(i-1) was issued ~a softmax block ago, so this is free).
       if (i > 0) mbar_wait(pv_done, (i - 1) & 1);
-      if (i > 0 && __any_sync(0xffffffffu, factor != 1.f)) {  // rare: rescale this warp's 32 rows of O
+      if (threadIdx.x == 64) AT_TRACE(11, i);
+      if (i > 0 && __any_sync(0xffffffffu, factor != 1.f)) {  // rare: rescale this warp's rows, its half of O's columns
         tc_fence_after();                                     // O quiescent: PV(i-1) done, PV(i) needs this P
 #pragma unroll 1
-        for (int c = 0; c < AT_HD / 32; ++c) {
+        for (int c = half * 4; c < half * 4 + 4; ++c) {
           uint32_t rr[32];
           tmem_ld32(tmem_o + lane_off + c * 32, rr);
           tmem_ld_wait();
@@ -294,42 +298,52 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
           tmem_st32(tmem_o + lane_off + c * 32, rr);
         }
       }
-      // P row r (64 bf16 = 32 columns) over the first half of S(i): the A operand of PV(i)
-      tmem_st32(tmem_s + lane_off + sb * AT_KV, pk);
+      // P row r, this half's 32 keys (16 columns of bf16 pairs) over the start of S(i): the A operand of PV(i)
+      tmem_st16(tmem_s + lane_off + sb * AT_KV + half * 16, pk);
       tmem_st_wait();
       tc_fence_before();
-      mbar_arrive(p_full(sb));
+      __syncwarp();
+      if (lane == 0) mbar_arrive(p_full(sb));  // 256 arrivals on one barrier would serialise on the critical path
       if (threadIdx.x == 64) AT_TRACE(5, i);
     }
-    // epilogue: O / l -> o[(token, head)]; row r = (token jj, head a) with r = jj * 8 + a.  Transposed
-    // through shared memory (stage 0 is free: every MMA has completed) for coalesced row stores.
+    // epilogue: O / l -> o[(token, head)]; row r = (token jj, head a) with r = jj * 8 + a.  Each half
+    // stores 128 of the 256 columns, transposed through shared memory (the K stages are free: every
+    // MMA has completed) for coalesced row stores.
     mbar_wait(pv_done, (nb - 1) & 1);
     tc_fence_after();
     if (threadIdx.x == 64) AT_TRACE(6, 1);
-    const float inv = 1.f / l_sum;
-    float* scr = reinterpret_cast<float*>(smem_raw + (base - smem_u32(smem_raw))) + q * (32 * 66);
+    xch[half * AT_ROWS + r] = l_sum;
+    named_bar_sync(1 + q, 64);
+    const float inv = 1.f / (l_sum + xch[(half ^ 1) * AT_ROWS + r]);
+    // 32 x 32 chunks through a private scratch (pitch 36 floats), then 8 lanes x 4 columns per row
+    constexpr int P = 36;
+    float* scr = reinterpret_cast<float*>(smem_raw) + (warp - 2) * (32 * P);
+    const int lr = lane >> 3, lc = (lane & 7) * 4;
+    size_t orow[8];   // output row offsets of the 8 rows this lane stores per chunk; -1 = padding row
+#pragma unroll
+    for (int x = 0; x < 8; ++x) {
+      const int row = q * 32 + x * 4 + lr, j = tt * AT_TOK + (row >> 3);
+      orow[x] = j < dm.H ? (size_t)(p * dm.H + j) * dm.q_n + (row & 7) * AT_HD + lc : (size_t)-1;
+    }
 #pragma unroll 1
-    for (int pass = 0; pass < AT_HD / 64; ++pass) {
+    for (int c = half * 4; c < half * 4 + 4; ++c) {
+      uint32_t rr[32];
+      tmem_ld32(tmem_o + lane_off + c * 32, rr);
+      tmem_ld_wait();
 #pragma unroll
-      for (int hh = 0; hh < 2; ++hh) {
-        uint32_t rr[32];
-        tmem_ld32(tmem_o + lane_off + pass * 64 + hh * 32, rr);
-        tmem_ld_wait();
-#pragma unroll
-        for (int e = 0; e < 32; e += 2)
-          *reinterpret_cast<float2*>(&scr[lane * 66 + hh * 32 + e]) =
-              make_float2(__uint_as_float(rr[e]) * inv, __uint_as_float(rr[e + 1]) * inv);
-      }
+      for (int e = 0; e < 32; e += 4)
+        *reinterpret_cast<float4*>(&scr[lane * P + e]) =
+            make_float4(__uint_as_float(rr[e]) * inv, __uint_as_float(rr[e + 1]) * inv, __uint_as_float(rr[e + 2]) * inv,
+                        __uint_as_float(rr[e + 3]) * inv);
       __syncwarp();
-      float2 ov[32];
+      float4 ov[8];
 #pragma unroll
-      for (int x = 0; x < 32; ++x) ov[x] = *reinterpret_cast<const float2*>(&scr[x * 66 + 2 * lane]);
+      for (int x = 0; x < 8; ++x) ov[x] = *reinterpret_cast<const float4*>(&scr[(x * 4 + lr) * P + lc]);
 #pragma unroll
-      for (int x = 0; x < 32; ++x) {
-        const int row = q * 32 + x, j = tt * AT_TOK + (row >> 3);
-        if (j < dm.H)
-          *reinterpret_cast<uint32_t*>(o + (size_t)(p * dm.H + j) * dm.q_n + (row & 7) * AT_HD + pass * 64 + 2 * lane) =
-              pack_op2(ov[x].x, ov[x].y, dm.fp16);
+      for (int x = 0; x < 8; ++x) {
+        if (orow[x] != (size_t)-1)
+          *reinterpret_cast<uint2*>(o + orow[x] + c * 32) =
+              make_uint2(pack_op2(ov[x].x, ov[x].y, dm.fp16), pack_op2(ov[x].z, ov[x].w, dm.fp16));
       }
       __syncwarp();
     }
@@ -348,7 +362,7 @@ static long long* g_attn_trace = nullptr;
 // copies the last trace (ROSA_DBG bit 4) to host: [2 CTAs][8 roles][32 blocks] clock64 values
 int tc_attn_read_trace(long long* host, int n) {
   if (!g_attn_trace) return 0;
-  if (n > 2 * 8 * 32) n = 2 * 8 * 32;
+  if (n > 2 * 16 * 32) n = 2 * 16 * 32;
   cudaMemcpy(host, g_attn_trace, n * sizeof(long long), cudaMemcpyDeviceToHost);
   return n;
 }
@@ -390,10 +404,9 @@ cudaError_t launch_attn_tc(const Dims& dm, const Tables& tb, int layer, const bf
   const int tpr = (dm.H + AT_TOK - 1) / AT_TOK;
   static int dbg = -1;  // ROSA_DBG bits 2-4: measurement aids (skip softmax arithmetic / skip the MMAs / trace)
   if (dbg < 0) { const char* e = getenv("ROSA_DBG"); dbg = e ? atoi(e) : 0; }
-  if ((dbg & 16) && !g_attn_trace) cudaMalloc((void**)&g_attn_trace, 2 * 8 * 32 * sizeof(long long));
-  k_attn_tc<<<tb.batch * tpr, AT_THREADS, AT_SMEM, s>>>(maps, (const CUtensorMap*)d_kv_maps, dm, tb, layer, o,
-                                                       k_iter, tpr, dbg, g_attn_trace);
-  return cudaGetLastError();
+  if ((dbg & 16) && !g_attn_trace) cudaMalloc((void**)&g_attn_trace, 2 * 16 * 32 * sizeof(long long));
+  return launch_k(k_attn_tc, dim3(tb.batch * tpr), dim3(AT_THREADS), AT_SMEM, s, maps, (const CUtensorMap*)d_kv_maps, dm,
+                  tb, layer, o, k_iter, tpr, dbg, g_attn_trace);
 }
 
 }  // namespace rosa

@@ -7,6 +7,13 @@
 
 namespace rosa {
 
+// Programmatic dependent launch: every kernel of the call is launched with the attribute (rosa_internal.h
+// launch_k), so its prologue overlaps the tail of the previous kernel.  pdl_wait() returns when the
+// previous kernel in the stream has completed and its writes are visible; nothing that depends on or
+// overwrites earlier kernels' data may happen before it.  pdl_trigger() lets the next kernel start launching.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);

@@ -293,6 +293,8 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
+  pdl_wait();     // everything above overlapped the previous kernel's tail
+  pdl_trigger();
 
   // Role loops run with whole warps (warp-uniform state stays in uniform registers); only the
   // TMA / tcgen05 issue is fenced to one elected lane.
@@ -438,6 +440,8 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
   cluster_sync_all();  // the peer's barriers are initialised before anything is signalled on them
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
+  pdl_wait();     // everything above overlapped the previous kernel's tail
+  pdl_trigger();
 
   if (warp == 0) {  // ---------------- TMA producer (both CTAs; completion counted in the leader)
     int s = 0;
@@ -607,8 +611,7 @@ static cudaError_t launch_one(const op16* A, const op16* W, int M, int N, int K,
     return cudaErrorInvalidValue;
   const int tiles = ((M + BM - 1) / BM) * (N / BN);
   const int grid = tiles < num_sms() ? tiles : num_sms();
-  k_gemm_tc<BN, EPI><<<grid, kGemmThreads, Cfg::SMEM, s>>>(tmA, tmB, M, N, K, a);
-  return cudaGetLastError();
+  return launch_k(k_gemm_tc<BN, EPI>, dim3(grid), dim3(kGemmThreads), Cfg::SMEM, s, tmA, tmB, M, N, K, a);
 }
 
 template <int BN, int EPI>
@@ -626,8 +629,7 @@ static cudaError_t launch_two(const op16* A, const op16* W, int M, int N, int K,
     return cudaErrorInvalidValue;
   const int tiles = ((M + 2 * BM - 1) / (2 * BM)) * (N / BN);
   const int pairs = tiles < num_sms() / 2 ? tiles : num_sms() / 2;
-  k_gemm_tc2<BN, EPI><<<2 * pairs, kGemmThreads, Cfg::SMEM, s>>>(tmA, tmB, M, N, K, a);
-  return cudaGetLastError();
+  return launch_k(k_gemm_tc2<BN, EPI>, dim3(2 * pairs), dim3(kGemmThreads), Cfg::SMEM, s, tmA, tmB, M, N, K, a);
 }
 
 template <int EPI>

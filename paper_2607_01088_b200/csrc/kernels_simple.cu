@@ -9,20 +9,24 @@ namespace rosa {
 
 // ------------------------------------------------------------------ x gather / scatter
 __global__ void k_gather_x(float* __restrict__ x, const CallPtrs* __restrict__ cp, Tables tb, int HA) {
+  pdl_wait();
+  pdl_trigger();
   int p = blockIdx.x;
   const float* s = cp->noise + (size_t)tb.src[p] * HA;
   for (int i = threadIdx.x; i < HA; i += blockDim.x) x[(size_t)p * HA + i] = s[i];
 }
 __global__ void k_scatter_x(const CallPtrs* __restrict__ cp, const float* __restrict__ x, Tables tb, int HA) {
+  pdl_wait();
+  pdl_trigger();
   int p = blockIdx.x;
   float* d = cp->out + (size_t)tb.src[p] * HA;
   for (int i = threadIdx.x; i < HA; i += blockDim.x) d[i] = x[(size_t)p * HA + i];
 }
 void launch_gather_x(float* x, const CallPtrs* cp, const Tables& tb, int HA, cudaStream_t s) {
-  k_gather_x<<<tb.batch, 128, 0, s>>>(x, cp, tb, HA);
+  launch_k(k_gather_x, dim3(tb.batch), dim3(128), 0, s, x, cp, tb, HA);
 }
 void launch_scatter_x(const CallPtrs* cp, const float* x, const Tables& tb, int HA, cudaStream_t s) {
-  k_scatter_x<<<tb.batch, 128, 0, s>>>(cp, x, tb, HA);
+  launch_k(k_scatter_x, dim3(tb.batch), dim3(128), 0, s, cp, x, tb, HA);
 }
 
 // ------------------------------------------------------------------ a1 (time half), hoisted
@@ -32,6 +36,8 @@ void launch_scatter_x(const CallPtrs* cp, const float* x, const Tables& tb, int 
 __global__ void k_timevec(float* __restrict__ tvec, const bf16* __restrict__ w_t1,
                           const float* __restrict__ b_t1, Dims dm, Tables tb, int max_batch) {
   extern __shared__ float tau[];  // [d]
+  pdl_wait();
+  pdl_trigger();
   const int p = blockIdx.x, k = blockIdx.y, d = dm.d, half = d / 2;
   if (k >= tb.nsteps[p]) return;
   const double t = (double)tb.t0[p] + (double)k * (double)tb.dt[p];
@@ -57,7 +63,7 @@ __global__ void k_timevec(float* __restrict__ tvec, const bf16* __restrict__ w_t
 void launch_timevec(float* tvec, const bf16* w_t1, const float* b_t1, const Dims& dm,
                     const Tables& tb, int nsteps_max, int max_batch, cudaStream_t s) {
   dim3 grid(tb.batch, nsteps_max);
-  k_timevec<<<grid, 256, dm.d * sizeof(float), s>>>(tvec, w_t1, b_t1, dm, tb, max_batch);
+  launch_k(k_timevec, grid, dim3(256), dm.d * sizeof(float), s, tvec, w_t1, b_t1, dm, tb, max_batch);
 }
 
 // ------------------------------------------------------------------ a1 (action half + swish)
@@ -71,6 +77,8 @@ __global__ void __launch_bounds__(256) k_embed1(op16* __restrict__ z, const floa
                                                 const float* __restrict__ tvec, int d, int A, int H, int fp16,
                                                 const int* __restrict__ m_active) {
   __shared__ float xs[EM_ROWS][64];
+  pdl_wait();
+  pdl_trigger();
   const int m0 = blockIdx.x * EM_ROWS, m_lim = *m_active;
   if (m0 >= m_lim) return;
   const int rows = min(EM_ROWS, m_lim - m0);
@@ -98,8 +106,8 @@ __global__ void __launch_bounds__(256) k_embed1(op16* __restrict__ z, const floa
 }
 void launch_embed1(op16* z, const float* x, const float* wca, const float* bca, const float* tvec_k,
                    const Dims& dm, const Tables& tb, int k_iter, int M, cudaStream_t s) {
-  k_embed1<<<(M + EM_ROWS - 1) / EM_ROWS, 256, 0, s>>>(z, x, wca, bca, tvec_k, dm.d, dm.A, dm.H, dm.fp16,
-                                                     tb.m_active + k_iter);
+  launch_k(k_embed1, dim3((M + EM_ROWS - 1) / EM_ROWS), dim3(256), 0, s, z, x, wca, bca, tvec_k, dm.d, dm.A, dm.H, dm.fp16,
+           tb.m_active + k_iter);
 }
 
 // ------------------------------------------------------------------ a2 RMSNorm (R5)
@@ -142,6 +150,8 @@ __global__ void __launch_bounds__(256) k_final(float* __restrict__ x, const Call
                                                const float* __restrict__ h, const float* __restrict__ g,
                                                const bf16* __restrict__ w_out, const float* __restrict__ b_out,
                                                int d, int A, int H, float eps, Tables tb, int k_iter) {
+  pdl_wait();
+  pdl_trigger();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int m = blockIdx.x * (blockDim.x >> 5) + warp;
   if (m >= tb.m_active[k_iter]) return;
@@ -195,8 +205,8 @@ void launch_final(float* x, const CallPtrs* cp, const float* h, const float* g, 
                   const float* b_out, const Dims& dm, const Tables& tb, int k_iter, int M,
                   cudaStream_t s) {
   const int wpb = 8;
-  k_final<<<(M + wpb - 1) / wpb, wpb * 32, 0, s>>>(x, cp, h, g, w_out, b_out, dm.d, dm.A, dm.H,
-                                                  dm.eps, tb, k_iter);
+  launch_k(k_final, dim3((M + wpb - 1) / wpb), dim3(wpb * 32), 0, s, x, cp, h, g, w_out, b_out, dm.d, dm.A, dm.H,
+           dm.eps, tb, k_iter);
 }
 
 __global__ void k_f32_to_bf16(bf16* __restrict__ dst, const float* __restrict__ src, size_t n) {

@@ -14,6 +14,11 @@ namespace rosa {
 
 static thread_local std::string g_err = "";
 void set_error(const std::string& msg) { g_err = msg; }
+bool pdl_enabled() {
+  static int on = -1;
+  if (on < 0) { const char* e = getenv("ROSA_PDL"); on = !(e && !strcmp(e, "0")); }
+  return on != 0;
+}
 
 #define CK(call)                                                                      \
   do {                                                                                \

@@ -122,4 +122,19 @@ cudaError_t launch_attn_tc(const Dims& dm, const Tables& tb, int layer, const bf
 
 void set_error(const std::string& msg);
 
+// Kernel launch with the programmatic-stream-serialization attribute (PDL; ROSA_PDL=0 turns it off).
+// Only for kernels that call pdl_wait() before touching global data produced or consumed by earlier kernels.
+bool pdl_enabled();
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, Args&&... args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = pdl_enabled() ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 }  // namespace rosa
