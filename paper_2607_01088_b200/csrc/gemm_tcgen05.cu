@@ -379,6 +379,15 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
   }
 }
 
+// measurement aid (ROSA_DBG bit 6): clock64 at the phases of CTA 0 of the last pair-kernel launch
+__device__ long long g_gemm_trace[16];
+#define GT_TRACE(slot) do { if ((ea.dbg & 64) && blockIdx.x == 0 && lane == 0) g_gemm_trace[slot] = clock64(); } while (0)
+int tc_gemm_read_trace(long long* host, int n) {
+  if (n > 16) n = 16;
+  cudaMemcpyFromSymbol(host, g_gemm_trace, n * sizeof(long long));
+  return n;
+}
+
 // ------------------------------------------------------------------ CTA-pair variant (cta_group::2)
 // Pair tile 256 x BN: CTA r of the cluster holds A rows [m0 + 128 r, +128) and B rows
 // [n0 + (BN/2) r, +BN/2) of every k-block; ONE tcgen05.mma (M = 256) issued by the leader reads
@@ -413,6 +422,7 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t rank = cluster_ctarank();
+  if (warp == 0) GT_TRACE(0);
   const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
   const int m_lim = ea.m_active ? min(M, *ea.m_active) : M;
   const int n_m = (m_lim + 2 * BM - 1) / (2 * BM), n_n = N / BN;
@@ -440,8 +450,10 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
   cluster_sync_all();  // the peer's barriers are initialised before anything is signalled on them
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
+  if (warp == 0) GT_TRACE(1);
   pdl_wait();     // everything above overlapped the previous kernel's tail
   pdl_trigger();
+  if (warp == 0) GT_TRACE(2);
 
   if (warp == 0) {  // ---------------- TMA producer (both CTAs; completion counted in the leader)
     int s = 0;
@@ -476,6 +488,8 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
         for (int kb = 0; kb < n_kb; ++kb) {
           mbar_wait(full_bar(s), ph);
           tc_fence_after();
+          if (it == 0 && kb == 0) GT_TRACE(3);
+          if (kb == n_kb - 1) GT_TRACE(4);
           if (elect_one()) {
             const uint32_t a_addr = smem_base + s * Cfg::STAGE_BYTES;
             const uint32_t b_addr = a_addr + Cfg::A_BYTES;
@@ -516,12 +530,16 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
         release();
         continue;
       }
+      if (warp == 2) GT_TRACE(5);
       epilogue_tile<BN, EPI>(ea, scr, t_acc, r0, n0, m_lim, N, lane, half, release);
+      if (warp == 2) GT_TRACE(6);
     }
   }
   tc_fence_before();
   __syncthreads();
+  if (warp == 0) GT_TRACE(7);
   cluster_sync_all();  // the leader's MMAs read the peer's shared memory; nobody leaves early
+  if (warp == 0) GT_TRACE(8);
   if (warp == 1) {
     tc_fence_after();
     tmem_dealloc_cg2(tmem_base, Cfg::TMEM_COLS);

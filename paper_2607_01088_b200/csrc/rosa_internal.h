@@ -115,6 +115,7 @@ cudaError_t launch_gemm_tc(Epi epi, const op16* A, const op16* W, int M, int N, 
 // tcgen05 attention (attn_tcgen05.cu)
 bool tc_attn_supported(const Dims& dm);
 int tc_attn_read_trace(long long* host, int n);
+int tc_gemm_read_trace(long long* host, int n);
 size_t tc_attn_map_bytes();  // sizeof(CUtensorMap)
 bool tc_attn_make_prefix_maps(void* out2_host, const bf16* k, const bf16* v, int len, const Dims& dm);
 cudaError_t launch_attn_tc(const Dims& dm, const Tables& tb, int layer, const bf16* qkv, op16* o, int k_iter,
