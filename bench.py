@@ -238,7 +238,8 @@ def run_ours(args, rank, world, local_rank):
     peaks = load_peaks()
 
     B = args.batch
-    case = cases.make_case(2, batch=B, robot_stream=rank)   # same weights on every rank, different robots
+    # same weights on every rank, different robots; --config 3 = the continuous-batching mix (extra line, not the contract metric)
+    case = cases.make_case(args.config, batch=B, robot_stream=rank)
     cfg = case.cfg
     lc = LoadedCase(case, device=dev)
     stream = torch.cuda.Stream(device=dev)
@@ -339,9 +340,11 @@ def run_ours(args, rank, world, local_rank):
             "warmup": args.warmup, "ms_per_step": ms_call, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "fp16 operands / fp32 accumulate" if os.environ.get("ROSA_GEMM_DTYPE") != "bf16"
             else "bf16 operands / fp32 accumulate", "data": "synthetic",
-            "config": {"workload": f"cfg2 fleet batch: B={B} robots/GPU, pi0-scale expert (18L d1024 8q/1kv hd256 "
-                                   f"ffn4096 H50 A32), ragged prefix U[600,1000] (sum L={int(case.prefix_lens.sum())}), "
-                                   "10 Euler steps per call, seed 2",
+            "config": {"workload": f"cfg{args.config} " + ("fleet batch" if args.config == 2 else "continuous-batching mix (t_i in {1.0..0.1}, n_i = 10 t_i)") + f": B={B} robots/GPU, pi0-scale expert (18L d1024 8q/1kv hd256 "
+                                   f"ffn4096 H50 A32), ragged prefix lengths (sum L={int(case.prefix_lens.sum())}), "
+                                   f"up to 10 Euler steps per call, seed {args.config}",
+                       "robot_steps_per_call": int(case.n_steps.sum()),
+                       "robot_steps_per_sec": float(world * case.n_steps.sum() * args.steps / (total_ms * 1e-3)),
                        "l2": "inputs exceed L2 (629 MB weights + %.2f GB prefix K/V streamed per Euler step)"
                              % (lc.kv_bytes() / 1e9),
                        "kernel_family": "tcgen05" if family == 1 else "cuda-core", "cuda_graph": True,
@@ -408,11 +411,14 @@ def main():
     ap.add_argument("--steps", type=int, default=30)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--batch", type=int, default=64, help="robots per GPU (the metric is quoted at 64)")
+    ap.add_argument("--batch", type=int, default=None, help="robots per GPU (default 64 for cfg2, 256 for cfg3)")
+    ap.add_argument("--config", type=int, default=2, choices=[2, 3], help="2 = fleet batch (the metric), 3 = continuous-batching mix")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true")
     ap.add_argument("--sweep-max", type=int, default=512)
     args = ap.parse_args()
+    if args.batch is None:
+        args.batch = 64 if args.config == 2 else 256
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                       # timing rule: W >= 3
     rank = int(os.environ.get("RANK", "0"))
