@@ -155,6 +155,43 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, float* scr, uin
         }
       }
     }
+  } else if constexpr (EPI == EPI_FINAL) {
+    // a9 + a10: columns are action dimensions (N = 64 covers A <= 64): v = r acc + b_out, x += dt_p v
+    static_assert(EPI != EPI_FINAL || BN == 64, "final projection uses one 64-column tile");
+    const float rs = row_rscale(ea, ok ? row : 0);
+    {
+      float v[32];
+      ld_acc32(t_acc + half * 32, v);
+      release();
+#pragma unroll
+      for (int i = 0; i < 32; ++i) v[i] *= rs;
+      to_scratch(v);
+    }
+    __syncwarp();
+    float4 o[8];
+    from_scratch(o);
+    float* vel_out = ea.cp->vel;
+    const int batch_ext = ea.cp->batch_ext;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const int m = r0 + i * 4 + lr;
+      if (m < m_lim) {
+        const int p = m / ea.H, j = m - p * ea.H;
+        const float dt = ea.dt[p];
+        const float vv[4] = {o[i].x, o[i].y, o[i].z, o[i].w};
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          const int a = half * 32 + lc + e;
+          if (a < ea.A) {
+            const float v = vv[e] + ea.bias[a];
+            float* xp = ea.x + (size_t)m * ea.A + a;
+            *xp = fmaf(dt, v, *xp);
+            if (vel_out) vel_out[(((size_t)ea.k_iter * batch_ext + ea.src[p]) * ea.H + j) * ea.A + a] = v;
+          }
+        }
+      }
+    }
+    __syncwarp();
   } else if constexpr (EPI == EPI_ROPE) {
     // BN == head_dim: the tile is exactly one head; pairs (c, c + hd/2) are both in TMEM.  This
     // warp covers low columns [64 half, 64 half + 64) and their partners 128 further on.
@@ -671,6 +708,9 @@ cudaError_t launch_gemm_tc(Epi epi, const op16* A, const op16* W, int M, int N, 
     case EPI_STORE_F32: return launch_by_n<EPI_STORE_F32>(A, W, M, N, K, a, s);
     case EPI_BIAS_F32: return launch_by_n<EPI_BIAS_F32>(A, W, M, N, K, a, s);
     case EPI_RESID: return launch_by_n<EPI_RESID>(A, W, M, N, K, a, s);
+    case EPI_FINAL:
+      if (N != 64) return cudaErrorNotSupported;
+      return use_pair(M) ? launch_two<64, EPI_FINAL>(A, W, M, N, K, a, s) : launch_one<64, EPI_FINAL>(A, W, M, N, K, a, s);
     case EPI_ROPE:
       if (a.hd != 256 || N % 256) return cudaErrorNotSupported;
       return use_pair(M) ? launch_two<256, EPI_ROPE>(A, W, M, N, K, a, s) : launch_one<256, EPI_ROPE>(A, W, M, N, K, a, s);

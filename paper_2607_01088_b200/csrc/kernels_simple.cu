@@ -67,7 +67,7 @@ void launch_timevec(float* tvec, const bf16* w_t1, const float* b_t1, const Dims
 }
 
 // ------------------------------------------------------------------ a1 (action half + swish)
-// z[m][n] = swish( sum_c x[m][c] Wca[n][c] + bca[n] + tvec[p][n] ), with Wca = W_1[:, d:] W_in and
+// z[m][n] = swish( sum_c x[m][c] Wca[c][n] + bca[n] + tvec[p][n] ), with Wca = (W_1[:, d:] W_in)^T and
 // bca = W_1[:, d:] b_in folded at create (fp64 on the host): W_1 [tau ; W_in x + b_in] + b_1 is
 // linear in x, so the K = A contraction runs in fp32 on CUDA cores straight from x (R11: x fp32).
 // Block = EM_ROWS token rows; thread = output columns n, n + 256, ...
@@ -92,9 +92,8 @@ __global__ void __launch_bounds__(256) k_embed1(op16* __restrict__ z, const floa
     const float b = bca[n];
 #pragma unroll
     for (int r = 0; r < EM_ROWS; ++r) acc[r] = b;
-    const float* wr = wca + (size_t)n * A;
     for (int c = 0; c < A; ++c) {
-      const float w = wr[c];
+      const float w = wca[(size_t)c * d + n];  // [A, d]: consecutive threads, consecutive addresses
 #pragma unroll
       for (int r = 0; r < EM_ROWS; ++r) acc[r] = fmaf(xs[r][c], w, acc[r]);
     }
@@ -145,67 +144,80 @@ void launch_rmsnorm(op16* out, const float* h, const Dims& dm, const Tables& tb,
 // v = RMSNorm(h; g_f) W_out^T + b_out ; x <- x + dt_p v.  One warp per token row.  The
 // normalised row stays in fp32 (no bf16 rounding of this operand).  Optional velocity export in
 // the caller's robot order.
-constexpr int FIN_AMAX = 64;  // action_dim <= 64 (rosa_expert_create)
+constexpr int FIN_AMAX = 64;   // action_dim <= 64 (rosa_expert_create)
+constexpr int FIN_ROWS = 32;   // token rows per block (4 per warp): W_out is staged once per block
 __global__ void __launch_bounds__(256) k_final(float* __restrict__ x, const CallPtrs* __restrict__ cp,
                                                const float* __restrict__ h, const float* __restrict__ g,
                                                const bf16* __restrict__ w_out, const float* __restrict__ b_out,
                                                int d, int A, int H, float eps, Tables tb, int k_iter) {
+  extern __shared__ __align__(16) uint8_t fin_smem[];
+  bf16* ws = reinterpret_cast<bf16*>(fin_smem);  // [A, d] copy of W_out (weights: no dependency on earlier kernels)
+  for (int i = threadIdx.x * 8; i < A * d; i += blockDim.x * 8)
+    *reinterpret_cast<uint4*>(ws + i) = *reinterpret_cast<const uint4*>(w_out + i);
   pdl_wait();
   pdl_trigger();
+  __syncthreads();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int m = blockIdx.x * (blockDim.x >> 5) + warp;
-  if (m >= tb.m_active[k_iter]) return;
-  const float* row = h + (size_t)m * d;
-  float ss = 0.f;
-  for (int c = lane * 4; c < d; c += 128) {
-    const float4 v = *reinterpret_cast<const float4*>(row + c);
-    ss += v.x * v.x + v.y * v.y + v.z * v.z + v.w * v.w;
-  }
-  ss = warp_sum(ss);
-  const float r = rsqrtf(ss / (float)d + eps);
-  // lane-private partial dot products for every action dimension, 4 columns per lane per chunk
-  float acc[FIN_AMAX];
+  const int m_lim = tb.m_active[k_iter];
+  float* vel_out = cp->vel;
+  const int batch_ext = cp->batch_ext;
+  for (int rr = 0; rr < FIN_ROWS / 8; ++rr) {
+    const int m = blockIdx.x * FIN_ROWS + rr * 8 + warp;
+    if (m >= m_lim) continue;  // warp-uniform
+    const float* row = h + (size_t)m * d;
+    float ss = 0.f;
+    for (int c = lane * 4; c < d; c += 128) {
+      const float4 v = *reinterpret_cast<const float4*>(row + c);
+      ss += v.x * v.x + v.y * v.y + v.z * v.z + v.w * v.w;
+    }
+    ss = warp_sum(ss);
+    const float r = rsqrtf(ss / (float)d + eps);
+    // lane-private partial dot products for every action dimension, 4 columns per lane per chunk
+    float acc[FIN_AMAX];
 #pragma unroll
-  for (int a = 0; a < FIN_AMAX; ++a) acc[a] = 0.f;
-  for (int c = lane * 4; c < d; c += 128) {
-    float4 v = *reinterpret_cast<const float4*>(row + c);
-    const float4 gg = *reinterpret_cast<const float4*>(g + c);
-    v.x *= r * gg.x; v.y *= r * gg.y; v.z *= r * gg.z; v.w *= r * gg.w;
+    for (int a = 0; a < FIN_AMAX; ++a) acc[a] = 0.f;
+    for (int c = lane * 4; c < d; c += 128) {
+      float4 v = *reinterpret_cast<const float4*>(row + c);
+      const float4 gg = *reinterpret_cast<const float4*>(g + c);
+      v.x *= r * gg.x; v.y *= r * gg.y; v.z *= r * gg.z; v.w *= r * gg.w;
+#pragma unroll
+      for (int a = 0; a < FIN_AMAX; ++a) {
+        if (a < A) {
+          const uint2 wb = *reinterpret_cast<const uint2*>(ws + (size_t)a * d + c);
+          const float2 w01 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&wb.x));
+          const float2 w23 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&wb.y));
+          acc[a] = fmaf(v.x, w01.x, fmaf(v.y, w01.y, fmaf(v.z, w23.x, fmaf(v.w, w23.y, acc[a]))));
+        }
+      }
+    }
+    float mine = 0.f, mine_hi = 0.f;  // lane a (and a + 32) keeps the reduced value of action dimension a
 #pragma unroll
     for (int a = 0; a < FIN_AMAX; ++a) {
       if (a < A) {
-        const uint2 wb = *reinterpret_cast<const uint2*>(w_out + (size_t)a * d + c);
-        const float2 w01 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&wb.x));
-        const float2 w23 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&wb.y));
-        acc[a] = fmaf(v.x, w01.x, fmaf(v.y, w01.y, fmaf(v.z, w23.x, fmaf(v.w, w23.y, acc[a]))));
+        const float v = warp_sum(acc[a]);
+        if ((a & 31) == lane) { if (a < 32) mine = v; else mine_hi = v; }
       }
     }
-  }
-  float mine = 0.f;  // lane a (and a + 32) keeps the reduced value of action dimension a
-  float mine_hi = 0.f;
-#pragma unroll
-  for (int a = 0; a < FIN_AMAX; ++a) {
-    if (a < A) {
-      const float v = warp_sum(acc[a]);
-      if ((a & 31) == lane) { if (a < 32) mine = v; else mine_hi = v; }
+    const int p = m / H, j = m - p * H;
+    const float dt = tb.dt[p];
+    for (int a = lane; a < A; a += 32) {
+      const float v = (a < 32 ? mine : mine_hi) + b_out[a];
+      float* xp = x + (size_t)m * A + a;
+      *xp = fmaf(dt, v, *xp);
+      if (vel_out) vel_out[(((size_t)k_iter * batch_ext + tb.src[p]) * H + j) * A + a] = v;
     }
-  }
-  float* vel_out = cp->vel;
-  const int batch_ext = cp->batch_ext;
-  const int p = m / H, j = m - p * H;
-  const float dt = tb.dt[p];
-  for (int a = lane; a < A; a += 32) {
-    const float v = (a < 32 ? mine : mine_hi) + b_out[a];
-    float* xp = x + (size_t)m * A + a;
-    *xp = fmaf(dt, v, *xp);
-    if (vel_out) vel_out[(((size_t)k_iter * batch_ext + tb.src[p]) * H + j) * A + a] = v;
   }
 }
 void launch_final(float* x, const CallPtrs* cp, const float* h, const float* g, const bf16* w_out,
                   const float* b_out, const Dims& dm, const Tables& tb, int k_iter, int M,
                   cudaStream_t s) {
-  const int wpb = 8;
-  launch_k(k_final, dim3((M + wpb - 1) / wpb), dim3(wpb * 32), 0, s, x, cp, h, g, w_out, b_out, dm.d, dm.A, dm.H,
+  const size_t smem = (size_t)dm.A * dm.d * sizeof(bf16);
+  static size_t configured = 0;
+  if (smem > configured) {
+    cudaFuncSetAttribute(k_final, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    configured = smem;
+  }
+  launch_k(k_final, dim3((M + FIN_ROWS - 1) / FIN_ROWS), dim3(256), smem, s, x, cp, h, g, w_out, b_out, dm.d, dm.A, dm.H,
            dm.eps, tb, k_iter);
 }
 

@@ -64,8 +64,9 @@ struct rosa_expert {
   int max_pos = 0;
   // weights
   bf16 *w_t1 = nullptr, *w_out = nullptr;  // CUDA-core steps: bf16 as given
-  float *wca = nullptr, *bca = nullptr;    // W_1[:, d:] W_in [d, A] and W_1[:, d:] b_in [d], folded in fp64
+  float *wca = nullptr, *bca = nullptr;    // (W_1[:, d:] W_in)^T [A, d] and W_1[:, d:] b_in [d], folded in fp64
   op16* w_t2 = nullptr;                    // GEMM operand: fp16 or bf16 (dm.fp16)
+  op16* w_out16 = nullptr;                 // [64, d]: W_out with the final-norm gain folded in, zero rows past A (tcgen05 family)
   float *b_t1 = nullptr, *b_t2 = nullptr, *b_out = nullptr, *g_final = nullptr;
   std::vector<LayerWeights> lw;
   float2* rope_tab = nullptr;
@@ -231,7 +232,7 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
         for (int c = 0; c < A; ++c) accr[c] += wj * wi[c];
         accb += wj * bin[j];
       }
-      for (int c = 0; c < A; ++c) wca[(size_t)n * A + c] = (float)accr[c];
+      for (int c = 0; c < A; ++c) wca[(size_t)c * d + n] = (float)accr[c];  // stored [A, d]: coalesced over n
       bca[n] = (float)accb;
     }
     if ((st = upload_f32(e, wca, &e->wca)) != ROSA_OK) return st;
@@ -241,6 +242,14 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
   FETCH(w->w_t2, (size_t)d * d); UPO(e->w_t2);
   FETCH(w->b_t2, d); UPF(e->b_t2);
   FETCH(w->w_out, (size_t)A * d); UPB(e->w_out);
+  {  // a9 on the tensor cores (family 1): [64, d] operand, gain folded (R23), rows >= A zero
+    std::vector<float> gf, wo = t;
+    if ((st = fetch_f32(w->g_final, (size_t)d, dt, od, gf)) != ROSA_OK) return st;
+    t.assign((size_t)64 * d, 0.f);
+    for (int a = 0; a < A; ++a)
+      for (int c = 0; c < d; ++c) t[(size_t)a * d + c] = wo[(size_t)a * d + c] * gf[c];
+    UPO(e->w_out16);
+  }
   FETCH(w->b_out, A); UPF(e->b_out);
   FETCH(w->g_final, d); UPF(e->g_final);
   e->lw.resize(dm.layers);
@@ -439,9 +448,14 @@ static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, cudaStream_
       ea.out_f32 = e->h; ea.ld_out = d;
       if ((err = gemm(e, ROSA_KC_GEMM_DOWN, EPI_RESID, e->mact, L.wdown, M, d, dm.F, ea, s)) != cudaSuccess) return err;   // a8
     }
-    mark(e, ROSA_KC_FINAL, s);
-    launch_final(e->x, cp, e->h, e->g_final, e->w_out, e->b_out, dm, tb, k, M, s);    // a9 + a10
-    e->last_launches += 1;
+    if (fused_norm) {                                                                 // a9 + a10
+      ea.bias = e->b_out; ea.x = e->x; ea.cp = cp; ea.dt = tb.dt; ea.src = tb.src; ea.A = dm.A; ea.k_iter = k;
+      if ((err = gemm(e, ROSA_KC_FINAL, EPI_FINAL, e->nrm, e->w_out16, M, 64, d, ea, s)) != cudaSuccess) return err;
+    } else {
+      mark(e, ROSA_KC_FINAL, s);
+      launch_final(e->x, cp, e->h, e->g_final, e->w_out, e->b_out, dm, tb, k, M, s);
+      e->last_launches += 1;
+    }
   }
   mark(e, ROSA_KC_GATHER_SCATTER, s);
   launch_scatter_x(cp, e->x, tb, dm.H * dm.A, s);
@@ -539,6 +553,9 @@ rosa_status_t rosa_expert_create(const rosa_expert_config_t* c, const rosa_weigh
   if (c->d_model % 64 || c->ffn % 64 || (c->n_q_heads * c->head_dim) % 64 || c->head_dim % 2 ||
       c->head_dim > 256 || c->n_q_heads % c->n_kv_heads || c->action_dim > 64 || c->horizon > 64) {
     set_error("unsupported shape (see rosa_expert_create in rosa.h)"); return ROSA_ERR_UNSUPPORTED;
+  }
+  if ((size_t)c->action_dim * c->d_model * 2 > 200 * 1024) {
+    set_error("action_dim * d_model too large for the final projection's shared-memory copy of W_out"); return ROSA_ERR_UNSUPPORTED;
   }
   if ((size_t)c->n_q_heads * (c->head_dim + c->max_prefix_len + c->horizon + 1) * 4 > 220 * 1024) {
     set_error("max_prefix_len too large for the attention kernel's shared memory"); return ROSA_ERR_UNSUPPORTED;

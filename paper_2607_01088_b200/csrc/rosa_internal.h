@@ -61,7 +61,8 @@ enum Epi : int {
   EPI_BIAS_F32 = 2,      // h fp32 = acc + bias[n]          (+ 16-bit copy and sum-of-squares partials)
   EPI_ROPE = 3,          // qkv bf16 = rope(r * acc) on q and k heads at pos = len + j; v = r * acc
   EPI_RESID = 4,         // h fp32 += acc                   (+ 16-bit copy and sum-of-squares partials)
-  EPI_GEGLU = 5          // out 16-bit [M, N/2] = gelu_tanh(r * gate) * (r * up) (interleaved columns)
+  EPI_GEGLU = 5,         // out 16-bit [M, N/2] = gelu_tanh(r * gate) * (r * up) (interleaved columns)
+  EPI_FINAL = 6          // a9 + a10: v = r * acc + b_out ; x += dt_p * v ; optional velocity export (N = 64 >= A)
 };
 
 struct EpiArgs {
@@ -82,6 +83,12 @@ struct EpiArgs {
   int gu_blk;             // GEGLU
   int ld_out;             // leading dimension (elements) of the output
   const int* m_active;    // device pointer to the active row count of this iteration (or null)
+  // EPI_FINAL
+  float* x;               // [M, A] current actions (internal robot order)
+  const CallPtrs* cp;     // velocity export pointer + caller batch
+  const float* dt;        // Tables::dt
+  const int* src;         // Tables::src
+  int A, k_iter;
   int dbg;                // measurement aid (ROSA_DBG): bit 0 skip the epilogue body, bit 1 skip the MMAs
 };
 
