@@ -55,7 +55,7 @@ __global__ void __launch_bounds__(AT_THREADS, 1)
 k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__ kv_maps, Dims dm, Tables tb,
           int layer, op16* __restrict__ o, int k_iter, int tiles_per_robot, int dbg, long long* __restrict__ trace) {
   extern __shared__ __align__(1024) uint8_t smem_raw[];
-  const int p = blockIdx.x / tiles_per_robot, tt = blockIdx.x % tiles_per_robot;
+  const int p = tb.attn_order[blockIdx.x / tiles_per_robot], tt = blockIdx.x % tiles_per_robot;
   if (p * dm.H >= tb.m_active[k_iter]) return;
   const int robot = tb.ids[p], L = tb.rlen[robot];
   const int nbp = (L + AT_KV - 1) / AT_KV, nb = nbp + 1;  // prefix blocks + one block of own tokens
@@ -128,8 +128,6 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
           mbar_expect_tx(k_full(s), AT_KV_BYTES);
           if (i == nbp) tma_load_3d(k_smem(s), &maps.own, k_full(s), 0, p * dm.H, dm.q_n / 64);
           else tma_load_3d(k_smem(s), kmap, k_full(s), 0, i * AT_KV, 0);
-          if (i == 1) for (int j = 2; j < AT_PF; ++j) prefetch_blk(j);
-          if (i >= 1) prefetch_blk(i + AT_PF - 1);
           AT_TRACE(0, i);
         }
         __syncwarp();
@@ -148,6 +146,9 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
           mbar_expect_tx(v_full(s), AT_KV_BYTES);
           if (i == nbp) tma_load_3d(v_smem(s), &maps.own, v_full(s), 0, p * dm.H, (dm.q_n + AT_HD) / 64);
           else tma_load_3d(v_smem(s), vmap, v_full(s), 0, i * AT_KV, 0);
+          // L2 prefetches go out only after everything the first MMAs wait for (Q, K0, K1, V0) is in flight
+          if (i == 0) for (int j = 2; j < AT_PF; ++j) prefetch_blk(j);
+          prefetch_blk(i + AT_PF);
           AT_TRACE(1, i);
         }
         __syncwarp();

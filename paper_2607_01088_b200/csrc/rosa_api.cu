@@ -92,7 +92,7 @@ struct rosa_expert {
   cudaEvent_t stage_ev[kStageRing] = {};
   int stage_next = 0;
   size_t call_bytes = 0;
-  size_t off_ids, off_src, off_t0, off_dt, off_ns, off_mact, off_ptrs;
+  size_t off_ids, off_src, off_t0, off_dt, off_ns, off_mact, off_order, off_ptrs;
   std::map<GraphKey, cudaGraphExec_t> graphs;
   std::map<GraphKey, int64_t> graph_launches;
   cudaStream_t cap_stream = nullptr;
@@ -171,6 +171,7 @@ static Tables make_tables(const rosa_expert* e, int batch) {
   tb.dt = (const float*)(e->d_call + e->off_dt);
   tb.nsteps = (const int*)(e->d_call + e->off_ns);
   tb.m_active = (const int*)(e->d_call + e->off_mact);
+  tb.attn_order = (const int*)(e->d_call + e->off_order);
   tb.rk = e->d_rk;
   tb.rv = e->d_rv;
   tb.rlen = e->d_rlen;
@@ -349,6 +350,7 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
   e->off_dt = take((size_t)c->max_batch * 4);
   e->off_ns = take((size_t)c->max_batch * 4);
   e->off_mact = take((size_t)c->max_steps * 4);
+  e->off_order = take((size_t)c->max_batch * 4);
   e->off_ptrs = take(sizeof(CallPtrs));
   e->call_bytes = off;
   WS(e->d_call, e->call_bytes);
@@ -504,6 +506,11 @@ static rosa_status_t denoise_impl(rosa_expert* e, int batch, const int32_t* ids,
     int act = 0;
     for (int p = 0; p < batch; ++p) act += h_ns[p] > k;
     h_ma[k] = act * dm.H;
+  }
+  {  // attention CTAs are issued longest prefix first: the second wave then pairs long with short (LPT)
+    int* h_ord = (int*)(hs + e->off_order);
+    std::iota(h_ord, h_ord + batch, 0);
+    std::stable_sort(h_ord, h_ord + batch, [&](int a, int b) { return e->h_rlen[h_ids[a]] > e->h_rlen[h_ids[b]]; });
   }
   CallPtrs* h_cp = (CallPtrs*)(hs + e->off_ptrs);
   h_cp->noise = noise; h_cp->out = out; h_cp->vel = out_vel; h_cp->batch_ext = batch;

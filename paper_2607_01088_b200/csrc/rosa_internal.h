@@ -34,6 +34,7 @@ struct Tables {
   const float* dt;      // [B]
   const int* nsteps;    // [B]
   const int* m_active;  // [max_steps] active token rows (= H * active robots) in iteration k
+  const int* attn_order;  // [B] internal positions sorted by prefix length, longest first (attention CTA order)
   const bf16* const* rk;  // [max_robots * layers] prefix K pointer of (robot, layer)
   const bf16* const* rv;  // [max_robots * layers]
   const int* rlen;        // [max_robots]
