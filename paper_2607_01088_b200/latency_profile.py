@@ -108,13 +108,15 @@ def feasible_configs(prof: Dict[int, dict], freq_hz: float, slo_ms: float, perce
     for b, p in sorted(prof.items()):
         rates = np.array([r["rate_per_s"] for r in p["rates"]])
         lats = np.array([r[percentile] for r in p["rates"]])
+        means = np.array([r.get("mean_ms", r[percentile]) for r in p["rates"]])
         best = None
         k = b
         while k * freq_hz <= rates[-1]:
             lam = k * freq_hz
             l = float(np.interp(lam, rates, lats)) if lam >= rates[0] else float(lats[0])
             if l <= slo_ms:
-                best = {"batch": int(b), "robots": int(k), "load_per_s": lam, percentile: l}
+                mean = float(np.interp(lam, rates, means)) if lam >= rates[0] else float(means[0])
+                best = {"batch": int(b), "robots": int(k), "load_per_s": lam, percentile: l, "mean_ms": mean}
                 out.append(dict(best))
             k += 1
         if best:
