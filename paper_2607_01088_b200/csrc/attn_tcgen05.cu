@@ -235,29 +235,39 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
     float m_ref = -INFINITY, l_sum = 0.f;                             // m_ref in log2 units; l_sum: this half's part
     for (int i = 0; i < nb; ++i) {
       const int sb = i & 1;
-      const int n_valid = (i == nbp ? dm.H : min(AT_KV, L - i * AT_KV)) - half * 32;  // valid columns of this half
+      const int n_tot = i == nbp ? dm.H : min(AT_KV, L - i * AT_KV);
+      const int n_valid = n_tot - half * 32, n_other = n_tot - (half ^ 1) * 32;  // valid columns of this / the other half
       mbar_wait(s_full(sb), (i >> 1) & 1);
       tc_fence_after();
       if (threadIdx.x == 64) AT_TRACE(4, i);
+      // Both warps of a row read all 64 scores for the row maximum (so they take the same rescale
+      // decision without an exchange); each exponentiates only its own 32.
       float sc[32];
+      float m_blk;
       {
-        uint32_t r0[32];
+        uint32_t r0[32], r1[32];
         tmem_ld32(tmem_s + lane_off + sb * AT_KV + half * 32, r0);
+        tmem_ld32(tmem_s + lane_off + sb * AT_KV + (half ^ 1) * 32, r1);
         tmem_ld_wait();
 #pragma unroll
         for (int c = 0; c < 32; ++c) sc[c] = __uint_as_float(r0[c]);
+        float mo = -INFINITY;
+        if (n_valid < 32 || n_other < 32) {  // warp-uniform; only the last prefix block and the own-token block
+#pragma unroll
+          for (int c = 0; c < 32; ++c) {
+            sc[c] = c < n_valid ? sc[c] : -INFINITY;
+            mo = fmaxf(mo, c < n_other ? __uint_as_float(r1[c]) : -INFINITY);
+          }
+        } else {
+#pragma unroll
+          for (int c = 0; c < 32; ++c) mo = fmaxf(mo, __uint_as_float(r1[c]));
+        }
+        m_blk = mo;
       }
       if (threadIdx.x == 64) AT_TRACE(8, i);
-      if (n_valid < 32) {  // warp-uniform; only the last prefix block and the own-token block
 #pragma unroll
-        for (int c = 0; c < 32; ++c) sc[c] = c < n_valid ? sc[c] : -INFINITY;
-      }
-      float m_blk = sc[0];
-#pragma unroll
-      for (int c = 1; c < 32; ++c) m_blk = fmaxf(m_blk, sc[c]);
-      xch[(sb * 2 + half) * AT_ROWS + r] = m_blk;
-      named_bar_sync(1 + q, 64);
-      m_blk = fmaxf(m_blk, xch[(sb * 2 + (half ^ 1)) * AT_ROWS + r]) * c_log2;
+      for (int c = 0; c < 32; ++c) m_blk = fmaxf(m_blk, sc[c]);
+      m_blk *= c_log2;
       if (threadIdx.x == 64) AT_TRACE(9, i);
       float factor = 1.f;
       if (m_blk > m_ref + AT_RESCALE_THR) {            // first block always lands here
