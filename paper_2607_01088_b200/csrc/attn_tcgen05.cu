@@ -181,7 +181,6 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
       AT_TRACE(6, 0);
       issue_s(0);
       for (int i = 0; i < nb; ++i) {
-        if ((dbg & 32) && i > 0) mbar_wait(pv_done, (i - 1) & 1);  // experiment: S(i+1) only after PV(i-1) completed
         if (i + 1 < nb) issue_s(i + 1);
         const int s = i % AT_ST;
         mbar_wait(v_full(s), (i / AT_ST) & 1);
