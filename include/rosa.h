@@ -137,7 +137,8 @@ typedef enum {
   ROSA_KC_GEMM_GATEUP = 8,    /* a7 */
   ROSA_KC_GEMM_DOWN = 9,      /* a8 */
   ROSA_KC_FINAL = 10,         /* a9 + a10 */
-  ROSA_KC_COUNT = 11
+  ROSA_KC_GEMM_FUSED = 11,    /* a6 -> a7 -> a8 in one persistent kernel (M > 128) */
+  ROSA_KC_COUNT = 12
 } rosa_kernel_class_t;
 
 /* Measurement aid for bench.py (SURVEY 8(d) "evidence per kernel"): runs the same call as

@@ -24,7 +24,7 @@ EXPORTS = ("rosa_expert_create", "rosa_expert_destroy", "rosa_prefix_kv_bind", "
            "rosa_profile_batch", "rosa_kernel_class_name", "rosa_debug_attn_trace",
            "rosa_last_launch_count", "rosa_kernel_family", "rosa_debug_gemm", "rosa_last_error",
            "rosa_version")
-ROSA_KC_COUNT = 11
+ROSA_KC_COUNT = 12
 
 
 class RosaError(RuntimeError):

@@ -8,9 +8,12 @@
 namespace rosa {
 
 // ------------------------------------------------------------------ x gather / scatter
-__global__ void k_gather_x(float* __restrict__ x, const CallPtrs* __restrict__ cp, Tables tb, int HA) {
+__global__ void k_gather_x(float* __restrict__ x, const CallPtrs* __restrict__ cp, Tables tb, int HA, int* __restrict__ zero,
+                           int n_zero) {
   pdl_wait();
   pdl_trigger();
+  if (blockIdx.x == 0)  // dependency counters of the fused GEMM kernels start every call at zero
+    for (int i = threadIdx.x; i < n_zero; i += blockDim.x) zero[i] = 0;
   int p = blockIdx.x;
   const float* s = cp->noise + (size_t)tb.src[p] * HA;
   for (int i = threadIdx.x; i < HA; i += blockDim.x) x[(size_t)p * HA + i] = s[i];
@@ -22,8 +25,8 @@ __global__ void k_scatter_x(const CallPtrs* __restrict__ cp, const float* __rest
   float* d = cp->out + (size_t)tb.src[p] * HA;
   for (int i = threadIdx.x; i < HA; i += blockDim.x) d[i] = x[(size_t)p * HA + i];
 }
-void launch_gather_x(float* x, const CallPtrs* cp, const Tables& tb, int HA, cudaStream_t s) {
-  launch_k(k_gather_x, dim3(tb.batch), dim3(128), 0, s, x, cp, tb, HA);
+void launch_gather_x(float* x, const CallPtrs* cp, const Tables& tb, int HA, int* zero, int n_zero, cudaStream_t s) {
+  launch_k(k_gather_x, dim3(tb.batch), dim3(128), 0, s, x, cp, tb, HA, zero, n_zero);
 }
 void launch_scatter_x(const CallPtrs* cp, const float* x, const Tables& tb, int HA, cudaStream_t s) {
   launch_k(k_scatter_x, dim3(tb.batch), dim3(128), 0, s, cp, x, tb, HA);

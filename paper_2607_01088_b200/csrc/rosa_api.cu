@@ -98,6 +98,11 @@ struct rosa_expert {
   cudaStream_t cap_stream = nullptr;
   int64_t last_launches = 0;
   float* e2e_dev = nullptr;  // staging for rosa_denoise_batch_host
+  // fused a6 -> a7 -> a8 kernel: static schedules for every number of row blocks + dependency counters
+  bool fused_ok = false;
+  uint16_t* d_sched = nullptr;
+  int* d_done = nullptr;  // [2][kFusedPhases][n_m_max]
+  int fused_slots = 0, fused_pairs = 0, n_m_max = 0;
   // per-launch event timing (rosa_profile_batch): boundary event before every launch
   bool prof_on = false;
   std::vector<cudaEvent_t> prof_ev;
@@ -318,6 +323,33 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
   WS(e->scratch, Mmax * (size_t)std::max(2 * F, dm.qkv_n) * 4);
   WS(e->e2e_dev, (size_t)c->max_batch * HA * 4);
   WS(e->ssq, Mmax * (d / 32) * 4);
+  {  // fused O -> gate/up -> down kernel (tcgen05 family, 256-column tiles)
+    const char* fz = getenv("ROSA_FUSED");
+    // opt-in (ROSA_FUSED=1): measured slower than the three separate PDL-chained launches
+    e->fused_ok = e->family == 1 && d % 256 == 0 && (2 * F) % 256 == 0 && dm.q_n % 64 == 0 && fz && !strcmp(fz, "1");
+    if (e->fused_ok) {
+      int sms = 0, dev = 0;
+      cudaGetDevice(&dev);
+      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+      e->fused_pairs = sms / 2;
+      e->n_m_max = (int)(Mmax / 256) + 1;
+      const int n_n[kFusedPhases] = {d / 256, 2 * F / 256, d / 256};
+      const int n_kb[kFusedPhases] = {dm.q_n / 64, d / 64, F / 64};
+      if (e->n_m_max > 127 || n_n[1] > 63) e->fused_ok = false;  // item code: 7 bits of row block, 6 bits of column tile
+    }
+    if (e->fused_ok) {
+      const int n_n[kFusedPhases] = {d / 256, 2 * F / 256, d / 256};
+      const int n_kb[kFusedPhases] = {dm.q_n / 64, d / 64, F / 64};
+      e->fused_slots = tc_fused_max_slots(e->n_m_max, n_n, n_kb, e->fused_pairs) + 1;
+      std::vector<uint16_t> tab((size_t)(e->n_m_max + 1) * e->fused_pairs * e->fused_slots, 0xFFFF);
+      for (int nm = 1; nm <= e->n_m_max; ++nm)
+        tc_fused_schedule(nm, n_n, n_kb, e->fused_pairs, e->fused_slots, tab.data() + (size_t)nm * e->fused_pairs * e->fused_slots);
+      WS(e->d_sched, tab.size() * 2);
+      CK(cudaMemcpy(e->d_sched, tab.data(), tab.size() * 2, cudaMemcpyHostToDevice));
+      WS(e->d_done, (size_t)2 * kFusedPhases * e->n_m_max * 4);
+      CK(cudaMemset(e->d_done, 0, (size_t)2 * kFusedPhases * e->n_m_max * 4));
+    }
+  }
   CK(cudaMemset(e->zbuf, 0, Mmax * d * 2));
   CK(cudaMemset(e->nrm, 0, Mmax * d * 2));
   CK(cudaMemset(e->qkv, 0, Mmax * dm.qkv_n * 2));
@@ -403,11 +435,13 @@ static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, cudaStream_
   cudaError_t err;
   e->last_launches = 0;
   mark(e, ROSA_KC_GATHER_SCATTER, s);
-  launch_gather_x(e->x, cp, tb, dm.H * dm.A, s);
+  launch_gather_x(e->x, cp, tb, dm.H * dm.A, e->d_done, e->fused_ok ? 2 * kFusedPhases * e->n_m_max : 0, s);
   mark(e, ROSA_KC_TIMEVEC, s);
   launch_timevec(e->tvec, e->w_t1, e->b_t1, dm, tb, nmax, e->cfg.max_batch, s);
   e->last_launches += 2;
   const bool fused_norm = e->family == 1;  // RMSNorm fused into the GEMM epilogues (tcgen05 family)
+  const bool use_fused = e->fused_ok && tc_use_pair(M);
+  int fused_idx = 0;
   for (int k = 0; k < nmax; ++k) {
     EpiArgs ea{};
     ea.m_active = tb.m_active + k;
@@ -438,17 +472,37 @@ static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, cudaStream_
         launch_attn_simple(dm, tb, l, e->qkv, e->obuf, k, e->cfg.max_prefix_len, s);
       }
       e->last_launches += 1;
-      ea.out_f32 = e->h; ea.ld_out = d;
-      if ((err = gemm(e, ROSA_KC_GEMM_O, EPI_RESID, e->obuf, L.wo, M, d, dm.q_n, ea, s)) != cudaSuccess) return err;    // a6
-      if (!fused_norm) {
-        mark(e, ROSA_KC_RMSNORM, s);
-        launch_rmsnorm(e->nrm, e->h, dm, tb, k, M, s);                               // a2
+      if (use_fused) {                                                              // a6 -> a7 -> a8, one launch
+        FusedMeta fm{};
+        const int n_n[kFusedPhases] = {d / 256, 2 * dm.F / 256, d / 256};
+        const int n_kb[kFusedPhases] = {dm.q_n / 64, d / 64, dm.F / 64};
+        const int epi[kFusedPhases] = {EPI_RESID, EPI_GEGLU, EPI_RESID};
+        for (int p = 0; p < kFusedPhases; ++p) { fm.n_n[p] = n_n[p]; fm.n_kb[p] = n_kb[p]; fm.epi[p] = epi[p]; fm.ea[p] = ea; }
+        fm.ea[0].out_f32 = e->h; fm.ea[0].ld_out = d;
+        fm.ea[1].out16 = e->mact; fm.ea[1].ld_out = dm.F;
+        fm.ea[2].out_f32 = e->h; fm.ea[2].ld_out = d;
+        fm.sched = e->d_sched; fm.pairs_max = e->fused_pairs; fm.slots = e->fused_slots; fm.n_m_max = e->n_m_max;
+        fm.done = e->d_done + (size_t)(fused_idx & 1) * kFusedPhases * e->n_m_max;
+        fm.done_next = e->d_done + (size_t)((fused_idx + 1) & 1) * kFusedPhases * e->n_m_max;
+        fused_idx += 1;
+        const op16* As[kFusedPhases] = {e->obuf, e->nrm, e->mact};
+        const op16* Ws[kFusedPhases] = {L.wo, L.wgu, L.wdown};
+        mark(e, ROSA_KC_GEMM_FUSED, s);
+        if ((err = launch_fused_tc(As, Ws, fm, M, tb.m_active + k, dm.fp16, s)) != cudaSuccess) return err;
         e->last_launches += 1;
+      } else {
+        ea.out_f32 = e->h; ea.ld_out = d;
+        if ((err = gemm(e, ROSA_KC_GEMM_O, EPI_RESID, e->obuf, L.wo, M, d, dm.q_n, ea, s)) != cudaSuccess) return err;    // a6
+        if (!fused_norm) {
+          mark(e, ROSA_KC_RMSNORM, s);
+          launch_rmsnorm(e->nrm, e->h, dm, tb, k, M, s);                               // a2
+          e->last_launches += 1;
+        }
+        ea.out16 = e->mact; ea.ld_out = dm.F;
+        if ((err = gemm(e, ROSA_KC_GEMM_GATEUP, EPI_GEGLU, e->nrm, L.wgu, M, 2 * dm.F, d, ea, s)) != cudaSuccess) return err;  // a2+a7
+        ea.out_f32 = e->h; ea.ld_out = d;
+        if ((err = gemm(e, ROSA_KC_GEMM_DOWN, EPI_RESID, e->mact, L.wdown, M, d, dm.F, ea, s)) != cudaSuccess) return err;   // a8
       }
-      ea.out16 = e->mact; ea.ld_out = dm.F;
-      if ((err = gemm(e, ROSA_KC_GEMM_GATEUP, EPI_GEGLU, e->nrm, L.wgu, M, 2 * dm.F, d, ea, s)) != cudaSuccess) return err;  // a2+a7
-      ea.out_f32 = e->h; ea.ld_out = d;
-      if ((err = gemm(e, ROSA_KC_GEMM_DOWN, EPI_RESID, e->mact, L.wdown, M, d, dm.F, ea, s)) != cudaSuccess) return err;   // a8
     }
     if (fused_norm) {                                                                 // a9 + a10
       ea.bias = e->b_out; ea.x = e->x; ea.cp = cp; ea.dt = tb.dt; ea.src = tb.src; ea.A = dm.A; ea.k_iter = k;
@@ -712,7 +766,7 @@ rosa_status_t rosa_profile_batch(rosa_expert_t* e, int32_t batch, const int32_t*
 const char* rosa_kernel_class_name(int32_t cls) {
   static const char* names[ROSA_KC_COUNT] = {"gather_scatter", "timevec", "inproj", "gemm_embed", "rmsnorm",
                                              "gemm_qkv_rope", "attention", "gemm_o_resid", "gemm_gateup_geglu",
-                                             "gemm_down_resid", "final_norm_outproj_euler"};
+                                             "gemm_down_resid", "final_norm_outproj_euler", "gemm_fused_o_gateup_down"};
   return cls >= 0 && cls < ROSA_KC_COUNT ? names[cls] : "";
 }
 

@@ -101,7 +101,7 @@ void launch_epilogue(Epi epi, const float* C, int M, int N, const EpiArgs& a, cu
 void launch_attn_simple(const Dims& dm, const Tables& tb, int layer, const bf16* qkv, op16* o,
                         int k_iter, int max_len, cudaStream_t s);
 // common elementwise kernels
-void launch_gather_x(float* x, const CallPtrs* cp, const Tables& tb, int HA, cudaStream_t s);
+void launch_gather_x(float* x, const CallPtrs* cp, const Tables& tb, int HA, int* zero, int n_zero, cudaStream_t s);
 void launch_scatter_x(const CallPtrs* cp, const float* x, const Tables& tb, int HA, cudaStream_t s);
 void launch_timevec(float* tvec, const bf16* w_t1, const float* b_t1, const Dims& dm,
                     const Tables& tb, int nsteps_max, int max_batch, cudaStream_t s);
@@ -119,6 +119,25 @@ int tc_ssq_cols(int N, int M);  // columns per sum-of-squares partial of the BIA
 // A [M,K] row-major, W [N,K] row-major, both fp16 or both bf16 (EpiArgs::in_fp16)
 cudaError_t launch_gemm_tc(Epi epi, const op16* A, const op16* W, int M, int N, int K,
                            const EpiArgs& a, cudaStream_t s);
+
+// fused dependent GEMMs a6 -> a7 -> a8 in one persistent CTA-pair kernel (gemm_tcgen05.cu)
+constexpr int kFusedPhases = 3;
+struct FusedMeta {
+  int n_n[kFusedPhases];     // column tiles (256 wide) per row block
+  int n_kb[kFusedPhases];    // k-blocks per tile
+  int epi[kFusedPhases];     // Epi
+  EpiArgs ea[kFusedPhases];
+  const uint16_t* sched;     // [n_m_max + 1][pairs_max][slots] item codes (phase << 13 | m << 6 | n), 0xFFFF = end
+  int pairs_max, slots;
+  int* done;                 // [kFusedPhases][n_m_max] epilogue-warp arrivals of this launch (zeroed by the previous one)
+  int* done_next;            // the other buffer: zeroed here for the next launch
+  int n_m_max;
+};
+bool tc_use_pair(int M);
+void tc_fused_schedule(int n_m, const int* n_n, const int* n_kb, int pairs, int slots, uint16_t* out);
+int tc_fused_max_slots(int n_m, const int* n_n, const int* n_kb, int pairs);
+cudaError_t launch_fused_tc(const op16* const* A, const op16* const* W, const FusedMeta& fm, int M, const int* m_active,
+                            int in_fp16, cudaStream_t s);
 
 // tcgen05 attention (attn_tcgen05.cu)
 bool tc_attn_supported(const Dims& dm);

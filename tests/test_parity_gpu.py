@@ -323,3 +323,21 @@ def test_bf16_operand_mode_measured(monkeypatch):
     assert res["bf16"][0] <= TOL_ACT_ABS and res["bf16"][1] <= TOL_ACT_REL
     assert res["fp16"][2] <= TOL_VEL_REL
     assert res["fp16"][2] < res["bf16"][2]
+
+
+def test_fused_dependent_gemm_kernel_opt_in(monkeypatch):
+    """ROSA_FUSED=1: O projection, gate/up and down GEMMs of a layer in ONE persistent kernel with a static
+    host-computed list schedule and per-row-block dependency counters (both priority orders)."""
+    case = edge_case([70, 150, 33, 90, 64, 200, 10, 129, 300, 17, 64, 65], n_steps=2)   # M = 600: three 256-row blocks
+    want_x, want_v = O.denoise_case(case, return_velocity=True)
+    for order in ("0", "1"):
+        monkeypatch.setenv("ROSA_FUSED", "1")
+        monkeypatch.setenv("ROSA_FUSED_ORDER", order)
+        lc = LoadedCase(case)
+        got_x, got_v = lc.run(want_velocity=True)
+        again, _ = lc.run()
+        n_launch = rosa.rosa_last_launch_count(lc.expert)
+        lc.close()
+        compare(f"fused-order{order}", got_x, got_v, want_x, want_v)
+        assert np.array_equal(got_x, again)                       # deterministic
+        assert n_launch == 2 + 2 * (2 + 2 * 3 + 1) + 1            # 3 kernels per layer instead of 5
