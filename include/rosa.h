@@ -160,9 +160,12 @@ rosa_status_t rosa_debug_gemm(int32_t family, int32_t M, int32_t N, int32_t K, c
 
 /* Measurement aid: with the environment variable ROSA_DBG bit 4 set, the attention kernel records
  * clock64() at its pipeline events for two CTAs; this copies [2][16 roles][32 key blocks] int64 values
- * of the last launch to host_out and returns the count (0 if tracing is off).  n < 0: the -n phase
- * timestamps of CTA 0 of the last CTA-pair GEMM launch instead (ROSA_DBG bit 6). */
+ * of the last launch to host_out and returns the count (0 if tracing is off). */
 int32_t rosa_debug_attn_trace(int64_t *host_out, int32_t n);
+/* Same for the CTA-pair GEMM (ROSA_DBG bit 6): up to 16 phase timestamps of CTA 0 of the last launch
+ * (entry, prologue done, dependency wait done, first stage full, last stage full, accumulator ready,
+ * epilogue done, block sync, cluster sync). */
+int32_t rosa_debug_gemm_trace(int64_t *host_out, int32_t n);
 
 const char *rosa_last_error(void); /* thread-local, never NULL */
 int32_t rosa_version(void);

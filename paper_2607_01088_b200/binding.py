@@ -21,7 +21,7 @@ ROSA_F32, ROSA_BF16 = 0, 1
 
 EXPORTS = ("rosa_expert_create", "rosa_expert_destroy", "rosa_prefix_kv_bind", "rosa_prefix_kv_unbind",
            "rosa_denoise_batch", "rosa_denoise_batch_ex", "rosa_denoise_batch_host",
-           "rosa_profile_batch", "rosa_kernel_class_name", "rosa_debug_attn_trace",
+           "rosa_profile_batch", "rosa_kernel_class_name", "rosa_debug_attn_trace", "rosa_debug_gemm_trace",
            "rosa_last_launch_count", "rosa_kernel_family", "rosa_debug_gemm", "rosa_last_error",
            "rosa_version")
 ROSA_KC_COUNT = 12
@@ -77,10 +77,12 @@ def load():
     lib.rosa_kernel_class_name.restype = C.c_char_p
     lib.rosa_debug_attn_trace.argtypes = [vp, i32]
     lib.rosa_debug_attn_trace.restype = i32
+    lib.rosa_debug_gemm_trace.argtypes = [vp, i32]
+    lib.rosa_debug_gemm_trace.restype = i32
     lib.rosa_last_error.restype = C.c_char_p
     lib.rosa_version.restype = i32
     for n in EXPORTS:
-        if n not in ("rosa_last_error", "rosa_version", "rosa_kernel_class_name", "rosa_debug_attn_trace"):
+        if n not in ("rosa_last_error", "rosa_version", "rosa_kernel_class_name", "rosa_debug_attn_trace", "rosa_debug_gemm_trace"):
             getattr(lib, n).restype = C.c_int
     _lib = lib
     return lib
@@ -238,6 +240,12 @@ def rosa_debug_gemm(family: int, M: int, N: int, K: int, A_bf16, W_bf16, C_f32, 
 def rosa_debug_attn_trace() -> np.ndarray:
     buf = np.zeros((2, 16, 32), dtype=np.int64)
     load().rosa_debug_attn_trace(_ptr(buf), buf.size)
+    return buf
+
+
+def rosa_debug_gemm_trace() -> np.ndarray:
+    buf = np.zeros(16, dtype=np.int64)
+    load().rosa_debug_gemm_trace(_ptr(buf), buf.size)
     return buf
 
 

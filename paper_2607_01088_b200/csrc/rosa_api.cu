@@ -798,9 +798,8 @@ rosa_status_t rosa_debug_gemm(int32_t family, int32_t M, int32_t N, int32_t K, c
   return ROSA_OK;
 }
 
-int32_t rosa_debug_attn_trace(int64_t* host_out, int32_t n) {
-  return n < 0 ? tc_gemm_read_trace((long long*)host_out, -n) : tc_attn_read_trace((long long*)host_out, n);
-}
+int32_t rosa_debug_attn_trace(int64_t* host_out, int32_t n) { return tc_attn_read_trace((long long*)host_out, n); }
+int32_t rosa_debug_gemm_trace(int64_t* host_out, int32_t n) { return tc_gemm_read_trace((long long*)host_out, n); }
 
 const char* rosa_last_error(void) { return g_err.c_str(); }
 int32_t rosa_version(void) { return 1; }
