@@ -910,9 +910,15 @@ bool tc_gemm_supported(int N, int K) { return N % 64 == 0 && K % 64 == 0 && N >=
 static bool use_pair(int M) { return M > BM; }
 bool tc_use_pair(int M) { return use_pair(M); }
 // N tile of the EPI_BIAS_F32 / EPI_RESID launches
+// Small batches are latency-bound (a serial K loop per tile), so narrower tiles are chosen until about
+// half of the CTAs (or CTA pairs) have a tile; from B = 64 on this is 256 (pairs) as before.
 static int resid_bn(int N, int M) {
-  if (use_pair(M) && N % 256 == 0) return 256;
-  return N % 128 == 0 ? 128 : 64;
+  const bool pair = use_pair(M);
+  const int units = pair ? num_sms() / 2 : num_sms();
+  const int n_m = pair ? (M + 2 * BM - 1) / (2 * BM) : (M + BM - 1) / BM;
+  for (int bn = pair ? 256 : 128; bn > 64; bn >>= 1)
+    if (N % bn == 0 && n_m * (N / bn) * 2 >= units) return bn;
+  return 64;
 }
 // columns per sum-of-squares partial written by those launches (half an N tile: two epilogue warps per row)
 int tc_ssq_cols(int N, int M) { return resid_bn(N, M) / 2; }
