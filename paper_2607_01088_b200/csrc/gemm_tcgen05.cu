@@ -963,7 +963,7 @@ template <int EPI>
 static cudaError_t launch_by_n(const op16* A, const op16* W, int M, int N, int K, const EpiArgs& a, cudaStream_t s) {
   const int forced = a.dbg >> 8;  // rosa_debug_gemm only: 1xx = single-CTA kernel, N tile xx0
   const bool pair = forced ? forced / 1000 == 2 : use_pair(M);
-  const int bn = forced ? forced % 1000 : resid_bn(N, M);
+  const int bn = forced ? forced % 1000 : (a.force_bn ? a.force_bn : resid_bn(N, M));
   if (pair) {
     if (bn == 256) return launch_two<256, EPI>(A, W, M, N, K, a, s);
     if (bn == 128) return launch_two<128, EPI>(A, W, M, N, K, a, s);

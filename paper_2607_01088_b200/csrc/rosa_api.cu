@@ -448,6 +448,7 @@ static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, cudaStream_
     ea.H = dm.H; ea.hd = dm.hd; ea.gu_blk = dm.gu_blk; ea.in_fp16 = dm.fp16; ea.out_fp16 = dm.fp16;
     ea.inv_d = 1.f / (float)d; ea.eps = dm.eps; ea.n_part = d / tc_ssq_cols(d, M);
     if (fused_norm) { ea.h16 = e->nrm; ea.ssq_out = e->ssq; ea.ssq_in = e->ssq; }
+    if (use_fused) { ea.force_bn = 256; ea.n_part = d / 128; }  // the fused kernel's tiles are 256 wide: every producer must match
     // a1: h0 = W2 swish(W1 [tau ; W_in x + b_in] + b1) + b2
     mark(e, ROSA_KC_INPROJ, s);
     launch_embed1(e->zbuf, e->x, e->wca, e->bca, e->tvec + (size_t)k * e->cfg.max_batch * d, dm, tb, k, M, s);

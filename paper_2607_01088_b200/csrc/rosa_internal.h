@@ -90,6 +90,7 @@ struct EpiArgs {
   const float* dt;        // Tables::dt
   const int* src;         // Tables::src
   int A, k_iter;
+  int force_bn;           // BIAS_F32 / RESID: N tile to use (0 = chosen from N and M)
   int dbg;                // measurement aid (ROSA_DBG): bit 0 skip the epilogue body, bit 1 skip the MMAs
 };
 
