@@ -123,7 +123,7 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
       auto load_k = [&](int i) {
         const int s = i % AT_KST;
         if (i == AT_KST - 2) mbar_wait(q_done, 0);  // Q has left the last two K stages
-        mbar_wait(k_empty(s), ((i / AT_KST) & 1) ^ 1);
+        mbar_wait_idle(k_empty(s), ((i / AT_KST) & 1) ^ 1);
         if (elect_one()) {
           mbar_expect_tx(k_full(s), AT_KV_BYTES);
           if (i == nbp) tma_load_3d(k_smem(s), &maps.own, k_full(s), 0, p * dm.H, dm.q_n / 64);
@@ -141,7 +141,7 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
       for (int i = 0; i < nb; ++i) {  // K runs one block ahead of V: it is needed a whole softmax earlier
         if (i + 1 < nb) load_k(i + 1);
         const int s = i % AT_ST;
-        mbar_wait(v_empty(s), ((i / AT_ST) & 1) ^ 1);
+        mbar_wait_idle(v_empty(s), ((i / AT_ST) & 1) ^ 1);
         if (elect_one()) {
           mbar_expect_tx(v_full(s), AT_KV_BYTES);
           if (i == nbp) tma_load_3d(v_smem(s), &maps.own, v_full(s), 0, p * dm.H, (dm.q_n + AT_HD) / 64);

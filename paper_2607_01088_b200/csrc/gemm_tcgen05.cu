@@ -346,7 +346,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
       const int m0 = (t % n_m) * BM, n0 = (t / n_m) * BN;
       for (int kb = 0; kb < n_kb; ++kb) {
-        mbar_wait(empty_bar(s), ph ^ 1);
+        mbar_wait_idle(empty_bar(s), ph ^ 1);
         if (elect_one()) {
           mbar_expect_tx(full_bar(s), Cfg::STAGE_BYTES);
           const uint32_t a_dst = smem_base + s * Cfg::STAGE_BYTES;
@@ -398,7 +398,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
       const uint32_t acc_ph = (it >> 1) & 1;
       const int m0 = (t % n_m) * BM, n0 = (t / n_m) * BN;
       const int r0 = m0 + q * 32;            // first row of this warp
-      mbar_wait(tfull_bar(acc), acc_ph);
+      mbar_wait_idle(tfull_bar(acc), acc_ph);
       tc_fence_after();
       const uint32_t t_acc = tmem_base + ((uint32_t)(q * 32) << 16) + acc * BN;
       auto release = [&] {
@@ -503,7 +503,7 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
     for (int t = pair; t < n_tiles; t += n_pairs) {
       const int m0 = (t % n_m) * (2 * BM) + (int)rank * BM, n0 = (t / n_m) * BN + (int)rank * (BN / 2);
       for (int kb = 0; kb < n_kb; ++kb) {
-        mbar_wait(empty_bar(s), ph ^ 1);
+        mbar_wait_idle(empty_bar(s), ph ^ 1);
         if (elect_one()) {
           const uint32_t lfull = mapa_shared(full_bar(s), 0);
           mbar_expect_tx_cluster(lfull, Cfg::STAGE_BYTES);
@@ -560,7 +560,7 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
       const uint32_t acc_ph = (it >> 1) & 1;
       const int m0 = (t % n_m) * (2 * BM) + (int)rank * BM, n0 = (t / n_m) * BN;
       const int r0 = m0 + q * 32;
-      mbar_wait(tfull_bar(acc), acc_ph);
+      mbar_wait_idle(tfull_bar(acc), acc_ph);
       tc_fence_after();
       const uint32_t t_acc = tmem_base + ((uint32_t)(q * 32) << 16) + acc * BN;
       auto release = [&] {
@@ -747,7 +747,7 @@ k_fused_tc2(const __grid_constant__ FusedMaps maps, const __grid_constant__ Fuse
       const int m0 = m * (2 * BM) + (int)rank * BM, n0 = n * BN + (int)rank * (BN / 2);
       const int n_kb = fm.n_kb[ph];
       for (int kb = 0; kb < n_kb; ++kb) {
-        mbar_wait(empty_bar(s), par ^ 1);
+        mbar_wait_idle(empty_bar(s), par ^ 1);
         if (elect_one()) {
           const uint32_t lfull = mapa_shared(full_bar(s), 0);
           mbar_expect_tx_cluster(lfull, Cfg::STAGE_BYTES);
@@ -797,7 +797,7 @@ k_fused_tc2(const __grid_constant__ FusedMaps maps, const __grid_constant__ Fuse
       const int acc = slot & 1;
       const uint32_t acc_ph = (slot >> 1) & 1;
       const int r0 = m * (2 * BM) + (int)rank * BM + q * 32, n0 = n * BN;
-      mbar_wait(tfull_bar(acc), acc_ph);
+      mbar_wait_idle(tfull_bar(acc), acc_ph);
       tc_fence_after();
       if (ph > 0) (void)ld_acquire_gpu(fm.done + (ph - 1) * fm.n_m_max + m);  // residual / partial sums of the previous phase
       const uint32_t t_acc = tmem_base + ((uint32_t)(q * 32) << 16) + acc * BN;

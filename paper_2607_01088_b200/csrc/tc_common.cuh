@@ -60,6 +60,15 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   }
 }
 
+// Same, for waits that are long by design (producer waiting for a free stage, epilogue waiting for an
+// accumulator): back off between polls so the idle warps do not burn issue slots and power.
+__device__ __forceinline__ void mbar_wait_idle(uint32_t bar, uint32_t parity) {
+  for (uint32_t spin = 0; !mbar_try_wait(bar, parity); ++spin) {
+    __nanosleep(40);
+    if (spin > (1u << 24)) __trap();
+  }
+}
+
 // ---------------------------------------------------------------- TMA
 __device__ __forceinline__ void prefetch_tensormap(const CUtensorMap* tm) {
   asm volatile("prefetch.tensormap [%0];" ::"l"(tm) : "memory");
