@@ -5,14 +5,16 @@
 // robot's key/value stream [prefix K/V (L_p rows, from the bound cache) ; own k/v (H rows, from
 // the qkv buffer)], walked in blocks of 64 keys:
 //     S = Q K_blk^T           tcgen05.mma  M=128 N=64  K=256   Q is the A operand FROM TENSOR MEMORY
-//     P = exp2(S*c - m_ref)   4 softmax warps, thread = query row, running (m_ref, l) in registers;
-//                             P (bf16) is written back into tensor memory over S
+//     P = exp2(S*c - m_ref)   8 softmax warps, two per query row (32 keys each; both read all 64 scores for
+//                             the row maximum), running (m_ref, partial l) in registers; P (bf16) is written
+//                             back into tensor memory over S
 //     O += P V_blk            tcgen05.mma  M=128 N=256 K=64    P is the A operand from tensor memory,
 //                             V the MN-major B operand from shared memory
 // Tensor memory (512 columns): O [0,256) | S/P double buffer [256,384) | Q [384,512).
-// Shared memory holds nothing but a 3-stage ring of K/V blocks (64 KB per stage) fed by TMA
-// (per-robot tensor maps made at bind time bound the ragged length: rows >= L_p are zero-filled
-// and masked), with L2 prefetches issued AT_PF blocks ahead.  Q passes through the last stage once.
+// Shared memory holds nothing but rings of K (4 stages) and V (3 stages) blocks of 32 KB, one 3-D TMA each
+// (per-robot tensor maps made at bind time bound the ragged length: rows >= L_p are zero-filled and masked),
+// K issued one block ahead of V, L2 prefetches AT_PF blocks ahead.  Q passes through the last two K stages once.
+// CTAs are issued longest prefix first (Tables::attn_order), so the second wave pairs long with short.
 // O stays in TMEM for the whole key stream; it is rescaled only when a row maximum grows by more
 // than 2^8 (lazy rescaling), which for N(0,1)-like logits almost never happens after block 0.
 #include <cstdlib>
@@ -35,7 +37,7 @@ constexpr int AT_PF = 6;          // L2 prefetch distance in blocks
 constexpr int AT_THREADS = 320;   // warp 0 TMA, warp 1 MMA, warps 2..9 softmax/epilogue (two per TMEM lane quarter)
 constexpr int AT_Q_BYTES = AT_ROWS * AT_HD * 2;     // 64 KB: 4 chunks [128 x 64] SW128
 constexpr int AT_KV_BYTES = AT_KV * AT_HD * 2;      // 32 KB: 4 chunks [64 x 64] SW128
-constexpr int AT_XCH_BYTES = 2 * 2 * AT_ROWS * 4;   // row-maximum / row-sum exchange between the two warps of a row
+constexpr int AT_XCH_BYTES = 2 * 2 * AT_ROWS * 4;   // row-sum exchange between the two warps of a row (epilogue)
 constexpr int AT_SMEM = (AT_KST + AT_ST) * AT_KV_BYTES + 256 + AT_XCH_BYTES;
 constexpr float AT_RESCALE_THR = 8.0f;              // log2 units
 
@@ -206,7 +208,7 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
   } else {
     // ---------------------------------------------------------- softmax + epilogue warps (2..9)
     // Two warps per TMEM lane quarter: a query row's 64 scores of a block are split 32 / 32 between
-    // warp w (half 0) and warp w + 4 (half 1).  They exchange the row maximum through shared memory
+    // warp w (half 0) and warp w + 4 (half 1).  Both read all 64 scores for the row maximum
     // (so both take the same rescale decision) and keep separate partial row sums until the end.
     const int q = warp & 3, half = (warp - 2) >> 2;
     const int r = q * 32 + lane;                       // query row of this thread

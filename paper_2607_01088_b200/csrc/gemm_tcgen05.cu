@@ -1,17 +1,19 @@
-// tcgen05 / TMEM / TMA bf16 GEMM with fused epilogues (steps a1, a3+a4, a6, a7, a8 of the path).
+// tcgen05 / TMEM / TMA GEMMs with fused epilogues (steps a1, a2+a3+a4, a6, a2+a7, a8, a9+a10 of the path).
 //
-//   C[M,N] = A[M,K] * W[N,K]^T   (A activations, W weights; both K-major bf16; fp32 accumulate)
+//   C[M,N] = A[M,K] * W[N,K]^T   (A activations, W weights; both K-major fp16 or bf16; fp32 accumulate)
 //
-// Persistent, warp-specialised, one CTA per SM:
-//   warp 0      TMA producer: A tile [128 x 64] + W tile [BN x 64] per k-block into a ring of
-//               SWIZZLE_128B stages, completion on "full" mbarriers
-//   warp 1      MMA issuer: one lane issues 4 x tcgen05.mma (M=128, N=BN, K=16) per stage into a
-//               TMEM accumulator; tcgen05.commit frees the stage ("empty") and, after the last
-//               k-block, publishes the accumulator ("tmem full")
-//   warps 2..5  epilogue: tcgen05.ld the accumulator (thread = one row, 32 columns at a time),
-//               apply the fused epilogue, store to global, release the accumulator ("tmem empty")
-// The accumulator is double-buffered in TMEM (2 x BN columns) so the epilogue of tile i overlaps
-// the MMAs of tile i+1.
+// Persistent, warp-specialised, one CTA per SM, 10 warps:
+//   warp 0      TMA producer: A tile [128 x 64] + W tile per k-block into a ring of SWIZZLE_128B
+//               stages, completion on "full" mbarriers
+//   warp 1      MMA issuer: the elected lane issues 4 x tcgen05.mma per stage into a TMEM accumulator;
+//               tcgen05.commit frees the stage ("empty") and, after the last k-block, publishes the
+//               accumulator ("tmem full")
+//   warps 2..9  epilogue, two warps per TMEM lane quarter (half of the tile's columns each): tcgen05.ld,
+//               fused epilogue (epilogue_tile below), coalesced global stores, release ("tmem empty")
+// The accumulator is double-buffered in TMEM (2 x BN columns) so the epilogue of tile i overlaps the
+// MMAs of tile i+1.  Three kernels share the pipeline: k_gemm_tc2 (CTA pairs, cta_group::2, 256-row tiles:
+// the workhorse for M > 128), k_gemm_tc (single CTA, 128-row tiles: small batches) and the opt-in
+// k_fused_tc2 (O -> gate/up -> down of a layer in one launch with dependency counters).
 #include <algorithm>
 #include <cstdlib>
 #include <map>
