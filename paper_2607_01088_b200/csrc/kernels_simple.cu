@@ -37,7 +37,7 @@ void launch_scatter_x(const CallPtrs* cp, const float* x, const Tables& tb, int 
 // The time half of W_1 u is per robot, not per token, and t_k is known at call time, so it is
 // computed once per call for every iteration.  sin/cos in fp64: angles reach ~1571 rad.
 __global__ void k_timevec(float* __restrict__ tvec, const bf16* __restrict__ w_t1,
-                          const float* __restrict__ b_t1, Dims dm, Tables tb, int max_batch) {
+                          const float* __restrict__ b_t1, Dims dm, Tables tb) {
   extern __shared__ float tau[];  // [d]
   pdl_wait();
   pdl_trigger();
@@ -54,7 +54,7 @@ __global__ void k_timevec(float* __restrict__ tvec, const bf16* __restrict__ w_t
   }
   __syncthreads();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
-  float* out = tvec + ((size_t)k * max_batch + p) * d;
+  float* out = tvec + ((size_t)k * tb.batch + p) * d;   // [k][batch][d], compact in the call's batch
   for (int n = warp; n < d; n += nw) {
     const bf16* wr = w_t1 + (size_t)n * 2 * d;
     float acc = 0.f;
@@ -64,17 +64,44 @@ __global__ void k_timevec(float* __restrict__ tvec, const bf16* __restrict__ w_t
   }
 }
 void launch_timevec(float* tvec, const bf16* w_t1, const float* b_t1, const Dims& dm,
-                    const Tables& tb, int nsteps_max, int max_batch, cudaStream_t s) {
+                    const Tables& tb, int nsteps_max, cudaStream_t s) {
   dim3 grid(tb.batch, nsteps_max);
-  launch_k(k_timevec, grid, dim3(256), dm.d * sizeof(float), s, tvec, w_t1, b_t1, dm, tb, max_batch);
+  launch_k(k_timevec, grid, dim3(256), dm.d * sizeof(float), s, tvec, w_t1, b_t1, dm, tb);
+}
+
+// The same time half as a tensor-core GEMM (tcgen05 family): this kernel writes the A operand, row
+// (k, p) = [hi(tau) | lo(tau)] with hi = op16(tau), lo = op16(tau - hi), so the 16-bit operand carries tau
+// to ~2^-22 (fp16) and the GEMM against [W_t | W_t] (K = 2d) + b_1 epilogue reproduces the fp32 dot product.
+__global__ void k_tau16(op16* __restrict__ a16, Dims dm, Tables tb) {
+  pdl_wait();
+  pdl_trigger();
+  const int p = blockIdx.x, k = blockIdx.y, d = dm.d, half = d / 2;
+  const double t = (double)tb.t0[p] + (double)k * (double)tb.dt[p];
+  op16* row = a16 + ((size_t)k * tb.batch + p) * 2 * d;
+  for (int j = threadIdx.x; j < half; j += blockDim.x) {
+    double frac = (double)j / (double)(half > 1 ? half - 1 : 1);
+    double period = (double)dm.pmin * pow((double)dm.pmax / (double)dm.pmin, frac);
+    double sn, cs;
+    sincos(6.283185307179586476925286766559 * t / period, &sn, &cs);
+    const float v[2] = {(float)sn, (float)cs};
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+      const op16 hi = f2op(v[i], dm.fp16);
+      row[i * half + j] = hi;
+      row[d + i * half + j] = f2op(v[i] - op2f(hi, dm.fp16), dm.fp16);
+    }
+  }
+}
+void launch_tau16(op16* a16, const Dims& dm, const Tables& tb, int nsteps_max, cudaStream_t s) {
+  launch_k(k_tau16, dim3(tb.batch, nsteps_max), dim3(256), 0, s, a16, dm, tb);
 }
 
 // ------------------------------------------------------------------ a1 (action half + swish)
 // z[m][n] = swish( sum_c x[m][c] Wca[c][n] + bca[n] + tvec[p][n] ), with Wca = (W_1[:, d:] W_in)^T and
 // bca = W_1[:, d:] b_in folded at create (fp64 on the host): W_1 [tau ; W_in x + b_in] + b_1 is
 // linear in x, so the K = A contraction runs in fp32 on CUDA cores straight from x (R11: x fp32).
-// Block = EM_ROWS token rows; thread = output columns n, n + 256, ...
-constexpr int EM_ROWS = 16;
+// Block = EM_ROWS token rows; thread = 4 adjacent output columns (float4 weight loads, 8-byte stores).
+constexpr int EM_ROWS = 8;
 __global__ void __launch_bounds__(256) k_embed1(op16* __restrict__ z, const float* __restrict__ x,
                                                 const float* __restrict__ wca, const float* __restrict__ bca,
                                                 const float* __restrict__ tvec, int d, int A, int H, int fp16,
@@ -90,19 +117,33 @@ __global__ void __launch_bounds__(256) k_embed1(op16* __restrict__ z, const floa
     xs[r][c] = r < rows ? x[(size_t)(m0 + r) * A + c] : 0.f;
   }
   __syncthreads();
-  for (int n = threadIdx.x; n < d; n += blockDim.x) {
-    float acc[EM_ROWS];
-    const float b = bca[n];
+  for (int n = 4 * threadIdx.x; n < d; n += 4 * blockDim.x) {
+    float4 acc[EM_ROWS];
+    const float4 b = *reinterpret_cast<const float4*>(bca + n);
 #pragma unroll
     for (int r = 0; r < EM_ROWS; ++r) acc[r] = b;
+#pragma unroll 8
     for (int c = 0; c < A; ++c) {
-      const float w = wca[(size_t)c * d + n];  // [A, d]: consecutive threads, consecutive addresses
+      const float4 w = *reinterpret_cast<const float4*>(wca + (size_t)c * d + n);  // [A, d]
 #pragma unroll
-      for (int r = 0; r < EM_ROWS; ++r) acc[r] = fmaf(xs[r][c], w, acc[r]);
+      for (int r = 0; r < EM_ROWS; ++r) {
+        const float xv = xs[r][c];
+        acc[r].x = fmaf(xv, w.x, acc[r].x);
+        acc[r].y = fmaf(xv, w.y, acc[r].y);
+        acc[r].z = fmaf(xv, w.z, acc[r].z);
+        acc[r].w = fmaf(xv, w.w, acc[r].w);
+      }
     }
-    for (int r = 0; r < rows; ++r) {
-      const int m = m0 + r;
-      z[(size_t)m * d + n] = f2op(swish_f(acc[r] + tvec[(size_t)(m / H) * d + n]), fp16);
+#pragma unroll
+    for (int r = 0; r < EM_ROWS; ++r) {
+      if (r < rows) {
+        const int m = m0 + r;
+        const float4 tv = *reinterpret_cast<const float4*>(tvec + (size_t)(m / H) * d + n);
+        uint2 o;
+        o.x = pack_op2(swish_f(acc[r].x + tv.x), swish_f(acc[r].y + tv.y), fp16);
+        o.y = pack_op2(swish_f(acc[r].z + tv.z), swish_f(acc[r].w + tv.w), fp16);
+        *reinterpret_cast<uint2*>(z + (size_t)m * d + n) = o;
+      }
     }
   }
 }

@@ -66,6 +66,7 @@ struct rosa_expert {
   bf16 *w_t1 = nullptr, *w_out = nullptr;  // CUDA-core steps: bf16 as given
   float *wca = nullptr, *bca = nullptr;    // (W_1[:, d:] W_in)^T [A, d] and W_1[:, d:] b_in [d], folded in fp64
   op16* w_t2 = nullptr;                    // GEMM operand: fp16 or bf16 (dm.fp16)
+  op16 *w_t1dup = nullptr, *tau16 = nullptr;  // tcgen05 family: [W_1[:, :d] | W_1[:, :d]] [d, 2d] and the [hi | lo] tau rows
   op16* w_out16 = nullptr;                 // [64, d]: W_out with the final-norm gain folded in, zero rows past A (tcgen05 family)
   float *b_t1 = nullptr, *b_t2 = nullptr, *b_out = nullptr, *g_final = nullptr;
   std::vector<LayerWeights> lw;
@@ -226,6 +227,12 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
     if ((st = fetch_f32(w->w_in, (size_t)d * A, dt, od, win)) != ROSA_OK) return st;
     if ((st = fetch_f32(w->b_in, (size_t)d, dt, od, bin)) != ROSA_OK) return st;
     FETCH(w->w_t1, (size_t)d * 2 * d); UPB(e->w_t1);
+    if (e->family == 1) {  // time half twice along K: pairs with the [hi(tau) | lo(tau)] operand rows of k_tau16
+      std::vector<float> dup((size_t)d * 2 * d);
+      for (int n = 0; n < d; ++n)
+        for (int c = 0; c < d; ++c) dup[(size_t)n * 2 * d + c] = dup[(size_t)n * 2 * d + d + c] = t[(size_t)n * 2 * d + c];
+      if ((st = upload_op16(e, dup, &e->w_t1dup)) != ROSA_OK) return st;
+    }
     std::vector<float> wca((size_t)d * A), bca(d);
     std::vector<double> accr(A);
     for (int n = 0; n < d; ++n) {
@@ -316,6 +323,7 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
   WS(e->h, Mmax * d * 4);
   WS(e->tvec, (size_t)c->max_steps * c->max_batch * d * 4);
   WS(e->zbuf, Mmax * d * 2);
+  if (e->family == 1) WS(e->tau16, ((size_t)c->max_steps * c->max_batch + 127) / 128 * 128 * 2 * d * 2);
   WS(e->nrm, Mmax * d * 2);
   WS(e->qkv, Mmax * dm.qkv_n * 2);
   WS(e->obuf, Mmax * dm.q_n * 2);
@@ -437,8 +445,16 @@ static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, cudaStream_
   mark(e, ROSA_KC_GATHER_SCATTER, s);
   launch_gather_x(e->x, cp, tb, dm.H * dm.A, e->d_done, e->fused_ok ? 2 * kFusedPhases * e->n_m_max : 0, s);
   mark(e, ROSA_KC_TIMEVEC, s);
-  launch_timevec(e->tvec, e->w_t1, e->b_t1, dm, tb, nmax, e->cfg.max_batch, s);
-  e->last_launches += 2;
+  if (e->family == 1 && tc_gemm_supported(d, 2 * d)) {  // a1 time half of every (step, robot) as one GEMM
+    launch_tau16(e->tau16, dm, tb, nmax, s);
+    EpiArgs et{};
+    et.in_fp16 = dm.fp16; et.out_f32 = e->tvec; et.ld_out = d; et.bias = e->b_t1;
+    if ((err = launch_gemm_tc(EPI_BIAS_F32, e->tau16, e->w_t1dup, nmax * batch, d, 2 * d, et, s)) != cudaSuccess) return err;
+    e->last_launches += 3;
+  } else {
+    launch_timevec(e->tvec, e->w_t1, e->b_t1, dm, tb, nmax, s);
+    e->last_launches += 2;
+  }
   const bool fused_norm = e->family == 1;  // RMSNorm fused into the GEMM epilogues (tcgen05 family)
   const bool use_fused = e->fused_ok && tc_use_pair(M);
   int fused_idx = 0;
@@ -451,7 +467,7 @@ static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, cudaStream_
     if (use_fused) { ea.force_bn = 256; ea.n_part = d / 128; }  // the fused kernel's tiles are 256 wide: every producer must match
     // a1: h0 = W2 swish(W1 [tau ; W_in x + b_in] + b1) + b2
     mark(e, ROSA_KC_INPROJ, s);
-    launch_embed1(e->zbuf, e->x, e->wca, e->bca, e->tvec + (size_t)k * e->cfg.max_batch * d, dm, tb, k, M, s);
+    launch_embed1(e->zbuf, e->x, e->wca, e->bca, e->tvec + (size_t)k * batch * d, dm, tb, k, M, s);
     e->last_launches += 1;
     ea.out_f32 = e->h; ea.ld_out = d; ea.bias = e->b_t2;
     if ((err = gemm(e, ROSA_KC_GEMM_EMBED, EPI_BIAS_F32, e->zbuf, e->w_t2, M, d, d, ea, s)) != cudaSuccess) return err;

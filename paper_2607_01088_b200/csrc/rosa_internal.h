@@ -105,7 +105,8 @@ void launch_attn_simple(const Dims& dm, const Tables& tb, int layer, const bf16*
 void launch_gather_x(float* x, const CallPtrs* cp, const Tables& tb, int HA, int* zero, int n_zero, cudaStream_t s);
 void launch_scatter_x(const CallPtrs* cp, const float* x, const Tables& tb, int HA, cudaStream_t s);
 void launch_timevec(float* tvec, const bf16* w_t1, const float* b_t1, const Dims& dm,
-                    const Tables& tb, int nsteps_max, int max_batch, cudaStream_t s);
+                    const Tables& tb, int nsteps_max, cudaStream_t s);
+void launch_tau16(op16* a16, const Dims& dm, const Tables& tb, int nsteps_max, cudaStream_t s);
 void launch_embed1(op16* z, const float* x, const float* wca, const float* bca, const float* tvec_k,
                    const Dims& dm, const Tables& tb, int k_iter, int M, cudaStream_t s);
 void launch_rmsnorm(op16* out, const float* h, const Dims& dm, const Tables& tb, int k_iter, int M,

@@ -342,4 +342,4 @@ def test_fused_dependent_gemm_kernel_opt_in(monkeypatch):
         lc.close()
         compare(f"fused-order{order}", got_x, got_v, want_x, want_v)
         assert np.array_equal(got_x, again)                       # deterministic
-        assert n_launch == 2 + 2 * (2 + 2 * 3 + 1) + 1            # 3 kernels per layer instead of 5
+        assert n_launch == 3 + 2 * (2 + 2 * 3 + 1) + 1            # gather, tau, time GEMM; per step 2 + 3 per layer (not 5) + 1; scatter
