@@ -102,24 +102,28 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, float* scr, uin
   if constexpr (EPI == EPI_STORE_F32 || EPI == EPI_BIAS_F32 || EPI == EPI_RESID) {
     // h (fp32) = acc [+ h] [+ bias]; optionally also the 16-bit copy of the new h (A operand of
     // the next GEMM) and this half-tile's partial sum of squares of each row (fused RMSNorm, a2)
-    constexpr int NC = BN / 64;  // 32-column chunks per half
+    // 32-column chunks: half 0 takes the first NC0, half 1 the rest.  BN need not divide N (nor be a
+    // multiple of 32): columns at or beyond min(n0 + BN, N) are masked, in groups of 4.
+    constexpr int NCT = (BN + 31) / 32, NC0 = (NCT + 1) / 2;
+    const int c_beg = half ? NC0 : 0, c_end = half ? NCT : NC0;
+    const int n_end = min(n0 + BN, N);
     float rowss[8];
 #pragma unroll
     for (int i = 0; i < 8; ++i) rowss[i] = 0.f;
     const bool want_h16 = EPI != EPI_STORE_F32 && ea.h16 != nullptr;
 #pragma unroll 1
-    for (int cc = 0; cc < NC; ++cc) {
-      const int c = half * NC + cc;
+    for (int c = c_beg; c < c_end; ++c) {
       {
         float v[32];
         ld_acc32(t_acc + c * 32, v);
-        if (cc == NC - 1) release();
+        if (c == c_end - 1) release();
         to_scratch(v);
       }
       __syncwarp();
       const int col = n0 + c * 32 + lc;
+      const bool colok = col < n_end;
       float4 add = make_float4(0.f, 0.f, 0.f, 0.f);
-      if constexpr (EPI == EPI_BIAS_F32) add = *reinterpret_cast<const float4*>(ea.bias + col);
+      if constexpr (EPI == EPI_BIAS_F32) { if (colok) add = *reinterpret_cast<const float4*>(ea.bias + col); }
       float* gp = ea.out_f32 + (size_t)(r0 + lr) * ea.ld_out + col;
       uint16_t* hp = (uint16_t*)ea.h16 + (size_t)(r0 + lr) * ea.ld_out + col;
       const size_t step = (size_t)4 * ea.ld_out;
@@ -128,7 +132,7 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, float* scr, uin
       if constexpr (EPI == EPI_RESID) {
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
-          if (r0 + i * 4 + lr < m_lim) {
+          if (colok && r0 + i * 4 + lr < m_lim) {
             const float4 h = *reinterpret_cast<const float4*>(gp + i * step);
             o[i].x += h.x; o[i].y += h.y; o[i].z += h.z; o[i].w += h.w;
           }
@@ -137,7 +141,7 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, float* scr, uin
 #pragma unroll
       for (int i = 0; i < 8; ++i) {
         o[i].x += add.x; o[i].y += add.y; o[i].z += add.z; o[i].w += add.w;
-        if (r0 + i * 4 + lr < m_lim) {
+        if (colok && r0 + i * 4 + lr < m_lim) {
           *reinterpret_cast<float4*>(gp + i * step) = o[i];
           if constexpr (EPI != EPI_STORE_F32) {
             if (want_h16)
@@ -158,7 +162,8 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, float* scr, uin
           v += __shfl_xor_sync(0xffffffffu, v, 2);
           v += __shfl_xor_sync(0xffffffffu, v, 4);
           const int rw = r0 + i * 4 + lr;
-          if ((lane & 7) == 0 && rw < m_lim) ea.ssq_out[(size_t)rw * (2 * N / BN) + 2 * (n0 / BN) + half] = v;
+          if ((lane & 7) == 0 && rw < m_lim)
+            ea.ssq_out[(size_t)rw * (2 * ((N + BN - 1) / BN)) + 2 * (n0 / BN) + half] = v;
         }
       }
     }
@@ -440,12 +445,16 @@ int tc_gemm_read_trace(long long* host, int n) {
 // the single-CTA tile, which is what bounds the single-CTA kernel (profiles/r1_gemm_notes.md).
 template <int BN>
 struct Gemm2Cfg {
-  static constexpr int STAGES = BN == 256 ? 5 : (BN == 128 ? 7 : 8);
+  static_assert(BN % 16 == 0 && BN >= 64 && BN <= 256, "pair tile width");
   static constexpr int A_BYTES = BM * BK * 2;
   static constexpr int B_BYTES = (BN / 2) * BK * 2;
-  static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
-  static constexpr int SMEM = STAGES * STAGE_BYTES + 1024 + 256 + kEpiWarps * kScrFloats * 4;
-  static constexpr int TMEM_COLS = 2 * BN < 32 ? 32 : 2 * BN;
+  static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;  // a multiple of 1024 for every BN % 16 == 0
+  static constexpr int FIXED = 1024 + 256 + kEpiWarps * kScrFloats * 4;
+  static constexpr int FIT = (232448 - FIXED) / STAGE_BYTES;
+  static constexpr int STAGES = FIT > 8 ? 8 : FIT;
+  static constexpr int SMEM = STAGES * STAGE_BYTES + FIXED;
+  static constexpr int ACC_STRIDE = BN <= 64 ? 64 : (BN <= 128 ? 128 : 256);  // columns between the two accumulators
+  static constexpr int TMEM_COLS = 2 * ACC_STRIDE;
 };
 
 template <int BN, int EPI>
@@ -469,7 +478,7 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
   if (warp == 0) GT_TRACE(0);
   const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
   const int m_lim = ea.m_active ? min(M, *ea.m_active) : M;
-  const int n_m = (m_lim + 2 * BM - 1) / (2 * BM), n_n = N / BN;
+  const int n_m = (m_lim + 2 * BM - 1) / (2 * BM), n_n = (N + BN - 1) / BN;  // the last column tile may hang over N
   const int n_tiles = n_m * n_n, n_kb = K / BK;
 
   if (warp == 0 && lane == 0) {
@@ -528,7 +537,7 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
         const uint32_t acc_ph = (it >> 1) & 1;
         mbar_wait(tempty_bar(acc), acc_ph ^ 1);
         tc_fence_after();
-        const uint32_t d_tmem = tmem_base + acc * BN;
+        const uint32_t d_tmem = tmem_base + acc * Cfg::ACC_STRIDE;
         for (int kb = 0; kb < n_kb; ++kb) {
           mbar_wait(full_bar(s), ph);
           tc_fence_after();
@@ -564,7 +573,7 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
       const int r0 = m0 + q * 32;
       mbar_wait_idle(tfull_bar(acc), acc_ph);
       tc_fence_after();
-      const uint32_t t_acc = tmem_base + ((uint32_t)(q * 32) << 16) + acc * BN;
+      const uint32_t t_acc = tmem_base + ((uint32_t)(q * 32) << 16) + acc * Cfg::ACC_STRIDE;
       auto release = [&] {
         tc_fence_before();
         __syncwarp();
@@ -911,19 +920,41 @@ bool tc_gemm_supported(int N, int K) { return N % 64 == 0 && K % 64 == 0 && N >=
 // CTA pairs (256-row tiles) once there is more than one 128-row tile of tokens
 static bool use_pair(int M) { return M > BM; }
 bool tc_use_pair(int M) { return use_pair(M); }
-// N tile of the EPI_BIAS_F32 / EPI_RESID launches
-// Small batches are latency-bound (a serial K loop per tile), so narrower tiles are chosen until about
-// half of the CTAs (or CTA pairs) have a tile; from B = 64 on this is 256 (pairs) as before.
+// N tile of the EPI_BIAS_F32 / EPI_RESID launches.
+// Single CTA (M <= 128): latency-bound (a serial K loop per tile), so narrower tiles are chosen until about
+// half of the CTAs have a tile.
+// CTA pairs: these GEMMs have few tiles (N = d), so whole rounds of tiles over the pairs decide the time:
+// 13 row blocks x 4 tiles of 256 columns leave 22 of 74 pairs idle, 13 x 5 tiles of 208 do not.  The width
+// is the candidate with the least rounds x (time per k-block + fixed cost per tile), where a k-block costs
+// max(MMA time ~ 2 BN, operand feed ~ 288 + BN) cycles (the L2 -> shared-memory feed bounds narrow tiles;
+// measured: profiles/r1_gemm_tile_width.md).
+static const int kPairBn[] = {256, 224, 192, 160, 128, 96, 64};
 static int resid_bn(int N, int M) {
-  const bool pair = use_pair(M);
-  const int units = pair ? num_sms() / 2 : num_sms();
-  const int n_m = pair ? (M + 2 * BM - 1) / (2 * BM) : (M + BM - 1) / BM;
-  for (int bn = pair ? 256 : 128; bn > 64; bn >>= 1)
-    if (N % bn == 0 && n_m * (N / bn) * 2 >= units) return bn;
-  return 64;
+  if (!use_pair(M)) {
+    const int units = num_sms(), n_m = (M + BM - 1) / BM;
+    for (int bn = 128; bn > 64; bn >>= 1)
+      if (N % bn == 0 && n_m * (N / bn) * 2 >= units) return bn;
+    return 64;
+  }
+  static const int forced = getenv("ROSA_RESID_BN") ? atoi(getenv("ROSA_RESID_BN")) : 0;  // experiments only
+  if (forced) return forced;
+  const int pairs = num_sms() / 2, n_m = (M + 2 * BM - 1) / (2 * BM);
+  int best = 256;
+  long best_cost = -1;
+  for (int bn : kPairBn) {
+    const int tiles = n_m * ((N + bn - 1) / bn);
+    const long rounds = (tiles + pairs - 1) / pairs;
+    const long per_kb = 2 * bn > 288 + bn ? 2 * bn : 288 + bn;
+    const long cost = rounds * (per_kb * 32 + 4000);  // 32 k-blocks (K = 2048) as the reference depth
+    if (best_cost < 0 || cost < best_cost) { best = bn; best_cost = cost; }
+  }
+  return best;
 }
-// columns per sum-of-squares partial written by those launches (half an N tile: two epilogue warps per row)
-int tc_ssq_cols(int N, int M) { return resid_bn(N, M) / 2; }
+// sum-of-squares partials per row written by those launches: one per half N tile (two epilogue warps per row)
+int tc_ssq_parts(int N, int M) {
+  const int bn = resid_bn(N, M);
+  return 2 * ((N + bn - 1) / bn);
+}
 
 template <int BN, int EPI>
 static cudaError_t launch_one(const op16* A, const op16* W, int M, int N, int K, const EpiArgs& a, cudaStream_t s) {
@@ -956,7 +987,7 @@ static cudaError_t launch_two(const op16* A, const op16* W, int M, int N, int K,
   if (!make_tmap_2d(&tmA, A, (uint64_t)M, (uint64_t)K, BM, a.in_fp16) ||
       !make_tmap_2d(&tmB, W, (uint64_t)N, (uint64_t)K, BN / 2, a.in_fp16))
     return cudaErrorInvalidValue;
-  const int tiles = ((M + 2 * BM - 1) / (2 * BM)) * (N / BN);
+  const int tiles = ((M + 2 * BM - 1) / (2 * BM)) * ((N + BN - 1) / BN);
   const int pairs = tiles < num_sms() / 2 ? tiles : num_sms() / 2;
   return launch_k(k_gemm_tc2<BN, EPI>, dim3(2 * pairs), dim3(kGemmThreads), Cfg::SMEM, s, tmA, tmB, M, N, K, a);
 }
@@ -967,9 +998,16 @@ static cudaError_t launch_by_n(const op16* A, const op16* W, int M, int N, int K
   const bool pair = forced ? forced / 1000 == 2 : use_pair(M);
   const int bn = forced ? forced % 1000 : (a.force_bn ? a.force_bn : resid_bn(N, M));
   if (pair) {
-    if (bn == 256) return launch_two<256, EPI>(A, W, M, N, K, a, s);
-    if (bn == 128) return launch_two<128, EPI>(A, W, M, N, K, a, s);
-    return launch_two<64, EPI>(A, W, M, N, K, a, s);
+    switch (bn) {
+      case 256: return launch_two<256, EPI>(A, W, M, N, K, a, s);
+      case 224: return launch_two<224, EPI>(A, W, M, N, K, a, s);
+      case 192: return launch_two<192, EPI>(A, W, M, N, K, a, s);
+      case 160: return launch_two<160, EPI>(A, W, M, N, K, a, s);
+      case 128: return launch_two<128, EPI>(A, W, M, N, K, a, s);
+      case 96: return launch_two<96, EPI>(A, W, M, N, K, a, s);
+      case 64: return launch_two<64, EPI>(A, W, M, N, K, a, s);
+      default: return cudaErrorNotSupported;
+    }
   }
   if (bn == 256) return launch_one<256, EPI>(A, W, M, N, K, a, s);
   if (bn == 128) return launch_one<128, EPI>(A, W, M, N, K, a, s);

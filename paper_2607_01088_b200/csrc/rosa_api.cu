@@ -462,7 +462,7 @@ static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, cudaStream_
     EpiArgs ea{};
     ea.m_active = tb.m_active + k;
     ea.H = dm.H; ea.hd = dm.hd; ea.gu_blk = dm.gu_blk; ea.in_fp16 = dm.fp16; ea.out_fp16 = dm.fp16;
-    ea.inv_d = 1.f / (float)d; ea.eps = dm.eps; ea.n_part = d / tc_ssq_cols(d, M);
+    ea.inv_d = 1.f / (float)d; ea.eps = dm.eps; ea.n_part = tc_ssq_parts(d, M);
     if (fused_norm) { ea.h16 = e->nrm; ea.ssq_out = e->ssq; ea.ssq_in = e->ssq; }
     if (use_fused) { ea.force_bn = 256; ea.n_part = d / 128; }  // the fused kernel's tiles are 256 wide: every producer must match
     // a1: h0 = W2 swish(W1 [tau ; W_in x + b_in] + b1) + b2
