@@ -14,8 +14,10 @@ library primitive used.  No blocking, fusion or reordering beyond the definition
 Pins (tests/test_oracle_pins.py): brute-force fp64 attention loops, closed forms (constant
 velocity, zero output projection, uniform attention, RoPE shift invariance, norm scale
 invariance), step composition, batch/permutation invariance, and torch fp64 library
-routines as an independent third opinion.  The numeric output of a *trained* model is
-"parity unpinned": no trained weights or published tensors exist for this path.
+routines as an independent third opinion.  The adaptive-norm variant (reading R25) is pinned by
+its reductions: zero modulation with unit gate equals the pinned blocks on the same normed input,
+zero gate is the identity, a hand-written per-element loop, and torch fp64.  The numeric output
+of a *trained* model is "parity unpinned": no trained weights or published tensors exist.
 """
 from __future__ import annotations
 
@@ -116,15 +118,12 @@ def embed(cfg, W: Dict, x: np.ndarray, t: np.ndarray, dtype=F) -> np.ndarray:
     return z @ _as(W["w_t2"], dtype).T + _as(W["b_t2"], dtype)
 
 
-def layer(cfg, W: Dict, l: int, h: np.ndarray, prefix_k: Sequence[np.ndarray],
-          prefix_v: Sequence[np.ndarray], dtype=F) -> np.ndarray:
-    """One pre-norm transformer block (step 4 of SURVEY 8(c)).
-
-    h: [B, H, d]; prefix_k[i], prefix_v[i]: [L_i, n_kv, hd] of THIS layer for robot i.
-    """
-    B, H, d = h.shape
+def attention_sublayer(cfg, W: Dict, l: int, n1: np.ndarray, prefix_k: Sequence[np.ndarray],
+                       prefix_v: Sequence[np.ndarray], dtype=F) -> np.ndarray:
+    """Attention half of a block, from the normed input n1 [B, H, d] to the W_o output [B, H, d]
+    (step 4 of SURVEY 8(c)).  prefix_k[i], prefix_v[i]: [L_i, n_kv, hd] of THIS layer for robot i."""
+    B, H, d = n1.shape
     nq, nkv, hd = cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim
-    n1 = rmsnorm(h, _as(W["g_attn"][l], dtype), cfg.rms_eps)
     q = (n1 @ _as(W["wq"][l], dtype).T).reshape(B, H, nq, hd)
     k = (n1 @ _as(W["wk"][l], dtype).T).reshape(B, H, nkv, hd)
     v = (n1 @ _as(W["wv"][l], dtype).T).reshape(B, H, nkv, hd)
@@ -137,15 +136,68 @@ def layer(cfg, W: Dict, l: int, h: np.ndarray, prefix_k: Sequence[np.ndarray],
         k_all = np.concatenate([_as(prefix_k[i], dtype), k_i], axis=0)    # prefix K is stored rotated
         v_all = np.concatenate([_as(prefix_v[i], dtype), v[i]], axis=0)
         o[i] = attention_robot(q_i, k_all, v_all)
-    h = h + o.reshape(B, H, nq * hd) @ _as(W["wo"][l], dtype).T
-    n2 = rmsnorm(h, _as(W["g_mlp"][l], dtype), cfg.rms_eps)
+    return o.reshape(B, H, nq * hd) @ _as(W["wo"][l], dtype).T
+
+
+def mlp_sublayer(cfg, W: Dict, l: int, n2: np.ndarray, dtype=F) -> np.ndarray:
+    """GeGLU MLP half of a block, from the normed input n2 to the W_down output (reading R6)."""
     m = gelu_tanh(n2 @ _as(W["w_gate"][l], dtype).T) * (n2 @ _as(W["w_up"][l], dtype).T)
-    return h + m @ _as(W["w_down"][l], dtype).T
+    return m @ _as(W["w_down"][l], dtype).T
+
+
+def layer(cfg, W: Dict, l: int, h: np.ndarray, prefix_k: Sequence[np.ndarray],
+          prefix_v: Sequence[np.ndarray], dtype=F) -> np.ndarray:
+    """One pre-norm transformer block (step 4 of SURVEY 8(c)); h: [B, H, d]."""
+    n1 = rmsnorm(h, _as(W["g_attn"][l], dtype), cfg.rms_eps)
+    h = h + attention_sublayer(cfg, W, l, n1, prefix_k, prefix_v, dtype)
+    n2 = rmsnorm(h, _as(W["g_mlp"][l], dtype), cfg.rms_eps)
+    return h + mlp_sublayer(cfg, W, l, n2, dtype)
+
+
+# ----------------------------------------------------------------------------- adaptive-norm variant
+# SURVEY.md 8(f) item 4 / PAPER.md:438: the paper also evaluates pi0.5, whose action expert takes the
+# flow-matching time through adaptive RMSNorm instead of the concatenated time MLP.  DESIGN.md reading
+# R25 fixes the form (cfg.time_conditioning == 1):
+#   cond   = swish(W_t2 swish(W_t1 tau(t) + b_t1) + b_t2)  in R^d       (W_t1 is [d, d] here)
+#   h0     = W_in x + b_in                                               (no time in the token embedding)
+#   every norm n:  (scale, shift, gate) = W_mod^n cond + b_mod^n  in R^{3d}, split in that order,
+#                  y = h rsqrt(mean(h^2) + eps) (1 + scale) + shift     (no learned gain),
+#                  h <- h + gate * sublayer(y);  the final norm uses scale and shift only.
+def time_condition(cfg, W: Dict, t: np.ndarray, dtype=F) -> np.ndarray:
+    """cond [B, d] of the adaptive-norm variant (reading R25)."""
+    tau = sinusoidal_time_embedding(t, cfg.d_model, cfg.time_min_period, cfg.time_max_period, dtype)
+    z = swish(tau @ _as(W["w_t1"], dtype).T + _as(W["b_t1"], dtype))
+    return swish(z @ _as(W["w_t2"], dtype).T + _as(W["b_t2"], dtype))
+
+
+def adarms(h: np.ndarray, cond: np.ndarray, w_mod: np.ndarray, b_mod: np.ndarray, eps: float):
+    """Adaptive RMSNorm (reading R25): h [B, H, d], cond [B, d] -> (y [B, H, d], gate [B, 1, d])."""
+    d = h.shape[-1]
+    mod = cond @ w_mod.T + b_mod                                          # [B, 3d]
+    scale, shift, gate = mod[:, None, :d], mod[:, None, d:2 * d], mod[:, None, 2 * d:]
+    ms = np.mean(h * h, axis=-1, keepdims=True)
+    return h / np.sqrt(ms + eps) * (1.0 + scale) + shift, gate
+
+
+def velocity_adarms(cfg, W: Dict, x: np.ndarray, t: np.ndarray, prefix_k: Sequence[np.ndarray],
+                    prefix_v: Sequence[np.ndarray], dtype=F) -> np.ndarray:
+    """v(x, t) of the adaptive-norm variant.  prefix_k[i]: [layers, L_i, n_kv, hd]."""
+    cond = time_condition(cfg, W, t, dtype)
+    h = x @ _as(W["w_in"], dtype).T + _as(W["b_in"], dtype)
+    for l in range(cfg.layers):
+        y, gate = adarms(h, cond, _as(W["w_mod_attn"][l], dtype), _as(W["b_mod_attn"][l], dtype), cfg.rms_eps)
+        h = h + gate * attention_sublayer(cfg, W, l, y, [pk[l] for pk in prefix_k], [pv[l] for pv in prefix_v], dtype)
+        y, gate = adarms(h, cond, _as(W["w_mod_mlp"][l], dtype), _as(W["b_mod_mlp"][l], dtype), cfg.rms_eps)
+        h = h + gate * mlp_sublayer(cfg, W, l, y, dtype)
+    y, _ = adarms(h, cond, _as(W["w_mod_final"], dtype), _as(W["b_mod_final"], dtype), cfg.rms_eps)
+    return y @ _as(W["w_out"], dtype).T + _as(W["b_out"], dtype)
 
 
 def velocity(cfg, W: Dict, x: np.ndarray, t: np.ndarray, prefix_k: Sequence[np.ndarray],
              prefix_v: Sequence[np.ndarray], dtype=F) -> np.ndarray:
     """v(x, t) for a batch of robots (steps 1-5).  prefix_k[i]: [layers, L_i, n_kv, hd]."""
+    if getattr(cfg, "time_conditioning", 0) == 1:
+        return velocity_adarms(cfg, W, x, t, prefix_k, prefix_v, dtype)
     h = embed(cfg, W, x, t, dtype)
     for l in range(cfg.layers):
         h = layer(cfg, W, l, h, [pk[l] for pk in prefix_k], [pv[l] for pv in prefix_v], dtype)

@@ -17,6 +17,10 @@ Draw order (one ``numpy.random.Generator(PCG64(seed))``, float32 ``standard_norm
   5. per robot i: per layer l: K then V, each [L_i, n_kv, head_dim]
   6. noise [B, H, A]
   7. config 3 only: per-robot start-time index
+Adaptive-norm variant (``time_conditioning=1``, reading R25): w_t1 is [d, d], and after
+step 4 a third generator ``PCG64([seed, 0x5eed])`` draws, per layer, w_mod_attn, w_mod_mlp [3d, d], then
+w_mod_final, then the biases b_mod_* [3d] in the same order, all N(0, 0.02), with +1 added to the gate
+third of every b_mod so the blocks contribute (a zero-mean gate would switch them off).
 """
 from __future__ import annotations
 
@@ -40,6 +44,7 @@ class ExpertConfig:
     rms_eps: float = 1e-6
     time_min_period: float = 4e-3
     time_max_period: float = 4.0
+    time_conditioning: int = 0       # 0: time concatenated into the embedding MLP (pi0-style); 1: adaptive RMSNorm (pi0.5-style, R25)
 
     def as_dict(self) -> dict:
         return asdict(self)
@@ -59,8 +64,10 @@ def weight_shapes(c: ExpertConfig) -> Dict[str, tuple]:
     """[out_features, in_features] row-major for every matrix (reading R10)."""
     d, a, f = c.d_model, c.action_dim, c.ffn
     nq, nkv, hd = c.n_q_heads, c.n_kv_heads, c.head_dim
+    ada = {"w_mod": (3 * d, d), "b_mod": (3 * d,)} if c.time_conditioning == 1 else {}   # per norm: 2 per layer + final
     return {
-        "w_in": (d, a), "w_t1": (d, 2 * d), "w_t2": (d, d), "w_out": (a, d),
+        **ada,
+        "w_in": (d, a), "w_t1": (d, d if c.time_conditioning == 1 else 2 * d), "w_t2": (d, d), "w_out": (a, d),
         "wq": (nq * hd, d), "wk": (nkv * hd, d), "wv": (nkv * hd, d), "wo": (d, nq * hd),
         "w_gate": (f, d), "w_up": (f, d), "w_down": (d, f),
         "b_in": (d,), "b_t1": (d,), "b_t2": (d,), "b_out": (a,),
@@ -168,6 +175,23 @@ def build_case(name: str, seed: int, cfg: ExpertConfig, *, bf16: bool,
     w["g_final"] = ones.copy()
     w["g_attn"] = [ones.copy() for _ in range(cfg.layers)]
     w["g_mlp"] = [ones.copy() for _ in range(cfg.layers)]
+    if cfg.time_conditioning == 1:
+        mrng = np.random.Generator(np.random.PCG64([seed, 0x5eed]))
+        w["w_mod_attn"], w["w_mod_mlp"] = [None] * cfg.layers, [None] * cfg.layers
+        for l in range(cfg.layers):
+            w["w_mod_attn"][l] = rnd(_normal(mrng, shp["w_mod"], 0.02))
+            w["w_mod_mlp"][l] = rnd(_normal(mrng, shp["w_mod"], 0.02))
+        w["w_mod_final"] = rnd(_normal(mrng, shp["w_mod"], 0.02))
+
+        def mod_bias():
+            b = _normal(mrng, shp["b_mod"], 0.02)
+            b[2 * cfg.d_model:] += np.float32(1.0)
+            return rnd(b)
+        w["b_mod_attn"], w["b_mod_mlp"] = [None] * cfg.layers, [None] * cfg.layers
+        for l in range(cfg.layers):
+            w["b_mod_attn"][l] = mod_bias()
+            w["b_mod_mlp"][l] = mod_bias()
+        w["b_mod_final"] = mod_bias()
 
     pk, pv = [], []
     if with_prefix:
@@ -216,6 +240,17 @@ def make_case(config: int, *, batch: Optional[int] = None, with_prefix: bool = T
         b = batch or 64
         return build_case(f"cfg4-sweep-b{b}", 4, PI0, bf16=True, prefix_lens=[816] * b, **kw)
     raise ValueError(f"unknown config {config}")
+
+
+def make_adarms_case(scale: str = "tiny", *, batch: int = 2, layers: Optional[int] = None, seed: int = 5) -> Case:
+    """Adaptive-norm variant (reading R25) on the tiny fp32 shapes or on pi0-scale bf16 shapes with fewer
+    layers (the oracle's time grows with layers x batch; kernels are exercised from 2 layers on)."""
+    from dataclasses import replace
+    if scale == "tiny":
+        cfg = replace(TINY, time_conditioning=1, layers=layers or TINY.layers)
+        return build_case("adarms-tiny", seed, cfg, bf16=False, prefix_lens=[48, 64][:batch] if batch <= 2 else [48 + 5 * i for i in range(batch)], n_steps=4)
+    cfg = replace(PI0, time_conditioning=1, layers=layers or 3)
+    return build_case(f"adarms-pi0-l{cfg.layers}-b{batch}", seed, cfg, bf16=True, draw_lens=(300, 500), batch=batch, n_steps=4)
 
 
 SWEEP_BATCHES = (1, 2, 4, 8, 16, 32, 64, 128, 256, 512)

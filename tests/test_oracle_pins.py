@@ -59,6 +59,42 @@ def _rope_vec(x, pos, base):
     return y
 
 
+def _brute_attention_rows(cfg, W, l, n1, pk, pv):
+    """W_o output rows of one robot's attention sublayer from its normed rows n1 [H][d] (scalar loops)."""
+    H = cfg.horizon
+    nq, nkv, hd = cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim
+    L = pk.shape[1]
+    q, k, v = [], [], []
+    for j in range(H):
+        qj = _matvec(W["wq"][l], n1[j])
+        kj = _matvec(W["wk"][l], n1[j])
+        vj = _matvec(W["wv"][l], n1[j])
+        q.append([_rope_vec(qj[a * hd:(a + 1) * hd], L + j, cfg.rope_base) for a in range(nq)])
+        k.append([_rope_vec(kj[g * hd:(g + 1) * hd], L + j, cfg.rope_base) for g in range(nkv)])
+        v.append([vj[g * hd:(g + 1) * hd] for g in range(nkv)])
+    rows = []
+    for j in range(H):
+        o = []
+        for a in range(nq):
+            g = a // (nq // nkv)
+            keys = [list(map(float, pk[l, s, g])) for s in range(L)] + [k[jj][g] for jj in range(H)]
+            vals = [list(map(float, pv[l, s, g])) for s in range(L)] + [v[jj][g] for jj in range(H)]
+            sc = [_dot(q[j][a], kk) / math.sqrt(hd) for kk in keys]
+            e = [math.exp(s) for s in sc]            # plain definition, no max subtraction
+            den = sum(e)
+            o += [sum(e[s] * vals[s][c] for s in range(L + H)) / den for c in range(hd)]
+        rows.append(_matvec(W["wo"][l], o))
+    return rows
+
+
+def _brute_mlp_row(W, l, n2):
+    gt = _matvec(W["w_gate"][l], n2)
+    up = _matvec(W["w_up"][l], n2)
+    m = [0.5 * a_ * (1 + math.tanh(math.sqrt(2 / math.pi) * (a_ + 0.044715 * a_ ** 3))) * b_
+         for a_, b_ in zip(gt, up)]
+    return _matvec(W["w_down"][l], m)
+
+
 def brute_velocity_robot(cfg, W, x, t, pk, pv):
     """v(x, t) of ONE robot with scalar loops only (math module), straight from the definitions."""
     d, H, A = cfg.d_model, cfg.horizon, cfg.action_dim
@@ -78,35 +114,12 @@ def brute_velocity_robot(cfg, W, x, t, pk, pv):
         z = [v / (1.0 + math.exp(-v)) for v in z]
         h.append(_matvec(W["w_t2"], z, W["b_t2"]))
     for l in range(cfg.layers):
-        q, k, v = [], [], []
+        proj = _brute_attention_rows(cfg, W, l, [_rms(h[j], W["g_attn"][l], cfg.rms_eps) for j in range(H)], pk, pv)
         for j in range(H):
-            n1 = _rms(h[j], W["g_attn"][l], cfg.rms_eps)
-            qj = _matvec(W["wq"][l], n1)
-            kj = _matvec(W["wk"][l], n1)
-            vj = _matvec(W["wv"][l], n1)
-            q.append([_rope_vec(qj[a * hd:(a + 1) * hd], L + j, cfg.rope_base) for a in range(nq)])
-            k.append([_rope_vec(kj[g * hd:(g + 1) * hd], L + j, cfg.rope_base) for g in range(nkv)])
-            v.append([vj[g * hd:(g + 1) * hd] for g in range(nkv)])
+            h[j] = [p + r for p, r in zip(h[j], proj[j])]
         for j in range(H):
-            o = []
-            for a in range(nq):
-                g = a // (nq // nkv)
-                keys = [list(map(float, pk[l, s, g])) for s in range(L)] + [k[jj][g] for jj in range(H)]
-                vals = [list(map(float, pv[l, s, g])) for s in range(L)] + [v[jj][g] for jj in range(H)]
-                sc = [_dot(q[j][a], kk) / math.sqrt(hd) for kk in keys]
-                e = [math.exp(s) for s in sc]            # plain definition, no max subtraction
-                den = sum(e)
-                o += [sum(e[s] * vals[s][c] for s in range(L + H)) / den for c in range(hd)]
-            proj = _matvec(W["wo"][l], o)
-            h[j] = [p + r for p, r in zip(h[j], proj)]
-        for j in range(H):
-            n2 = _rms(h[j], W["g_mlp"][l], cfg.rms_eps)
-            gt = _matvec(W["w_gate"][l], n2)
-            up = _matvec(W["w_up"][l], n2)
-            m = [0.5 * a_ * (1 + math.tanh(math.sqrt(2 / math.pi) * (a_ + 0.044715 * a_ ** 3))) * b_
-                 for a_, b_ in zip(gt, up)]
-            proj = _matvec(W["w_down"][l], m)
-            h[j] = [p + r for p, r in zip(h[j], proj)]
+            proj_j = _brute_mlp_row(W, l, _rms(h[j], W["g_mlp"][l], cfg.rms_eps))
+            h[j] = [p + r for p, r in zip(h[j], proj_j)]
     out = []
     for j in range(H):
         n = _rms(h[j], W["g_final"], cfg.rms_eps)
@@ -381,3 +394,159 @@ def test_cases_generator_contract():
     assert set(np.round(c3.t_start * 10).astype(int)) <= set(range(1, 11))
     np.testing.assert_array_equal(c3.n_steps, np.round(c3.t_start * 10).astype(np.int32))
     assert c3.prefix_lens.min() >= 400 and c3.prefix_lens.max() <= 1200
+
+
+# ------------------------------------------------------------------ adaptive-norm variant (reading R25)
+MICRO_ADA = cases.ExpertConfig(layers=2, d_model=16, n_q_heads=4, n_kv_heads=2, head_dim=8,
+                               ffn=24, horizon=3, action_dim=3, time_conditioning=1)
+
+
+def micro_ada_case(seed=21, lens=(5, 7)):
+    c = cases.build_case("micro-ada", seed, MICRO_ADA, bf16=False, prefix_lens=list(lens), n_steps=3)
+    for k in cases.GLOBAL_WEIGHTS + cases.BIASES:
+        c.weights[k] = (c.weights[k] * 12).astype(np.float32)
+    for k in cases.LAYER_WEIGHTS + ("w_mod_attn", "w_mod_mlp"):
+        c.weights[k] = [(w * 12).astype(np.float32) for w in c.weights[k]]
+    c.weights["w_mod_final"] = (c.weights["w_mod_final"] * 12).astype(np.float32)
+    return c
+
+
+def brute_velocity_adarms_robot(cfg, W, x, t, pk, pv):
+    """v(x, t) of ONE robot of the adaptive-norm variant, scalar loops only, from reading R25."""
+    d, H = cfg.d_model, cfg.horizon
+    half = d // 2
+    tau = [0.0] * d
+    for j in range(half):
+        period = cfg.time_min_period * (cfg.time_max_period / cfg.time_min_period) ** (j / (half - 1))
+        tau[j] = math.sin(2 * math.pi * t / period)
+        tau[half + j] = math.cos(2 * math.pi * t / period)
+    z = [v / (1.0 + math.exp(-v)) for v in _matvec(W["w_t1"], tau, W["b_t1"])]
+    cond = [v / (1.0 + math.exp(-v)) for v in _matvec(W["w_t2"], z, W["b_t2"])]
+
+    def ada(row, wm, bm):
+        mod = _matvec(wm, cond, bm)                       # [scale | shift | gate]
+        r = 1.0 / math.sqrt(sum(v * v for v in row) / d + cfg.rms_eps)
+        return [row[c] * r * (1.0 + mod[c]) + mod[d + c] for c in range(d)], mod[2 * d:]
+
+    h = [_matvec(W["w_in"], x[j], W["b_in"]) for j in range(H)]
+    for l in range(cfg.layers):
+        ys, gate = [], None
+        for j in range(H):
+            y, gate = ada(h[j], W["w_mod_attn"][l], W["b_mod_attn"][l])
+            ys.append(y)
+        proj = _brute_attention_rows(cfg, W, l, ys, pk, pv)
+        for j in range(H):
+            h[j] = [p + g * r for p, g, r in zip(h[j], gate, proj[j])]
+        for j in range(H):
+            y, gate = ada(h[j], W["w_mod_mlp"][l], W["b_mod_mlp"][l])
+            h[j] = [p + g * r for p, g, r in zip(h[j], gate, _brute_mlp_row(W, l, y))]
+    out = []
+    for j in range(H):
+        y, _ = ada(h[j], W["w_mod_final"], W["b_mod_final"])
+        out.append(_matvec(W["w_out"], y, W["b_out"]))
+    return np.array(out)
+
+
+def test_adarms_bruteforce_velocity_and_denoise():
+    c = micro_ada_case()
+    ts = np.array([0.7, 0.3])
+    pk = [c.prefix_k[i] for i in range(2)]
+    pv = [c.prefix_v[i] for i in range(2)]
+    v = O.velocity(c.cfg, c.weights, c.noise.astype(np.float64), ts, pk, pv)
+    for i in range(2):
+        vb = brute_velocity_adarms_robot(c.cfg, c.weights, c.noise[i].astype(np.float64), float(ts[i]), pk[i], pv[i])
+        assert np.abs(vb).max() > 1e-2
+        np.testing.assert_allclose(v[i], vb, rtol=0, atol=1e-11)
+    x, vel = O.denoise_case(c, return_velocity=True)
+    for i in range(2):
+        xb = c.noise[i].astype(np.float64)
+        for k in range(int(c.n_steps[i])):
+            vb = brute_velocity_adarms_robot(c.cfg, c.weights, xb, float(c.t_start[i]) + k * float(c.dt[i]), pk[i], pv[i])
+            np.testing.assert_allclose(vel[k][i], vb, rtol=0, atol=1e-10)
+            xb = xb + float(c.dt[i]) * vb
+        np.testing.assert_allclose(x[i], xb, rtol=0, atol=1e-10)
+    # time really conditions the output, and through the modulation only
+    v2 = O.velocity(c.cfg, c.weights, c.noise.astype(np.float64), ts[::-1].copy(), pk, pv)
+    assert np.abs(v2 - v).max() > 1e-3
+
+
+def _zero_mod(c, scale=0.0, shift=0.0, gate=1.0):
+    d = c.cfg.d_model
+    b = np.concatenate([np.full(d, scale), np.full(d, shift), np.full(d, gate)]).astype(np.float32)
+    for k in ("w_mod_attn", "w_mod_mlp"):
+        c.weights[k] = [np.zeros_like(w) for w in c.weights[k]]
+    c.weights["w_mod_final"] = np.zeros_like(c.weights["w_mod_final"])
+    c.weights["b_mod_attn"] = [b.copy() for _ in range(c.cfg.layers)]
+    c.weights["b_mod_mlp"] = [b.copy() for _ in range(c.cfg.layers)]
+    c.weights["b_mod_final"] = b.copy()
+    return c
+
+
+def test_adarms_reduces_to_plain_blocks_with_identity_modulation():
+    """scale = shift = 0, gate = 1: the stack is the pinned pre-norm blocks (gains 1) on h0 = W_in x + b_in."""
+    c = _zero_mod(micro_ada_case())
+    W, cfg = c.weights, c.cfg
+    x = c.noise.astype(np.float64)
+    pk = [c.prefix_k[i] for i in range(2)]
+    pv = [c.prefix_v[i] for i in range(2)]
+    v = O.velocity(cfg, W, x, np.array([0.9, 0.2]), pk, pv)
+    h = x @ W["w_in"].astype(np.float64).T + W["b_in"]
+    for l in range(cfg.layers):
+        h = O.layer(cfg, W, l, h, [p[l] for p in pk], [p[l] for p in pv])     # g_attn = g_mlp = 1 in the generator
+    want = O.rmsnorm(h, np.ones(cfg.d_model), cfg.rms_eps) @ W["w_out"].astype(np.float64).T + W["b_out"]
+    np.testing.assert_allclose(v, want, rtol=0, atol=1e-12)
+    # ... and then the output does not depend on t at all
+    v2 = O.velocity(cfg, W, x, np.array([0.1, 0.6]), pk, pv)
+    np.testing.assert_allclose(v2, v, rtol=0, atol=1e-13)
+
+
+def test_adarms_zero_gate_is_identity_and_shift_only_closed_form():
+    c = _zero_mod(micro_ada_case(), gate=0.0)
+    W, cfg = c.weights, c.cfg
+    x = c.noise.astype(np.float64)
+    pk = [c.prefix_k[i] for i in range(2)]
+    pv = [c.prefix_v[i] for i in range(2)]
+    v = O.velocity(cfg, W, x, np.array([0.9, 0.2]), pk, pv)
+    h0 = x @ W["w_in"].astype(np.float64).T + W["b_in"]
+    want = h0 / np.sqrt(np.mean(h0 * h0, axis=-1, keepdims=True) + cfg.rms_eps) @ W["w_out"].astype(np.float64).T + W["b_out"]
+    np.testing.assert_allclose(v, want, rtol=0, atol=1e-12)
+    # scale = -1 removes the token entirely: y = shift, so v = W_out (s 1) + b_out for every token
+    c = _zero_mod(micro_ada_case(), scale=-1.0, shift=0.37, gate=0.0)
+    v = O.velocity(c.cfg, c.weights, x, np.array([0.9, 0.2]), pk, pv)
+    want_row = c.weights["w_out"].astype(np.float64) @ np.full(cfg.d_model, np.float64(np.float32(0.37))) + c.weights["b_out"]
+    np.testing.assert_allclose(v, np.broadcast_to(want_row, v.shape), rtol=0, atol=1e-12)
+
+
+def test_adarms_torch_third_opinion():
+    c = micro_ada_case()
+    W, cfg = c.weights, c.cfg
+    d = cfg.d_model
+    t = np.array([0.65, 0.15])
+    cond = O.time_condition(cfg, W, t)
+    tau = torch.from_numpy(O.sinusoidal_time_embedding(t, d, cfg.time_min_period, cfg.time_max_period))
+    tl = lambda k: torch.from_numpy(W[k].astype(np.float64))
+    z = torch.nn.functional.silu(torch.nn.functional.linear(tau, tl("w_t1"), tl("b_t1")))
+    want = torch.nn.functional.silu(torch.nn.functional.linear(z, tl("w_t2"), tl("b_t2"))).numpy()
+    np.testing.assert_allclose(cond, want, rtol=0, atol=1e-13)
+    rng = np.random.default_rng(3)
+    h = rng.standard_normal((2, cfg.horizon, d))
+    wm, bm = W["w_mod_attn"][1].astype(np.float64), W["b_mod_attn"][1].astype(np.float64)
+    y, gate = O.adarms(h, cond, wm, bm, cfg.rms_eps)
+    mod = torch.nn.functional.linear(torch.from_numpy(cond), torch.from_numpy(wm), torch.from_numpy(bm))
+    sc, sh, gt = mod.chunk(3, dim=-1)
+    yt = torch.nn.functional.rms_norm(torch.from_numpy(h), (d,), eps=cfg.rms_eps) * (1 + sc[:, None]) + sh[:, None]
+    np.testing.assert_allclose(y, yt.numpy(), rtol=0, atol=1e-13)
+    np.testing.assert_allclose(gate[:, 0], gt.numpy(), rtol=0, atol=1e-15)
+
+
+def test_adarms_batch_invariance_and_generator_contract():
+    c = cases.make_adarms_case("tiny")
+    assert c.cfg.time_conditioning == 1 and c.weights["w_t1"].shape == (128, 128)
+    assert c.weights["w_mod_attn"][0].shape == (384, 128) and abs(float(c.weights["b_mod_mlp"][1][256:].mean()) - 1.0) < 0.01
+    x, _ = O.denoise_case(c)
+    for i in range(c.batch):
+        xi, _ = O.denoise_case(c, robots=[i])
+        np.testing.assert_allclose(xi[0], x[i], rtol=0, atol=1e-13)       # BLAS blocking differs with the batch
+    # the modulation weights come from their own generator: the first draw of the main stream is the base one's
+    base = cases.build_case("b", 5, cases.TINY, bf16=False, prefix_lens=[48, 64], n_steps=4)
+    np.testing.assert_array_equal(base.weights["w_in"], c.weights["w_in"])
