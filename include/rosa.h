@@ -51,6 +51,12 @@ typedef struct {
   float rms_eps;          /* 1e-6 */
   float time_min_period;  /* 4e-3 */
   float time_max_period;  /* 4.0  */
+  int32_t time_conditioning; /* 0: time concatenated into the embedding MLP (pi0-style, BJ cfg0; the path of
+                              * every BASELINE.json config).  1: adaptive RMSNorm (pi0.5-style, PAPER.md:438,
+                              * DESIGN.md reading R25): cond = swish(W_t2 swish(W_t1 tau(t) + b_t1) + b_t2),
+                              * h0 = W_in x + b_in, every norm y = h rsqrt(mean h^2 + eps)(1 + scale) + shift
+                              * with (scale, shift, gate) = W_mod cond + b_mod, h += gate * sublayer(y).
+                              * Needs the tcgen05 shapes (head_dim 256), else ROSA_ERR_UNSUPPORTED. */
 } rosa_expert_config_t;
 
 /* Weights.  Every matrix is [out_features, in_features] row-major (R10); q/k/v rows are
@@ -59,13 +65,18 @@ typedef struct {
  * `layers` pointers.  Shapes: w_in [d,A] b_in [d]; w_t1 [d,2d] (columns 0..d-1 multiply the
  * sinusoidal time embedding, d..2d-1 the projected action, R2) b_t1 [d]; w_t2 [d,d] b_t2 [d];
  * w_out [A,d] b_out [A]; g_final [d]; per layer g_attn [d], wq [nq*hd,d], wk [nkv*hd,d],
- * wv [nkv*hd,d], wo [d,nq*hd], g_mlp [d], w_gate [F,d], w_up [F,d], w_down [d,F]. */
+ * wv [nkv*hd,d], wo [d,nq*hd], g_mlp [d], w_gate [F,d], w_up [F,d], w_down [d,F].
+ * time_conditioning == 1 only (ignored otherwise): w_t1 is [d,d]; w_mod_* [3d,d] and b_mod_* [3d], rows
+ * ordered scale | shift | gate, one pair per norm (per layer: attention, MLP; and the final norm);
+ * g_attn, g_mlp, g_final are not read. */
 typedef struct {
   rosa_dtype_t dtype;
   int32_t on_device;
   const void *w_in, *b_in, *w_t1, *b_t1, *w_t2, *b_t2, *w_out, *b_out, *g_final;
   const void *const *g_attn, *const *wq, *const *wk, *const *wv, *const *wo;
   const void *const *g_mlp, *const *w_gate, *const *w_up, *const *w_down;
+  const void *const *w_mod_attn, *const *b_mod_attn, *const *w_mod_mlp, *const *b_mod_mlp;
+  const void *w_mod_final, *b_mod_final;
 } rosa_weights_t;
 
 /* Create an expert on the current CUDA device.  Copies and repacks every weight into

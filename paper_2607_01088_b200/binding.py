@@ -37,16 +37,20 @@ class rosa_expert_config_t(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ("layers", "d_model", "n_q_heads", "n_kv_heads", "head_dim", "ffn",
                                          "horizon", "action_dim", "max_robots", "max_batch",
                                          "max_prefix_len", "max_steps")] + \
-               [(n, C.c_float) for n in ("rope_base", "rms_eps", "time_min_period", "time_max_period")]
+               [(n, C.c_float) for n in ("rope_base", "rms_eps", "time_min_period", "time_max_period")] + \
+               [("time_conditioning", C.c_int32)]
 
 
 _GLOBAL = ("w_in", "b_in", "w_t1", "b_t1", "w_t2", "b_t2", "w_out", "b_out", "g_final")
 _LAYER = ("g_attn", "wq", "wk", "wv", "wo", "g_mlp", "w_gate", "w_up", "w_down")
+_LAYER_ADA = ("w_mod_attn", "b_mod_attn", "w_mod_mlp", "b_mod_mlp")      # time_conditioning == 1 only
+_GLOBAL_ADA = ("w_mod_final", "b_mod_final")
 
 
 class rosa_weights_t(C.Structure):
     _fields_ = [("dtype", C.c_int), ("on_device", C.c_int32)] + [(n, C.c_void_p) for n in _GLOBAL] + \
-               [(n, C.POINTER(C.c_void_p)) for n in _LAYER]
+               [(n, C.POINTER(C.c_void_p)) for n in _LAYER] + [(n, C.POINTER(C.c_void_p)) for n in _LAYER_ADA] + \
+               [(n, C.c_void_p) for n in _GLOBAL_ADA]
 
 
 _lib = None
@@ -143,14 +147,16 @@ def rosa_expert_create(cfg: dict, weights: Dict[str, object], *, max_robots: int
     c.max_robots, c.max_batch, c.max_prefix_len, c.max_steps = max_robots, max_batch, max_prefix_len, max_steps
     c.rope_base, c.rms_eps = float(cfg["rope_base"]), float(cfg["rms_eps"])
     c.time_min_period, c.time_max_period = float(cfg["time_min_period"]), float(cfg["time_max_period"])
+    c.time_conditioning = int(cfg.get("time_conditioning", 0))
+    ada = c.time_conditioning == 1
     w = rosa_weights_t()
     w.dtype, w.on_device = ROSA_F32, 0
     keep = []
-    for n in _GLOBAL:
+    for n in _GLOBAL + (_GLOBAL_ADA if ada else ()):
         a = np.ascontiguousarray(weights[n], dtype=np.float32)
         keep.append(a)
         setattr(w, n, a.ctypes.data)
-    for n in _LAYER:
+    for n in _LAYER + (_LAYER_ADA if ada else ()):
         arrs = [np.ascontiguousarray(a, dtype=np.float32) for a in weights[n]]
         keep.append(arrs)
         pa = (C.c_void_p * len(arrs))(*[a.ctypes.data for a in arrs])

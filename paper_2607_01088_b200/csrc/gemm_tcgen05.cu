@@ -133,6 +133,10 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, float* scr, uin
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
           if (colok && r0 + i * 4 + lr < m_lim) {
+            if (ea.gate) {  // adaptive-norm variant (R25): per-robot gate on the sublayer output
+              const float4 g = *reinterpret_cast<const float4*>(ea.gate + (size_t)((r0 + i * 4 + lr) / ea.H) * ea.gate_ld + col);
+              o[i].x *= g.x; o[i].y *= g.y; o[i].z *= g.z; o[i].w *= g.w;
+            }
             const float4 h = *reinterpret_cast<const float4*>(gp + i * step);
             o[i].x += h.x; o[i].y += h.y; o[i].z += h.z; o[i].w += h.w;
           }

@@ -447,4 +447,106 @@ void launch_attn_simple(const Dims& dm, const Tables& tb, int layer, const bf16*
   k_attn_simple<<<tb.batch * dm.H, 256, smem, s>>>(dm, tb, layer, qkv, o, k_iter);
 }
 
+
+// ------------------------------------------------------------------ adaptive-norm variant (reading R25)
+// The tcgen05 GEMMs, the attention kernel and the final-projection epilogue are the base path's; the
+// variant adds three small kernels (time-MLP activation, plain action embedding, adaptive RMSNorm) and a
+// per-robot gate in the residual epilogue.  The norm is NOT fused into the GEMMs here: (1 + scale) runs
+// along K and shift adds a per-robot row, so the normalised, modulated operand is written once by
+// k_adarms and the consuming GEMMs run with a unit row scale.
+namespace {
+// out16 = op16(swish(in)) over a [rows, d] fp32 matrix (the two layers of the time MLP)
+__global__ void k_swish16(op16* __restrict__ out, const float* __restrict__ in, size_t n4, int fp16) {
+  pdl_wait();
+  pdl_trigger();
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n4) return;
+  const float4 v = reinterpret_cast<const float4*>(in)[i];
+  reinterpret_cast<uint2*>(out)[i] = make_uint2(pack_op2(swish_f(v.x), swish_f(v.y), fp16), pack_op2(swish_f(v.z), swish_f(v.w), fp16));
+}
+
+// h0[m][n] = b_in[n] + sum_c x[m][c] W_in[n][c]  (fp32, K = A on CUDA cores; w_inT is [A, d])
+__global__ void __launch_bounds__(256) k_embed_lin(float* __restrict__ h, const float* __restrict__ x,
+                                                   const float* __restrict__ w_inT, const float* __restrict__ b_in,
+                                                   int d, int A, const int* __restrict__ m_active) {
+  __shared__ float xs[EM_ROWS][64];
+  pdl_wait();
+  pdl_trigger();
+  const int m0 = blockIdx.x * EM_ROWS, m_lim = *m_active;
+  if (m0 >= m_lim) return;
+  const int rows = min(EM_ROWS, m_lim - m0);
+  for (int i = threadIdx.x; i < EM_ROWS * A; i += blockDim.x) {
+    const int r = i / A, c = i - r * A;
+    xs[r][c] = r < rows ? x[(size_t)(m0 + r) * A + c] : 0.f;
+  }
+  __syncthreads();
+  for (int n = 4 * threadIdx.x; n < d; n += 4 * blockDim.x) {
+    float4 acc[EM_ROWS];
+    const float4 b = *reinterpret_cast<const float4*>(b_in + n);
+#pragma unroll
+    for (int r = 0; r < EM_ROWS; ++r) acc[r] = b;
+#pragma unroll 8
+    for (int c = 0; c < A; ++c) {
+      const float4 w = *reinterpret_cast<const float4*>(w_inT + (size_t)c * d + n);
+#pragma unroll
+      for (int r = 0; r < EM_ROWS; ++r) {
+        const float xv = xs[r][c];
+        acc[r].x = fmaf(xv, w.x, acc[r].x);
+        acc[r].y = fmaf(xv, w.y, acc[r].y);
+        acc[r].z = fmaf(xv, w.z, acc[r].z);
+        acc[r].w = fmaf(xv, w.w, acc[r].w);
+      }
+    }
+#pragma unroll
+    for (int r = 0; r < EM_ROWS; ++r)
+      if (r < rows) *reinterpret_cast<float4*>(h + (size_t)(m0 + r) * d + n) = acc[r];
+  }
+}
+
+// out16[m][c] = op16( h[m][c] rsqrt(mean(h[m]^2) + eps) (1 + scale[p][c]) + shift[p][c] ), p = m / H.
+// mod points at this norm's [scale | shift | gate] block of robot 0; robots are mod_ld floats apart.
+__global__ void k_adarms(op16* __restrict__ out, const float* __restrict__ h, const float* __restrict__ mod, int mod_ld,
+                         int d, int H, float eps, int fp16, const int* __restrict__ m_active) {
+  pdl_wait();
+  pdl_trigger();
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int m = blockIdx.x * (blockDim.x >> 5) + warp;
+  if (m >= *m_active) return;
+  const float* row = h + (size_t)m * d;
+  float ss = 0.f;
+  for (int c = lane * 4; c < d; c += 128) {
+    const float4 v = *reinterpret_cast<const float4*>(row + c);
+    ss += v.x * v.x + v.y * v.y + v.z * v.z + v.w * v.w;
+  }
+  ss = warp_sum(ss);
+  const float r = rsqrtf(ss / (float)d + eps);
+  const float* sc = mod + (size_t)(m / H) * mod_ld;
+  const float* sh = sc + d;
+  for (int c = lane * 4; c < d; c += 128) {
+    const float4 v = *reinterpret_cast<const float4*>(row + c);
+    const float4 a = *reinterpret_cast<const float4*>(sc + c);
+    const float4 b = *reinterpret_cast<const float4*>(sh + c);
+    uint2 pk;
+    pk.x = pack_op2(fmaf(v.x * r, 1.f + a.x, b.x), fmaf(v.y * r, 1.f + a.y, b.y), fp16);
+    pk.y = pack_op2(fmaf(v.z * r, 1.f + a.z, b.z), fmaf(v.w * r, 1.f + a.w, b.w), fp16);
+    *reinterpret_cast<uint2*>(out + (size_t)m * d + c) = pk;
+  }
+}
+}  // namespace
+
+void launch_swish16(op16* out, const float* in, size_t n, int fp16, cudaStream_t s) {
+  const size_t n4 = n / 4;
+  launch_k(k_swish16, dim3((unsigned)((n4 + 255) / 256)), dim3(256), 0, s, out, in, n4, fp16);
+}
+void launch_embed_lin(float* h, const float* x, const float* w_inT, const float* b_in, const Dims& dm, const Tables& tb,
+                      int k_iter, int M, cudaStream_t s) {
+  launch_k(k_embed_lin, dim3((M + EM_ROWS - 1) / EM_ROWS), dim3(256), 0, s, h, x, w_inT, b_in, dm.d, dm.A, tb.m_active + k_iter);
+}
+void launch_adarms(op16* out, const float* h, const float* mod, int mod_ld, const Dims& dm, const Tables& tb, int k_iter,
+                   int M, cudaStream_t s) {
+  const int wpb = 8;
+  launch_k(k_adarms, dim3((M + wpb - 1) / wpb), dim3(wpb * 32), 0, s, out, h, mod, mod_ld, dm.d, dm.H, dm.eps, dm.fp16,
+           tb.m_active + k_iter);
+}
+
 }  // namespace rosa

@@ -66,7 +66,12 @@ struct rosa_expert {
   bf16 *w_t1 = nullptr, *w_out = nullptr;  // CUDA-core steps: bf16 as given
   float *wca = nullptr, *bca = nullptr;    // (W_1[:, d:] W_in)^T [A, d] and W_1[:, d:] b_in [d], folded in fp64
   op16* w_t2 = nullptr;                    // GEMM operand: fp16 or bf16 (dm.fp16)
-  op16 *w_t1dup = nullptr, *tau16 = nullptr;  // tcgen05 family: [W_1[:, :d] | W_1[:, :d]] [d, 2d] and the [hi | lo] tau rows
+  op16 *w_t1dup = nullptr, *tau16 = nullptr;
+  // adaptive-norm variant (R25): all 2L+1 modulation matrices stacked [(2L+1) 3d, d] (norm n = 2l attention,
+  // 2l+1 MLP, 2L final; rows scale | shift | gate), their biases, the 16-bit time-MLP activations and the
+  // per-step modulation vectors [max_batch, (2L+1) 3d]
+  op16 *w_mod = nullptr, *z16 = nullptr, *cond16 = nullptr;
+  float *b_mod = nullptr, *mod = nullptr;  // tcgen05 family: [W_1[:, :d] | W_1[:, :d]] [d, 2d] and the [hi | lo] tau rows
   op16* w_out16 = nullptr;                 // [64, d]: W_out with the final-norm gain folded in, zero rows past A (tcgen05 family)
   float *b_t1 = nullptr, *b_t2 = nullptr, *b_out = nullptr, *g_final = nullptr;
   std::vector<LayerWeights> lw;
@@ -208,6 +213,7 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
   dm.qkv_n = (dm.nq + 2 * dm.nkv) * dm.hd;
   dm.q_n = dm.nq * dm.hd;
   dm.gu_blk = 64;
+  dm.ada = c->time_conditioning == 1;
   {  // GEMM operand format: fp16 by default (reading R19), ROSA_GEMM_DTYPE=bf16 to compare
     const char* gd = getenv("ROSA_GEMM_DTYPE");
     dm.fp16 = (gd && !strcmp(gd, "bf16")) ? 0 : 1;
@@ -222,7 +228,33 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
 #define UPB(dst) if ((st = upload_bf16(e, t, &(dst))) != ROSA_OK) return st
 #define UPO(dst) if ((st = upload_op16(e, t, &(dst))) != ROSA_OK) return st
 #define UPF(dst) if ((st = upload_f32(e, t, &(dst))) != ROSA_OK) return st
-  {  // a1 folding (exact algebra, fp64): Wca = W_1[:, d:] W_in, bca = W_1[:, d:] b_in
+  if (dm.ada) {  // R25: h0 = W_in x + b_in on CUDA cores (W_in^T as [A, d]); time MLP first layer [d, d], doubled along K
+    std::vector<float> win, bin;
+    if ((st = fetch_f32(w->w_in, (size_t)d * A, dt, od, win)) != ROSA_OK) return st;
+    if ((st = fetch_f32(w->b_in, (size_t)d, dt, od, bin)) != ROSA_OK) return st;
+    std::vector<float> wt((size_t)A * d);
+    for (int n = 0; n < d; ++n)
+      for (int c2 = 0; c2 < A; ++c2) wt[(size_t)c2 * d + n] = win[(size_t)n * A + c2];
+    if ((st = upload_f32(e, wt, &e->wca)) != ROSA_OK) return st;
+    if ((st = upload_f32(e, bin, &e->bca)) != ROSA_OK) return st;
+    FETCH(w->w_t1, (size_t)d * d);
+    std::vector<float> dup((size_t)d * 2 * d);
+    for (int n = 0; n < d; ++n)
+      for (int c2 = 0; c2 < d; ++c2) dup[(size_t)n * 2 * d + c2] = dup[(size_t)n * 2 * d + d + c2] = t[(size_t)n * d + c2];
+    if ((st = upload_op16(e, dup, &e->w_t1dup)) != ROSA_OK) return st;
+    // modulation matrices, stacked in norm order
+    const size_t blk = (size_t)3 * d * d;
+    std::vector<float> wm((size_t)(2 * dm.layers + 1) * blk), bm((size_t)(2 * dm.layers + 1) * 3 * d);
+    for (int nrm = 0; nrm <= 2 * dm.layers; ++nrm) {
+      const void* wp = nrm == 2 * dm.layers ? w->w_mod_final : (nrm & 1 ? w->w_mod_mlp[nrm / 2] : w->w_mod_attn[nrm / 2]);
+      const void* bp = nrm == 2 * dm.layers ? w->b_mod_final : (nrm & 1 ? w->b_mod_mlp[nrm / 2] : w->b_mod_attn[nrm / 2]);
+      if (!wp || !bp) { set_error("NULL modulation weight pointer"); return ROSA_ERR_INVALID_ARG; }
+      FETCH(wp, blk); memcpy(&wm[nrm * blk], t.data(), blk * 4);
+      FETCH(bp, (size_t)3 * d); memcpy(&bm[(size_t)nrm * 3 * d], t.data(), (size_t)3 * d * 4);
+    }
+    if ((st = upload_op16(e, wm, &e->w_mod)) != ROSA_OK) return st;
+    if ((st = upload_f32(e, bm, &e->b_mod)) != ROSA_OK) return st;
+  } else {  // a1 folding (exact algebra, fp64): Wca = W_1[:, d:] W_in, bca = W_1[:, d:] b_in
     std::vector<float> win, bin;
     if ((st = fetch_f32(w->w_in, (size_t)d * A, dt, od, win)) != ROSA_OK) return st;
     if ((st = fetch_f32(w->b_in, (size_t)d, dt, od, bin)) != ROSA_OK) return st;
@@ -256,22 +288,22 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
   FETCH(w->b_t2, d); UPF(e->b_t2);
   FETCH(w->w_out, (size_t)A * d); UPB(e->w_out);
   {  // a9 on the tensor cores (family 1): [64, d] operand, gain folded (R23), rows >= A zero
-    std::vector<float> gf, wo = t;
-    if ((st = fetch_f32(w->g_final, (size_t)d, dt, od, gf)) != ROSA_OK) return st;
+    std::vector<float> gf(d, 1.f), wo = t;
+    if (!dm.ada && (st = fetch_f32(w->g_final, (size_t)d, dt, od, gf)) != ROSA_OK) return st;
     t.assign((size_t)64 * d, 0.f);
     for (int a = 0; a < A; ++a)
       for (int c = 0; c < d; ++c) t[(size_t)a * d + c] = wo[(size_t)a * d + c] * gf[c];
     UPO(e->w_out16);
   }
   FETCH(w->b_out, A); UPF(e->b_out);
-  FETCH(w->g_final, d); UPF(e->g_final);
+  if (!dm.ada) { FETCH(w->g_final, d); UPF(e->g_final); }
   e->lw.resize(dm.layers);
   for (int l = 0; l < dm.layers; ++l) {
     LayerWeights& L = e->lw[l];
     // RMSNorm gains are folded into the columns of the consuming matrices: (h r g) W^T = r h (W g)^T
-    std::vector<float> g1, g2;
-    if ((st = fetch_f32(w->g_attn[l], (size_t)d, dt, od, g1)) != ROSA_OK) return st;
-    if ((st = fetch_f32(w->g_mlp[l], (size_t)d, dt, od, g2)) != ROSA_OK) return st;
+    std::vector<float> g1(d, 1.f), g2(d, 1.f);  // the adaptive norms (R25) have no learned gain
+    if (!dm.ada && (st = fetch_f32(w->g_attn[l], (size_t)d, dt, od, g1)) != ROSA_OK) return st;
+    if (!dm.ada && (st = fetch_f32(w->g_mlp[l], (size_t)d, dt, od, g2)) != ROSA_OK) return st;
     // packed [wq ; wk ; wv]  -> one QKV GEMM (step a3)
     std::vector<float> pk((size_t)dm.qkv_n * d);
     FETCH(w->wq[l], (size_t)dm.q_n * d); memcpy(pk.data(), t.data(), t.size() * 4);
@@ -323,6 +355,12 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
   WS(e->h, Mmax * d * 4);
   WS(e->tvec, (size_t)c->max_steps * c->max_batch * d * 4);
   WS(e->zbuf, Mmax * d * 2);
+  if (dm.ada) {
+    const size_t rows = ((size_t)c->max_steps * c->max_batch + 127) / 128 * 128;
+    WS(e->z16, rows * d * 2);
+    WS(e->cond16, rows * d * 2);
+    WS(e->mod, (size_t)c->max_batch * (2 * dm.layers + 1) * 3 * d * 4);
+  }
   if (e->family == 1) WS(e->tau16, ((size_t)c->max_steps * c->max_batch + 127) / 128 * 128 * 2 * d * 2);
   WS(e->nrm, Mmax * d * 2);
   WS(e->qkv, Mmax * dm.qkv_n * 2);
@@ -433,10 +471,89 @@ static cudaError_t gemm(rosa_expert* e, int cls, Epi epi, const op16* A, const o
   return cudaGetLastError();
 }
 
+// The call of the adaptive-norm variant (reading R25; tcgen05 family only).  Same GEMM, attention and
+// final-projection kernels as the base path; the norms are k_adarms launches (normalised, modulated 16-bit
+// operand; the GEMMs then run with a unit row scale) and the residual epilogues take the per-robot gate.
+static cudaError_t enqueue_call_ada(rosa_expert* e, int batch, int nmax, cudaStream_t s) {
+  const Dims& dm = e->dm;
+  const Tables tb = make_tables(e, batch);
+  const CallPtrs* cp = (const CallPtrs*)(e->d_call + e->off_ptrs);
+  const int M = batch * dm.H, d = dm.d, R = nmax * batch;
+  const int n_mod = (2 * dm.layers + 1) * 3 * d;
+  cudaError_t err;
+  e->last_launches = 0;
+  mark(e, ROSA_KC_GATHER_SCATTER, s);
+  launch_gather_x(e->x, cp, tb, dm.H * dm.A, e->d_done, 0, s);
+  e->last_launches += 1;
+  // cond of every (step, robot) row: swish(W_t2 swish(W_t1 tau + b_t1) + b_t2), rows [k][batch]
+  mark(e, ROSA_KC_TIMEVEC, s);
+  launch_tau16(e->tau16, dm, tb, nmax, s);
+  EpiArgs et{};
+  et.in_fp16 = dm.fp16; et.out_f32 = e->tvec; et.ld_out = d; et.bias = e->b_t1;
+  if ((err = launch_gemm_tc(EPI_BIAS_F32, e->tau16, e->w_t1dup, R, d, 2 * d, et, s)) != cudaSuccess) return err;
+  launch_swish16(e->z16, e->tvec, (size_t)R * d, dm.fp16, s);
+  et.bias = e->b_t2;
+  if ((err = launch_gemm_tc(EPI_BIAS_F32, e->z16, e->w_t2, R, d, d, et, s)) != cudaSuccess) return err;
+  launch_swish16(e->cond16, e->tvec, (size_t)R * d, dm.fp16, s);
+  e->last_launches += 5;
+  for (int k = 0; k < nmax; ++k) {
+    EpiArgs ea{};
+    ea.m_active = tb.m_active + k;
+    ea.H = dm.H; ea.hd = dm.hd; ea.gu_blk = dm.gu_blk; ea.in_fp16 = dm.fp16; ea.out_fp16 = dm.fp16;
+    ea.inv_d = 1.f / (float)d; ea.eps = dm.eps;
+    // (scale, shift, gate) of all 2L+1 norms for this step's robots: mod[p][norm][3d]
+    EpiArgs em{};
+    em.in_fp16 = dm.fp16; em.out_f32 = e->mod; em.ld_out = n_mod; em.bias = e->b_mod;
+    mark(e, ROSA_KC_TIMEVEC, s);
+    if ((err = launch_gemm_tc(EPI_BIAS_F32, e->cond16 + (size_t)k * batch * d, e->w_mod, batch, n_mod, d, em, s)) != cudaSuccess) return err;
+    mark(e, ROSA_KC_INPROJ, s);
+    launch_embed_lin(e->h, e->x, e->wca, e->bca, dm, tb, k, M, s);
+    e->last_launches += 2;
+    for (int l = 0; l < dm.layers; ++l) {
+      const LayerWeights& L = e->lw[l];
+      const float* mod_a = e->mod + (size_t)(2 * l) * 3 * d;
+      const float* mod_m = e->mod + (size_t)(2 * l + 1) * 3 * d;
+      mark(e, ROSA_KC_RMSNORM, s);
+      launch_adarms(e->nrm, e->h, mod_a, n_mod, dm, tb, k, M, s);
+      e->last_launches += 1;
+      ea.gate = nullptr;
+      ea.out16 = e->qkv; ea.ld_out = dm.qkv_n;
+      ea.rope_tab = e->rope_tab; ea.ids = tb.ids; ea.rlen = tb.rlen;
+      ea.rope_cols = dm.q_n + dm.nkv * dm.hd;
+      if ((err = gemm(e, ROSA_KC_GEMM_QKV, EPI_ROPE, e->nrm, L.wqkv, M, dm.qkv_n, d, ea, s)) != cudaSuccess) return err;
+      mark(e, ROSA_KC_ATTN, s);
+      if ((err = launch_attn_tc(dm, tb, l, e->qkv, e->obuf, k, M, e->d_kv_maps, s)) != cudaSuccess) return err;
+      e->last_launches += 1;
+      ea.out_f32 = e->h; ea.ld_out = d; ea.gate = mod_a + 2 * d; ea.gate_ld = n_mod;
+      if ((err = gemm(e, ROSA_KC_GEMM_O, EPI_RESID, e->obuf, L.wo, M, d, dm.q_n, ea, s)) != cudaSuccess) return err;
+      mark(e, ROSA_KC_RMSNORM, s);
+      launch_adarms(e->nrm, e->h, mod_m, n_mod, dm, tb, k, M, s);
+      e->last_launches += 1;
+      ea.gate = nullptr;
+      ea.out16 = e->mact; ea.ld_out = dm.F;
+      if ((err = gemm(e, ROSA_KC_GEMM_GATEUP, EPI_GEGLU, e->nrm, L.wgu, M, 2 * dm.F, d, ea, s)) != cudaSuccess) return err;
+      ea.out_f32 = e->h; ea.ld_out = d; ea.gate = mod_m + 2 * d; ea.gate_ld = n_mod;
+      if ((err = gemm(e, ROSA_KC_GEMM_DOWN, EPI_RESID, e->mact, L.wdown, M, d, dm.F, ea, s)) != cudaSuccess) return err;
+    }
+    mark(e, ROSA_KC_RMSNORM, s);
+    launch_adarms(e->nrm, e->h, e->mod + (size_t)(2 * dm.layers) * 3 * d, n_mod, dm, tb, k, M, s);
+    e->last_launches += 1;
+    ea.gate = nullptr;
+    ea.bias = e->b_out; ea.x = e->x; ea.cp = cp; ea.dt = tb.dt; ea.src = tb.src; ea.A = dm.A; ea.k_iter = k;
+    if ((err = gemm(e, ROSA_KC_FINAL, EPI_FINAL, e->nrm, e->w_out16, M, 64, d, ea, s)) != cudaSuccess) return err;
+  }
+  mark(e, ROSA_KC_GATHER_SCATTER, s);
+  launch_scatter_x(cp, e->x, tb, dm.H * dm.A, s);
+  e->last_launches += 1;
+  mark(e, -1, s);
+  return cudaGetLastError();
+}
+
 // Enqueue the whole call (steps a1..a11) on `s`.  Everything that changes from call to call is
 // read from the device tables, so the same sequence can be captured once per (batch, nmax).
 static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, cudaStream_t s) {
   const Dims& dm = e->dm;
+  if (dm.ada) return enqueue_call_ada(e, batch, nmax, s);
   const Tables tb = make_tables(e, batch);
   const CallPtrs* cp = (const CallPtrs*)(e->d_call + e->off_ptrs);
   const int M = batch * dm.H, d = dm.d;
@@ -638,9 +755,17 @@ rosa_status_t rosa_expert_create(const rosa_expert_config_t* c, const rosa_weigh
   if ((size_t)c->n_q_heads * (c->head_dim + c->max_prefix_len + c->horizon + 1) * 4 > 220 * 1024) {
     set_error("max_prefix_len too large for the attention kernel's shared memory"); return ROSA_ERR_UNSUPPORTED;
   }
-  const void* must[] = {w->w_in, w->b_in, w->w_t1, w->b_t1, w->w_t2, w->b_t2, w->w_out, w->b_out, w->g_final,
-                        w->g_attn, w->wq, w->wk, w->wv, w->wo, w->g_mlp, w->w_gate, w->w_up, w->w_down};
+  const void* must[] = {w->w_in, w->b_in, w->w_t1, w->b_t1, w->w_t2, w->b_t2, w->w_out, w->b_out,
+                        w->wq, w->wk, w->wv, w->wo, w->w_gate, w->w_up, w->w_down};
   for (const void* p : must) if (!p) { set_error("NULL weight pointer"); return ROSA_ERR_INVALID_ARG; }
+  if (c->time_conditioning != 1 && (!w->g_final || !w->g_attn || !w->g_mlp)) {
+    set_error("NULL weight pointer"); return ROSA_ERR_INVALID_ARG;
+  }
+  if (c->time_conditioning != 0 && c->time_conditioning != 1) { set_error("time_conditioning must be 0 or 1"); return ROSA_ERR_INVALID_ARG; }
+  if (c->time_conditioning == 1) {
+    const void* must_ada[] = {w->w_mod_attn, w->b_mod_attn, w->w_mod_mlp, w->b_mod_mlp, w->w_mod_final, w->b_mod_final};
+    for (const void* p : must_ada) if (!p) { set_error("NULL modulation weight pointer"); return ROSA_ERR_INVALID_ARG; }
+  }
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
     cudaGetLastError();
@@ -652,6 +777,11 @@ rosa_status_t rosa_expert_create(const rosa_expert_config_t* c, const rosa_weigh
   // tcgen05 family needs head_dim == 256 (RoPE epilogue tile = one head) and 128/256-wide N tiles
   const bool tc_shape = c->head_dim == 256 && c->d_model % 128 == 0 && (2 * c->ffn) % 256 == 0;
   e->family = (fam && !strcmp(fam, "simple")) || !tc_shape ? 0 : 1;
+  if (c->time_conditioning == 1 && e->family != 1) {
+    delete e;
+    set_error("time_conditioning = 1 needs the tcgen05 kernels (head_dim 256, d_model % 128 == 0, ROSA_KERNELS unset)");
+    return ROSA_ERR_UNSUPPORTED;
+  }
   const char* gr = getenv("ROSA_GRAPH");
   e->use_graph = !(gr && !strcmp(gr, "0"));
   rosa_status_t st = create_impl(c, w, e);

@@ -22,6 +22,7 @@ struct Dims {
   int q_n;     // nq * hd
   int gu_blk;  // gate/up interleave block: packed rows [b*2g, b*2g+g) = gate, next g = up
   int fp16;    // GEMM operands (weights + activations) held as fp16 (1) or bf16 (0); R19
+  int ada;     // time conditioning by adaptive RMSNorm (reading R25) instead of the concatenated time MLP
   float rope_base, eps, pmin, pmax;
 };
 
@@ -91,6 +92,8 @@ struct EpiArgs {
   const int* src;         // Tables::src
   int A, k_iter;
   int force_bn;           // BIAS_F32 / RESID: N tile to use (0 = chosen from N and M)
+  const float* gate;      // RESID, adaptive-norm variant: h += gate[row / H][col] * acc (null = 1); rows gate_ld floats apart
+  int gate_ld;
   int dbg;                // measurement aid (ROSA_DBG): bit 0 skip the epilogue body, bit 1 skip the MMAs
 };
 
@@ -107,6 +110,12 @@ void launch_scatter_x(const CallPtrs* cp, const float* x, const Tables& tb, int 
 void launch_timevec(float* tvec, const bf16* w_t1, const float* b_t1, const Dims& dm,
                     const Tables& tb, int nsteps_max, cudaStream_t s);
 void launch_tau16(op16* a16, const Dims& dm, const Tables& tb, int nsteps_max, cudaStream_t s);
+// adaptive-norm variant (reading R25)
+void launch_swish16(op16* out, const float* in, size_t n, int fp16, cudaStream_t s);
+void launch_embed_lin(float* h, const float* x, const float* w_inT, const float* b_in, const Dims& dm, const Tables& tb,
+                      int k_iter, int M, cudaStream_t s);
+void launch_adarms(op16* out, const float* h, const float* mod, int mod_ld, const Dims& dm, const Tables& tb, int k_iter,
+                   int M, cudaStream_t s);
 void launch_embed1(op16* z, const float* x, const float* wca, const float* bca, const float* tvec_k,
                    const Dims& dm, const Tables& tb, int k_iter, int M, cudaStream_t s);
 void launch_rmsnorm(op16* out, const float* h, const Dims& dm, const Tables& tb, int k_iter, int M,

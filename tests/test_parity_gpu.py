@@ -343,3 +343,47 @@ def test_fused_dependent_gemm_kernel_opt_in(monkeypatch):
         compare(f"fused-order{order}", got_x, got_v, want_x, want_v)
         assert np.array_equal(got_x, again)                       # deterministic
         assert n_launch == 3 + 2 * (2 + 2 * 3 + 1) + 1            # gather, tau, time GEMM; per step 2 + 3 per layer (not 5) + 1; scatter
+
+
+# ------------------------------------------------------------------ adaptive-norm variant (reading R25)
+def test_adarms_variant_pi0_shapes():
+    """pi0-scale widths (d 1024, F 4096, 8q/1kv x 256), 3 layers, ragged prefixes: CTA-pair GEMMs (M = 300)."""
+    case = cases.make_adarms_case("pi0", batch=6, layers=3)
+    assert case.cfg.time_conditioning == 1 and case.cfg.d_model == 1024
+    lc = LoadedCase(case)
+    assert rosa.rosa_kernel_family(lc.expert) == 1
+    got_x, _ = check_against_oracle(case, lc, list(range(6)), "adarms-pi0-b6")
+    again, _ = lc.run(robots=list(range(6)))
+    assert np.array_equal(got_x, again)                                   # P13
+    # M = 100 rows: the single-CTA GEMM kernels; batch invariance against the batched run (P2)
+    sub, _ = check_against_oracle(case, lc, [4, 1], "adarms-pi0-b2")
+    assert np.abs(sub - got_x[[4, 1]]).max() <= 5e-3
+    lc.close()
+
+
+def test_adarms_variant_mixed_steps_and_gate_wiring():
+    """Narrow model, robots at different denoise stages (shrinking active set), then the closed forms."""
+    from dataclasses import replace
+    cfg = replace(MINI, time_conditioning=1)
+    case = cases.build_case("adarms-mini-mix", 23, cfg, bf16=True, draw_lens=(0, 200), batch=5, cfg3_mix=True)
+    lc = LoadedCase(case)
+    check_against_oracle(case, lc, list(range(5)), "adarms-mini-mix")
+    lc.close()
+    # zero gate: blocks are the identity, v = (h0 r)(1 + scale) + shift through W_out: oracle closed form pinned on CPU
+    d = cfg.d_model
+    for k in ("b_mod_attn", "b_mod_mlp"):
+        case.weights[k] = [np.concatenate([b[:2 * d], np.zeros(d, np.float32)]) for b in case.weights[k]]
+    for k in ("w_mod_attn", "w_mod_mlp"):
+        case.weights[k] = [np.concatenate([w[:2 * d], np.zeros((d, d), np.float32)]) for w in case.weights[k]]
+    lc = LoadedCase(case)
+    got_x, got_v = lc.run(want_velocity=True)
+    want_x, want_v = O.denoise_case(case, return_velocity=True)
+    compare("adarms-zero-gate", got_x, got_v, want_x, want_v)
+    lc.close()
+
+
+def test_adarms_variant_needs_tcgen05_shapes():
+    case = cases.make_adarms_case("tiny")
+    with pytest.raises(rosa.RosaError) as ei:
+        LoadedCase(case)
+    assert ei.value.status == rosa.ROSA_ERR_UNSUPPORTED
