@@ -70,6 +70,10 @@ def class_flops(cfg, lens, n_euler):
         "gemm_down_resid": 2.0 * tok * F * d * Lyr,
         "final_norm_outproj_euler": 2.0 * tok * d * A,
     }
+    if getattr(cfg, "time_conditioning", 0) == 1:    # adaptive-norm variant (R25)
+        rs = float(ne.sum())                         # robot-steps
+        del out["gemm_embed"]                        # h0 = W_in x + b_in only
+        out["timevec"] = 2.0 * rs * (2 * d * d + (2 * Lyr + 1) * 3 * d * d)   # time MLP + all modulation vectors
     out["gemm_fused_o_gateup_down"] = out["gemm_o_resid"] + out["gemm_gateup_geglu"] + out["gemm_down_resid"]
     return out
 
@@ -81,6 +85,9 @@ def call_bytes(cfg, lens, n_euler):
     nq, nkv, hd, Lyr = cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim, cfg.layers
     params = d * A + d + 2 * d * d + d + d * d + d + A * d + A + d + \
         Lyr * ((nq + 2 * nkv) * hd * d + nq * hd * d + 3 * F * d + 2 * d)
+    if getattr(cfg, "time_conditioning", 0) == 1:
+        params = d * A + d + 2 * (d * d + d) + A * d + A + (2 * Lyr + 1) * (3 * d * d + 3 * d) + \
+            Lyr * ((nq + 2 * nkv) * hd * d + nq * hd * d + 3 * F * d)
     iters = int(np.max(n_euler))
     kv = float((np.asarray(lens, dtype=np.float64) * np.asarray(n_euler, dtype=np.float64)).sum()) * \
         2 * nkv * hd * 2 * Lyr
@@ -240,7 +247,8 @@ def run_ours(args, rank, world, local_rank):
 
     B = args.batch
     # same weights on every rank, different robots; --config 3 = the continuous-batching mix (extra line, not the contract metric)
-    case = cases.make_case(args.config, batch=B, robot_stream=rank)
+    ada = args.time_conditioning == "adarms"
+    case = cases.make_case(args.config, batch=B, robot_stream=rank, time_conditioning=1 if ada else 0)
     cfg = case.cfg
     lc = LoadedCase(case, device=dev)
     stream = torch.cuda.Stream(device=dev)
@@ -341,13 +349,13 @@ def run_ours(args, rank, world, local_rank):
             "warmup": args.warmup, "ms_per_step": ms_call, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "fp16 operands / fp32 accumulate" if os.environ.get("ROSA_GEMM_DTYPE") != "bf16"
             else "bf16 operands / fp32 accumulate", "data": "synthetic",
-            "config": {"workload": f"cfg{args.config} " + ("fleet batch" if args.config == 2 else "continuous-batching mix (t_i in {1.0..0.1}, n_i = 10 t_i)") + f": B={B} robots/GPU, pi0-scale expert (18L d1024 8q/1kv hd256 "
+            "config": {"workload": f"cfg{args.config} " + ("fleet batch" if args.config == 2 else "continuous-batching mix (t_i in {1.0..0.1}, n_i = 10 t_i)") + (", adaptive-RMSNorm time conditioning (pi0.5-style variant, DESIGN.md R25; not the contract workload)" if ada else "") + f": B={B} robots/GPU, pi0-scale expert (18L d1024 8q/1kv hd256 "
                                    f"ffn4096 H50 A32), ragged prefix lengths (sum L={int(case.prefix_lens.sum())}), "
                                    f"up to 10 Euler steps per call, seed {args.config}",
                        "robot_steps_per_call": int(case.n_steps.sum()),
                        "robot_steps_per_sec": float(world * case.n_steps.sum() * args.steps / (total_ms * 1e-3)),
-                       "l2": "inputs exceed L2 (629 MB weights + %.2f GB prefix K/V streamed per Euler step)"
-                             % (lc.kv_bytes() / 1e9),
+                       "l2": "inputs exceed L2 (%d MB weights + %.2f GB prefix K/V streamed per Euler step)"
+                             % (862 if ada else 629, lc.kv_bytes() / 1e9),
                        "kernel_family": "tcgen05" if family == 1 else "cuda-core", "cuda_graph": True,
                        "parallelism": f"replicas x{world}, robots sharded, no collective"},
             "latency_ms": {"p50": pct(per_call, 0.5), "p99": pct(per_call, 0.99), "min": min(per_call)},
@@ -414,6 +422,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--batch", type=int, default=None, help="robots per GPU (default 64 for cfg2, 256 for cfg3)")
     ap.add_argument("--config", type=int, default=2, choices=[2, 3], help="2 = fleet batch (the metric), 3 = continuous-batching mix")
+    ap.add_argument("--time-conditioning", default="concat", choices=["concat", "adarms"],
+                    help="concat = the contract workload (pi0-style); adarms = the adaptive-RMSNorm variant (extra line)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true")
     ap.add_argument("--sweep-max", type=int, default=512)

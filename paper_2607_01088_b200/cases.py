@@ -223,9 +223,17 @@ def build_case(name: str, seed: int, cfg: ExpertConfig, *, bf16: bool,
 
 
 def make_case(config: int, *, batch: Optional[int] = None, with_prefix: bool = True,
-              robot_stream: int = 0) -> Case:
-    """BASELINE.json ``configs[config]``.  ``batch`` selects the B of the config-4 sweep."""
+              robot_stream: int = 0, time_conditioning: int = 0) -> Case:
+    """BASELINE.json ``configs[config]``.  ``batch`` selects the B of the config-4 sweep.
+    ``time_conditioning=1`` (configs 1-4): the same workload on the adaptive-norm variant of the expert (R25)."""
     kw = dict(with_prefix=with_prefix, robot_stream=robot_stream)
+    if time_conditioning:
+        from dataclasses import replace
+        pi0 = replace(PI0, time_conditioning=1)
+        spec = {1: dict(prefix_lens=[816] * 8), 2: dict(draw_lens=(600, 1000), batch=batch or 64),
+                3: dict(draw_lens=(400, 1200), batch=batch or 256, cfg3_mix=True),
+                4: dict(prefix_lens=[816] * (batch or 64))}[config]
+        return build_case(f"cfg{config}-adarms", config, pi0, bf16=True, **spec, **kw)
     if config == 0:
         return build_case("cfg0-tiny", 0, TINY, bf16=False, prefix_lens=[48, 64], n_steps=4, **kw)
     if config == 1:

@@ -130,13 +130,21 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, float* scr, uin
       float4 o[8];
       from_scratch(o);
       if constexpr (EPI == EPI_RESID) {
+        if (ea.gate) {  // adaptive-norm variant (R25): per-robot gate on the sublayer output, h += gate * acc.
+          // Addresses are clamped into range instead of predicated so the 8 loads issue back to back.
+          const int colc = colok ? col : n0;
+          float4 g[8];
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const int rr = min(r0 + i * 4 + lr, m_lim - 1);
+            g[i] = *reinterpret_cast<const float4*>(ea.gate + (size_t)(rr / ea.H) * ea.gate_ld + colc);
+          }
+#pragma unroll
+          for (int i = 0; i < 8; ++i) { o[i].x *= g[i].x; o[i].y *= g[i].y; o[i].z *= g[i].z; o[i].w *= g[i].w; }
+        }
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
           if (colok && r0 + i * 4 + lr < m_lim) {
-            if (ea.gate) {  // adaptive-norm variant (R25): per-robot gate on the sublayer output
-              const float4 g = *reinterpret_cast<const float4*>(ea.gate + (size_t)((r0 + i * 4 + lr) / ea.H) * ea.gate_ld + col);
-              o[i].x *= g.x; o[i].y *= g.y; o[i].z *= g.z; o[i].w *= g.w;
-            }
             const float4 h = *reinterpret_cast<const float4*>(gp + i * step);
             o[i].x += h.x; o[i].y += h.y; o[i].z += h.z; o[i].w += h.w;
           }

@@ -387,3 +387,40 @@ def test_adarms_variant_needs_tcgen05_shapes():
     with pytest.raises(rosa.RosaError) as ei:
         LoadedCase(case)
     assert ei.value.status == rosa.ROSA_ERR_UNSUPPORTED
+
+
+def test_adarms_variant_full_depth_cfg1_sampled():
+    """All 18 layers and 10 Euler steps of the cfg1 workload on the variant; oracle on two of the eight robots.
+
+    Final actions: north_star tolerances.  Per-step velocity: 5e-3 holds when both sides evaluate v at the SAME x
+    (each Euler step launched from the oracle's x_k: the arithmetic error of one velocity evaluation).  Along the
+    free-running trajectory the variant's velocity is more sensitive to the accumulated difference in x than the
+    base model's (x enters the residual stream through W_in alone, R25), so there the bound is 1e-2, stated here."""
+    case = cases.make_case(1, time_conditioning=1)
+    assert case.cfg.layers == 18 and case.batch == 8
+    lc = LoadedCase(case)
+    sample = [0, 5]
+    got_x, got_v = lc.run(want_velocity=True)
+    want_x, want_v = O.denoise_case(case, robots=sample, return_velocity=True)
+    free = [rel_l2(got_v[k][sample], want_v[k]) for k in range(len(want_v))]
+    print(f"[adarms-cfg1 free-running] actions max-abs {np.abs(got_x[sample] - want_x).max():.3e} rel-L2 "
+          f"{rel_l2(got_x[sample], want_x):.3e}; velocity rel-L2 per step {[f'{v:.2e}' for v in free]}")
+    assert np.abs(got_x[sample] - want_x).max() <= TOL_ACT_ABS and rel_l2(got_x[sample], want_x) <= TOL_ACT_REL
+    assert free[0] <= TOL_VEL_REL and max(free) <= 1e-2
+    # teacher-forced: step k from the oracle's x_k at t_k
+    dev = lc.device
+    ids = np.asarray(sample, dtype=np.int32)
+    xk = case.noise[sample].astype(np.float64)
+    forced = []
+    for k in range(len(want_v)):
+        x_in = torch.from_numpy(xk.astype(np.float32)).to(dev)
+        out = torch.empty_like(x_in)
+        vel = torch.empty((1,) + tuple(x_in.shape), dtype=torch.float32, device=dev)
+        t_k = (case.t_start[sample] + k * case.dt[sample]).astype(np.float32)
+        rosa.rosa_denoise_batch_ex(lc.expert, ids, x_in, t_k, case.dt[sample], np.ones(len(sample), np.int32), out, vel, None)
+        torch.cuda.synchronize()
+        forced.append(rel_l2(vel[0].cpu().numpy(), want_v[k]))
+        xk = xk + case.dt[sample].astype(np.float64)[:, None, None] * want_v[k]
+    print(f"[adarms-cfg1 same-x] velocity rel-L2 per step max {max(forced):.3e}")
+    assert max(forced) <= TOL_VEL_REL, forced
+    lc.close()
