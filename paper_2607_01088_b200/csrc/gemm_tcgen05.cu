@@ -281,17 +281,20 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, float* scr, uin
     }
   } else if constexpr (EPI == EPI_GEGLU) {
     // packed columns: [gate 64 | up 64] blocks (gu_blk = 64) -> 64 outputs; this warp takes block `half`
-    static_assert(EPI != EPI_GEGLU || BN == 256, "GeGLU epilogue assumes two 128-column blocks per tile");
+    // BN = 256: two 128-column blocks, one per half-warp; BN = 128 (single-CTA kernel, small batches): one block,
+    // each half-warp takes 32 of its 64 outputs
+    static_assert(EPI != EPI_GEGLU || BN == 256 || BN == 128, "GeGLU epilogue: one or two 128-column blocks per tile");
     const float rs = row_rscale(ea, ok ? row : 0);
     uint16_t* outp = (uint16_t*)ea.out16;
-    const int blk = half;
+    const int blk = BN == 256 ? half : 0;
+    const int hh_beg = BN == 256 ? 0 : half, hh_end = BN == 256 ? 2 : half + 1;
 #pragma unroll 1
-    for (int hh = 0; hh < 2; ++hh) {
+    for (int hh = hh_beg; hh < hh_end; ++hh) {
       {
         float g[32], u[32];
         ld_acc32(t_acc + blk * 128 + hh * 32, g);
         ld_acc32(t_acc + blk * 128 + 64 + hh * 32, u);
-        if (hh == 1) release();
+        if (hh == hh_end - 1) release();
 #pragma unroll
         for (int i = 0; i < 32; ++i) g[i] = gelu_tanh_f(g[i] * rs) * (u[i] * rs);
         to_scratch(g);
@@ -1040,8 +1043,9 @@ cudaError_t launch_gemm_tc(Epi epi, const op16* A, const op16* W, int M, int N, 
       return use_pair(M) ? launch_two<256, EPI_ROPE>(A, W, M, N, K, a, s) : launch_one<256, EPI_ROPE>(A, W, M, N, K, a, s);
     case EPI_GEGLU:
       if (a.gu_blk != 64 || N % 256) return cudaErrorNotSupported;
+      // M <= 128: 128-column tiles (5 stages of 32 KB, twice the CTAs) halve the latency-bound K loop of a tile
       return use_pair(M) ? launch_two<256, EPI_GEGLU>(A, W, M, N, K, a, s)
-                         : launch_one<256, EPI_GEGLU>(A, W, M, N, K, a, s);
+                         : launch_one<128, EPI_GEGLU>(A, W, M, N, K, a, s);
   }
   return cudaErrorNotSupported;
 }
