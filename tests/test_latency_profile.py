@@ -70,3 +70,25 @@ def test_profile_on_gpu_small():
     prof = lp.profile([1, 8], pools, n_requests=500)
     assert all(t > 0 for b in pools for t in pools[b])
     assert prof[8]["max_throughput_per_s"] > prof[1]["max_throughput_per_s"]
+
+
+def test_bench_work_accounting_for_both_time_conditionings():
+    """bench.py's algorithmic FLOPs / bytes: SURVEY 8(d) figures for the base path, and the variant's extra terms."""
+    import importlib.util, os
+    from dataclasses import replace
+    from paper_2607_01088_b200 import cases
+    spec = importlib.util.spec_from_file_location("bench", os.path.join(os.path.dirname(__file__), "..", "bench.py"))
+    bench = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(bench)
+    lens, ns = [816] * 64, [10] * 64
+    fl = bench.class_flops(cases.PI0, lens, ns)
+    tot = sum(v for k, v in fl.items() if k != "gemm_fused_o_gateup_down")
+    assert abs(tot / 1e12 - 24.16) < 0.02       # SURVEY 8(a): 24.22 TFLOP per call, minus the hoisted per-token time half of W_1
+    assert abs(bench.call_bytes(cases.PI0, lens, ns) / 1e9 - 15.92) < 0.05   # 10 x (629.36 MB + 64 x 15.04 MB)
+    ada = replace(cases.PI0, time_conditioning=1)
+    fa = bench.class_flops(ada, lens, ns)
+    assert "gemm_embed" not in fa and fa["timevec"] == 2.0 * 640 * (2 * 1024 ** 2 + 37 * 3 * 1024 ** 2)
+    assert fa["attention"] == fl["attention"] and fa["gemm_gateup_geglu"] == fl["gemm_gateup_geglu"]
+    extra = bench.call_bytes(ada, lens, ns) - bench.call_bytes(cases.PI0, lens, ns)
+    # parameters per step (2 B each): + 37 modulation matrices and biases, - the action half of W_1, - the 37 gain vectors
+    assert abs(extra / 10 / 2 - (37 * (3 * 1024 ** 2 + 3 * 1024) - 1024 ** 2 - 37 * 1024)) < 1
