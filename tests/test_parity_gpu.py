@@ -424,3 +424,36 @@ def test_adarms_variant_full_depth_cfg1_sampled():
     print(f"[adarms-cfg1 same-x] velocity rel-L2 per step max {max(forced):.3e}")
     assert max(forced) <= TOL_VEL_REL, forced
     lc.close()
+
+
+def test_soak_random_batch_compositions_are_reproducible():
+    """~10 s of back-to-back calls with random batch sizes, robot subsets and per-robot step counts on the cfg2
+    fleet (every call replays or captures a graph keyed by (batch, max steps)): each call is issued twice and must
+    agree bitwise (P13: no order-dependent arithmetic, no race between the graph's kernels), stay finite, and robots
+    that run all 10 steps must match their single-robot result (P2)."""
+    import time
+    case = cases.make_case(2)
+    lc = LoadedCase(case)
+    single = {r: lc.run(robots=[r])[0][0] for r in (0, 13, 63)}
+    rng = np.random.default_rng(7)
+    t_end, calls = time.time() + 10.0, 0
+    while time.time() < t_end:
+        b = int(rng.choice([1, 2, 3, 5, 8, 13, 21, 34, 50, 64]))
+        idx = rng.permutation(64)[:b].astype(np.int32)
+        ns = rng.integers(1, 11, size=b).astype(np.int32)
+        tst = np.ones(b, np.float32)
+        dt = (-tst / ns).astype(np.float32)
+        noise = torch.from_numpy(case.noise[idx]).to(lc.device)
+        o1, o2 = torch.empty_like(noise), torch.empty_like(noise)
+        rosa.rosa_denoise_batch_ex(lc.expert, idx, noise, tst, dt, ns, o1, None, None)
+        rosa.rosa_denoise_batch_ex(lc.expert, idx, noise, tst, dt, ns, o2, None, None)
+        torch.cuda.synchronize()
+        a = o1.cpu().numpy()
+        assert np.all(np.isfinite(a)) and np.array_equal(a, o2.cpu().numpy()), (b, idx[:4], ns[:4])
+        for j, r in enumerate(idx):
+            if int(r) in single and ns[j] == 10:
+                assert np.abs(a[j] - single[int(r)]).max() <= 5e-3
+        calls += 2
+    print(f"[soak] {calls} calls")
+    assert calls >= 100
+    lc.close()
