@@ -358,6 +358,8 @@ def test_adarms_variant_pi0_shapes():
     # M = 100 rows: the single-CTA GEMM kernels; batch invariance against the batched run (P2)
     sub, _ = check_against_oracle(case, lc, [4, 1], "adarms-pi0-b2")
     assert np.abs(sub - got_x[[4, 1]]).max() <= 5e-3
+    one, _ = check_against_oracle(case, lc, [3], "adarms-pi0-b1")         # one robot: one row of cond / modulation
+    assert np.abs(one[0] - got_x[3]).max() <= 5e-3
     lc.close()
 
 
