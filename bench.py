@@ -403,7 +403,10 @@ def run_sweep(args):
         t_c, t_m = fl_tot / (peaks["bf16_tflops"] * 1e12) * 1e3, by / (peaks["hbm_gbs"] * 1e9) * 1e3
         row = {"B": B, "chunks_per_s": B / (ms * 1e-3), "ms_per_call": ms, "p50_ms": pct(per_call, 0.5),
                "p99_ms": pct(per_call, 0.99), "bound": "tensor" if t_c > t_m else "hbm",
-               "roofline_ms": max(t_c, t_m), "roofline_frac": max(t_c, t_m) / ms, "steps": steps}
+               "roofline_ms": max(t_c, t_m), "roofline_frac": max(t_c, t_m) / ms,
+               # also against the sustained measured peak and the nominal 2250 TFLOP/s / 8 TB/s
+               "roofline_frac_sustained": max(fl_tot / (peaks["bf16_tflops_sustained"] * 1e12) * 1e3, t_m) / ms,
+               "roofline_frac_nominal": max(fl_tot / 2250e12, by / 8000e9) * 1e3 / ms, "steps": steps}
         rows.append(row)
         print(json.dumps(row), flush=True)
         fl.close()
