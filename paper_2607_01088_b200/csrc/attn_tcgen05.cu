@@ -91,6 +91,9 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
   if (warp == 0 && lane == 0) {
     prefetch_tensormap(&maps.q);
     prefetch_tensormap(&maps.own);
+    // the per-robot prefix maps live in global memory
+    prefetch_tensormap(kmap);
+    prefetch_tensormap(vmap);
     for (int s = 0; s < AT_KST; ++s) { mbar_init(k_full(s), 1); mbar_init(k_empty(s), 1); }
     for (int s = 0; s < AT_ST; ++s) { mbar_init(v_full(s), 1); mbar_init(v_empty(s), 1); }
     mbar_init(s_full(0), 1); mbar_init(s_full(1), 1);
@@ -134,12 +137,14 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
         }
         __syncwarp();
       };
+      // K(0) first: it usually comes from HBM (the prefix cache is streamed once per layer) while Q was just
+      // written by the QKV GEMM and hits L2, so queueing Q's 64 KB ahead of it delayed the first S MMA
+      load_k(0);
       if (elect_one()) {
         mbar_expect_tx(q_full, AT_Q_BYTES);
         for (int c = 0; c < 4; ++c) tma_load_3d(q_smem + c * (AT_ROWS * 128), &maps.q, q_full, c * 64, 0, tok0);
       }
       __syncwarp();
-      load_k(0);  // what the first MMAs need goes out before any prefetch
       for (int i = 0; i < nb; ++i) {  // K runs one block ahead of V: it is needed a whole softmax earlier
         if (i + 1 < nb) load_k(i + 1);
         const int s = i % AT_ST;
@@ -337,11 +342,14 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
       const int row = q * 32 + x * 4 + lr, j = tt * AT_TOK + (row >> 3);
       orow[x] = j < dm.H ? (size_t)(p * dm.H + j) * dm.q_n + (row & 7) * AT_HD + lc : (size_t)-1;
     }
-#pragma unroll 1
-    for (int c = half * 4; c < half * 4 + 4; ++c) {
-      uint32_t rr[32];
-      tmem_ld32(tmem_o + lane_off + c * 32, rr);
+    uint32_t rbuf[2][32];  // the next chunk's TMEM load is in flight while this one is transposed and stored
+    tmem_ld32(tmem_o + lane_off + (half * 4) * 32, rbuf[0]);
+#pragma unroll
+    for (int cc = 0; cc < 4; ++cc) {
+      const int c = half * 4 + cc;
+      uint32_t (&rr)[32] = rbuf[cc & 1];
       tmem_ld_wait();
+      if (cc + 1 < 4) tmem_ld32(tmem_o + lane_off + (c + 1) * 32, rbuf[(cc + 1) & 1]);
 #pragma unroll
       for (int e = 0; e < 32; e += 4)
         *reinterpret_cast<float4*>(&scr[lane * P + e]) =
