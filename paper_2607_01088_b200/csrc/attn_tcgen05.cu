@@ -258,12 +258,15 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
 #pragma unroll
         for (int c = 0; c < 32; ++c) sc[c] = __uint_as_float(r0[c]);
         float mo = -INFINITY;
-        if (n_valid < 32 || n_other < 32) {  // warp-uniform; only the last prefix block and the own-token block
+        // warp-uniform branches; only the last prefix block and the own-token block are ragged, and there
+        // only one of the two halves of a row is short
+        if (n_valid < 32) {
 #pragma unroll
-          for (int c = 0; c < 32; ++c) {
-            sc[c] = c < n_valid ? sc[c] : -INFINITY;
-            mo = fmaxf(mo, c < n_other ? __uint_as_float(r1[c]) : -INFINITY);
-          }
+          for (int c = 0; c < 32; ++c) sc[c] = c < n_valid ? sc[c] : -INFINITY;
+        }
+        if (n_other < 32) {
+#pragma unroll
+          for (int c = 0; c < 32; ++c) mo = fmaxf(mo, c < n_other ? __uint_as_float(r1[c]) : -INFINITY);
         } else {
 #pragma unroll
           for (int c = 0; c < 32; ++c) mo = fmaxf(mo, __uint_as_float(r1[c]));
