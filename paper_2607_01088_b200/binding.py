@@ -250,7 +250,7 @@ def rosa_debug_attn_trace() -> np.ndarray:
 
 
 def rosa_debug_gemm_trace() -> np.ndarray:
-    buf = np.zeros(16, dtype=np.int64)
+    buf = np.zeros((16, 2, 16), dtype=np.int64)  # [2 * EPI + (K > 2048)][CTA 0 | CTA 64][slot]
     load().rosa_debug_gemm_trace(_ptr(buf), buf.size)
     return buf
 

@@ -76,6 +76,54 @@ __device__ __forceinline__ float row_rscale(const EpiArgs& ea, int row) {
   return rsqrtf(ss * ea.inv_d + ea.eps);
 }
 
+// What an epilogue warp fetches BEFORE it waits for its accumulator, so that the latency sits under the main
+// loop instead of after it (clock trace, profiles/r1_gemm_epilogue_trace.md: the residual epilogue's h loads were
+// four exposed round trips, 17k cycles of a 39k-cycle O-projection launch; the RoPE epilogue began with three
+// dependent ones: ids -> rlen, the sum-of-squares partials, the cos/sin rows).
+struct EpiPre {
+  float rs;            // row_rscale of this thread's row (ROPE / GEGLU / FINAL)
+  int posr;            // ROPE: position L_p + j of this thread's row
+  float4 cs0[8], cs1[8];  // ROPE: (cos, sin) of the first 32-column chunk, rows i * 4 + lr, columns lc..lc+3
+};
+template <int BN, int EPI>
+__device__ __forceinline__ void rope_load_cs(const EpiArgs& ea, int posr, int c, int lane, float4 (&cs0)[8], float4 (&cs1)[8]) {
+  const int lr = lane >> 3, lc = (lane & 7) * 4;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const int pos = __shfl_sync(0xffffffffu, posr, i * 4 + lr);
+    const float4* tp = reinterpret_cast<const float4*>(ea.rope_tab + (size_t)pos * (BN / 2) + c * 32 + lc);
+    cs0[i] = tp[0];
+    cs1[i] = tp[1];
+  }
+}
+template <int BN, int EPI>
+__device__ __forceinline__ void epilogue_pre(EpiPre& pre, const EpiArgs& ea, int r0, int n0, int m_lim, int N, int lane, int half) {
+  const int row = r0 + lane;
+  const bool ok = row < m_lim;
+  if constexpr (EPI == EPI_RESID) {
+    // h (32 rows x half a tile of fp32) towards L2: the weights streamed since it was written may have pushed it out
+    constexpr int NCT = (BN + 31) / 32, NC0 = (NCT + 1) / 2;
+    const int c_beg = half ? NC0 : 0, c_end = half ? NCT : NC0;
+    const int n_end = min(n0 + BN, N);
+    if (ok) {
+      const float* hp = ea.out_f32 + (size_t)row * ea.ld_out;
+      for (int col = n0 + c_beg * 32; col < min(n0 + c_end * 32, n_end); col += 32)
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(hp + col));
+    }
+  }
+  if constexpr (EPI == EPI_ROPE || EPI == EPI_GEGLU || EPI == EPI_FINAL) pre.rs = row_rscale(ea, ok ? row : 0);
+  if constexpr (EPI == EPI_ROPE) {
+    pre.posr = 0;
+    if (n0 < ea.rope_cols) {  // warp-uniform (one head per tile)
+      if (ok) {
+        const int p = row / ea.H;
+        pre.posr = ea.rlen[ea.ids[p]] + (row - p * ea.H);
+      }
+      rope_load_cs<BN, EPI>(ea, pre.posr, half * 2, lane, pre.cs0, pre.cs1);
+    }
+  }
+}
+
 // Epilogue of one accumulator tile for one warp: its 32 rows (TMEM lane quarter) x ONE HALF of the
 // tile's BN columns (`half`: the 8 epilogue warps are two per lane quarter).  `release()` is called
 // once, as soon as this warp has read its part of the accumulator.
@@ -84,12 +132,10 @@ __device__ __forceinline__ float row_rscale(const EpiArgs& ea, int row) {
 // rows, conflict-free both ways) and then works with 8 lanes x 4 columns per row, 4 rows per
 // instruction, so every global access is a coalesced 64..128-byte row segment.
 template <int BN, int EPI, typename Release>
-__device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, float* scr, uint32_t t_acc, int r0, int n0, int m_lim,
+__device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, EpiPre& pre, float* scr, uint32_t t_acc, int r0, int n0, int m_lim,
                                               int N, int lane, int half, Release release) {
   constexpr int P = 36;
   const int lr = lane >> 3, lc = (lane & 7) * 4;
-  const int row = r0 + lane;  // row of this thread in the thread = row domain
-  const bool ok = row < m_lim;
   auto to_scratch = [&](const float (&v)[32]) {
 #pragma unroll
     for (int i = 0; i < 32; i += 4)
@@ -113,13 +159,6 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, float* scr, uin
     const bool want_h16 = EPI != EPI_STORE_F32 && ea.h16 != nullptr;
 #pragma unroll 1
     for (int c = c_beg; c < c_end; ++c) {
-      {
-        float v[32];
-        ld_acc32(t_acc + c * 32, v);
-        if (c == c_end - 1) release();
-        to_scratch(v);
-      }
-      __syncwarp();
       const int col = n0 + c * 32 + lc;
       const bool colok = col < n_end;
       float4 add = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -127,6 +166,22 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, float* scr, uin
       float* gp = ea.out_f32 + (size_t)(r0 + lr) * ea.ld_out + col;
       uint16_t* hp = (uint16_t*)ea.h16 + (size_t)(r0 + lr) * ea.ld_out + col;
       const size_t step = (size_t)4 * ea.ld_out;
+      // the residual rows are requested first: their latency (L2, after epilogue_prefetch) overlaps the
+      // accumulator load and the transpose
+      float4 hres[8];
+      if constexpr (EPI == EPI_RESID) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+          hres[i] = colok && r0 + i * 4 + lr < m_lim ? *reinterpret_cast<const float4*>(gp + i * step)
+                                                      : make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+      {
+        float v[32];
+        ld_acc32(t_acc + c * 32, v);
+        if (c == c_end - 1) release();
+        to_scratch(v);
+      }
+      __syncwarp();
       float4 o[8];
       from_scratch(o);
       if constexpr (EPI == EPI_RESID) {
@@ -143,12 +198,7 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, float* scr, uin
           for (int i = 0; i < 8; ++i) { o[i].x *= g[i].x; o[i].y *= g[i].y; o[i].z *= g[i].z; o[i].w *= g[i].w; }
         }
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
-          if (colok && r0 + i * 4 + lr < m_lim) {
-            const float4 h = *reinterpret_cast<const float4*>(gp + i * step);
-            o[i].x += h.x; o[i].y += h.y; o[i].z += h.z; o[i].w += h.w;
-          }
-        }
+        for (int i = 0; i < 8; ++i) { o[i].x += hres[i].x; o[i].y += hres[i].y; o[i].z += hres[i].z; o[i].w += hres[i].w; }
       }
 #pragma unroll
       for (int i = 0; i < 8; ++i) {
@@ -182,7 +232,7 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, float* scr, uin
   } else if constexpr (EPI == EPI_FINAL) {
     // a9 + a10: columns are action dimensions (N = 64 covers A <= 64): v = r acc + b_out, x += dt_p v
     static_assert(EPI != EPI_FINAL || BN == 64, "final projection uses one 64-column tile");
-    const float rs = row_rscale(ea, ok ? row : 0);
+    const float rs = pre.rs;
     {
       float v[32];
       ld_acc32(t_acc + half * 32, v);
@@ -221,12 +271,8 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, float* scr, uin
     // warp covers low columns [64 half, 64 half + 64) and their partners 128 further on.
     static_assert(EPI != EPI_ROPE || BN == 256, "RoPE epilogue assumes BN == head_dim == 256");
     const bool rot = n0 < ea.rope_cols;
-    const float rs = row_rscale(ea, ok ? row : 0);
-    int posr = 0;
-    if (ok && rot) {
-      const int p = row / ea.H;
-      posr = ea.rlen[ea.ids[p]] + (row - p * ea.H);
-    }
+    const float rs = pre.rs;
+    const int posr = pre.posr;
     uint16_t* outp = (uint16_t*)ea.out16;
 #pragma unroll 1
     for (int cc = 0; cc < 2; ++cc) {
@@ -250,22 +296,17 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, float* scr, uin
         from_scratch(hi);
       }
       if (rot) {  // warp-uniform (one head per tile)
-        float4 cs0[8], cs1[8];  // (cos, sin) of columns lc, lc+1 | lc+2, lc+3
+        // (cos, sin) of columns lc, lc+1 | lc+2, lc+3: chunk cc = 0 was loaded before the accumulator wait
+        // (epilogue_pre), chunk 1 is requested below while chunk 0 is stored
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
-          const int pos = __shfl_sync(0xffffffffu, posr, i * 4 + lr);
-          const float4* tp = reinterpret_cast<const float4*>(ea.rope_tab + (size_t)pos * (BN / 2) + c * 32 + lc);
-          cs0[i] = tp[0];
-          cs1[i] = tp[1];
+          const float4 a = lo[i], b = hi[i], cs0 = pre.cs0[i], cs1 = pre.cs1[i];
+          lo[i].x = a.x * cs0.x - b.x * cs0.y; hi[i].x = b.x * cs0.x + a.x * cs0.y;
+          lo[i].y = a.y * cs0.z - b.y * cs0.w; hi[i].y = b.y * cs0.z + a.y * cs0.w;
+          lo[i].z = a.z * cs1.x - b.z * cs1.y; hi[i].z = b.z * cs1.x + a.z * cs1.y;
+          lo[i].w = a.w * cs1.z - b.w * cs1.w; hi[i].w = b.w * cs1.z + a.w * cs1.w;
         }
-#pragma unroll
-        for (int i = 0; i < 8; ++i) {
-          const float4 a = lo[i], b = hi[i];
-          lo[i].x = a.x * cs0[i].x - b.x * cs0[i].y; hi[i].x = b.x * cs0[i].x + a.x * cs0[i].y;
-          lo[i].y = a.y * cs0[i].z - b.y * cs0[i].w; hi[i].y = b.y * cs0[i].z + a.y * cs0[i].w;
-          lo[i].z = a.z * cs1[i].x - b.z * cs1[i].y; hi[i].z = b.z * cs1[i].x + a.z * cs1[i].y;
-          lo[i].w = a.w * cs1[i].z - b.w * cs1[i].w; hi[i].w = b.w * cs1[i].z + a.w * cs1[i].w;
-        }
+        if (cc == 0) rope_load_cs<BN, EPI>(ea, posr, c + 1, lane, pre.cs0, pre.cs1);
       }
       uint16_t* dst = outp + (size_t)(r0 + lr) * ea.ld_out + n0 + c * 32 + lc;
       const size_t step = (size_t)4 * ea.ld_out;
@@ -284,7 +325,7 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, float* scr, uin
     // BN = 256: two 128-column blocks, one per half-warp; BN = 128 (single-CTA kernel, small batches): one block,
     // each half-warp takes 32 of its 64 outputs
     static_assert(EPI != EPI_GEGLU || BN == 256 || BN == 128, "GeGLU epilogue: one or two 128-column blocks per tile");
-    const float rs = row_rscale(ea, ok ? row : 0);
+    const float rs = pre.rs;
     uint16_t* outp = (uint16_t*)ea.out16;
     const int blk = BN == 256 ? half : 0;
     const int hh_beg = BN == 256 ? 0 : half, hh_end = BN == 256 ? 2 : half + 1;
@@ -428,6 +469,8 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
       const uint32_t acc_ph = (it >> 1) & 1;
       const int m0 = (t % n_m) * BM, n0 = (t / n_m) * BN;
       const int r0 = m0 + q * 32;            // first row of this warp
+      EpiPre pre;
+      epilogue_pre<BN, EPI>(pre, ea, r0, n0, m_lim, N, lane, half);
       mbar_wait_idle(tfull_bar(acc), acc_ph);
       tc_fence_after();
       const uint32_t t_acc = tmem_base + ((uint32_t)(q * 32) << 16) + acc * BN;
@@ -440,7 +483,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         release();
         continue;
       }
-      epilogue_tile<BN, EPI>(ea, scr, t_acc, r0, n0, m_lim, N, lane, half, release);
+      epilogue_tile<BN, EPI>(ea, pre, scr, t_acc, r0, n0, m_lim, N, lane, half, release);
     }
   }
   tc_fence_before();
@@ -452,10 +495,12 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
 }
 
 // measurement aid (ROSA_DBG bit 6): clock64 at the phases of CTA 0 of the last pair-kernel launch
-__device__ long long g_gemm_trace[16];
-#define GT_TRACE(slot) do { if ((ea.dbg & 64) && blockIdx.x == 0 && lane == 0) g_gemm_trace[slot] = clock64(); } while (0)
+// [class = 2 * EPI + (K > 2048)][CTA 0 | CTA 64][slot]: the last launch of each class wins
+__device__ long long g_gemm_trace[16 * 2 * 16];
+#define GT_TRACE(slot) do { if ((ea.dbg & 64) && (blockIdx.x == 0 || blockIdx.x == 64) && lane == 0) \
+  g_gemm_trace[((2 * EPI + (K > 2048)) * 2 + (blockIdx.x != 0)) * 16 + (slot)] = clock64(); } while (0)
 int tc_gemm_read_trace(long long* host, int n) {
-  if (n > 16) n = 16;
+  if (n > 16 * 2 * 16) n = 16 * 2 * 16;
   cudaMemcpyFromSymbol(host, g_gemm_trace, n * sizeof(long long));
   return n;
 }
@@ -538,6 +583,7 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
       const int m0 = (t % n_m) * (2 * BM) + (int)rank * BM, n0 = (t / n_m) * BN + (int)rank * (BN / 2);
       for (int kb = 0; kb < n_kb; ++kb) {
         mbar_wait_idle(empty_bar(s), ph ^ 1);
+        if (t == pair && kb == 0) GT_TRACE(10);
         if (elect_one()) {
           const uint32_t lfull = mapa_shared(full_bar(s), 0);
           mbar_expect_tx_cluster(lfull, Cfg::STAGE_BYTES);
@@ -566,6 +612,8 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
           tc_fence_after();
           if (it == 0 && kb == 0) GT_TRACE(3);
           if (kb == n_kb - 1) GT_TRACE(4);
+          if (it == 0 && kb == n_kb - 1) GT_TRACE(9);
+          if (it == 0 && kb == 8) GT_TRACE(13);
           if (elect_one()) {
             const uint32_t a_addr = smem_base + s * Cfg::STAGE_BYTES;
             const uint32_t b_addr = a_addr + Cfg::A_BYTES;
@@ -594,6 +642,8 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
       const uint32_t acc_ph = (it >> 1) & 1;
       const int m0 = (t % n_m) * (2 * BM) + (int)rank * BM, n0 = (t / n_m) * BN;
       const int r0 = m0 + q * 32;
+      EpiPre pre;
+      epilogue_pre<BN, EPI>(pre, ea, r0, n0, m_lim, N, lane, half);
       mbar_wait_idle(tfull_bar(acc), acc_ph);
       tc_fence_after();
       const uint32_t t_acc = tmem_base + ((uint32_t)(q * 32) << 16) + acc * Cfg::ACC_STRIDE;
@@ -607,8 +657,10 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
         continue;
       }
       if (warp == 2) GT_TRACE(5);
-      epilogue_tile<BN, EPI>(ea, scr, t_acc, r0, n0, m_lim, N, lane, half, release);
+      if (warp == 2 && it == 0) GT_TRACE(11);
+      epilogue_tile<BN, EPI>(ea, pre, scr, t_acc, r0, n0, m_lim, N, lane, half, release);
       if (warp == 2) GT_TRACE(6);
+      if (warp == 2 && it == 0) GT_TRACE(12);
     }
   }
   tc_fence_before();
@@ -841,9 +893,17 @@ k_fused_tc2(const __grid_constant__ FusedMaps maps, const __grid_constant__ Fuse
         if (lane == 0) mbar_arrive_cluster(mapa_shared(tempty_bar(acc), 0));
       };
       const int N = fm.n_n[ph] * BN;
-      if (fm.epi[ph] == EPI_RESID) epilogue_tile<BN, EPI_RESID>(fm.ea[ph], scr, t_acc, r0, n0, m_lim, N, lane, half, release);
-      else if (fm.epi[ph] == EPI_GEGLU) epilogue_tile<BN, EPI_GEGLU>(fm.ea[ph], scr, t_acc, r0, n0, m_lim, N, lane, half, release);
-      else epilogue_tile<BN, EPI_ROPE>(fm.ea[ph], scr, t_acc, r0, n0, m_lim, N, lane, half, release);
+      EpiPre pre;  // after the acquire here: what it fetches is written by the previous phase of this kernel
+      if (fm.epi[ph] == EPI_RESID) {
+        epilogue_pre<BN, EPI_RESID>(pre, fm.ea[ph], r0, n0, m_lim, N, lane, half);
+        epilogue_tile<BN, EPI_RESID>(fm.ea[ph], pre, scr, t_acc, r0, n0, m_lim, N, lane, half, release);
+      } else if (fm.epi[ph] == EPI_GEGLU) {
+        epilogue_pre<BN, EPI_GEGLU>(pre, fm.ea[ph], r0, n0, m_lim, N, lane, half);
+        epilogue_tile<BN, EPI_GEGLU>(fm.ea[ph], pre, scr, t_acc, r0, n0, m_lim, N, lane, half, release);
+      } else {
+        epilogue_pre<BN, EPI_ROPE>(pre, fm.ea[ph], r0, n0, m_lim, N, lane, half);
+        epilogue_tile<BN, EPI_ROPE>(fm.ea[ph], pre, scr, t_acc, r0, n0, m_lim, N, lane, half, release);
+      }
       if (ph + 1 < kFusedPhases) {  // publish: this warp's part of tile (ph, m, n) is in global memory
         __threadfence();
         fence_proxy_async_all();
@@ -952,7 +1012,7 @@ bool tc_use_pair(int M) { return use_pair(M); }
 // max(MMA time ~ 2 BN, operand feed ~ 288 + BN) cycles (the L2 -> shared-memory feed bounds narrow tiles;
 // measured: profiles/r1_gemm_tile_width.md).
 static const int kPairBn[] = {256, 224, 192, 160, 128, 96, 64};
-static int resid_bn(int N, int M) {
+static int resid_bn(int N, int M, int share = 1) {  // share: lanes the CTA pairs are divided between
   if (!use_pair(M)) {
     const int units = num_sms(), n_m = (M + BM - 1) / BM;
     for (int bn = 128; bn > 64; bn >>= 1)
@@ -961,7 +1021,7 @@ static int resid_bn(int N, int M) {
   }
   static const int forced = getenv("ROSA_RESID_BN") ? atoi(getenv("ROSA_RESID_BN")) : 0;  // experiments only
   if (forced) return forced;
-  const int pairs = num_sms() / 2, n_m = (M + 2 * BM - 1) / (2 * BM);
+  const int pairs = num_sms() / 2 / share, n_m = (M + 2 * BM - 1) / (2 * BM);
   int best = 256;
   long best_cost = -1;
   for (int bn : kPairBn) {
@@ -978,6 +1038,7 @@ int tc_ssq_parts(int N, int M) {
   const int bn = resid_bn(N, M);
   return 2 * ((N + bn - 1) / bn);
 }
+int tc_resid_bn(int N, int M, int share) { return resid_bn(N, M, share); }
 
 // ROSA_WPREFETCH=0 switches the pre-wait weight prefetch off (A/B measurements)
 static int wprefetch_off_bit() {

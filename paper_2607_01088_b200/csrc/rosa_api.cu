@@ -103,6 +103,13 @@ struct rosa_expert {
   std::map<GraphKey, int64_t> graph_launches;
   cudaStream_t cap_stream = nullptr;
   int64_t last_launches = 0;
+  // Two lanes: robots are independent, so a large batch is cut into two sub-batches whose
+  // kernel chains run on two streams (two branches of the captured graph).  One lane's partial last round of
+  // tiles, prologue and exposed epilogue then overlap the other lane's main loop.  ROSA_LANES=1 turns it off.
+  int lanes = 1, lane_min_batch = 1 << 30;
+  cudaStream_t lane_stream = nullptr;
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+  size_t lane_row_align = 256;  // lane 1 starts on a fresh 256-row tile of every workspace
   float* e2e_dev = nullptr;  // staging for rosa_denoise_batch_host
   // fused a6 -> a7 -> a8 kernel: static schedules for every number of row blocks + dependency counters
   bool fused_ok = false;
@@ -174,20 +181,35 @@ static rosa_status_t upload_f32(rosa_expert* e, const std::vector<float>& v, flo
   return ROSA_OK;
 }
 
-static Tables make_tables(const rosa_expert* e, int batch) {
+// Tables of the robots at internal positions [p0, p0 + batch) (a lane of the call, or all of it: p0 = 0, lane 0);
+// every per-robot array is indexed by the position within the lane.
+static Tables make_tables(const rosa_expert* e, int batch, int p0 = 0, int lane = 0) {
   Tables tb;
-  tb.ids = (const int*)(e->d_call + e->off_ids);
-  tb.src = (const int*)(e->d_call + e->off_src);
-  tb.t0 = (const float*)(e->d_call + e->off_t0);
-  tb.dt = (const float*)(e->d_call + e->off_dt);
-  tb.nsteps = (const int*)(e->d_call + e->off_ns);
-  tb.m_active = (const int*)(e->d_call + e->off_mact);
-  tb.attn_order = (const int*)(e->d_call + e->off_order);
+  tb.ids = (const int*)(e->d_call + e->off_ids) + p0;
+  tb.src = (const int*)(e->d_call + e->off_src) + p0;
+  tb.t0 = (const float*)(e->d_call + e->off_t0) + p0;
+  tb.dt = (const float*)(e->d_call + e->off_dt) + p0;
+  tb.nsteps = (const int*)(e->d_call + e->off_ns) + p0;
+  tb.m_active = (const int*)(e->d_call + e->off_mact) + (size_t)lane * e->cfg.max_steps;
+  tb.attn_order = (const int*)(e->d_call + e->off_order) + p0;
   tb.rk = e->d_rk;
   tb.rv = e->d_rv;
   tb.rlen = e->d_rlen;
   tb.batch = batch;
   return tb;
+}
+
+// Robots of lane 0 when a batch is cut in two (0 = one lane).  Near half, moved down as far as a quarter of the
+// batch if that saves a 256-row tile block: B = 64, H = 50 gives 30 + 34 robots = 6 + 7 row blocks, where
+// 32 + 32 would pad to 7 + 7.
+static int lane_split(const rosa_expert* e, int batch) {
+  if (e->lanes < 2 || batch < e->lane_min_batch || e->prof_on) return 0;
+  const int H = e->dm.H;
+  auto blocks = [&](int b) { return (b * H + 255) / 256; };
+  int best = batch / 2;
+  for (int b0 = batch / 2; b0 >= batch / 2 - batch / 4 && b0 >= 1; --b0)
+    if (blocks(b0) + blocks(batch - b0) < blocks(best) + blocks(batch - best)) best = b0;
+  return best;
 }
 
 static void destroy_impl(rosa_expert* e) {
@@ -202,6 +224,9 @@ static void destroy_impl(rosa_expert* e) {
     if (e->stage_ev[i]) cudaEventDestroy(e->stage_ev[i]);
   }
   if (e->cap_stream) cudaStreamDestroy(e->cap_stream);
+  if (e->lane_stream) cudaStreamDestroy(e->lane_stream);
+  if (e->ev_fork) cudaEventDestroy(e->ev_fork);
+  if (e->ev_join) cudaEventDestroy(e->ev_join);
   for (cudaEvent_t ev : e->prof_ev) cudaEventDestroy(ev);
   delete e;
 }
@@ -348,7 +373,8 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
     CK(cudaMemcpy(e->rope_tab, tab.data(), tab.size() * sizeof(float2), cudaMemcpyHostToDevice));
   }
   // workspaces (rows padded to a multiple of 128 for the tile kernels)
-  const size_t Mmax = ((size_t)c->max_batch * dm.H + 127) / 128 * 128;
+  // + 256: lane 1 of a split batch starts on the next 256-row boundary after lane 0's rows
+  const size_t Mmax = ((size_t)c->max_batch * dm.H + 127) / 128 * 128 + 256;
   const size_t HA = (size_t)dm.H * A;
 #define WS(ptr, bytes) if ((st = dev_alloc(e, (void**)&(ptr), (bytes))) != ROSA_OK) return st
   WS(e->x, (size_t)c->max_batch * HA * 4);
@@ -427,7 +453,7 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
   e->off_t0 = take((size_t)c->max_batch * 4);
   e->off_dt = take((size_t)c->max_batch * 4);
   e->off_ns = take((size_t)c->max_batch * 4);
-  e->off_mact = take((size_t)c->max_steps * 4);
+  e->off_mact = take((size_t)2 * c->max_steps * 4);  // one list per lane
   e->off_order = take((size_t)c->max_batch * 4);
   e->off_ptrs = take(sizeof(CallPtrs));
   e->call_bytes = off;
@@ -438,6 +464,15 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
     CK(cudaEventCreateWithFlags(&e->stage_ev[i], cudaEventDisableTiming));
   }
   CK(cudaStreamCreateWithFlags(&e->cap_stream, cudaStreamNonBlocking));
+  CK(cudaStreamCreateWithFlags(&e->lane_stream, cudaStreamNonBlocking));
+  CK(cudaEventCreateWithFlags(&e->ev_fork, cudaEventDisableTiming));
+  CK(cudaEventCreateWithFlags(&e->ev_join, cudaEventDisableTiming));
+  {
+    const char* ln = getenv("ROSA_LANES");
+    const char* lb = getenv("ROSA_LANE_MIN_BATCH");
+    e->lanes = e->family == 1 && !dm.ada && !e->fused_ok && ln && atoi(ln) == 2 ? 2 : 1;
+    e->lane_min_batch = lb ? atoi(lb) : 32;
+  }
   return ROSA_OK;
 }
 
@@ -463,6 +498,12 @@ static cudaError_t gemm(rosa_expert* e, int cls, Epi epi, const op16* A, const o
   mark(e, cls, s);
   if (e->family == 1 && tc_gemm_supported(N, K)) {
     e->last_launches += 1;
+    static const int trace_bit = getenv("ROSA_DBG") ? atoi(getenv("ROSA_DBG")) & 64 : 0;  // clock trace of CTAs 0 and 64
+    if (trace_bit) {
+      EpiArgs at = a;
+      at.dbg |= trace_bit;
+      return launch_gemm_tc(epi, A, W, M, N, K, at, s);
+    }
     return launch_gemm_tc(epi, A, W, M, N, K, a, s);
   }
   launch_gemm_naive(A, W, e->scratch, M, N, K, a.in_fp16, a.m_active, s);
@@ -549,14 +590,120 @@ static cudaError_t enqueue_call_ada(rosa_expert* e, int batch, int nmax, cudaStr
   return cudaGetLastError();
 }
 
+// A lane of a call: the robots at internal positions [p0, p0 + tb.batch), their token rows starting at row0 of
+// every workspace; `share` lanes divide the GPU between them.
+struct LaneView {
+  Tables tb;
+  int p0;
+  size_t row0;
+  int share;
+};
+
+// All Euler iterations (a1..a10 x nmax) of one lane on `s`.
+static cudaError_t enqueue_steps(rosa_expert* e, const LaneView& lv, int batch_full, int nmax, cudaStream_t s) {
+  const Dims& dm = e->dm;
+  const Tables& tb = lv.tb;
+  const CallPtrs* cp = (const CallPtrs*)(e->d_call + e->off_ptrs);
+  const int batch = tb.batch, M = batch * dm.H, d = dm.d;
+  const size_t r0 = lv.row0;
+  float* x = e->x + (size_t)lv.p0 * dm.H * dm.A;
+  float* h = e->h + r0 * d;
+  op16 *zbuf = e->zbuf + r0 * d, *nrm = e->nrm + r0 * d, *obuf = e->obuf + r0 * dm.q_n, *mact = e->mact + r0 * dm.F;
+  bf16* qkv = e->qkv + r0 * dm.qkv_n;
+  float* ssq = e->ssq + r0 * (d / 32);
+  cudaError_t err;
+  const bool fused_norm = e->family == 1;  // RMSNorm fused into the GEMM epilogues (tcgen05 family)
+  const bool use_fused = e->fused_ok && tc_use_pair(M);
+  int fused_idx = 0;
+  for (int k = 0; k < nmax; ++k) {
+    EpiArgs ea{};
+    ea.m_active = tb.m_active + k;
+    ea.H = dm.H; ea.hd = dm.hd; ea.gu_blk = dm.gu_blk; ea.in_fp16 = dm.fp16; ea.out_fp16 = dm.fp16;
+    ea.inv_d = 1.f / (float)d; ea.eps = dm.eps; ea.n_part = tc_ssq_parts(d, M);
+    if (fused_norm) { ea.h16 = nrm; ea.ssq_out = ssq; ea.ssq_in = ssq; }
+    if (use_fused) { ea.force_bn = 256; ea.n_part = d / 128; }  // the fused kernel's tiles are 256 wide: every producer must match
+    if (lv.share > 1 && tc_use_pair(M)) {  // tile width for half of the CTA pairs; every producer of ssq must match
+      ea.force_bn = tc_resid_bn(d, M, lv.share);
+      ea.n_part = 2 * ((d + ea.force_bn - 1) / ea.force_bn);
+    }
+    // a1: h0 = W2 swish(W1 [tau ; W_in x + b_in] + b1) + b2
+    mark(e, ROSA_KC_INPROJ, s);
+    launch_embed1(zbuf, x, e->wca, e->bca, e->tvec + ((size_t)k * batch_full + lv.p0) * d, dm, tb, k, M, s);
+    e->last_launches += 1;
+    ea.out_f32 = h; ea.ld_out = d; ea.bias = e->b_t2;
+    if ((err = gemm(e, ROSA_KC_GEMM_EMBED, EPI_BIAS_F32, zbuf, e->w_t2, M, d, d, ea, s)) != cudaSuccess) return err;
+    for (int l = 0; l < dm.layers; ++l) {
+      const LayerWeights& L = e->lw[l];
+      if (!fused_norm) {
+        mark(e, ROSA_KC_RMSNORM, s);
+        launch_rmsnorm(nrm, h, dm, tb, k, M, s);                               // a2
+        e->last_launches += 1;
+      }
+      ea.out16 = qkv; ea.ld_out = dm.qkv_n;
+      ea.rope_tab = e->rope_tab; ea.ids = tb.ids; ea.rlen = tb.rlen;
+      ea.rope_cols = dm.q_n + dm.nkv * dm.hd;
+      if ((err = gemm(e, ROSA_KC_GEMM_QKV, EPI_ROPE, nrm, L.wqkv, M, dm.qkv_n, d, ea, s)) != cudaSuccess) return err;  // a2+a3+a4
+      mark(e, ROSA_KC_ATTN, s);
+      if (e->attn_tc) {                                                              // a5
+        if ((err = launch_attn_tc(dm, tb, l, qkv, obuf, k, M, e->d_kv_maps, s)) != cudaSuccess) return err;
+      } else {
+        launch_attn_simple(dm, tb, l, qkv, obuf, k, e->cfg.max_prefix_len, s);
+      }
+      e->last_launches += 1;
+      if (use_fused) {                                                              // a6 -> a7 -> a8, one launch
+        FusedMeta fm{};
+        const int n_n[kFusedPhases] = {d / 256, 2 * dm.F / 256, d / 256};
+        const int n_kb[kFusedPhases] = {dm.q_n / 64, d / 64, dm.F / 64};
+        const int epi[kFusedPhases] = {EPI_RESID, EPI_GEGLU, EPI_RESID};
+        for (int p = 0; p < kFusedPhases; ++p) { fm.n_n[p] = n_n[p]; fm.n_kb[p] = n_kb[p]; fm.epi[p] = epi[p]; fm.ea[p] = ea; }
+        fm.ea[0].out_f32 = h; fm.ea[0].ld_out = d;
+        fm.ea[1].out16 = mact; fm.ea[1].ld_out = dm.F;
+        fm.ea[2].out_f32 = h; fm.ea[2].ld_out = d;
+        fm.sched = e->d_sched; fm.pairs_max = e->fused_pairs; fm.slots = e->fused_slots; fm.n_m_max = e->n_m_max;
+        fm.done = e->d_done + (size_t)(fused_idx & 1) * kFusedPhases * e->n_m_max;
+        fm.done_next = e->d_done + (size_t)((fused_idx + 1) & 1) * kFusedPhases * e->n_m_max;
+        fused_idx += 1;
+        const op16* As[kFusedPhases] = {obuf, nrm, mact};
+        const op16* Ws[kFusedPhases] = {L.wo, L.wgu, L.wdown};
+        mark(e, ROSA_KC_GEMM_FUSED, s);
+        if ((err = launch_fused_tc(As, Ws, fm, M, tb.m_active + k, dm.fp16, s)) != cudaSuccess) return err;
+        e->last_launches += 1;
+      } else {
+        ea.out_f32 = h; ea.ld_out = d;
+        if ((err = gemm(e, ROSA_KC_GEMM_O, EPI_RESID, obuf, L.wo, M, d, dm.q_n, ea, s)) != cudaSuccess) return err;    // a6
+        if (!fused_norm) {
+          mark(e, ROSA_KC_RMSNORM, s);
+          launch_rmsnorm(nrm, h, dm, tb, k, M, s);                               // a2
+          e->last_launches += 1;
+        }
+        ea.out16 = mact; ea.ld_out = dm.F;
+        if ((err = gemm(e, ROSA_KC_GEMM_GATEUP, EPI_GEGLU, nrm, L.wgu, M, 2 * dm.F, d, ea, s)) != cudaSuccess) return err;  // a2+a7
+        ea.out_f32 = h; ea.ld_out = d;
+        if ((err = gemm(e, ROSA_KC_GEMM_DOWN, EPI_RESID, mact, L.wdown, M, d, dm.F, ea, s)) != cudaSuccess) return err;   // a8
+      }
+    }
+    if (fused_norm) {                                                                 // a9 + a10
+      ea.bias = e->b_out; ea.x = x; ea.cp = cp; ea.dt = tb.dt; ea.src = tb.src; ea.A = dm.A; ea.k_iter = k;
+      if ((err = gemm(e, ROSA_KC_FINAL, EPI_FINAL, nrm, e->w_out16, M, 64, d, ea, s)) != cudaSuccess) return err;
+    } else {
+      mark(e, ROSA_KC_FINAL, s);
+      launch_final(x, cp, h, e->g_final, e->w_out, e->b_out, dm, tb, k, M, s);
+      e->last_launches += 1;
+    }
+  }
+  return cudaSuccess;
+}
+
 // Enqueue the whole call (steps a1..a11) on `s`.  Everything that changes from call to call is
 // read from the device tables, so the same sequence can be captured once per (batch, nmax).
-static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, cudaStream_t s) {
+// b0 > 0: robots [0, b0) and [b0, batch) run as two lanes, the second on e->lane_stream between a
+// fork and a join event (two branches when `s` is being captured).
+static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, int b0, cudaStream_t s) {
   const Dims& dm = e->dm;
   if (dm.ada) return enqueue_call_ada(e, batch, nmax, s);
   const Tables tb = make_tables(e, batch);
   const CallPtrs* cp = (const CallPtrs*)(e->d_call + e->off_ptrs);
-  const int M = batch * dm.H, d = dm.d;
+  const int d = dm.d;
   cudaError_t err;
   e->last_launches = 0;
   mark(e, ROSA_KC_GATHER_SCATTER, s);
@@ -572,80 +719,19 @@ static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, cudaStream_
     launch_timevec(e->tvec, e->w_t1, e->b_t1, dm, tb, nmax, s);
     e->last_launches += 2;
   }
-  const bool fused_norm = e->family == 1;  // RMSNorm fused into the GEMM epilogues (tcgen05 family)
-  const bool use_fused = e->fused_ok && tc_use_pair(M);
-  int fused_idx = 0;
-  for (int k = 0; k < nmax; ++k) {
-    EpiArgs ea{};
-    ea.m_active = tb.m_active + k;
-    ea.H = dm.H; ea.hd = dm.hd; ea.gu_blk = dm.gu_blk; ea.in_fp16 = dm.fp16; ea.out_fp16 = dm.fp16;
-    ea.inv_d = 1.f / (float)d; ea.eps = dm.eps; ea.n_part = tc_ssq_parts(d, M);
-    if (fused_norm) { ea.h16 = e->nrm; ea.ssq_out = e->ssq; ea.ssq_in = e->ssq; }
-    if (use_fused) { ea.force_bn = 256; ea.n_part = d / 128; }  // the fused kernel's tiles are 256 wide: every producer must match
-    // a1: h0 = W2 swish(W1 [tau ; W_in x + b_in] + b1) + b2
-    mark(e, ROSA_KC_INPROJ, s);
-    launch_embed1(e->zbuf, e->x, e->wca, e->bca, e->tvec + (size_t)k * batch * d, dm, tb, k, M, s);
-    e->last_launches += 1;
-    ea.out_f32 = e->h; ea.ld_out = d; ea.bias = e->b_t2;
-    if ((err = gemm(e, ROSA_KC_GEMM_EMBED, EPI_BIAS_F32, e->zbuf, e->w_t2, M, d, d, ea, s)) != cudaSuccess) return err;
-    for (int l = 0; l < dm.layers; ++l) {
-      const LayerWeights& L = e->lw[l];
-      if (!fused_norm) {
-        mark(e, ROSA_KC_RMSNORM, s);
-        launch_rmsnorm(e->nrm, e->h, dm, tb, k, M, s);                               // a2
-        e->last_launches += 1;
-      }
-      ea.out16 = e->qkv; ea.ld_out = dm.qkv_n;
-      ea.rope_tab = e->rope_tab; ea.ids = tb.ids; ea.rlen = tb.rlen;
-      ea.rope_cols = dm.q_n + dm.nkv * dm.hd;
-      if ((err = gemm(e, ROSA_KC_GEMM_QKV, EPI_ROPE, e->nrm, L.wqkv, M, dm.qkv_n, d, ea, s)) != cudaSuccess) return err;  // a2+a3+a4
-      mark(e, ROSA_KC_ATTN, s);
-      if (e->attn_tc) {                                                              // a5
-        if ((err = launch_attn_tc(dm, tb, l, e->qkv, e->obuf, k, M, e->d_kv_maps, s)) != cudaSuccess) return err;
-      } else {
-        launch_attn_simple(dm, tb, l, e->qkv, e->obuf, k, e->cfg.max_prefix_len, s);
-      }
-      e->last_launches += 1;
-      if (use_fused) {                                                              // a6 -> a7 -> a8, one launch
-        FusedMeta fm{};
-        const int n_n[kFusedPhases] = {d / 256, 2 * dm.F / 256, d / 256};
-        const int n_kb[kFusedPhases] = {dm.q_n / 64, d / 64, dm.F / 64};
-        const int epi[kFusedPhases] = {EPI_RESID, EPI_GEGLU, EPI_RESID};
-        for (int p = 0; p < kFusedPhases; ++p) { fm.n_n[p] = n_n[p]; fm.n_kb[p] = n_kb[p]; fm.epi[p] = epi[p]; fm.ea[p] = ea; }
-        fm.ea[0].out_f32 = e->h; fm.ea[0].ld_out = d;
-        fm.ea[1].out16 = e->mact; fm.ea[1].ld_out = dm.F;
-        fm.ea[2].out_f32 = e->h; fm.ea[2].ld_out = d;
-        fm.sched = e->d_sched; fm.pairs_max = e->fused_pairs; fm.slots = e->fused_slots; fm.n_m_max = e->n_m_max;
-        fm.done = e->d_done + (size_t)(fused_idx & 1) * kFusedPhases * e->n_m_max;
-        fm.done_next = e->d_done + (size_t)((fused_idx + 1) & 1) * kFusedPhases * e->n_m_max;
-        fused_idx += 1;
-        const op16* As[kFusedPhases] = {e->obuf, e->nrm, e->mact};
-        const op16* Ws[kFusedPhases] = {L.wo, L.wgu, L.wdown};
-        mark(e, ROSA_KC_GEMM_FUSED, s);
-        if ((err = launch_fused_tc(As, Ws, fm, M, tb.m_active + k, dm.fp16, s)) != cudaSuccess) return err;
-        e->last_launches += 1;
-      } else {
-        ea.out_f32 = e->h; ea.ld_out = d;
-        if ((err = gemm(e, ROSA_KC_GEMM_O, EPI_RESID, e->obuf, L.wo, M, d, dm.q_n, ea, s)) != cudaSuccess) return err;    // a6
-        if (!fused_norm) {
-          mark(e, ROSA_KC_RMSNORM, s);
-          launch_rmsnorm(e->nrm, e->h, dm, tb, k, M, s);                               // a2
-          e->last_launches += 1;
-        }
-        ea.out16 = e->mact; ea.ld_out = dm.F;
-        if ((err = gemm(e, ROSA_KC_GEMM_GATEUP, EPI_GEGLU, e->nrm, L.wgu, M, 2 * dm.F, d, ea, s)) != cudaSuccess) return err;  // a2+a7
-        ea.out_f32 = e->h; ea.ld_out = d;
-        if ((err = gemm(e, ROSA_KC_GEMM_DOWN, EPI_RESID, e->mact, L.wdown, M, d, dm.F, ea, s)) != cudaSuccess) return err;   // a8
-      }
-    }
-    if (fused_norm) {                                                                 // a9 + a10
-      ea.bias = e->b_out; ea.x = e->x; ea.cp = cp; ea.dt = tb.dt; ea.src = tb.src; ea.A = dm.A; ea.k_iter = k;
-      if ((err = gemm(e, ROSA_KC_FINAL, EPI_FINAL, e->nrm, e->w_out16, M, 64, d, ea, s)) != cudaSuccess) return err;
-    } else {
-      mark(e, ROSA_KC_FINAL, s);
-      launch_final(e->x, cp, e->h, e->g_final, e->w_out, e->b_out, dm, tb, k, M, s);
-      e->last_launches += 1;
-    }
+  if (b0 > 0) {
+    const size_t row1 = ((size_t)b0 * dm.H + e->lane_row_align - 1) / e->lane_row_align * e->lane_row_align;
+    const LaneView l0{make_tables(e, b0, 0, 0), 0, 0, 2};
+    const LaneView l1{make_tables(e, batch - b0, b0, 1), b0, row1, 2};
+    if ((err = cudaEventRecord(e->ev_fork, s)) != cudaSuccess) return err;
+    if ((err = cudaStreamWaitEvent(e->lane_stream, e->ev_fork, 0)) != cudaSuccess) return err;
+    if ((err = enqueue_steps(e, l0, batch, nmax, s)) != cudaSuccess) return err;
+    if ((err = enqueue_steps(e, l1, batch, nmax, e->lane_stream)) != cudaSuccess) return err;
+    if ((err = cudaEventRecord(e->ev_join, e->lane_stream)) != cudaSuccess) return err;
+    if ((err = cudaStreamWaitEvent(s, e->ev_join, 0)) != cudaSuccess) return err;
+  } else {
+    const LaneView l0{tb, 0, 0, 1};
+    if ((err = enqueue_steps(e, l0, batch, nmax, s)) != cudaSuccess) return err;
   }
   mark(e, ROSA_KC_GATHER_SCATTER, s);
   launch_scatter_x(cp, e->x, tb, dm.H * dm.A, s);
@@ -676,6 +762,18 @@ static rosa_status_t denoise_impl(rosa_expert* e, int batch, const int32_t* ids,
   std::vector<int> order(batch);
   std::iota(order.begin(), order.end(), 0);
   std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return n_steps[a] > n_steps[b]; });
+  // two lanes: positions [0, b0) and [b0, batch); the sorted robots are dealt to the lanes in proportion
+  // (each lane keeps the descending order, and both lose their robots at about the same iterations)
+  const int b0 = lane_split(e, batch);
+  if (b0 > 0) {
+    std::vector<int> l0, l1;
+    for (int q = 0; q < batch; ++q) {
+      const bool to0 = (long)(q + 1) * b0 / batch > (long)q * b0 / batch;
+      (to0 ? l0 : l1).push_back(order[q]);
+    }
+    std::copy(l0.begin(), l0.end(), order.begin());
+    std::copy(l1.begin(), l1.end(), order.begin() + b0);
+  }
   const int slot = e->stage_next;
   e->stage_next = (slot + 1) % kStageRing;
   CK(cudaEventSynchronize(e->stage_ev[slot]));  // the copy that last used this slot has completed
@@ -690,15 +788,20 @@ static rosa_status_t denoise_impl(rosa_expert* e, int batch, const int32_t* ids,
     h_dt[p] = dt ? dt[i] : -h_t0[p] / (float)n_steps[i];
     h_ns[p] = n_steps[i];
   }
-  for (int k = 0; k < e->cfg.max_steps; ++k) {
-    int act = 0;
-    for (int p = 0; p < batch; ++p) act += h_ns[p] > k;
-    h_ma[k] = act * dm.H;
-  }
-  {  // attention CTAs are issued longest prefix first: the second wave then pairs long with short (LPT)
-    int* h_ord = (int*)(hs + e->off_order);
-    std::iota(h_ord, h_ord + batch, 0);
-    std::stable_sort(h_ord, h_ord + batch, [&](int a, int b) { return e->h_rlen[h_ids[a]] > e->h_rlen[h_ids[b]]; });
+  const int lane_p0[3] = {0, b0 > 0 ? b0 : batch, batch};
+  for (int lane = 0; lane < 2; ++lane) {
+    // active token rows of iteration k per lane (one lane: the whole batch in list 0)
+    for (int k = 0; k < e->cfg.max_steps; ++k) {
+      int act = 0;
+      for (int p = lane_p0[lane]; p < lane_p0[lane + 1]; ++p) act += h_ns[p] > k;
+      h_ma[lane * e->cfg.max_steps + k] = act * dm.H;
+    }
+    // attention CTAs are issued longest prefix first: the second wave then pairs long with short (LPT);
+    // positions are counted within the lane
+    int* h_ord = (int*)(hs + e->off_order) + lane_p0[lane];
+    const int nb = lane_p0[lane + 1] - lane_p0[lane], p0 = lane_p0[lane];
+    std::iota(h_ord, h_ord + nb, 0);
+    std::stable_sort(h_ord, h_ord + nb, [&](int a, int b) { return e->h_rlen[h_ids[p0 + a]] > e->h_rlen[h_ids[p0 + b]]; });
   }
   CallPtrs* h_cp = (CallPtrs*)(hs + e->off_ptrs);
   h_cp->noise = noise; h_cp->out = out; h_cp->vel = out_vel; h_cp->batch_ext = batch;
@@ -706,7 +809,7 @@ static rosa_status_t denoise_impl(rosa_expert* e, int batch, const int32_t* ids,
   CK(cudaEventRecord(e->stage_ev[slot], stream));
   if (out_vel) CK(cudaMemsetAsync(out_vel, 0, (size_t)nmax * batch * dm.H * dm.A * 4, stream));
   if (!e->use_graph || e->prof_on) {
-    CK(enqueue_call(e, batch, nmax, stream));
+    CK(enqueue_call(e, batch, nmax, b0, stream));
     return ROSA_OK;
   }
   const GraphKey key{batch, nmax, 0};
@@ -714,7 +817,7 @@ static rosa_status_t denoise_impl(rosa_expert* e, int batch, const int32_t* ids,
   if (it == e->graphs.end()) {
     cudaGraph_t g = nullptr;
     CK(cudaStreamBeginCapture(e->cap_stream, cudaStreamCaptureModeThreadLocal));
-    cudaError_t err = enqueue_call(e, batch, nmax, e->cap_stream);
+    cudaError_t err = enqueue_call(e, batch, nmax, b0, e->cap_stream);
     cudaError_t err2 = cudaStreamEndCapture(e->cap_stream, &g);
     if (err != cudaSuccess || err2 != cudaSuccess) {
       if (g) cudaGraphDestroy(g);

@@ -345,6 +345,26 @@ def test_fused_dependent_gemm_kernel_opt_in(monkeypatch):
         assert n_launch == 3 + 2 * (2 + 2 * 3 + 1) + 1            # gather, tau, time GEMM; per step 2 + 3 per layer (not 5) + 1; scatter
 
 
+def test_two_lane_opt_in(monkeypatch):
+    """ROSA_LANES=2: a batch cut into two sub-batches whose kernel chains run as two branches of the captured graph
+    (measured slower at B=64 and left opt-in).  Mixed step counts, so each lane has its own shrinking
+    active set; the split 5 + 7 robots puts lane 1 on its own 256-row block of every workspace."""
+    case = edge_case([70, 150, 33, 90, 64, 200, 10, 129, 300, 17, 64, 65], n_steps=3)
+    case.n_steps[:] = np.array([3, 1, 2, 3, 1, 1, 2, 3, 3, 2, 1, 3], dtype=case.n_steps.dtype)
+    case.dt[:] = (-case.t_start / case.n_steps).astype(case.dt.dtype)
+    want_x, want_v = O.denoise_case(case, return_velocity=True)
+    monkeypatch.setenv("ROSA_LANES", "2")
+    monkeypatch.setenv("ROSA_LANE_MIN_BATCH", "4")
+    lc = LoadedCase(case)
+    got_x, got_v = lc.run(want_velocity=True)
+    again, _ = lc.run()
+    n_launch = rosa.rosa_last_launch_count(lc.expert)
+    lc.close()
+    compare("two-lane", got_x, got_v, want_x, want_v)
+    assert np.array_equal(got_x, again)                           # deterministic
+    assert n_launch == 3 + 2 * 3 * (2 + 5 * MINI.layers + 1) + 1  # both lanes run every kernel of the three steps
+
+
 # ------------------------------------------------------------------ adaptive-norm variant (reading R25, SURVEY 8(f) item 4)
 def test_adarms_variant_pi0_shapes():
     """pi0-scale widths (d 1024, F 4096, 8q/1kv x 256), 3 layers, ragged prefixes: CTA-pair GEMMs (M = 300)."""
