@@ -76,6 +76,12 @@ __device__ __forceinline__ float row_rscale(const EpiArgs& ea, int row) {
   return rsqrtf(ss * ea.inv_d + ea.eps);
 }
 
+// Clock traces (ROSA_DBG=64): [class = 2 * EPI + (K > 2048)][CTA 0 | CTA 64][slot], the last launch of each class wins;
+// class 15 holds the inside of the last residual epilogue of CTA 64, warp 2 (chunk c: slots 5 c .. 5 c + 4).
+__device__ long long g_gemm_trace[16 * 2 * 16];
+#define EPI_TRACE(slot) do { if ((ea.dbg & 64) && blockIdx.x == 64 && lane == 0 && half == 0 && ((r0 >> 5) & 3) == 2 && (slot) < 32) \
+  g_gemm_trace[15 * 32 + (slot)] = clock64(); } while (0)
+
 // What an epilogue warp fetches BEFORE it waits for its accumulator, so that the latency sits under the main
 // loop instead of after it (clock trace, profiles/r1_gemm_epilogue_trace.md: the residual epilogue's h loads were
 // four exposed round trips, 17k cycles of a 39k-cycle O-projection launch; the RoPE epilogue began with three
@@ -169,21 +175,24 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, EpiPre& pre, fl
       // the residual rows are requested first: their latency (L2, after epilogue_prefetch) overlaps the
       // accumulator load and the transpose
       float4 hres[8];
+      if constexpr (EPI == EPI_RESID) EPI_TRACE(5 * (c - c_beg));
       if constexpr (EPI == EPI_RESID) {
 #pragma unroll
         for (int i = 0; i < 8; ++i)
-          hres[i] = colok && r0 + i * 4 + lr < m_lim ? *reinterpret_cast<const float4*>(gp + i * step)
+          hres[i] = colok && r0 + i * 4 + lr < m_lim && !(ea.epi_dbg & 1) ? *reinterpret_cast<const float4*>(gp + i * step)
                                                       : make_float4(0.f, 0.f, 0.f, 0.f);
       }
       {
         float v[32];
         ld_acc32(t_acc + c * 32, v);
+        if constexpr (EPI == EPI_RESID) EPI_TRACE(5 * (c - c_beg) + 1);
         if (c == c_end - 1) release();
         to_scratch(v);
       }
       __syncwarp();
       float4 o[8];
       from_scratch(o);
+      if constexpr (EPI == EPI_RESID) EPI_TRACE(5 * (c - c_beg) + 2);
       if constexpr (EPI == EPI_RESID) {
         if (ea.gate) {  // adaptive-norm variant (R25): per-robot gate on the sublayer output, h += gate * acc.
           // Addresses are clamped into range instead of predicated so the 8 loads issue back to back.
@@ -199,14 +208,15 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, EpiPre& pre, fl
         }
 #pragma unroll
         for (int i = 0; i < 8; ++i) { o[i].x += hres[i].x; o[i].y += hres[i].y; o[i].z += hres[i].z; o[i].w += hres[i].w; }
+        if (o[0].x != 12345.678f) EPI_TRACE(5 * (c - c_beg) + 3);
       }
 #pragma unroll
       for (int i = 0; i < 8; ++i) {
         o[i].x += add.x; o[i].y += add.y; o[i].z += add.z; o[i].w += add.w;
         if (colok && r0 + i * 4 + lr < m_lim) {
-          *reinterpret_cast<float4*>(gp + i * step) = o[i];
+          if (!(ea.epi_dbg & 2)) *reinterpret_cast<float4*>(gp + i * step) = o[i];
           if constexpr (EPI != EPI_STORE_F32) {
-            if (want_h16)
+            if (want_h16 && !(ea.epi_dbg & 4))
               *reinterpret_cast<uint2*>(hp + i * step) =
                   make_uint2(pack_op2(o[i].x, o[i].y, ea.out_fp16), pack_op2(o[i].z, o[i].w, ea.out_fp16));
             rowss[i] += o[i].x * o[i].x + o[i].y * o[i].y + o[i].z * o[i].z + o[i].w * o[i].w;
@@ -214,6 +224,7 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, EpiPre& pre, fl
         }
       }
       __syncwarp();
+      if constexpr (EPI == EPI_RESID) EPI_TRACE(5 * (c - c_beg) + 4);
     }
     if constexpr (EPI != EPI_STORE_F32) {
       if (ea.ssq_out) {
@@ -495,8 +506,6 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
 }
 
 // measurement aid (ROSA_DBG bit 6): clock64 at the phases of CTA 0 of the last pair-kernel launch
-// [class = 2 * EPI + (K > 2048)][CTA 0 | CTA 64][slot]: the last launch of each class wins
-__device__ long long g_gemm_trace[16 * 2 * 16];
 #define GT_TRACE(slot) do { if ((ea.dbg & 64) && (blockIdx.x == 0 || blockIdx.x == 64) && lane == 0) \
   g_gemm_trace[((2 * EPI + (K > 2048)) * 2 + (blockIdx.x != 0)) * 16 + (slot)] = clock64(); } while (0)
 int tc_gemm_read_trace(long long* host, int n) {
