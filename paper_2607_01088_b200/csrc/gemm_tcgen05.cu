@@ -20,6 +20,8 @@
 #include <vector>
 #include <mutex>
 
+#include <type_traits>
+
 #include "device_math.cuh"
 #include "rosa_internal.h"
 #include "tc_common.cuh"
@@ -58,6 +60,16 @@ __device__ __forceinline__ void store_op16x32(uint16_t* dst, const float (&v)[32
     d[i] = u;
   }
 }
+template <bool FP16>
+__device__ __forceinline__ uint32_t pack_op2_t(float lo, float hi) {  // pack_op2 with the format fixed at compile time
+  if constexpr (FP16) {
+    __half2 v = __floats2half2_rn(lo, hi);
+    return *reinterpret_cast<uint32_t*>(&v);
+  } else {
+    __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+    return *reinterpret_cast<uint32_t*>(&v);
+  }
+}
 __device__ __forceinline__ void ld_acc32(uint32_t taddr, float (&v)[32]) {
   uint32_t r[32];
   tmem_ld32(taddr, r);
@@ -75,12 +87,6 @@ __device__ __forceinline__ float row_rscale(const EpiArgs& ea, int row) {
   for (int i = 0; i < ea.n_part; ++i) ss += ea.ssq_in[(size_t)row * ea.n_part + i];
   return rsqrtf(ss * ea.inv_d + ea.eps);
 }
-
-// Clock traces (ROSA_DBG=64): [class = 2 * EPI + (K > 2048)][CTA 0 | CTA 64][slot], the last launch of each class wins;
-// class 15 holds the inside of the last residual epilogue of CTA 64, warp 2 (chunk c: slots 5 c .. 5 c + 4).
-__device__ long long g_gemm_trace[16 * 2 * 16];
-#define EPI_TRACE(slot) do { if ((ea.dbg & 64) && blockIdx.x == 64 && lane == 0 && half == 0 && ((r0 >> 5) & 3) == 2 && (slot) < 32) \
-  g_gemm_trace[15 * 32 + (slot)] = clock64(); } while (0)
 
 // What an epilogue warp fetches BEFORE it waits for its accumulator, so that the latency sits under the main
 // loop instead of after it (clock trace, profiles/r1_gemm_epilogue_trace.md: the residual epilogue's h loads were
@@ -163,6 +169,54 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, EpiPre& pre, fl
 #pragma unroll
     for (int i = 0; i < 8; ++i) rowss[i] = 0.f;
     const bool want_h16 = EPI != EPI_STORE_F32 && ea.h16 != nullptr;
+    // Fast path (every interior tile): no row or column masks, the 16-bit format fixed at compile time, row
+    // offsets kept in registers.  The clock trace showed this epilogue bound by instruction issue (about 600
+    // SASS instructions per 32 x 32 chunk, most of them 64-bit address arithmetic, mask predicates and the
+    // per-value format branch), not by memory.
+    const bool fast = EPI != EPI_STORE_F32 && BN % 32 == 0 && want_h16 && ea.ssq_out && !ea.gate && r0 + 32 <= m_lim && n0 + BN <= N;
+    if (fast) {
+      auto run = [&](auto fp16_tag) {
+        constexpr bool FP16 = decltype(fp16_tag)::value;
+        float* const gbase = ea.out_f32 + (size_t)r0 * ea.ld_out + n0 + lc;
+        uint16_t* const hbase = (uint16_t*)ea.h16 + (size_t)r0 * ea.ld_out + n0 + lc;
+        uint32_t off[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) off[i] = (uint32_t)(i * 4 + lr) * (uint32_t)ea.ld_out;
+#pragma unroll 1
+        for (int c = c_beg; c < c_end; ++c) {
+          float* const gc = gbase + c * 32;
+          uint16_t* const hc = hbase + c * 32;
+          float4 hres[8];
+          if constexpr (EPI == EPI_RESID) {  // requested first: the latency overlaps the accumulator load and the transpose
+#pragma unroll
+            for (int i = 0; i < 8; ++i) hres[i] = *reinterpret_cast<const float4*>(gc + off[i]);
+          } else {
+            const float4 b = *reinterpret_cast<const float4*>(ea.bias + n0 + c * 32 + lc);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) hres[i] = b;
+          }
+          {
+            float v[32];
+            ld_acc32(t_acc + c * 32, v);
+            if (c == c_end - 1) release();
+            to_scratch(v);
+          }
+          __syncwarp();
+          float4 o[8];
+          from_scratch(o);
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            o[i].x += hres[i].x; o[i].y += hres[i].y; o[i].z += hres[i].z; o[i].w += hres[i].w;
+            *reinterpret_cast<float4*>(gc + off[i]) = o[i];
+            *reinterpret_cast<uint2*>(hc + off[i]) = make_uint2(pack_op2_t<FP16>(o[i].x, o[i].y), pack_op2_t<FP16>(o[i].z, o[i].w));
+            rowss[i] += o[i].x * o[i].x + o[i].y * o[i].y + o[i].z * o[i].z + o[i].w * o[i].w;
+          }
+          __syncwarp();
+        }
+      };
+      if (ea.out_fp16) run(std::true_type{});
+      else run(std::false_type{});
+    } else
 #pragma unroll 1
     for (int c = c_beg; c < c_end; ++c) {
       const int col = n0 + c * 32 + lc;
@@ -175,24 +229,21 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, EpiPre& pre, fl
       // the residual rows are requested first: their latency (L2, after epilogue_prefetch) overlaps the
       // accumulator load and the transpose
       float4 hres[8];
-      if constexpr (EPI == EPI_RESID) EPI_TRACE(5 * (c - c_beg));
       if constexpr (EPI == EPI_RESID) {
 #pragma unroll
         for (int i = 0; i < 8; ++i)
-          hres[i] = colok && r0 + i * 4 + lr < m_lim && !(ea.epi_dbg & 1) ? *reinterpret_cast<const float4*>(gp + i * step)
+          hres[i] = colok && r0 + i * 4 + lr < m_lim ? *reinterpret_cast<const float4*>(gp + i * step)
                                                       : make_float4(0.f, 0.f, 0.f, 0.f);
       }
       {
         float v[32];
         ld_acc32(t_acc + c * 32, v);
-        if constexpr (EPI == EPI_RESID) EPI_TRACE(5 * (c - c_beg) + 1);
         if (c == c_end - 1) release();
         to_scratch(v);
       }
       __syncwarp();
       float4 o[8];
       from_scratch(o);
-      if constexpr (EPI == EPI_RESID) EPI_TRACE(5 * (c - c_beg) + 2);
       if constexpr (EPI == EPI_RESID) {
         if (ea.gate) {  // adaptive-norm variant (R25): per-robot gate on the sublayer output, h += gate * acc.
           // Addresses are clamped into range instead of predicated so the 8 loads issue back to back.
@@ -208,15 +259,14 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, EpiPre& pre, fl
         }
 #pragma unroll
         for (int i = 0; i < 8; ++i) { o[i].x += hres[i].x; o[i].y += hres[i].y; o[i].z += hres[i].z; o[i].w += hres[i].w; }
-        if (o[0].x != 12345.678f) EPI_TRACE(5 * (c - c_beg) + 3);
       }
 #pragma unroll
       for (int i = 0; i < 8; ++i) {
         o[i].x += add.x; o[i].y += add.y; o[i].z += add.z; o[i].w += add.w;
         if (colok && r0 + i * 4 + lr < m_lim) {
-          if (!(ea.epi_dbg & 2)) *reinterpret_cast<float4*>(gp + i * step) = o[i];
+          *reinterpret_cast<float4*>(gp + i * step) = o[i];
           if constexpr (EPI != EPI_STORE_F32) {
-            if (want_h16 && !(ea.epi_dbg & 4))
+            if (want_h16)
               *reinterpret_cast<uint2*>(hp + i * step) =
                   make_uint2(pack_op2(o[i].x, o[i].y, ea.out_fp16), pack_op2(o[i].z, o[i].w, ea.out_fp16));
             rowss[i] += o[i].x * o[i].x + o[i].y * o[i].y + o[i].z * o[i].z + o[i].w * o[i].w;
@@ -224,7 +274,6 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, EpiPre& pre, fl
         }
       }
       __syncwarp();
-      if constexpr (EPI == EPI_RESID) EPI_TRACE(5 * (c - c_beg) + 4);
     }
     if constexpr (EPI != EPI_STORE_F32) {
       if (ea.ssq_out) {
@@ -356,11 +405,16 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, EpiPre& pre, fl
       from_scratch(o);
       uint16_t* dst = outp + (size_t)(r0 + lr) * ea.ld_out + n0 / 2 + blk * 64 + hh * 32 + lc;
       const size_t step = (size_t)4 * ea.ld_out;
+      if (ea.out_fp16) {  // warp-uniform: one branch per chunk, not one per value
 #pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        if (r0 + i * 4 + lr < m_lim)
-          *reinterpret_cast<uint2*>(dst + i * step) =
-              make_uint2(pack_op2(o[i].x, o[i].y, ea.out_fp16), pack_op2(o[i].z, o[i].w, ea.out_fp16));
+        for (int i = 0; i < 8; ++i)
+          if (r0 + i * 4 + lr < m_lim)
+            *reinterpret_cast<uint2*>(dst + i * step) = make_uint2(pack_op2_t<true>(o[i].x, o[i].y), pack_op2_t<true>(o[i].z, o[i].w));
+      } else {
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+          if (r0 + i * 4 + lr < m_lim)
+            *reinterpret_cast<uint2*>(dst + i * step) = make_uint2(pack_op2_t<false>(o[i].x, o[i].y), pack_op2_t<false>(o[i].z, o[i].w));
       }
       __syncwarp();
     }
@@ -506,6 +560,8 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
 }
 
 // measurement aid (ROSA_DBG bit 6): clock64 at the phases of CTA 0 of the last pair-kernel launch
+// [class = 2 * EPI + (K > 2048)][CTA 0 | CTA 64][slot]: the last launch of each class wins
+__device__ long long g_gemm_trace[16 * 2 * 16];
 #define GT_TRACE(slot) do { if ((ea.dbg & 64) && (blockIdx.x == 0 || blockIdx.x == 64) && lane == 0) \
   g_gemm_trace[((2 * EPI + (K > 2048)) * 2 + (blockIdx.x != 0)) * 16 + (slot)] = clock64(); } while (0)
 int tc_gemm_read_trace(long long* host, int n) {

@@ -502,8 +502,6 @@ static cudaError_t gemm(rosa_expert* e, int cls, Epi epi, const op16* A, const o
     if (trace_bit) {
       EpiArgs at = a;
       at.dbg |= trace_bit;
-      static const int ed = getenv("ROSA_EPI_DBG") ? atoi(getenv("ROSA_EPI_DBG")) : 0;
-      at.epi_dbg = ed;
       return launch_gemm_tc(epi, A, W, M, N, K, at, s);
     }
     return launch_gemm_tc(epi, A, W, M, N, K, a, s);

@@ -94,7 +94,6 @@ struct EpiArgs {
   int force_bn;           // BIAS_F32 / RESID: N tile to use (0 = chosen from N and M)
   const float* gate;      // RESID, adaptive-norm variant: h += gate[row / H][col] * acc (null = 1); rows gate_ld floats apart
   int gate_ld;
-  int epi_dbg;
   int dbg;                // measurement aid (ROSA_DBG): bit 0 skip the epilogue body, bit 1 skip the MMAs
 };
 
