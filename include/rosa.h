@@ -173,10 +173,21 @@ rosa_status_t rosa_debug_gemm(int32_t family, int32_t M, int32_t N, int32_t K, c
  * clock64() at its pipeline events for two CTAs; this copies [2][16 roles][32 key blocks] int64 values
  * of the last launch to host_out and returns the count (0 if tracing is off). */
 int32_t rosa_debug_attn_trace(int64_t *host_out, int32_t n);
-/* Same for the CTA-pair GEMM (ROSA_DBG bit 6): up to 16 phase timestamps of CTA 0 of the last launch
- * (entry, prologue done, dependency wait done, first stage full, last stage full, accumulator ready,
- * epilogue done, block sync, cluster sync). */
+/* Same for the CTA-pair GEMM (ROSA_DBG bit 6): int64 [16 classes][2 CTAs][16 slots]; class = 2 * epilogue kind +
+ * (K > 2048), CTAs 0 and 64, the last launch of each class wins.  Slots: 0 entry, 1 prologue done, 2 dependency
+ * wait done, 10 first TMA issued, 3 first stage full, 13 ninth stage full, 9 / 4 last k-block of the first / last
+ * tile issued, 11-12 / 5-6 first / last tile's epilogue, 7 block sync, 8 cluster sync.  Read it with
+ * `python -m paper_2607_01088_b200.clock_trace`. */
 int32_t rosa_debug_gemm_trace(int64_t *host_out, int32_t n);
+
+/* Host logic of the opt-in two-lane split of a call (environment ROSA_LANES=2), exposed so that it
+ * can be tested without a device.  Robots are independent (one request per robot, batched on a GPU
+ * worker), so a batch may be cut into two sub-batches whose kernel chains run side by side.  Given the batch
+ * size (>= 2), the action horizon H and the host array n_steps[batch], writes the internal robot order to the host
+ * array order_out[batch] (indices into the caller's arrays: lane 0 first, each lane sorted by n_steps descending,
+ * stable) and returns the number of robots in lane 0 (chosen near batch / 2 so that the two lanes need the fewest
+ * 256-row tile blocks), or a negative rosa_status_t.  Touches no device and no expert. */
+int32_t rosa_debug_lane_plan(int32_t batch, int32_t horizon, const int32_t *n_steps, int32_t *order_out);
 
 const char *rosa_last_error(void); /* thread-local, never NULL */
 int32_t rosa_version(void);

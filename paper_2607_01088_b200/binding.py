@@ -21,7 +21,7 @@ ROSA_F32, ROSA_BF16 = 0, 1
 
 EXPORTS = ("rosa_expert_create", "rosa_expert_destroy", "rosa_prefix_kv_bind", "rosa_prefix_kv_unbind",
            "rosa_denoise_batch", "rosa_denoise_batch_ex", "rosa_denoise_batch_host",
-           "rosa_profile_batch", "rosa_kernel_class_name", "rosa_debug_attn_trace", "rosa_debug_gemm_trace",
+           "rosa_profile_batch", "rosa_kernel_class_name", "rosa_debug_attn_trace", "rosa_debug_gemm_trace", "rosa_debug_lane_plan",
            "rosa_last_launch_count", "rosa_kernel_family", "rosa_debug_gemm", "rosa_last_error",
            "rosa_version")
 ROSA_KC_COUNT = 12
@@ -83,10 +83,12 @@ def load():
     lib.rosa_debug_attn_trace.restype = i32
     lib.rosa_debug_gemm_trace.argtypes = [vp, i32]
     lib.rosa_debug_gemm_trace.restype = i32
+    lib.rosa_debug_lane_plan.argtypes = [i32, i32, vp, vp]
+    lib.rosa_debug_lane_plan.restype = i32
     lib.rosa_last_error.restype = C.c_char_p
     lib.rosa_version.restype = i32
     for n in EXPORTS:
-        if n not in ("rosa_last_error", "rosa_version", "rosa_kernel_class_name", "rosa_debug_attn_trace", "rosa_debug_gemm_trace"):
+        if n not in ("rosa_last_error", "rosa_version", "rosa_kernel_class_name", "rosa_debug_attn_trace", "rosa_debug_gemm_trace", "rosa_debug_lane_plan"):
             getattr(lib, n).restype = C.c_int
     _lib = lib
     return lib
@@ -253,6 +255,16 @@ def rosa_debug_gemm_trace() -> np.ndarray:
     buf = np.zeros((16, 2, 16), dtype=np.int64)  # [2 * EPI + (K > 2048)][CTA 0 | CTA 64][slot]
     load().rosa_debug_gemm_trace(_ptr(buf), buf.size)
     return buf
+
+
+def rosa_debug_lane_plan(n_steps, horizon: int):
+    """(robots in lane 0, internal order) of the opt-in two-lane split; host logic only, no device."""
+    ns = np.ascontiguousarray(n_steps, dtype=np.int32)
+    order = np.zeros(ns.shape[0], dtype=np.int32)
+    b0 = load().rosa_debug_lane_plan(int(ns.shape[0]), int(horizon), _ptr(ns), _ptr(order))
+    if b0 < 0:
+        raise RuntimeError(rosa_last_error())
+    return int(b0), order
 
 
 def rosa_last_error() -> str:

@@ -199,17 +199,36 @@ static Tables make_tables(const rosa_expert* e, int batch, int p0 = 0, int lane 
   return tb;
 }
 
-// Robots of lane 0 when a batch is cut in two (0 = one lane).  Near half, moved down as far as a quarter of the
-// batch if that saves a 256-row tile block: B = 64, H = 50 gives 30 + 34 robots = 6 + 7 row blocks, where
-// 32 + 32 would pad to 7 + 7.
-static int lane_split(const rosa_expert* e, int batch) {
-  if (e->lanes < 2 || batch < e->lane_min_batch || e->prof_on) return 0;
-  const int H = e->dm.H;
+// Robots of lane 0 when a batch is cut in two.  Near half, moved down as far as a quarter of the batch if that
+// saves a 256-row tile block: B = 64, H = 50 gives 30 + 34 robots = 6 + 7 row blocks, where 32 + 32 would pad to 7 + 7.
+static int lane_split_rows(int batch, int H) {
   auto blocks = [&](int b) { return (b * H + 255) / 256; };
   int best = batch / 2;
   for (int b0 = batch / 2; b0 >= batch / 2 - batch / 4 && b0 >= 1; --b0)
     if (blocks(b0) + blocks(batch - b0) < blocks(best) + blocks(batch - best)) best = b0;
   return best;
+}
+static int lane_split(const rosa_expert* e, int batch) {  // 0 = one lane
+  if (e->lanes < 2 || batch < e->lane_min_batch || batch < 2 || e->prof_on) return 0;
+  return lane_split_rows(batch, e->dm.H);
+}
+// Internal order of a call: n_steps descending (stable), so that the active set of iteration k is a row prefix.  With two
+// lanes (b0 > 0) the sorted robots are dealt to the lanes in proportion (each lane keeps the descending order and both lose
+// their robots at about the same iterations); lane 0 takes positions [0, b0), lane 1 [b0, batch).
+static std::vector<int> call_order(int batch, const int32_t* n_steps, int b0) {
+  std::vector<int> order(batch);
+  std::iota(order.begin(), order.end(), 0);
+  std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return n_steps[a] > n_steps[b]; });
+  if (b0 > 0) {
+    std::vector<int> l0, l1;
+    for (int q = 0; q < batch; ++q) {
+      const bool to0 = (long)(q + 1) * b0 / batch > (long)q * b0 / batch;
+      (to0 ? l0 : l1).push_back(order[q]);
+    }
+    std::copy(l0.begin(), l0.end(), order.begin());
+    std::copy(l1.begin(), l1.end(), order.begin() + b0);
+  }
+  return order;
 }
 
 static void destroy_impl(rosa_expert* e) {
@@ -758,22 +777,9 @@ static rosa_status_t denoise_impl(rosa_expert* e, int batch, const int32_t* ids,
     if (n_steps[i] > e->cfg.max_steps) { set_error("n_steps > max_steps"); return ROSA_ERR_CAPACITY; }
     nmax = std::max(nmax, (int)n_steps[i]);
   }
-  // internal order: n_steps descending (stable) -> the active set of iteration k is a row prefix
-  std::vector<int> order(batch);
-  std::iota(order.begin(), order.end(), 0);
-  std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return n_steps[a] > n_steps[b]; });
-  // two lanes: positions [0, b0) and [b0, batch); the sorted robots are dealt to the lanes in proportion
-  // (each lane keeps the descending order, and both lose their robots at about the same iterations)
+  // internal order: n_steps descending; two lanes: positions [0, b0) and [b0, batch) (call_order)
   const int b0 = lane_split(e, batch);
-  if (b0 > 0) {
-    std::vector<int> l0, l1;
-    for (int q = 0; q < batch; ++q) {
-      const bool to0 = (long)(q + 1) * b0 / batch > (long)q * b0 / batch;
-      (to0 ? l0 : l1).push_back(order[q]);
-    }
-    std::copy(l0.begin(), l0.end(), order.begin());
-    std::copy(l1.begin(), l1.end(), order.begin() + b0);
-  }
+  const std::vector<int> order = call_order(batch, n_steps, b0);
   const int slot = e->stage_next;
   e->stage_next = (slot + 1) % kStageRing;
   CK(cudaEventSynchronize(e->stage_ev[slot]));  // the copy that last used this slot has completed
@@ -1048,6 +1054,13 @@ rosa_status_t rosa_debug_gemm(int32_t family, int32_t M, int32_t N, int32_t K, c
   return ROSA_OK;
 }
 
+int32_t rosa_debug_lane_plan(int32_t batch, int32_t horizon, const int32_t* n_steps, int32_t* order_out) {
+  if (batch < 2 || horizon < 1 || !n_steps || !order_out) { set_error("bad argument"); return ROSA_ERR_INVALID_ARG; }
+  const int b0 = lane_split_rows(batch, horizon);
+  const std::vector<int> order = call_order(batch, n_steps, b0);
+  std::copy(order.begin(), order.end(), order_out);
+  return b0;
+}
 int32_t rosa_debug_attn_trace(int64_t* host_out, int32_t n) { return tc_attn_read_trace((long long*)host_out, n); }
 int32_t rosa_debug_gemm_trace(int64_t* host_out, int32_t n) { return tc_gemm_read_trace((long long*)host_out, n); }
 
