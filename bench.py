@@ -74,7 +74,6 @@ def class_flops(cfg, lens, n_euler):
         rs = float(ne.sum())                         # robot-steps
         del out["gemm_embed"]                        # h0 = W_in x + b_in only
         out["timevec"] = 2.0 * rs * (2 * d * d + (2 * Lyr + 1) * 3 * d * d)   # time MLP + all modulation vectors
-    out["gemm_fused_o_gateup_down"] = out["gemm_o_resid"] + out["gemm_gateup_geglu"] + out["gemm_down_resid"]
     return out
 
 
@@ -309,7 +308,7 @@ def run_ours(args, rank, world, local_rank):
             cls_ms[k] = cls_ms.get(k, 0.0) + ms / n_prof
             cls_n[k] = n
     flops = class_flops(cfg, case.prefix_lens, case.n_steps)
-    tot_flops = sum(v for k, v in flops.items() if k != "gemm_fused_o_gateup_down")
+    tot_flops = sum(flops.values())
     tot_bytes = call_bytes(cfg, case.prefix_lens, case.n_steps)
     classes = {}
     for k, ms in cls_ms.items():
@@ -398,7 +397,7 @@ def run_sweep(args):
         with torch.cuda.stream(stream):
             total_ms, per_call = measure(torch, rosa, fl.expert, ids, fl.noise, t0, dt, ns, out, stream, steps, 5)
         ms = total_ms / steps
-        fl_tot = sum(v for k, v in class_flops(cfg, [816] * B, ns).items() if k != "gemm_fused_o_gateup_down")
+        fl_tot = sum(class_flops(cfg, [816] * B, ns).values())
         by = call_bytes(cfg, [816] * B, ns)
         t_c, t_m = fl_tot / (peaks["bf16_tflops"] * 1e12) * 1e3, by / (peaks["hbm_gbs"] * 1e9) * 1e3
         row = {"B": B, "chunks_per_s": B / (ms * 1e-3), "ms_per_call": ms, "p50_ms": pct(per_call, 0.5),
@@ -417,56 +416,6 @@ def run_sweep(args):
         json.dump({"peaks": peaks, "rows": rows}, f, indent=1)
 
 
-def run_library_gemms(args):
-    """Context line, not the product path and not part of the metric: cuBLAS through torch.matmul (fp16 operands,
-    fp32 accumulate, plain fp16 output, no fused epilogue) on the four layer-GEMM shapes of the pi0-scale expert at
-    M = batch x H token rows, streamed in layer order over 18 layers of distinct weights (629 MB, larger than L2) like
-    the path does, event-timed between launches like `rosa_profile_batch`, so the numbers compare with `classes` of
-    the default line."""
-    import torch
-    dev = torch.device("cuda:0")
-    H, d, F, layers = 50, 1024, 4096, 18
-    M = args.batch * H
-    shapes = {"gemm_qkv_rope": (2560, d), "gemm_o_resid": (d, 2048), "gemm_gateup_geglu": (2 * F, d), "gemm_down_resid": (d, F)}
-    g = torch.Generator(device=dev)
-    g.manual_seed(0)
-    A = {k: torch.randn((M, K), generator=g, device=dev).half() for k, (N, K) in shapes.items()}
-    W = {k: [(0.02 * torch.randn((N, K), generator=g, device=dev)).half() for _ in range(layers)] for k, (N, K) in shapes.items()}
-    out = {k: torch.empty((M, N), dtype=torch.float16, device=dev) for k, (N, K) in shapes.items()}
-    n_ev = layers * len(shapes) + 1
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(n_ev)]
-    tot = {k: 0.0 for k in shapes}
-    passes = max(args.steps, 10)
-    clk = ClockSampler(0)
-    for it in range(args.warmup + passes):
-        if it == args.warmup:
-            torch.cuda.synchronize()
-            clk.start()
-        i = 0
-        ev[0].record()
-        for l in range(layers):
-            for k in shapes:
-                torch.matmul(A[k], W[k][l].t(), out=out[k])
-                i += 1
-                ev[i].record()
-        torch.cuda.synchronize()
-        if it >= args.warmup:
-            i = 0
-            for l in range(layers):
-                for k in shapes:
-                    tot[k] += ev[i].elapsed_time(ev[i + 1])
-                    i += 1
-    clocks = clk.stop()
-    res = {}
-    for k, (N, K) in shapes.items():
-        us = tot[k] / (passes * layers) * 1e3
-        res[k] = {"us_per_launch": round(us, 2), "tflops": round(2.0 * M * N * K / (us * 1e-6) / 1e12, 1), "N": N, "K": K}
-    print(json.dumps({"impl": "library-gemms", "what": "torch.matmul fp16 (cuBLAS), no epilogue; context only", "M": M,
-                      "layers_streamed": layers, "passes": passes, "shapes": res,
-                      "ms_per_euler_step_gemms_only": round(sum(v["us_per_launch"] for v in res.values()) * layers / 1e3, 3),
-                      "clocks": clocks}))
-
-
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -480,8 +429,6 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true")
     ap.add_argument("--sweep-max", type=int, default=512)
-    ap.add_argument("--library-gemms", action="store_true",
-                    help="context only: cuBLAS on the four layer-GEMM shapes at M = batch x 50 (not the product path)")
     args = ap.parse_args()
     if args.batch is None:
         args.batch = 64 if args.config == 2 else 256
@@ -492,8 +439,6 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         run_reference(args, rank, world)
-    elif args.library_gemms:
-        run_library_gemms(args)
     elif args.sweep:
         run_sweep(args)
     else:

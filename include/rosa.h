@@ -17,6 +17,8 @@
  * thrown across the ABI.  Arguments are validated before any launch.  There is no CPU
  * fallback: without a CUDA device every compute entry point returns ROSA_ERR_CUDA.
  * Pointers are marked [host] or [dev].  The library is not thread-safe per expert handle.
+ * Measurement and unit-test hooks (per-class timing, the GEMM unit test, host-side planners) are declared in
+ * rosa_debug.h; they are exported by the same library and are not needed to use it.
  */
 #ifndef ROSA_H_
 #define ROSA_H_
@@ -129,65 +131,6 @@ rosa_status_t rosa_denoise_batch_host(rosa_expert_t *e, int32_t batch, const int
                                       const float *noise_host, const float *t_start,
                                       const float *dt, const int32_t *n_steps,
                                       float *out_actions_host, void *stream);
-
-/* Introspection for the bench: number of kernel launches (graph nodes) the last denoise call
- * issued, and which kernel family runs (0 = simple CUDA-core, 1 = tcgen05). */
-rosa_status_t rosa_last_launch_count(rosa_expert_t *e, int64_t *n_kernels);
-rosa_status_t rosa_kernel_family(rosa_expert_t *e, int32_t *family);
-
-/* Kernel classes of the hot path, for rosa_profile_batch. */
-typedef enum {
-  ROSA_KC_GATHER_SCATTER = 0, /* x gather at call start / scatter at call end */
-  ROSA_KC_TIMEVEC = 1,        /* a1, time half of W_1 (hoisted, once per call) */
-  ROSA_KC_INPROJ = 2,         /* a1, W_in x + b_in */
-  ROSA_KC_GEMM_EMBED = 3,     /* a1, the two d x d GEMMs of the time MLP */
-  ROSA_KC_RMSNORM = 4,        /* a2 */
-  ROSA_KC_GEMM_QKV = 5,       /* a3 + a4 */
-  ROSA_KC_ATTN = 6,           /* a5 */
-  ROSA_KC_GEMM_O = 7,         /* a6 */
-  ROSA_KC_GEMM_GATEUP = 8,    /* a7 */
-  ROSA_KC_GEMM_DOWN = 9,      /* a8 */
-  ROSA_KC_FINAL = 10,         /* a9 + a10 */
-  ROSA_KC_GEMM_FUSED = 11,    /* a6 -> a7 -> a8 in one persistent kernel (M > 128) */
-  ROSA_KC_COUNT = 12
-} rosa_kernel_class_t;
-
-/* Measurement aid for bench.py (SURVEY 8(d) "evidence per kernel"): runs the same call as
- * rosa_denoise_batch_ex, NOT through the CUDA graph, with a CUDA event recorded on `stream`
- * between consecutive launches, synchronises, and returns per kernel class the summed device
- * time in milliseconds (ms_out [host] float[ROSA_KC_COUNT]) and the number of launches
- * (launches_out [host] int32[ROSA_KC_COUNT]).  Results are identical to the graphed call. */
-rosa_status_t rosa_profile_batch(rosa_expert_t *e, int32_t batch, const int32_t *robot_ids,
-                                 const float *noise, const float *t_start, const float *dt,
-                                 const int32_t *n_steps, float *out_actions, void *stream,
-                                 float *ms_out, int32_t *launches_out);
-const char *rosa_kernel_class_name(int32_t cls); /* "" if out of range */
-
-/* Kernel unit-test hook: C[M,N] (float32, [dev]) = A[M,K] * W[N,K]^T with bf16 [dev]
- * operands through the tcgen05/TMA GEMM (family 1) or the CUDA-core GEMM (family 0).
- * K % 64 == 0 and N % 64 == 0 required for family 1. */
-rosa_status_t rosa_debug_gemm(int32_t family, int32_t M, int32_t N, int32_t K, const void *A_bf16,
-                              const void *W_bf16, float *C, void *stream);
-
-/* Measurement aid: with the environment variable ROSA_DBG bit 4 set, the attention kernel records
- * clock64() at its pipeline events for two CTAs; this copies [2][16 roles][32 key blocks] int64 values
- * of the last launch to host_out and returns the count (0 if tracing is off). */
-int32_t rosa_debug_attn_trace(int64_t *host_out, int32_t n);
-/* Same for the CTA-pair GEMM (ROSA_DBG bit 6): int64 [16 classes][2 CTAs][16 slots]; class = 2 * epilogue kind +
- * (K > 2048), CTAs 0 and 64, the last launch of each class wins.  Slots: 0 entry, 1 prologue done, 2 dependency
- * wait done, 10 first TMA issued, 3 first stage full, 13 ninth stage full, 9 / 4 last k-block of the first / last
- * tile issued, 11-12 / 5-6 first / last tile's epilogue, 7 block sync, 8 cluster sync.  Read it with
- * `python -m paper_2607_01088_b200.clock_trace`. */
-int32_t rosa_debug_gemm_trace(int64_t *host_out, int32_t n);
-
-/* Host logic of the opt-in two-lane split of a call (environment ROSA_LANES=2), exposed so that it
- * can be tested without a device.  Robots are independent (one request per robot, batched on a GPU
- * worker), so a batch may be cut into two sub-batches whose kernel chains run side by side.  Given the batch
- * size (>= 2), the action horizon H and the host array n_steps[batch], writes the internal robot order to the host
- * array order_out[batch] (indices into the caller's arrays: lane 0 first, each lane sorted by n_steps descending,
- * stable) and returns the number of robots in lane 0 (chosen near batch / 2 so that the two lanes need the fewest
- * 256-row tile blocks), or a negative rosa_status_t.  Touches no device and no expert. */
-int32_t rosa_debug_lane_plan(int32_t batch, int32_t horizon, const int32_t *n_steps, int32_t *order_out);
 
 const char *rosa_last_error(void); /* thread-local, never NULL */
 int32_t rosa_version(void);

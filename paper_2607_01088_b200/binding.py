@@ -1,4 +1,4 @@
-"""ctypes binding of librosa.so — same names as include/rosa.h, argument marshalling only.
+"""ctypes binding of librosa.so — same names as include/rosa.h and include/rosa_debug.h, argument marshalling only.
 
 PyTorch is used by callers for device memory and streams; this module only reads
 ``tensor.data_ptr()``.  Every step of the path runs inside the library's CUDA kernels.
@@ -21,10 +21,12 @@ ROSA_F32, ROSA_BF16 = 0, 1
 
 EXPORTS = ("rosa_expert_create", "rosa_expert_destroy", "rosa_prefix_kv_bind", "rosa_prefix_kv_unbind",
            "rosa_denoise_batch", "rosa_denoise_batch_ex", "rosa_denoise_batch_host",
-           "rosa_profile_batch", "rosa_kernel_class_name", "rosa_debug_attn_trace", "rosa_debug_gemm_trace", "rosa_debug_lane_plan",
-           "rosa_last_launch_count", "rosa_kernel_family", "rosa_debug_gemm", "rosa_last_error",
-           "rosa_version")
-ROSA_KC_COUNT = 12
+           "rosa_last_error", "rosa_version")
+# include/rosa_debug.h: measurement and unit-test hooks
+DEBUG_EXPORTS = ("rosa_profile_batch", "rosa_kernel_class_name", "rosa_last_launch_count", "rosa_kernel_family",
+                 "rosa_debug_graph_captures", "rosa_debug_gemm", "rosa_debug_attn_plan")
+ROSA_KC_COUNT = 11
+EPI_STORE_F32, EPI_BIAS_F32, EPI_RESID = 0, 2, 4
 
 
 class RosaError(RuntimeError):
@@ -75,20 +77,17 @@ def load():
     lib.rosa_denoise_batch_host.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp]
     lib.rosa_last_launch_count.argtypes = [vp, C.POINTER(i64)]
     lib.rosa_kernel_family.argtypes = [vp, C.POINTER(i32)]
-    lib.rosa_debug_gemm.argtypes = [i32, i32, i32, i32, vp, vp, vp, vp]
+    lib.rosa_debug_graph_captures.argtypes = [vp, C.POINTER(i64)]
+    lib.rosa_debug_gemm.argtypes = [i32, i32, i32, i32, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
+    lib.rosa_debug_attn_plan.argtypes = [i32, i32, vp, i32, vp, vp, i32]
+    lib.rosa_debug_attn_plan.restype = i32
     lib.rosa_profile_batch.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.rosa_kernel_class_name.argtypes = [i32]
     lib.rosa_kernel_class_name.restype = C.c_char_p
-    lib.rosa_debug_attn_trace.argtypes = [vp, i32]
-    lib.rosa_debug_attn_trace.restype = i32
-    lib.rosa_debug_gemm_trace.argtypes = [vp, i32]
-    lib.rosa_debug_gemm_trace.restype = i32
-    lib.rosa_debug_lane_plan.argtypes = [i32, i32, vp, vp]
-    lib.rosa_debug_lane_plan.restype = i32
     lib.rosa_last_error.restype = C.c_char_p
     lib.rosa_version.restype = i32
-    for n in EXPORTS:
-        if n not in ("rosa_last_error", "rosa_version", "rosa_kernel_class_name", "rosa_debug_attn_trace", "rosa_debug_gemm_trace", "rosa_debug_lane_plan"):
+    for n in EXPORTS + DEBUG_EXPORTS:
+        if n not in ("rosa_last_error", "rosa_version", "rosa_kernel_class_name", "rosa_debug_attn_plan"):
             getattr(lib, n).restype = C.c_int
     _lib = lib
     return lib
@@ -241,30 +240,29 @@ def rosa_kernel_family(e: Expert) -> int:
     return n.value
 
 
-def rosa_debug_gemm(family: int, M: int, N: int, K: int, A_bf16, W_bf16, C_f32, stream=None):
-    _check(load().rosa_debug_gemm(family, M, N, K, _ptr(A_bf16), _ptr(W_bf16), _ptr(C_f32), _stream_handle(stream)))
+def rosa_debug_graph_captures(e: Expert) -> int:
+    n = C.c_int64()
+    _check(load().rosa_debug_graph_captures(e.handle, C.byref(n)))
+    return n.value
 
 
-def rosa_debug_attn_trace() -> np.ndarray:
-    buf = np.zeros((2, 16, 32), dtype=np.int64)
-    load().rosa_debug_attn_trace(_ptr(buf), buf.size)
-    return buf
+def rosa_debug_gemm(family: int, M: int, N: int, K: int, A16, W16, C_f32, *, epi: int = EPI_STORE_F32, pair: int = -1,
+                    bn: int = 0, fp16: int = 0, bias=None, h16=None, ssq=None, stream=None):
+    _check(load().rosa_debug_gemm(family, epi, pair, bn, fp16, M, N, K, _ptr(A16), _ptr(W16), _ptr(C_f32), _ptr(bias),
+                                  _ptr(h16), _ptr(ssq), _stream_handle(stream)))
 
 
-def rosa_debug_gemm_trace() -> np.ndarray:
-    buf = np.zeros((16, 2, 16), dtype=np.int64)  # [2 * EPI + (K > 2048)][CTA 0 | CTA 64][slot]
-    load().rosa_debug_gemm_trace(_ptr(buf), buf.size)
-    return buf
-
-
-def rosa_debug_lane_plan(n_steps, horizon: int):
-    """(robots in lane 0, internal order) of the opt-in two-lane split; host logic only, no device."""
-    ns = np.ascontiguousarray(n_steps, dtype=np.int32)
-    order = np.zeros(ns.shape[0], dtype=np.int32)
-    b0 = load().rosa_debug_lane_plan(int(ns.shape[0]), int(horizon), _ptr(ns), _ptr(order))
-    if b0 < 0:
-        raise RuntimeError(rosa_last_error())
-    return int(b0), order
+def rosa_debug_attn_plan(horizon: int, lens, n_cta: int):
+    """Host logic of the attention work split (no device): returns (offs [n_cta + 1], segs [n, 6] int32 with columns
+    robot, tile, kb0, kb1, n_part, part0)."""
+    ln = np.ascontiguousarray(lens, dtype=np.int32)
+    cap = int(ln.shape[0]) * ((int(horizon) + 15) // 16) + 4 * int(n_cta)
+    offs = np.zeros(n_cta + 1, dtype=np.int32)
+    segs = np.zeros((cap, 8), dtype=np.int32)
+    n = load().rosa_debug_attn_plan(int(horizon), int(ln.shape[0]), _ptr(ln), int(n_cta), _ptr(offs), _ptr(segs), cap)
+    if n < 0:
+        raise RosaError(n, rosa_last_error())
+    return offs, segs[:n, :6].copy()
 
 
 def rosa_last_error() -> str:

@@ -21,7 +21,8 @@ def sources():
 
 
 def _deps_mtime() -> float:
-    files = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(ROOT, "include", "rosa.h")]
+    files = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + \
+        [os.path.join(ROOT, "include", h) for h in ("rosa.h", "rosa_debug.h")]
     return max(os.path.getmtime(f) for f in files)
 
 
@@ -32,7 +33,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
     hdr_time = max(os.path.getmtime(os.path.join(CSRC, f)) for f in os.listdir(CSRC)
                    if f.endswith((".h", ".cuh")))
-    hdr_time = max(hdr_time, os.path.getmtime(os.path.join(ROOT, "include", "rosa.h")))
+    hdr_time = max([hdr_time] + [os.path.getmtime(os.path.join(ROOT, "include", h)) for h in ("rosa.h", "rosa_debug.h")])
 
     def compile_one(src: str) -> str:
         obj = os.path.join(OBJ, os.path.basename(src)[:-3] + ".o")

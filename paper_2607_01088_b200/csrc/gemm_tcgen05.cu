@@ -467,7 +467,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
   // for it (small batches: the K loop is bound by TMA round trips, and an L2 hit is a shorter trip than HBM;
   // the previous kernel leaves HBM mostly idle there).  Measured: B=1 14.04 -> 13.64 ms per call; in the pair
   // kernel it is neutral at B = 8..32 and costs 3% at B = 64, so only this kernel does it.
-  if (warp == 0 && !(ea.dbg & 128) && (int)blockIdx.x < n_tiles && elect_one()) {
+  if (warp == 0 && (int)blockIdx.x < n_tiles && elect_one()) {
     const int n0 = ((int)blockIdx.x / n_m) * BN;
     for (int kb = 0; kb < n_kb; ++kb) tma_prefetch_2d(&tmB, kb * BK, n0);
   }
@@ -510,12 +510,10 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         if (elect_one()) {
           const uint32_t a_addr = smem_base + s * Cfg::STAGE_BYTES;
           const uint32_t b_addr = a_addr + Cfg::A_BYTES;
-          if (!(ea.dbg & 2)) {
 #pragma unroll
-            for (int kk = 0; kk < BK / 16; ++kk) {
-              umma_bf16(d_tmem, make_sdesc_k128(a_addr + kk * 32), make_sdesc_k128(b_addr + kk * 32), idesc,
-                        (kb | kk) != 0);
-            }
+          for (int kk = 0; kk < BK / 16; ++kk) {
+            umma_bf16(d_tmem, make_sdesc_k128(a_addr + kk * 32), make_sdesc_k128(b_addr + kk * 32), idesc,
+                      (kb | kk) != 0);
           }
           umma_commit(empty_bar(s));
           if (kb == n_kb - 1) umma_commit(tfull_bar(acc));
@@ -544,10 +542,6 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         __syncwarp();
         if (lane == 0) mbar_arrive(tempty_bar(acc));
       };
-      if (ea.dbg & 1) {  // measurement aid: mainloop only
-        release();
-        continue;
-      }
       epilogue_tile<BN, EPI>(ea, pre, scr, t_acc, r0, n0, m_lim, N, lane, half, release);
     }
   }
@@ -559,16 +553,15 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
   }
 }
 
-// measurement aid (ROSA_DBG bit 6): clock64 at the phases of CTA 0 of the last pair-kernel launch
-// [class = 2 * EPI + (K > 2048)][CTA 0 | CTA 64][slot]: the last launch of each class wins
+// Measurement aid, compiled in only with -DROSA_TRACE: clock64 at the phases of CTAs 0 and 64 of the last pair-kernel
+// launch of each class [class = 2 * EPI + (K > 2048)][CTA 0 | CTA 64][slot].
+#ifdef ROSA_TRACE
 __device__ long long g_gemm_trace[16 * 2 * 16];
-#define GT_TRACE(slot) do { if ((ea.dbg & 64) && (blockIdx.x == 0 || blockIdx.x == 64) && lane == 0) \
+#define GT_TRACE(slot) do { if ((blockIdx.x == 0 || blockIdx.x == 64) && lane == 0) \
   g_gemm_trace[((2 * EPI + (K > 2048)) * 2 + (blockIdx.x != 0)) * 16 + (slot)] = clock64(); } while (0)
-int tc_gemm_read_trace(long long* host, int n) {
-  if (n > 16 * 2 * 16) n = 16 * 2 * 16;
-  cudaMemcpyFromSymbol(host, g_gemm_trace, n * sizeof(long long));
-  return n;
-}
+#else
+#define GT_TRACE(slot) do { } while (0)
+#endif
 
 // ------------------------------------------------------------------ CTA-pair variant (cta_group::2)
 // Pair tile 256 x BN: CTA r of the cluster holds A rows [m0 + 128 r, +128) and B rows
@@ -682,12 +675,10 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
           if (elect_one()) {
             const uint32_t a_addr = smem_base + s * Cfg::STAGE_BYTES;
             const uint32_t b_addr = a_addr + Cfg::A_BYTES;
-            if (!(ea.dbg & 2)) {
 #pragma unroll
-              for (int kk = 0; kk < BK / 16; ++kk) {
-                umma_bf16_cg2(d_tmem, make_sdesc_k128(a_addr + kk * 32), make_sdesc_k128(b_addr + kk * 32), idesc,
-                              (kb | kk) != 0);
-              }
+            for (int kk = 0; kk < BK / 16; ++kk) {
+              umma_bf16_cg2(d_tmem, make_sdesc_k128(a_addr + kk * 32), make_sdesc_k128(b_addr + kk * 32), idesc,
+                            (kb | kk) != 0);
             }
             umma_commit_cg2(empty_bar(s));
             if (kb == n_kb - 1) umma_commit_cg2(tfull_bar(acc));
@@ -717,10 +708,6 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
         __syncwarp();
         if (lane == 0) mbar_arrive_cluster(mapa_shared(tempty_bar(acc), 0));
       };
-      if (ea.dbg & 1) {
-        release();
-        continue;
-      }
       if (warp == 2) GT_TRACE(5);
       if (warp == 2 && it == 0) GT_TRACE(11);
       epilogue_tile<BN, EPI>(ea, pre, scr, t_acc, r0, n0, m_lim, N, lane, half, release);
@@ -737,274 +724,6 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
     tc_fence_after();
     tmem_dealloc_cg2(tmem_base, Cfg::TMEM_COLS);
   }
-}
-
-// ------------------------------------------------------------------ fused dependent GEMMs (a6 -> a7 -> a8)
-// One persistent CTA-pair kernel runs the O projection, the gate/up GEMM and the down projection of a
-// layer.  Work items are pair tiles (phase, m, n); an item of phase p may start once every tile of
-// phase p-1 in the same 256-row block m has finished (per-block completion counters in global memory).
-// Which pair runs which items, in which order, is a STATIC list schedule computed on the host for every
-// possible number of active row blocks (durations ~ k-blocks, priority m-major then phase), so long items of
-// early row blocks back-fill the tail of the previous phase and the single-round O / down GEMMs no longer
-// leave 30% of the SMs idle.  Executing a valid list schedule in start-time order cannot deadlock: the
-// unfinished item with the earliest scheduled start has all its dependencies finished and heads its pair's list.
-// Host: list scheduling of the items of `n_m` row blocks on `pairs` CTA pairs.
-void tc_fused_schedule(int n_m, const int* n_n, const int* n_kb, int pairs, int slots, uint16_t* out /*[pairs][slots]*/) {
-  // priority order of the items: mode 0 = row-block-major (m, phase, n): early row blocks finish all phases
-  // early and their long down tiles back-fill; mode 1 = phase-major with m fastest (ph, n, m): the order of the
-  // separate kernels (consecutive pairs share a weight tile)
-  static int mode = -1;
-  if (mode < 0) { const char* e = getenv("ROSA_FUSED_ORDER"); mode = e ? atoi(e) : 0; }
-  struct Item { int ph, m, n; };
-  std::vector<Item> items;
-  if (mode == 1) {
-    for (int p = 0; p < kFusedPhases; ++p)
-      for (int n = 0; n < n_n[p]; ++n)
-        for (int m = 0; m < n_m; ++m) items.push_back({p, m, n});
-  } else {
-    for (int m = 0; m < n_m; ++m)
-      for (int p = 0; p < kFusedPhases; ++p)
-        for (int n = 0; n < n_n[p]; ++n) items.push_back({p, m, n});
-  }
-  std::vector<char> taken(items.size(), 0);
-  std::vector<std::vector<uint16_t>> lists(pairs);
-  std::vector<double> free_at(pairs, 0.0);
-  std::vector<double> fin(kFusedPhases * n_m, 0.0);   // finish time of (phase, m) = max over its tiles
-  std::vector<int> left(kFusedPhases * n_m);          // tiles of (phase, m) not yet scheduled
-  for (int p = 0; p < kFusedPhases; ++p)
-    for (int m = 0; m < n_m; ++m) left[p * n_m + m] = n_n[p];
-  size_t first = 0, remaining = items.size();
-  while (remaining > 0) {
-    int pr = 0;
-    for (int q = 1; q < pairs; ++q) if (free_at[q] < free_at[pr]) pr = q;
-    double t = free_at[pr];
-    while (first < items.size() && taken[first]) ++first;
-    // first item in priority order that is released at time t; else the one released earliest
-    long pick = -1, soon = -1;
-    double soon_t = 1e300;
-    for (size_t i = first; i < items.size(); ++i) {
-      if (taken[i]) continue;
-      const Item& it = items[i];
-      if (it.ph > 0 && left[(it.ph - 1) * n_m + it.m] != 0) continue;  // dependency not even scheduled yet
-      const double rel = it.ph == 0 ? 0.0 : fin[(it.ph - 1) * n_m + it.m];
-      if (rel <= t) { pick = (long)i; break; }
-      if (rel < soon_t) { soon_t = rel; soon = (long)i; }
-    }
-    if (pick < 0) { pick = soon; t = soon_t; }
-    const Item& it = items[pick];
-    taken[pick] = 1;
-    const double end = t + n_kb[it.ph] + 2.0;
-    free_at[pr] = end;
-    fin[it.ph * n_m + it.m] = std::max(fin[it.ph * n_m + it.m], end);
-    left[it.ph * n_m + it.m] -= 1;
-    lists[pr].push_back((uint16_t)((it.ph << 13) | (it.m << 6) | it.n));
-    remaining -= 1;
-  }
-  for (int q = 0; q < pairs; ++q)
-    for (int sidx = 0; sidx < slots; ++sidx)
-      out[(size_t)q * slots + sidx] = sidx < (int)lists[q].size() ? lists[q][sidx] : (uint16_t)0xFFFF;
-}
-// largest list length of that schedule (to size `slots`)
-int tc_fused_max_slots(int n_m, const int* n_n, const int* n_kb, int pairs) {
-  std::vector<uint16_t> tmp((size_t)pairs * 4096, 0xFFFF);
-  tc_fused_schedule(n_m, n_n, n_kb, pairs, 4096, tmp.data());
-  int mx = 0;
-  for (int q = 0; q < pairs; ++q) {
-    int c = 0;
-    while (c < 4096 && tmp[(size_t)q * 4096 + c] != 0xFFFF) ++c;
-    mx = std::max(mx, c);
-  }
-  return mx;
-}
-
-__device__ __forceinline__ int ld_acquire_gpu(const int* p) {
-  int v;
-  asm volatile("ld.acquire.gpu.global.b32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-  return v;
-}
-// generic-proxy global writes of other SMs -> visible to this thread's TMA (async proxy) reads, and back
-__device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
-
-struct FusedMaps { CUtensorMap a[kFusedPhases], b[kFusedPhases]; };
-
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1)
-k_fused_tc2(const __grid_constant__ FusedMaps maps, const __grid_constant__ FusedMeta fm, int M, const int* __restrict__ m_active,
-            int in_fp16) {
-  constexpr int BN = 256;
-  using Cfg = Gemm2Cfg<BN>;
-  extern __shared__ uint8_t smem_raw[];
-  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t bar_base = smem_base + Cfg::STAGES * Cfg::STAGE_BYTES;
-  auto full_bar = [&](int s) { return bar_base + 8u * s; };
-  auto empty_bar = [&](int s) { return bar_base + 8u * (Cfg::STAGES + s); };
-  auto tfull_bar = [&](int a) { return bar_base + 8u * (2 * Cfg::STAGES + a); };
-  auto tempty_bar = [&](int a) { return bar_base + 8u * (2 * Cfg::STAGES + 2 + a); };
-  const uint32_t tmem_slot = bar_base + 8u * (2 * Cfg::STAGES + 4);
-  volatile uint32_t* tmem_slot_ptr =
-      reinterpret_cast<volatile uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
-
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const uint32_t rank = cluster_ctarank();
-  const int pair = blockIdx.x >> 1;
-  const int m_lim = min(M, *m_active);
-  const int n_m = (m_lim + 2 * BM - 1) / (2 * BM);
-  const uint16_t* my = fm.sched + ((size_t)n_m * fm.pairs_max + pair) * fm.slots;  // this pair's item list
-
-  if (warp == 0 && lane == 0) {
-    for (int p = 0; p < kFusedPhases; ++p) { prefetch_tensormap(&maps.a[p]); prefetch_tensormap(&maps.b[p]); }
-    for (int s = 0; s < Cfg::STAGES; ++s) { mbar_init(full_bar(s), 2); mbar_init(empty_bar(s), 1); }
-    for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), 2 * kEpiWarps); }
-    fence_barrier_init();
-  }
-  if (warp == 1) {
-    tmem_alloc_cg2(tmem_slot, Cfg::TMEM_COLS);
-    tmem_relinquish_cg2();
-  }
-  tc_fence_before();
-  __syncthreads();
-  cluster_sync_all();
-  tc_fence_after();
-  const uint32_t tmem_base = *tmem_slot_ptr;
-  pdl_wait();
-  pdl_trigger();
-  if (blockIdx.x == 0)  // the counters of the NEXT launch (other buffer; its last user finished a launch ago)
-    for (int i = threadIdx.x; i < kFusedPhases * fm.n_m_max; i += blockDim.x) fm.done_next[i] = 0;
-
-  auto decode = [&](int slot, int& ph, int& m, int& n) {
-    const uint16_t c = slot < fm.slots ? my[slot] : (uint16_t)0xFFFF;
-    if (c == 0xFFFF) return false;
-    ph = c >> 13; m = (c >> 6) & 127; n = c & 63;
-    return true;
-  };
-  // every epilogue warp of both CTAs arrives once per tile: a row block is complete at n_n * 2 * kEpiWarps
-  auto dep_target = [&](int ph) { return fm.n_n[ph] * 2 * kEpiWarps; };
-
-  if (warp == 0) {  // ---------------- TMA producer
-    int s = 0, ph, m, n;
-    uint32_t par = 0;
-    for (int slot = 0; decode(slot, ph, m, n); ++slot) {
-      if (ph > 0) {  // the A operand (and the residual) of this item come from the previous phase's tiles
-        if (lane == 0) {
-          const int* c = fm.done + (ph - 1) * fm.n_m_max + m;
-          const int want = dep_target(ph - 1);
-          for (uint32_t spin = 0; ld_acquire_gpu(c) < want; ++spin) {
-            __nanosleep(64);
-            if (spin > (1u << 24)) __trap();
-          }
-          fence_proxy_async_all();
-        }
-        __syncwarp();
-      }
-      const int m0 = m * (2 * BM) + (int)rank * BM, n0 = n * BN + (int)rank * (BN / 2);
-      const int n_kb = fm.n_kb[ph];
-      for (int kb = 0; kb < n_kb; ++kb) {
-        mbar_wait_idle(empty_bar(s), par ^ 1);
-        if (elect_one()) {
-          const uint32_t lfull = mapa_shared(full_bar(s), 0);
-          mbar_expect_tx_cluster(lfull, Cfg::STAGE_BYTES);
-          const uint32_t a_dst = smem_base + s * Cfg::STAGE_BYTES;
-          tma_load_2d_cg2(a_dst, &maps.a[ph], lfull, kb * BK, m0);
-          tma_load_2d_cg2(a_dst + Cfg::A_BYTES, &maps.b[ph], lfull, kb * BK, n0);
-        }
-        __syncwarp();
-        if (++s == Cfg::STAGES) { s = 0; par ^= 1; }
-      }
-    }
-  } else if (warp == 1) {
-    if (rank == 0) {  // ---------------- MMA issuer (leader CTA only)
-      const uint32_t idesc =
-          in_fp16 ? (make_idesc_bf16(2 * BM, BN) & ~((1u << 7) | (1u << 10))) : make_idesc_bf16(2 * BM, BN);
-      int s = 0, ph, m, n;
-      uint32_t par = 0;
-      for (int slot = 0; decode(slot, ph, m, n); ++slot) {
-        const int acc = slot & 1;
-        const uint32_t acc_ph = (slot >> 1) & 1;
-        mbar_wait(tempty_bar(acc), acc_ph ^ 1);
-        tc_fence_after();
-        const uint32_t d_tmem = tmem_base + acc * BN;
-        const int n_kb = fm.n_kb[ph];
-        for (int kb = 0; kb < n_kb; ++kb) {
-          mbar_wait(full_bar(s), par);
-          tc_fence_after();
-          if (elect_one()) {
-            const uint32_t a_addr = smem_base + s * Cfg::STAGE_BYTES;
-            const uint32_t b_addr = a_addr + Cfg::A_BYTES;
-#pragma unroll
-            for (int kk = 0; kk < BK / 16; ++kk)
-              umma_bf16_cg2(d_tmem, make_sdesc_k128(a_addr + kk * 32), make_sdesc_k128(b_addr + kk * 32), idesc, (kb | kk) != 0);
-            umma_commit_cg2(empty_bar(s));
-            if (kb == n_kb - 1) umma_commit_cg2(tfull_bar(acc));
-          }
-          __syncwarp();
-          if (++s == Cfg::STAGES) { s = 0; par ^= 1; }
-        }
-      }
-    }
-  } else {  // ---------------- epilogue warps 2..9
-    const int q = warp & 3, half = (warp - 2) >> 2;
-    float* scr = reinterpret_cast<float*>(smem_raw + (bar_base + 256u - smem_u32(smem_raw))) + (warp - 2) * kScrFloats;
-    int ph, m, n;
-    for (int slot = 0; decode(slot, ph, m, n); ++slot) {
-      const int acc = slot & 1;
-      const uint32_t acc_ph = (slot >> 1) & 1;
-      const int r0 = m * (2 * BM) + (int)rank * BM + q * 32, n0 = n * BN;
-      mbar_wait_idle(tfull_bar(acc), acc_ph);
-      tc_fence_after();
-      if (ph > 0) (void)ld_acquire_gpu(fm.done + (ph - 1) * fm.n_m_max + m);  // residual / partial sums of the previous phase
-      const uint32_t t_acc = tmem_base + ((uint32_t)(q * 32) << 16) + acc * BN;
-      auto release = [&] {
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive_cluster(mapa_shared(tempty_bar(acc), 0));
-      };
-      const int N = fm.n_n[ph] * BN;
-      EpiPre pre;  // after the acquire here: what it fetches is written by the previous phase of this kernel
-      if (fm.epi[ph] == EPI_RESID) {
-        epilogue_pre<BN, EPI_RESID>(pre, fm.ea[ph], r0, n0, m_lim, N, lane, half);
-        epilogue_tile<BN, EPI_RESID>(fm.ea[ph], pre, scr, t_acc, r0, n0, m_lim, N, lane, half, release);
-      } else if (fm.epi[ph] == EPI_GEGLU) {
-        epilogue_pre<BN, EPI_GEGLU>(pre, fm.ea[ph], r0, n0, m_lim, N, lane, half);
-        epilogue_tile<BN, EPI_GEGLU>(fm.ea[ph], pre, scr, t_acc, r0, n0, m_lim, N, lane, half, release);
-      } else {
-        epilogue_pre<BN, EPI_ROPE>(pre, fm.ea[ph], r0, n0, m_lim, N, lane, half);
-        epilogue_tile<BN, EPI_ROPE>(fm.ea[ph], pre, scr, t_acc, r0, n0, m_lim, N, lane, half, release);
-      }
-      if (ph + 1 < kFusedPhases) {  // publish: this warp's part of tile (ph, m, n) is in global memory
-        __threadfence();
-        fence_proxy_async_all();
-        __syncwarp();
-        if (lane == 0) atomicAdd(fm.done + ph * fm.n_m_max + m, 1);
-      }
-    }
-  }
-  tc_fence_before();
-  __syncthreads();
-  cluster_sync_all();
-  if (warp == 1) {
-    tc_fence_after();
-    tmem_dealloc_cg2(tmem_base, Cfg::TMEM_COLS);
-  }
-}
-
-cudaError_t launch_fused_tc(const op16* const* A, const op16* const* W, const FusedMeta& fm, int M, const int* m_active, int in_fp16,
-                            cudaStream_t s) {
-  using Cfg = Gemm2Cfg<256>;
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(k_fused_tc2, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
-  FusedMaps maps;
-  for (int p = 0; p < kFusedPhases; ++p) {
-    const uint64_t N = (uint64_t)fm.n_n[p] * 256, K = (uint64_t)fm.n_kb[p] * BK;
-    if (!make_tmap_2d(&maps.a[p], A[p], (uint64_t)M, K, BM, in_fp16) || !make_tmap_2d(&maps.b[p], W[p], N, K, 128, in_fp16))
-      return cudaErrorInvalidValue;
-  }
-  const int n_m = (M + 2 * BM - 1) / (2 * BM);
-  int pairs = fm.pairs_max;
-  (void)n_m;
-  return launch_k(k_fused_tc2, dim3(2 * pairs), dim3(kGemmThreads), Cfg::SMEM, s, maps, fm, M, m_active, in_fp16);
 }
 
 // ------------------------------------------------------------------ host side
@@ -1077,16 +796,14 @@ bool tc_use_pair(int M) { return use_pair(M); }
 // max(MMA time ~ 2 BN, operand feed ~ 288 + BN) cycles (the L2 -> shared-memory feed bounds narrow tiles;
 // measured: profiles/r1_gemm_tile_width.md).
 static const int kPairBn[] = {256, 224, 192, 160, 128, 96, 64};
-static int resid_bn(int N, int M, int share = 1) {  // share: lanes the CTA pairs are divided between
+static int resid_bn(int N, int M) {
   if (!use_pair(M)) {
     const int units = num_sms(), n_m = (M + BM - 1) / BM;
     for (int bn = 128; bn > 64; bn >>= 1)
       if (N % bn == 0 && n_m * (N / bn) * 2 >= units) return bn;
     return 64;
   }
-  static const int forced = getenv("ROSA_RESID_BN") ? atoi(getenv("ROSA_RESID_BN")) : 0;  // experiments only
-  if (forced) return forced;
-  const int pairs = num_sms() / 2 / share, n_m = (M + 2 * BM - 1) / (2 * BM);
+  const int pairs = num_sms() / 2, n_m = (M + 2 * BM - 1) / (2 * BM);
   int best = 256;
   long best_cost = -1;
   for (int bn : kPairBn) {
@@ -1103,13 +820,7 @@ int tc_ssq_parts(int N, int M) {
   const int bn = resid_bn(N, M);
   return 2 * ((N + bn - 1) / bn);
 }
-int tc_resid_bn(int N, int M, int share) { return resid_bn(N, M, share); }
-
-// ROSA_WPREFETCH=0 switches the pre-wait weight prefetch off (A/B measurements)
-static int wprefetch_off_bit() {
-  static const int bit = getenv("ROSA_WPREFETCH") && !strcmp(getenv("ROSA_WPREFETCH"), "0") ? 128 : 0;
-  return bit;
-}
+int tc_resid_bn(int N, int M) { return resid_bn(N, M); }
 
 template <int BN, int EPI>
 static cudaError_t launch_one(const op16* A, const op16* W, int M, int N, int K, const EpiArgs& a, cudaStream_t s) {
@@ -1126,9 +837,7 @@ static cudaError_t launch_one(const op16* A, const op16* W, int M, int N, int K,
     return cudaErrorInvalidValue;
   const int tiles = ((M + BM - 1) / BM) * (N / BN);
   const int grid = tiles < num_sms() ? tiles : num_sms();
-  EpiArgs ea = a;
-  ea.dbg |= wprefetch_off_bit();
-  return launch_k(k_gemm_tc<BN, EPI>, dim3(grid), dim3(kGemmThreads), Cfg::SMEM, s, tmA, tmB, M, N, K, ea);
+  return launch_k(k_gemm_tc<BN, EPI>, dim3(grid), dim3(kGemmThreads), Cfg::SMEM, s, tmA, tmB, M, N, K, a);
 }
 
 template <int BN, int EPI>
@@ -1151,9 +860,8 @@ static cudaError_t launch_two(const op16* A, const op16* W, int M, int N, int K,
 
 template <int EPI>
 static cudaError_t launch_by_n(const op16* A, const op16* W, int M, int N, int K, const EpiArgs& a, cudaStream_t s) {
-  const int forced = a.dbg >> 8;  // rosa_debug_gemm only: 1xx = single-CTA kernel, N tile xx0
-  const bool pair = forced ? forced / 1000 == 2 : use_pair(M);
-  const int bn = forced ? forced % 1000 : (a.force_bn ? a.force_bn : resid_bn(N, M));
+  const bool pair = a.force_pair ? a.force_pair == 2 : use_pair(M);
+  const int bn = a.force_bn ? a.force_bn : resid_bn(N, M);
   if (pair) {
     switch (bn) {
       case 256: return launch_two<256, EPI>(A, W, M, N, K, a, s);
@@ -1166,9 +874,11 @@ static cudaError_t launch_by_n(const op16* A, const op16* W, int M, int N, int K
       default: return cudaErrorNotSupported;
     }
   }
+  if (N % bn) return cudaErrorNotSupported;   // the single-CTA kernel has no masked column tile
   if (bn == 256) return launch_one<256, EPI>(A, W, M, N, K, a, s);
   if (bn == 128) return launch_one<128, EPI>(A, W, M, N, K, a, s);
-  return launch_one<64, EPI>(A, W, M, N, K, a, s);
+  if (bn == 64) return launch_one<64, EPI>(A, W, M, N, K, a, s);
+  return cudaErrorNotSupported;
 }
 
 cudaError_t launch_gemm_tc(Epi epi, const op16* A, const op16* W, int M, int N, int K, const EpiArgs& a,

@@ -8,13 +8,12 @@
 namespace rosa {
 
 // ------------------------------------------------------------------ x gather / scatter
-__global__ void k_gather_x(float* __restrict__ x, const CallPtrs* __restrict__ cp, Tables tb, int HA, int* __restrict__ zero,
-                           int n_zero) {
+// Grids are sized for the graph's batch bucket (tb.batch); robots at positions >= *tb.batch_dev do not exist.
+__global__ void k_gather_x(float* __restrict__ x, const CallPtrs* __restrict__ cp, Tables tb, int HA) {
   pdl_wait();
   pdl_trigger();
-  if (blockIdx.x == 0)  // dependency counters of the fused GEMM kernels start every call at zero
-    for (int i = threadIdx.x; i < n_zero; i += blockDim.x) zero[i] = 0;
   int p = blockIdx.x;
+  if (p >= *tb.batch_dev) return;
   const float* s = cp->noise + (size_t)tb.src[p] * HA;
   for (int i = threadIdx.x; i < HA; i += blockDim.x) x[(size_t)p * HA + i] = s[i];
 }
@@ -22,11 +21,12 @@ __global__ void k_scatter_x(const CallPtrs* __restrict__ cp, const float* __rest
   pdl_wait();
   pdl_trigger();
   int p = blockIdx.x;
+  if (p >= *tb.batch_dev) return;
   float* d = cp->out + (size_t)tb.src[p] * HA;
   for (int i = threadIdx.x; i < HA; i += blockDim.x) d[i] = x[(size_t)p * HA + i];
 }
-void launch_gather_x(float* x, const CallPtrs* cp, const Tables& tb, int HA, int* zero, int n_zero, cudaStream_t s) {
-  launch_k(k_gather_x, dim3(tb.batch), dim3(128), 0, s, x, cp, tb, HA, zero, n_zero);
+void launch_gather_x(float* x, const CallPtrs* cp, const Tables& tb, int HA, cudaStream_t s) {
+  launch_k(k_gather_x, dim3(tb.batch), dim3(128), 0, s, x, cp, tb, HA);
 }
 void launch_scatter_x(const CallPtrs* cp, const float* x, const Tables& tb, int HA, cudaStream_t s) {
   launch_k(k_scatter_x, dim3(tb.batch), dim3(128), 0, s, cp, x, tb, HA);
@@ -42,7 +42,7 @@ __global__ void k_timevec(float* __restrict__ tvec, const bf16* __restrict__ w_t
   pdl_wait();
   pdl_trigger();
   const int p = blockIdx.x, k = blockIdx.y, d = dm.d, half = d / 2;
-  if (k >= tb.nsteps[p]) return;
+  if (p >= *tb.batch_dev || k >= tb.nsteps[p]) return;
   const double t = (double)tb.t0[p] + (double)k * (double)tb.dt[p];
   for (int j = threadIdx.x; j < half; j += blockDim.x) {
     double frac = (double)j / (double)(half > 1 ? half - 1 : 1);
@@ -76,8 +76,12 @@ __global__ void k_tau16(op16* __restrict__ a16, Dims dm, Tables tb) {
   pdl_wait();
   pdl_trigger();
   const int p = blockIdx.x, k = blockIdx.y, d = dm.d, half = d / 2;
-  const double t = (double)tb.t0[p] + (double)k * (double)tb.dt[p];
   op16* row = a16 + ((size_t)k * tb.batch + p) * 2 * d;
+  if (p >= *tb.batch_dev) {  // bucket padding: a finite operand row (the GEMM reads every row of the bucket)
+    for (int j = threadIdx.x; j < 2 * d; j += blockDim.x) row[j] = 0;
+    return;
+  }
+  const double t = (double)tb.t0[p] + (double)k * (double)tb.dt[p];
   for (int j = threadIdx.x; j < half; j += blockDim.x) {
     double frac = (double)j / (double)(half > 1 ? half - 1 : 1);
     double period = (double)dm.pmin * pow((double)dm.pmax / (double)dm.pmin, frac);

@@ -98,30 +98,24 @@ struct rosa_expert {
   cudaEvent_t stage_ev[kStageRing] = {};
   int stage_next = 0;
   size_t call_bytes = 0;
-  size_t off_ids, off_src, off_t0, off_dt, off_ns, off_mact, off_order, off_ptrs;
+  size_t off_ids, off_src, off_t0, off_dt, off_ns, off_mact, off_ptrs, off_aiter, off_aoffs, off_asegs;
+  size_t seg_cap = 0;              // capacity of the attention segment table (entries)
+  int n_cta = 0;                   // CTAs of the persistent attention kernel (= SMs of the device)
+  float* attn_part = nullptr;      // per-CTA partial (O, m, l) of items cut between CTAs
+  int* attn_flag = nullptr;        // [n_cta][8] ready flags of those partials
+  int64_t graph_captures = 0;      // graphs captured so far (rosa_debug_graph_captures)
   std::map<GraphKey, cudaGraphExec_t> graphs;
   std::map<GraphKey, int64_t> graph_launches;
   cudaStream_t cap_stream = nullptr;
   int64_t last_launches = 0;
-  // Two lanes: robots are independent, so a large batch is cut into two sub-batches whose
-  // kernel chains run on two streams (two branches of the captured graph).  One lane's partial last round of
-  // tiles, prologue and exposed epilogue then overlap the other lane's main loop.  ROSA_LANES=1 turns it off.
-  int lanes = 1, lane_min_batch = 1 << 30;
-  cudaStream_t lane_stream = nullptr;
-  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
-  size_t lane_row_align = 256;  // lane 1 starts on a fresh 256-row tile of every workspace
   float* e2e_dev = nullptr;  // staging for rosa_denoise_batch_host
-  // fused a6 -> a7 -> a8 kernel: static schedules for every number of row blocks + dependency counters
-  bool fused_ok = false;
-  uint16_t* d_sched = nullptr;
-  int* d_done = nullptr;  // [2][kFusedPhases][n_m_max]
-  int fused_slots = 0, fused_pairs = 0, n_m_max = 0;
   // per-launch event timing (rosa_profile_batch): boundary event before every launch
   bool prof_on = false;
   std::vector<cudaEvent_t> prof_ev;
   std::vector<int> prof_cls;
   size_t prof_n = 0;
   std::vector<void*> allocs;
+  std::vector<rosa::AttnSeg> seg_tmp;
 };
 
 namespace rosa {
@@ -181,17 +175,20 @@ static rosa_status_t upload_f32(rosa_expert* e, const std::vector<float>& v, flo
   return ROSA_OK;
 }
 
-// Tables of the robots at internal positions [p0, p0 + batch) (a lane of the call, or all of it: p0 = 0, lane 0);
-// every per-robot array is indexed by the position within the lane.
-static Tables make_tables(const rosa_expert* e, int batch, int p0 = 0, int lane = 0) {
+// Device tables of the current call (robots in internal order).
+static Tables make_tables(const rosa_expert* e, int batch) {
+  const int p0 = 0;
   Tables tb;
   tb.ids = (const int*)(e->d_call + e->off_ids) + p0;
   tb.src = (const int*)(e->d_call + e->off_src) + p0;
   tb.t0 = (const float*)(e->d_call + e->off_t0) + p0;
   tb.dt = (const float*)(e->d_call + e->off_dt) + p0;
   tb.nsteps = (const int*)(e->d_call + e->off_ns) + p0;
-  tb.m_active = (const int*)(e->d_call + e->off_mact) + (size_t)lane * e->cfg.max_steps;
-  tb.attn_order = (const int*)(e->d_call + e->off_order) + p0;
+  tb.m_active = (const int*)(e->d_call + e->off_mact);
+  tb.attn_iter = (const int*)(e->d_call + e->off_aiter);
+  tb.attn_offs = (const int*)(e->d_call + e->off_aoffs);
+  tb.attn_segs = (const AttnSeg*)(e->d_call + e->off_asegs);
+  tb.batch_dev = &((const CallPtrs*)(e->d_call + e->off_ptrs))->batch_ext;
   tb.rk = e->d_rk;
   tb.rv = e->d_rv;
   tb.rlen = e->d_rlen;
@@ -199,35 +196,11 @@ static Tables make_tables(const rosa_expert* e, int batch, int p0 = 0, int lane 
   return tb;
 }
 
-// Robots of lane 0 when a batch is cut in two.  Near half, moved down as far as a quarter of the batch if that
-// saves a 256-row tile block: B = 64, H = 50 gives 30 + 34 robots = 6 + 7 row blocks, where 32 + 32 would pad to 7 + 7.
-static int lane_split_rows(int batch, int H) {
-  auto blocks = [&](int b) { return (b * H + 255) / 256; };
-  int best = batch / 2;
-  for (int b0 = batch / 2; b0 >= batch / 2 - batch / 4 && b0 >= 1; --b0)
-    if (blocks(b0) + blocks(batch - b0) < blocks(best) + blocks(batch - best)) best = b0;
-  return best;
-}
-static int lane_split(const rosa_expert* e, int batch) {  // 0 = one lane
-  if (e->lanes < 2 || batch < e->lane_min_batch || batch < 2 || e->prof_on) return 0;
-  return lane_split_rows(batch, e->dm.H);
-}
-// Internal order of a call: n_steps descending (stable), so that the active set of iteration k is a row prefix.  With two
-// lanes (b0 > 0) the sorted robots are dealt to the lanes in proportion (each lane keeps the descending order and both lose
-// their robots at about the same iterations); lane 0 takes positions [0, b0), lane 1 [b0, batch).
-static std::vector<int> call_order(int batch, const int32_t* n_steps, int b0) {
+// Internal order of a call: n_steps descending (stable), so that the active set of iteration k is a row prefix.
+static std::vector<int> call_order(int batch, const int32_t* n_steps) {
   std::vector<int> order(batch);
   std::iota(order.begin(), order.end(), 0);
   std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return n_steps[a] > n_steps[b]; });
-  if (b0 > 0) {
-    std::vector<int> l0, l1;
-    for (int q = 0; q < batch; ++q) {
-      const bool to0 = (long)(q + 1) * b0 / batch > (long)q * b0 / batch;
-      (to0 ? l0 : l1).push_back(order[q]);
-    }
-    std::copy(l0.begin(), l0.end(), order.begin());
-    std::copy(l1.begin(), l1.end(), order.begin() + b0);
-  }
   return order;
 }
 
@@ -243,9 +216,6 @@ static void destroy_impl(rosa_expert* e) {
     if (e->stage_ev[i]) cudaEventDestroy(e->stage_ev[i]);
   }
   if (e->cap_stream) cudaStreamDestroy(e->cap_stream);
-  if (e->lane_stream) cudaStreamDestroy(e->lane_stream);
-  if (e->ev_fork) cudaEventDestroy(e->ev_fork);
-  if (e->ev_join) cudaEventDestroy(e->ev_join);
   for (cudaEvent_t ev : e->prof_ev) cudaEventDestroy(ev);
   delete e;
 }
@@ -414,33 +384,6 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
   WS(e->scratch, Mmax * (size_t)std::max(2 * F, dm.qkv_n) * 4);
   WS(e->e2e_dev, (size_t)c->max_batch * HA * 4);
   WS(e->ssq, Mmax * (d / 32) * 4);
-  {  // fused O -> gate/up -> down kernel (tcgen05 family, 256-column tiles)
-    const char* fz = getenv("ROSA_FUSED");
-    // opt-in (ROSA_FUSED=1): measured slower than the three separate PDL-chained launches
-    e->fused_ok = e->family == 1 && d % 256 == 0 && (2 * F) % 256 == 0 && dm.q_n % 64 == 0 && fz && !strcmp(fz, "1");
-    if (e->fused_ok) {
-      int sms = 0, dev = 0;
-      cudaGetDevice(&dev);
-      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-      e->fused_pairs = sms / 2;
-      e->n_m_max = (int)(Mmax / 256) + 1;
-      const int n_n[kFusedPhases] = {d / 256, 2 * F / 256, d / 256};
-      const int n_kb[kFusedPhases] = {dm.q_n / 64, d / 64, F / 64};
-      if (e->n_m_max > 127 || n_n[1] > 63) e->fused_ok = false;  // item code: 7 bits of row block, 6 bits of column tile
-    }
-    if (e->fused_ok) {
-      const int n_n[kFusedPhases] = {d / 256, 2 * F / 256, d / 256};
-      const int n_kb[kFusedPhases] = {dm.q_n / 64, d / 64, F / 64};
-      e->fused_slots = tc_fused_max_slots(e->n_m_max, n_n, n_kb, e->fused_pairs) + 1;
-      std::vector<uint16_t> tab((size_t)(e->n_m_max + 1) * e->fused_pairs * e->fused_slots, 0xFFFF);
-      for (int nm = 1; nm <= e->n_m_max; ++nm)
-        tc_fused_schedule(nm, n_n, n_kb, e->fused_pairs, e->fused_slots, tab.data() + (size_t)nm * e->fused_pairs * e->fused_slots);
-      WS(e->d_sched, tab.size() * 2);
-      CK(cudaMemcpy(e->d_sched, tab.data(), tab.size() * 2, cudaMemcpyHostToDevice));
-      WS(e->d_done, (size_t)2 * kFusedPhases * e->n_m_max * 4);
-      CK(cudaMemset(e->d_done, 0, (size_t)2 * kFusedPhases * e->n_m_max * 4));
-    }
-  }
   CK(cudaMemset(e->zbuf, 0, Mmax * d * 2));
   CK(cudaMemset(e->nrm, 0, Mmax * d * 2));
   CK(cudaMemset(e->qkv, 0, Mmax * dm.qkv_n * 2));
@@ -460,6 +403,12 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
       const size_t nb = (size_t)c->max_robots * dm.layers * 2 * tc_attn_map_bytes();
       WS(e->d_kv_maps, nb);
       CK(cudaMemset(e->d_kv_maps, 0, nb));
+      int sms = 1, dev = 0;
+      cudaGetDevice(&dev);
+      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+      WS(e->attn_part, tc_attn_part_bytes(sms));
+      WS(e->attn_flag, (size_t)sms * 8 * 4);
+      CK(cudaMemset(e->attn_flag, 0, (size_t)sms * 8 * 4));
     }
   }
   e->h_rlen.assign(c->max_robots, -1);
@@ -472,9 +421,19 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
   e->off_t0 = take((size_t)c->max_batch * 4);
   e->off_dt = take((size_t)c->max_batch * 4);
   e->off_ns = take((size_t)c->max_batch * 4);
-  e->off_mact = take((size_t)2 * c->max_steps * 4);  // one list per lane
-  e->off_order = take((size_t)c->max_batch * 4);
+  e->off_mact = take((size_t)c->max_steps * 4);
   e->off_ptrs = take(sizeof(CallPtrs));
+  // attention work lists: one list per distinct active-robot count of the call, the used part is copied per call
+  e->n_cta = 1;
+  {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&e->n_cta, cudaDevAttrMultiProcessorCount, dev);
+  }
+  e->off_aiter = take((size_t)c->max_steps * 4);
+  e->off_aoffs = take((size_t)c->max_steps * (e->n_cta + 1) * 4);
+  e->seg_cap = (size_t)c->max_steps * ((size_t)c->max_batch * tc_attn_tiles(dm) + 4 * e->n_cta);
+  e->off_asegs = take(e->seg_cap * sizeof(AttnSeg));
   e->call_bytes = off;
   WS(e->d_call, e->call_bytes);
 #undef WS
@@ -483,15 +442,6 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
     CK(cudaEventCreateWithFlags(&e->stage_ev[i], cudaEventDisableTiming));
   }
   CK(cudaStreamCreateWithFlags(&e->cap_stream, cudaStreamNonBlocking));
-  CK(cudaStreamCreateWithFlags(&e->lane_stream, cudaStreamNonBlocking));
-  CK(cudaEventCreateWithFlags(&e->ev_fork, cudaEventDisableTiming));
-  CK(cudaEventCreateWithFlags(&e->ev_join, cudaEventDisableTiming));
-  {
-    const char* ln = getenv("ROSA_LANES");
-    const char* lb = getenv("ROSA_LANE_MIN_BATCH");
-    e->lanes = e->family == 1 && !dm.ada && !e->fused_ok && ln && atoi(ln) == 2 ? 2 : 1;
-    e->lane_min_batch = lb ? atoi(lb) : 32;
-  }
   return ROSA_OK;
 }
 
@@ -517,12 +467,6 @@ static cudaError_t gemm(rosa_expert* e, int cls, Epi epi, const op16* A, const o
   mark(e, cls, s);
   if (e->family == 1 && tc_gemm_supported(N, K)) {
     e->last_launches += 1;
-    static const int trace_bit = getenv("ROSA_DBG") ? atoi(getenv("ROSA_DBG")) & 64 : 0;  // clock trace of CTAs 0 and 64
-    if (trace_bit) {
-      EpiArgs at = a;
-      at.dbg |= trace_bit;
-      return launch_gemm_tc(epi, A, W, M, N, K, at, s);
-    }
     return launch_gemm_tc(epi, A, W, M, N, K, a, s);
   }
   launch_gemm_naive(A, W, e->scratch, M, N, K, a.in_fp16, a.m_active, s);
@@ -543,7 +487,7 @@ static cudaError_t enqueue_call_ada(rosa_expert* e, int batch, int nmax, cudaStr
   cudaError_t err;
   e->last_launches = 0;
   mark(e, ROSA_KC_GATHER_SCATTER, s);
-  launch_gather_x(e->x, cp, tb, dm.H * dm.A, e->d_done, 0, s);
+  launch_gather_x(e->x, cp, tb, dm.H * dm.A, s);
   e->last_launches += 1;
   // cond of every (step, robot) row: swish(W_t2 swish(W_t1 tau + b_t1) + b_t2), rows [k][batch]
   mark(e, ROSA_KC_TIMEVEC, s);
@@ -582,7 +526,7 @@ static cudaError_t enqueue_call_ada(rosa_expert* e, int batch, int nmax, cudaStr
       ea.rope_cols = dm.q_n + dm.nkv * dm.hd;
       if ((err = gemm(e, ROSA_KC_GEMM_QKV, EPI_ROPE, e->nrm, L.wqkv, M, dm.qkv_n, d, ea, s)) != cudaSuccess) return err;
       mark(e, ROSA_KC_ATTN, s);
-      if ((err = launch_attn_tc(dm, tb, l, e->qkv, e->obuf, k, M, e->d_kv_maps, s)) != cudaSuccess) return err;
+      if ((err = launch_attn_tc(dm, tb, l, e->qkv, e->obuf, k, M, e->d_kv_maps, e->attn_part, e->attn_flag, e->n_cta, s)) != cudaSuccess) return err;
       e->last_launches += 1;
       ea.out_f32 = e->h; ea.ld_out = d; ea.gate = mod_a + 2 * d; ea.gate_ld = n_mod;
       if ((err = gemm(e, ROSA_KC_GEMM_O, EPI_RESID, e->obuf, L.wo, M, d, dm.q_n, ea, s)) != cudaSuccess) return err;
@@ -609,45 +553,26 @@ static cudaError_t enqueue_call_ada(rosa_expert* e, int batch, int nmax, cudaStr
   return cudaGetLastError();
 }
 
-// A lane of a call: the robots at internal positions [p0, p0 + tb.batch), their token rows starting at row0 of
-// every workspace; `share` lanes divide the GPU between them.
-struct LaneView {
-  Tables tb;
-  int p0;
-  size_t row0;
-  int share;
-};
-
-// All Euler iterations (a1..a10 x nmax) of one lane on `s`.
-static cudaError_t enqueue_steps(rosa_expert* e, const LaneView& lv, int batch_full, int nmax, cudaStream_t s) {
+// All Euler iterations (a1..a10 x nmax) of a call on `s`.  `batch` is the graph's batch BUCKET: grids and row counts
+// are sized for it, the rows that are live in iteration k come from the device table m_active[k].
+static cudaError_t enqueue_steps(rosa_expert* e, const Tables& tb, int nmax, cudaStream_t s) {
   const Dims& dm = e->dm;
-  const Tables& tb = lv.tb;
   const CallPtrs* cp = (const CallPtrs*)(e->d_call + e->off_ptrs);
   const int batch = tb.batch, M = batch * dm.H, d = dm.d;
-  const size_t r0 = lv.row0;
-  float* x = e->x + (size_t)lv.p0 * dm.H * dm.A;
-  float* h = e->h + r0 * d;
-  op16 *zbuf = e->zbuf + r0 * d, *nrm = e->nrm + r0 * d, *obuf = e->obuf + r0 * dm.q_n, *mact = e->mact + r0 * dm.F;
-  bf16* qkv = e->qkv + r0 * dm.qkv_n;
-  float* ssq = e->ssq + r0 * (d / 32);
+  float *x = e->x, *h = e->h, *ssq = e->ssq;
+  op16 *zbuf = e->zbuf, *nrm = e->nrm, *obuf = e->obuf, *mact = e->mact;
+  bf16* qkv = e->qkv;
   cudaError_t err;
   const bool fused_norm = e->family == 1;  // RMSNorm fused into the GEMM epilogues (tcgen05 family)
-  const bool use_fused = e->fused_ok && tc_use_pair(M);
-  int fused_idx = 0;
   for (int k = 0; k < nmax; ++k) {
     EpiArgs ea{};
     ea.m_active = tb.m_active + k;
     ea.H = dm.H; ea.hd = dm.hd; ea.gu_blk = dm.gu_blk; ea.in_fp16 = dm.fp16; ea.out_fp16 = dm.fp16;
     ea.inv_d = 1.f / (float)d; ea.eps = dm.eps; ea.n_part = tc_ssq_parts(d, M);
     if (fused_norm) { ea.h16 = nrm; ea.ssq_out = ssq; ea.ssq_in = ssq; }
-    if (use_fused) { ea.force_bn = 256; ea.n_part = d / 128; }  // the fused kernel's tiles are 256 wide: every producer must match
-    if (lv.share > 1 && tc_use_pair(M)) {  // tile width for half of the CTA pairs; every producer of ssq must match
-      ea.force_bn = tc_resid_bn(d, M, lv.share);
-      ea.n_part = 2 * ((d + ea.force_bn - 1) / ea.force_bn);
-    }
     // a1: h0 = W2 swish(W1 [tau ; W_in x + b_in] + b1) + b2
     mark(e, ROSA_KC_INPROJ, s);
-    launch_embed1(zbuf, x, e->wca, e->bca, e->tvec + ((size_t)k * batch_full + lv.p0) * d, dm, tb, k, M, s);
+    launch_embed1(zbuf, x, e->wca, e->bca, e->tvec + (size_t)k * batch * d, dm, tb, k, M, s);
     e->last_launches += 1;
     ea.out_f32 = h; ea.ld_out = d; ea.bias = e->b_t2;
     if ((err = gemm(e, ROSA_KC_GEMM_EMBED, EPI_BIAS_F32, zbuf, e->w_t2, M, d, d, ea, s)) != cudaSuccess) return err;
@@ -664,42 +589,22 @@ static cudaError_t enqueue_steps(rosa_expert* e, const LaneView& lv, int batch_f
       if ((err = gemm(e, ROSA_KC_GEMM_QKV, EPI_ROPE, nrm, L.wqkv, M, dm.qkv_n, d, ea, s)) != cudaSuccess) return err;  // a2+a3+a4
       mark(e, ROSA_KC_ATTN, s);
       if (e->attn_tc) {                                                              // a5
-        if ((err = launch_attn_tc(dm, tb, l, qkv, obuf, k, M, e->d_kv_maps, s)) != cudaSuccess) return err;
+        if ((err = launch_attn_tc(dm, tb, l, qkv, obuf, k, M, e->d_kv_maps, e->attn_part, e->attn_flag, e->n_cta, s)) != cudaSuccess) return err;
       } else {
         launch_attn_simple(dm, tb, l, qkv, obuf, k, e->cfg.max_prefix_len, s);
       }
       e->last_launches += 1;
-      if (use_fused) {                                                              // a6 -> a7 -> a8, one launch
-        FusedMeta fm{};
-        const int n_n[kFusedPhases] = {d / 256, 2 * dm.F / 256, d / 256};
-        const int n_kb[kFusedPhases] = {dm.q_n / 64, d / 64, dm.F / 64};
-        const int epi[kFusedPhases] = {EPI_RESID, EPI_GEGLU, EPI_RESID};
-        for (int p = 0; p < kFusedPhases; ++p) { fm.n_n[p] = n_n[p]; fm.n_kb[p] = n_kb[p]; fm.epi[p] = epi[p]; fm.ea[p] = ea; }
-        fm.ea[0].out_f32 = h; fm.ea[0].ld_out = d;
-        fm.ea[1].out16 = mact; fm.ea[1].ld_out = dm.F;
-        fm.ea[2].out_f32 = h; fm.ea[2].ld_out = d;
-        fm.sched = e->d_sched; fm.pairs_max = e->fused_pairs; fm.slots = e->fused_slots; fm.n_m_max = e->n_m_max;
-        fm.done = e->d_done + (size_t)(fused_idx & 1) * kFusedPhases * e->n_m_max;
-        fm.done_next = e->d_done + (size_t)((fused_idx + 1) & 1) * kFusedPhases * e->n_m_max;
-        fused_idx += 1;
-        const op16* As[kFusedPhases] = {obuf, nrm, mact};
-        const op16* Ws[kFusedPhases] = {L.wo, L.wgu, L.wdown};
-        mark(e, ROSA_KC_GEMM_FUSED, s);
-        if ((err = launch_fused_tc(As, Ws, fm, M, tb.m_active + k, dm.fp16, s)) != cudaSuccess) return err;
+      ea.out_f32 = h; ea.ld_out = d;
+      if ((err = gemm(e, ROSA_KC_GEMM_O, EPI_RESID, obuf, L.wo, M, d, dm.q_n, ea, s)) != cudaSuccess) return err;    // a6
+      if (!fused_norm) {
+        mark(e, ROSA_KC_RMSNORM, s);
+        launch_rmsnorm(nrm, h, dm, tb, k, M, s);                               // a2
         e->last_launches += 1;
-      } else {
-        ea.out_f32 = h; ea.ld_out = d;
-        if ((err = gemm(e, ROSA_KC_GEMM_O, EPI_RESID, obuf, L.wo, M, d, dm.q_n, ea, s)) != cudaSuccess) return err;    // a6
-        if (!fused_norm) {
-          mark(e, ROSA_KC_RMSNORM, s);
-          launch_rmsnorm(nrm, h, dm, tb, k, M, s);                               // a2
-          e->last_launches += 1;
-        }
-        ea.out16 = mact; ea.ld_out = dm.F;
-        if ((err = gemm(e, ROSA_KC_GEMM_GATEUP, EPI_GEGLU, nrm, L.wgu, M, 2 * dm.F, d, ea, s)) != cudaSuccess) return err;  // a2+a7
-        ea.out_f32 = h; ea.ld_out = d;
-        if ((err = gemm(e, ROSA_KC_GEMM_DOWN, EPI_RESID, mact, L.wdown, M, d, dm.F, ea, s)) != cudaSuccess) return err;   // a8
       }
+      ea.out16 = mact; ea.ld_out = dm.F;
+      if ((err = gemm(e, ROSA_KC_GEMM_GATEUP, EPI_GEGLU, nrm, L.wgu, M, 2 * dm.F, d, ea, s)) != cudaSuccess) return err;  // a2+a7
+      ea.out_f32 = h; ea.ld_out = d;
+      if ((err = gemm(e, ROSA_KC_GEMM_DOWN, EPI_RESID, mact, L.wdown, M, d, dm.F, ea, s)) != cudaSuccess) return err;   // a8
     }
     if (fused_norm) {                                                                 // a9 + a10
       ea.bias = e->b_out; ea.x = x; ea.cp = cp; ea.dt = tb.dt; ea.src = tb.src; ea.A = dm.A; ea.k_iter = k;
@@ -713,11 +618,10 @@ static cudaError_t enqueue_steps(rosa_expert* e, const LaneView& lv, int batch_f
   return cudaSuccess;
 }
 
-// Enqueue the whole call (steps a1..a11) on `s`.  Everything that changes from call to call is
-// read from the device tables, so the same sequence can be captured once per (batch, nmax).
-// b0 > 0: robots [0, b0) and [b0, batch) run as two lanes, the second on e->lane_stream between a
-// fork and a join event (two branches when `s` is being captured).
-static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, int b0, cudaStream_t s) {
+// Enqueue the whole call (steps a1..a11) on `s`.  Everything that changes from call to call (robots, their order,
+// times, step counts, the number of live robots, the caller's pointers) is read from the device tables, so the
+// sequence is captured once per (batch bucket, nmax) and replayed for any call that fits the bucket.
+static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, cudaStream_t s) {
   const Dims& dm = e->dm;
   if (dm.ada) return enqueue_call_ada(e, batch, nmax, s);
   const Tables tb = make_tables(e, batch);
@@ -726,7 +630,7 @@ static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, int b0, cud
   cudaError_t err;
   e->last_launches = 0;
   mark(e, ROSA_KC_GATHER_SCATTER, s);
-  launch_gather_x(e->x, cp, tb, dm.H * dm.A, e->d_done, e->fused_ok ? 2 * kFusedPhases * e->n_m_max : 0, s);
+  launch_gather_x(e->x, cp, tb, dm.H * dm.A, s);
   mark(e, ROSA_KC_TIMEVEC, s);
   if (e->family == 1 && tc_gemm_supported(d, 2 * d)) {  // a1 time half of every (step, robot) as one GEMM
     launch_tau16(e->tau16, dm, tb, nmax, s);
@@ -738,20 +642,7 @@ static cudaError_t enqueue_call(rosa_expert* e, int batch, int nmax, int b0, cud
     launch_timevec(e->tvec, e->w_t1, e->b_t1, dm, tb, nmax, s);
     e->last_launches += 2;
   }
-  if (b0 > 0) {
-    const size_t row1 = ((size_t)b0 * dm.H + e->lane_row_align - 1) / e->lane_row_align * e->lane_row_align;
-    const LaneView l0{make_tables(e, b0, 0, 0), 0, 0, 2};
-    const LaneView l1{make_tables(e, batch - b0, b0, 1), b0, row1, 2};
-    if ((err = cudaEventRecord(e->ev_fork, s)) != cudaSuccess) return err;
-    if ((err = cudaStreamWaitEvent(e->lane_stream, e->ev_fork, 0)) != cudaSuccess) return err;
-    if ((err = enqueue_steps(e, l0, batch, nmax, s)) != cudaSuccess) return err;
-    if ((err = enqueue_steps(e, l1, batch, nmax, e->lane_stream)) != cudaSuccess) return err;
-    if ((err = cudaEventRecord(e->ev_join, e->lane_stream)) != cudaSuccess) return err;
-    if ((err = cudaStreamWaitEvent(s, e->ev_join, 0)) != cudaSuccess) return err;
-  } else {
-    const LaneView l0{tb, 0, 0, 1};
-    if ((err = enqueue_steps(e, l0, batch, nmax, s)) != cudaSuccess) return err;
-  }
+  if ((err = enqueue_steps(e, tb, nmax, s)) != cudaSuccess) return err;
   mark(e, ROSA_KC_GATHER_SCATTER, s);
   launch_scatter_x(cp, e->x, tb, dm.H * dm.A, s);
   e->last_launches += 1;
@@ -777,9 +668,8 @@ static rosa_status_t denoise_impl(rosa_expert* e, int batch, const int32_t* ids,
     if (n_steps[i] > e->cfg.max_steps) { set_error("n_steps > max_steps"); return ROSA_ERR_CAPACITY; }
     nmax = std::max(nmax, (int)n_steps[i]);
   }
-  // internal order: n_steps descending; two lanes: positions [0, b0) and [b0, batch) (call_order)
-  const int b0 = lane_split(e, batch);
-  const std::vector<int> order = call_order(batch, n_steps, b0);
+  // internal order: n_steps descending, so the robots live in iteration k are a prefix
+  const std::vector<int> order = call_order(batch, n_steps);
   const int slot = e->stage_next;
   e->stage_next = (slot + 1) % kStageRing;
   CK(cudaEventSynchronize(e->stage_ev[slot]));  // the copy that last used this slot has completed
@@ -794,36 +684,52 @@ static rosa_status_t denoise_impl(rosa_expert* e, int batch, const int32_t* ids,
     h_dt[p] = dt ? dt[i] : -h_t0[p] / (float)n_steps[i];
     h_ns[p] = n_steps[i];
   }
-  const int lane_p0[3] = {0, b0 > 0 ? b0 : batch, batch};
-  for (int lane = 0; lane < 2; ++lane) {
-    // active token rows of iteration k per lane (one lane: the whole batch in list 0)
-    for (int k = 0; k < e->cfg.max_steps; ++k) {
-      int act = 0;
-      for (int p = lane_p0[lane]; p < lane_p0[lane + 1]; ++p) act += h_ns[p] > k;
-      h_ma[lane * e->cfg.max_steps + k] = act * dm.H;
+  std::vector<int> act(e->cfg.max_steps, 0);
+  for (int k = 0; k < e->cfg.max_steps; ++k) {  // active token rows of iteration k
+    for (int p = 0; p < batch; ++p) act[k] += h_ns[p] > k;
+    h_ma[k] = act[k] * dm.H;
+  }
+  size_t copy_bytes = e->off_aiter;
+  if (e->attn_tc) {
+    // attention work lists (stream-K over the live robots' key streams): one per distinct live count
+    std::vector<int> len(batch);
+    for (int p = 0; p < batch; ++p) len[p] = e->h_rlen[h_ids[p]];
+    int* h_iter = (int*)(hs + e->off_aiter);
+    int* h_offs = (int*)(hs + e->off_aoffs);
+    std::vector<AttnSeg>& segs = e->seg_tmp;
+    segs.clear();
+    int n_lists = 0;
+    for (int k = 0; k < nmax; ++k) {
+      if (k > 0 && act[k] == act[k - 1]) { h_iter[k] = h_iter[k - 1]; continue; }
+      h_iter[k] = n_lists * (e->n_cta + 1);
+      attn_build_list(dm, act[k], len.data(), e->n_cta, segs, h_offs + h_iter[k]);
+      ++n_lists;
     }
-    // attention CTAs are issued longest prefix first: the second wave then pairs long with short (LPT);
-    // positions are counted within the lane
-    int* h_ord = (int*)(hs + e->off_order) + lane_p0[lane];
-    const int nb = lane_p0[lane + 1] - lane_p0[lane], p0 = lane_p0[lane];
-    std::iota(h_ord, h_ord + nb, 0);
-    std::stable_sort(h_ord, h_ord + nb, [&](int a, int b) { return e->h_rlen[h_ids[p0 + a]] > e->h_rlen[h_ids[p0 + b]]; });
+    for (int k = nmax; k < e->cfg.max_steps; ++k) h_iter[k] = 0;
+    if (segs.size() > e->seg_cap) { set_error("attention work list overflow"); return ROSA_ERR_CAPACITY; }
+    memcpy(hs + e->off_asegs, segs.data(), segs.size() * sizeof(AttnSeg));
+    copy_bytes = e->off_asegs + segs.size() * sizeof(AttnSeg);
   }
   CallPtrs* h_cp = (CallPtrs*)(hs + e->off_ptrs);
   h_cp->noise = noise; h_cp->out = out; h_cp->vel = out_vel; h_cp->batch_ext = batch;
-  CK(cudaMemcpyAsync(e->d_call, hs, e->call_bytes, cudaMemcpyHostToDevice, stream));
+  CK(cudaMemcpyAsync(e->d_call, hs, copy_bytes, cudaMemcpyHostToDevice, stream));
   CK(cudaEventRecord(e->stage_ev[slot], stream));
   if (out_vel) CK(cudaMemsetAsync(out_vel, 0, (size_t)nmax * batch * dm.H * dm.A * 4, stream));
+  // The captured sequence is sized for a batch BUCKET (next power of two, at most max_batch): rows, robots and
+  // work lists of the call itself come from the device tables, so one graph serves every call that fits the bucket.
+  int bucket = 1;
+  while (bucket < batch) bucket <<= 1;
+  bucket = std::min(bucket, e->cfg.max_batch);
   if (!e->use_graph || e->prof_on) {
-    CK(enqueue_call(e, batch, nmax, b0, stream));
+    CK(enqueue_call(e, bucket, nmax, stream));
     return ROSA_OK;
   }
-  const GraphKey key{batch, nmax, 0};
+  const GraphKey key{bucket, nmax, 0};
   auto it = e->graphs.find(key);
   if (it == e->graphs.end()) {
     cudaGraph_t g = nullptr;
     CK(cudaStreamBeginCapture(e->cap_stream, cudaStreamCaptureModeThreadLocal));
-    cudaError_t err = enqueue_call(e, batch, nmax, b0, e->cap_stream);
+    cudaError_t err = enqueue_call(e, bucket, nmax, e->cap_stream);
     cudaError_t err2 = cudaStreamEndCapture(e->cap_stream, &g);
     if (err != cudaSuccess || err2 != cudaSuccess) {
       if (g) cudaGraphDestroy(g);
@@ -835,6 +741,7 @@ static rosa_status_t denoise_impl(rosa_expert* e, int batch, const int32_t* ids,
     cudaGraphDestroy(g);
     it = e->graphs.emplace(key, ex).first;
     e->graph_launches[key] = e->last_launches;
+    e->graph_captures += 1;
   }
   e->last_launches = e->graph_launches[key];
   CK(cudaGraphLaunch(it->second, stream));
@@ -1022,7 +929,7 @@ rosa_status_t rosa_profile_batch(rosa_expert_t* e, int32_t batch, const int32_t*
 const char* rosa_kernel_class_name(int32_t cls) {
   static const char* names[ROSA_KC_COUNT] = {"gather_scatter", "timevec", "inproj", "gemm_embed", "rmsnorm",
                                              "gemm_qkv_rope", "attention", "gemm_o_resid", "gemm_gateup_geglu",
-                                             "gemm_down_resid", "final_norm_outproj_euler", "gemm_fused_o_gateup_down"};
+                                             "gemm_down_resid", "final_norm_outproj_euler"};
   return cls >= 0 && cls < ROSA_KC_COUNT ? names[cls] : "";
 }
 
@@ -1037,32 +944,51 @@ rosa_status_t rosa_kernel_family(rosa_expert_t* e, int32_t* family) {
   return ROSA_OK;
 }
 
-rosa_status_t rosa_debug_gemm(int32_t family, int32_t M, int32_t N, int32_t K, const void* A, const void* W,
-                              float* C, void* stream) {
+rosa_status_t rosa_debug_graph_captures(rosa_expert_t* e, int64_t* n) {
+  if (!e || !n) { set_error("NULL argument"); return ROSA_ERR_INVALID_ARG; }
+  *n = e->graph_captures;
+  return ROSA_OK;
+}
+
+rosa_status_t rosa_debug_gemm(int32_t family, int32_t epi, int32_t pair, int32_t bn, int32_t fp16, int32_t M, int32_t N,
+                              int32_t K, const void* A, const void* W, float* C, const float* bias, void* h16,
+                              float* ssq, void* stream) {
   if (!A || !W || !C || M < 1 || N < 1 || K < 1) { set_error("bad argument"); return ROSA_ERR_INVALID_ARG; }
+  if (epi != EPI_STORE_F32 && epi != EPI_BIAS_F32 && epi != EPI_RESID) { set_error("epi must be 0, 2 or 4"); return ROSA_ERR_INVALID_ARG; }
+  if (epi == EPI_BIAS_F32 && !bias) { set_error("bias is NULL"); return ROSA_ERR_INVALID_ARG; }
   cudaStream_t s = (cudaStream_t)stream;
   if (family == 0) {
-    launch_gemm_naive((const op16*)A, (const op16*)W, C, M, N, K, 0, nullptr, s);
+    if (epi != EPI_STORE_F32) { set_error("family 0: epi 0 only"); return ROSA_ERR_UNSUPPORTED; }
+    launch_gemm_naive((const op16*)A, (const op16*)W, C, M, N, K, fp16, nullptr, s);
     CK(cudaGetLastError());
     return ROSA_OK;
   }
   if (!tc_gemm_supported(N, K)) { set_error("shape not supported by the tcgen05 GEMM"); return ROSA_ERR_UNSUPPORTED; }
   EpiArgs ea{};
-  ea.out_f32 = C; ea.ld_out = N;
-  if (const char* dbg = getenv("ROSA_DBG")) ea.dbg = atoi(dbg);  // bits 0-1 skip epilogue / MMA; >> 8: 1256 = single-CTA BN 256, 2128 = pair BN 128 ...
-  CK(launch_gemm_tc(EPI_STORE_F32, (const op16*)A, (const op16*)W, M, N, K, ea, s));
+  ea.out_f32 = C; ea.ld_out = N; ea.bias = bias; ea.h16 = h16; ea.ssq_out = ssq;
+  ea.in_fp16 = fp16; ea.out_fp16 = fp16;
+  ea.force_bn = bn; ea.force_pair = pair < 0 ? 0 : (pair ? 2 : 1);
+  cudaError_t err = launch_gemm_tc((Epi)epi, (const op16*)A, (const op16*)W, M, N, K, ea, s);
+  if (err == cudaErrorNotSupported) { set_error("no kernel for this (pair, bn)"); return ROSA_ERR_UNSUPPORTED; }
+  CK(err);
   return ROSA_OK;
 }
 
-int32_t rosa_debug_lane_plan(int32_t batch, int32_t horizon, const int32_t* n_steps, int32_t* order_out) {
-  if (batch < 2 || horizon < 1 || !n_steps || !order_out) { set_error("bad argument"); return ROSA_ERR_INVALID_ARG; }
-  const int b0 = lane_split_rows(batch, horizon);
-  const std::vector<int> order = call_order(batch, n_steps, b0);
-  std::copy(order.begin(), order.end(), order_out);
-  return b0;
+int32_t rosa_debug_attn_plan(int32_t horizon, int32_t n_robots, const int32_t* len, int32_t n_cta, int32_t* offs_out,
+                             int32_t* segs_out, int32_t cap) {
+  if (horizon < 1 || n_robots < 1 || !len || n_cta < 1 || !offs_out || !segs_out) { set_error("bad argument"); return ROSA_ERR_INVALID_ARG; }
+  Dims dm{};
+  dm.H = horizon;
+  std::vector<AttnSeg> segs;
+  const int n = attn_build_list(dm, n_robots, len, n_cta, segs, offs_out);
+  if (n > cap) { set_error("cap too small"); return ROSA_ERR_CAPACITY; }
+  for (int i = 0; i < n; ++i) {
+    int32_t* o = segs_out + 8 * i;
+    o[0] = segs[i].p; o[1] = segs[i].tt; o[2] = segs[i].kb0; o[3] = segs[i].kb1;
+    o[4] = segs[i].n_part; o[5] = segs[i].part0; o[6] = 0; o[7] = 0;
+  }
+  return n;
 }
-int32_t rosa_debug_attn_trace(int64_t* host_out, int32_t n) { return tc_attn_read_trace((long long*)host_out, n); }
-int32_t rosa_debug_gemm_trace(int64_t* host_out, int32_t n) { return tc_gemm_read_trace((long long*)host_out, n); }
 
 const char* rosa_last_error(void) { return g_err.c_str(); }
 int32_t rosa_version(void) { return 1; }

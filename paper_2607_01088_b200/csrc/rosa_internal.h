@@ -9,6 +9,7 @@
 #include <vector>
 
 #include "rosa.h"
+#include "rosa_debug.h"
 
 typedef __nv_bfloat16 bf16;
 typedef uint16_t op16;  // 16-bit GEMM operand storage: fp16 or bf16 bits, chosen per expert (Dims::fp16)
@@ -35,12 +36,25 @@ struct Tables {
   const float* dt;      // [B]
   const int* nsteps;    // [B]
   const int* m_active;  // [max_steps] active token rows (= H * active robots) in iteration k
-  const int* attn_order;  // [B] internal positions sorted by prefix length, longest first (attention CTA order)
+  // attention work lists (attn_tcgen05.cu): offs + attn_iter[k] = the n_cta + 1 segment offsets of iteration k
+  const int* attn_iter;     // [max_steps]
+  const int* attn_offs;
+  const struct AttnSeg* attn_segs;
+  const int* batch_dev;     // live robots of this call (<= batch, the graph's bucket)
   const bf16* const* rk;  // [max_robots * layers] prefix K pointer of (robot, layer)
   const bf16* const* rv;  // [max_robots * layers]
   const int* rlen;        // [max_robots]
-  int batch;
+  int batch;                // the captured graph's batch bucket: grids and row counts are sized for it
 };
+
+// One entry of a CTA's attention work list: key blocks [kb0, kb1) of item (robot position p, token tile tt).
+// n_part >= 0: head segment (kb0 = 0): writes the output after merging the partials of CTAs part0 .. part0 + n_part - 1;
+// n_part < 0: continuation: leaves its partial (O, m, l) in the scratch slot of its CTA.
+struct AttnSeg {
+  int32_t p;
+  int16_t tt, kb0, kb1, n_part, part0, pad;
+};
+static_assert(sizeof(AttnSeg) == 16, "AttnSeg is copied to the device as 16-byte records");
 
 // Caller pointers of the current call live in device memory so that a captured graph can be
 // replayed for a different call (the kernels read them through this struct).
@@ -94,7 +108,7 @@ struct EpiArgs {
   int force_bn;           // BIAS_F32 / RESID: N tile to use (0 = chosen from N and M)
   const float* gate;      // RESID, adaptive-norm variant: h += gate[row / H][col] * acc (null = 1); rows gate_ld floats apart
   int gate_ld;
-  int dbg;                // measurement aid (ROSA_DBG): bit 0 skip the epilogue body, bit 1 skip the MMAs
+  int force_pair;         // rosa_debug_gemm only: 0 = kernel chosen by M (the path), 1 = single-CTA kernel, 2 = CTA-pair kernel
 };
 
 // ---- launchers (each checks nothing; callers validated shapes) -------------------------
@@ -105,7 +119,7 @@ void launch_epilogue(Epi epi, const float* C, int M, int N, const EpiArgs& a, cu
 void launch_attn_simple(const Dims& dm, const Tables& tb, int layer, const bf16* qkv, op16* o,
                         int k_iter, int max_len, cudaStream_t s);
 // common elementwise kernels
-void launch_gather_x(float* x, const CallPtrs* cp, const Tables& tb, int HA, int* zero, int n_zero, cudaStream_t s);
+void launch_gather_x(float* x, const CallPtrs* cp, const Tables& tb, int HA, cudaStream_t s);
 void launch_scatter_x(const CallPtrs* cp, const float* x, const Tables& tb, int HA, cudaStream_t s);
 void launch_timevec(float* tvec, const bf16* w_t1, const float* b_t1, const Dims& dm,
                     const Tables& tb, int nsteps_max, cudaStream_t s);
@@ -126,39 +140,23 @@ void launch_final(float* x, const CallPtrs* cp, const float* h, const float* g, 
 void launch_f32_to_bf16(bf16* dst, const float* src, size_t n, cudaStream_t s);
 // tcgen05 family (gemm_tcgen05.cu)
 bool tc_gemm_supported(int N, int K);
-int tc_resid_bn(int N, int M, int share);  // N tile of the BIAS_F32 / RESID launches when `share` lanes divide the CTA pairs
+int tc_resid_bn(int N, int M);  // N tile of the BIAS_F32 / RESID launches
 int tc_ssq_parts(int N, int M);  // sum-of-squares partials per row written by the BIAS_F32 / RESID launches (two per N tile)
 // A [M,K] row-major, W [N,K] row-major, both fp16 or both bf16 (EpiArgs::in_fp16)
 cudaError_t launch_gemm_tc(Epi epi, const op16* A, const op16* W, int M, int N, int K,
                            const EpiArgs& a, cudaStream_t s);
 
-// fused dependent GEMMs a6 -> a7 -> a8 in one persistent CTA-pair kernel (gemm_tcgen05.cu)
-constexpr int kFusedPhases = 3;
-struct FusedMeta {
-  int n_n[kFusedPhases];     // column tiles (256 wide) per row block
-  int n_kb[kFusedPhases];    // k-blocks per tile
-  int epi[kFusedPhases];     // Epi
-  EpiArgs ea[kFusedPhases];
-  const uint16_t* sched;     // [n_m_max + 1][pairs_max][slots] item codes (phase << 13 | m << 6 | n), 0xFFFF = end
-  int pairs_max, slots;
-  int* done;                 // [kFusedPhases][n_m_max] epilogue-warp arrivals of this launch (zeroed by the previous one)
-  int* done_next;            // the other buffer: zeroed here for the next launch
-  int n_m_max;
-};
 bool tc_use_pair(int M);
-void tc_fused_schedule(int n_m, const int* n_n, const int* n_kb, int pairs, int slots, uint16_t* out);
-int tc_fused_max_slots(int n_m, const int* n_n, const int* n_kb, int pairs);
-cudaError_t launch_fused_tc(const op16* const* A, const op16* const* W, const FusedMeta& fm, int M, const int* m_active,
-                            int in_fp16, cudaStream_t s);
 
 // tcgen05 attention (attn_tcgen05.cu)
 bool tc_attn_supported(const Dims& dm);
-int tc_attn_read_trace(long long* host, int n);
-int tc_gemm_read_trace(long long* host, int n);
 size_t tc_attn_map_bytes();  // sizeof(CUtensorMap)
 bool tc_attn_make_prefix_maps(void* out2_host, const bf16* k, const bf16* v, int len, const Dims& dm);
+size_t tc_attn_part_bytes(int n_cta);  // scratch for the partial results of items cut between CTAs
+int tc_attn_tiles(const Dims& dm);     // token tiles (items) per robot
+int attn_build_list(const Dims& dm, int n_active, const int* len, int n_cta, std::vector<AttnSeg>& segs, int* offs);
 cudaError_t launch_attn_tc(const Dims& dm, const Tables& tb, int layer, const bf16* qkv, op16* o, int k_iter,
-                           int M, const void* d_kv_maps, cudaStream_t s);
+                           int M, const void* d_kv_maps, float* part, int* part_flag, int n_cta, cudaStream_t s);
 
 void set_error(const std::string& msg);
 

@@ -1,4 +1,5 @@
-"""The C-ABI library loads and exports every symbol include/rosa.h declares (CPU only; no compute)."""
+"""The C-ABI library loads and exports every symbol include/*.h declares (CPU only; no compute), and the host
+logic behind it that needs no device."""
 import os
 import re
 
@@ -18,17 +19,19 @@ def lib():
     return rosa.load()
 
 
-def declared_symbols():
-    text = open(os.path.join(ROOT, "include", "rosa.h")).read()
+def declared_symbols(header):
+    text = open(os.path.join(ROOT, "include", header)).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(rosa_[a-z_0-9]+)\s*\(", text)))
 
 
 def test_header_symbols_exported(lib):
-    syms = declared_symbols()
-    assert set(syms) == set(rosa.EXPORTS), (syms, rosa.EXPORTS)
-    for s in syms:
-        assert hasattr(lib, s), s
+    assert sorted(os.listdir(os.path.join(ROOT, "include"))) == ["rosa.h", "rosa_debug.h"]
+    for header, names in (("rosa.h", rosa.EXPORTS), ("rosa_debug.h", rosa.DEBUG_EXPORTS)):
+        syms = declared_symbols(header)
+        assert set(syms) == set(names), (header, syms, names)
+        for s in syms:
+            assert hasattr(lib, s), s
     assert rosa.rosa_version() >= 1
     assert isinstance(rosa.rosa_last_error(), str)
 
@@ -55,30 +58,56 @@ def test_argument_validation_without_gpu(lib):
     assert ei.value.status == rosa.ROSA_ERR_UNSUPPORTED
 
 
-def test_lane_plan_host_logic(lib):
-    """Host logic of the opt-in two-lane split, through the C ABI without a device: the split
-    point minimises 256-row tile blocks near batch / 2, the order is a permutation, and each lane is the stable
-    descending sort of its robots by n_steps with the two lanes interleaved in proportion."""
-    blocks = lambda b, H: (b * H + 255) // 256
-    rng = np.random.default_rng(7)
-    b0, order = rosa.rosa_debug_lane_plan(np.full(64, 10), 50)
-    assert b0 == 30 and blocks(30, 50) + blocks(34, 50) == 13 == blocks(64, 50)   # BASELINE.json configs[2]: 6 + 7 row blocks
-    assert sorted(order.tolist()) == list(range(64))
-    for batch, H in [(2, 50), (3, 8), (12, 50), (64, 50), (256, 50), (37, 7), (512, 50)]:
-        ns = rng.integers(1, 11, size=batch).astype(np.int32)
-        b0, order = rosa.rosa_debug_lane_plan(ns, H)
-        assert 1 <= b0 <= batch // 2 or (batch < 4 and b0 == batch // 2)
-        cand = range(max(batch // 2 - batch // 4, 1), batch // 2 + 1)
-        assert blocks(b0, H) + blocks(batch - b0, H) == min(blocks(c, H) + blocks(batch - c, H) for c in cand)
-        assert sorted(order.tolist()) == list(range(batch))
-        want = sorted(range(batch), key=lambda i: -int(ns[i]))                      # stable descending
-        for lane in (order[:b0], order[b0:]):
-            assert all(ns[a] >= ns[b] for a, b in zip(lane[:-1], lane[1:]))
-            assert [i for i in want if i in set(lane.tolist())] == lane.tolist()    # a subsequence of the stable sort
-        # dealt in proportion: after any prefix of the sorted robots the lanes hold their share to within one robot
-        pos = {int(r): q for q, r in enumerate(want)}
-        for q in range(1, batch + 1):
-            in0 = sum(1 for r in order[:b0] if pos[int(r)] < q)
-            assert abs(in0 - q * b0 / batch) < 1.0
-    with pytest.raises(RuntimeError):
-        rosa.rosa_debug_lane_plan(np.array([3], dtype=np.int32), 50)
+def check_attn_plan(H, lens, n_cta):
+    """Invariants of the stream-K split of the attention step (attn_tcgen05.cu): every key block of every item is
+    covered exactly once; a head segment (kb0 = 0) is the last entry of its CTA's list unless the item is whole;
+    a continuation is the FIRST entry of its CTA's list and sits on the CTAs part0 .. part0 + n_part - 1 right
+    after the head's CTA; nothing is shorter than 2 blocks unless the item is."""
+    offs, segs = rosa.rosa_debug_attn_plan(H, lens, n_cta)
+    tiles = (H + 15) // 16
+    assert offs[0] == 0 and offs[-1] == len(segs) and np.all(np.diff(offs) >= 0)
+    cta_of = np.repeat(np.arange(n_cta), np.diff(offs))
+    cover = {}
+    for i, (p, tt, kb0, kb1, n_part, part0) in enumerate(segs):
+        nb = (lens[p] + 63) // 64 + 1
+        assert 0 <= tt < tiles and 0 <= kb0 < kb1 <= nb
+        cover.setdefault((p, tt), []).append((kb0, kb1, n_part, part0, cta_of[i], i))
+    assert set(cover) == {(p, t) for p in range(len(lens)) for t in range(tiles)}
+    loads = np.zeros(n_cta)
+    for (p, tt), parts in cover.items():
+        nb = (lens[p] + 63) // 64 + 1
+        parts.sort()
+        assert parts[0][0] == 0 and parts[-1][1] == nb
+        for a, b in zip(parts, parts[1:]):
+            assert a[1] == b[0]                                   # contiguous, no overlap
+        head = parts[0]
+        assert head[2] == len(parts) - 1 and len(parts) <= 4       # n_part of the head = number of continuations
+        if len(parts) > 1:
+            assert head[5] == offs[head[4] + 1] - 1               # the head ends its CTA's list
+            assert head[3] == head[4] + 1                         # the continuations follow on the next CTAs
+            for k, c in enumerate(parts[1:]):
+                assert c[2] == -1 and c[4] == head[4] + 1 + k and c[5] == offs[c[4]]   # first entry of that CTA
+            assert all(b - a >= 2 for a, b, *_ in parts)
+        for a, b, _, _, cta, _ in parts:
+            loads[cta] += b - a + 2.0
+    return loads
+
+
+def test_attn_plan_host_logic(lib):
+    """Host logic of the attention work split through the C ABI without a device (pins: brute-force invariants
+    above; balance: no CTA carries more than its equal share plus one item's worth)."""
+    rng = np.random.default_rng(3)
+    # cfg2-like fleet on 148 CTAs: shares are balanced to within a few blocks
+    lens = rng.integers(600, 1001, size=64)
+    loads = check_attn_plan(50, lens, 148)
+    assert np.count_nonzero(loads) == 148
+    assert loads.max() <= loads.sum() / 148 + 4.0, (loads.max(), loads.sum() / 148)
+    # one robot: the four items are cut so that several CTAs share each key stream
+    loads = check_attn_plan(50, [816], 148)
+    assert np.count_nonzero(loads) >= 8
+    # degenerate and ragged cases, few CTAs, L = 0
+    for lens, n_cta, H in (([0], 148, 50), ([0, 1, 63, 64, 65], 7, 50), ([5000], 3, 8), (list(rng.integers(0, 1300, size=256)), 148, 50),
+                           ([816] * 512, 148, 50), ([100, 100], 1, 50), ([1200] * 3, 148, 64)):
+        check_attn_plan(H, np.asarray(lens), n_cta)
+    with pytest.raises(rosa.RosaError):
+        rosa.rosa_debug_attn_plan(0, [1], 4)

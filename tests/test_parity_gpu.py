@@ -288,21 +288,73 @@ def test_rebind_unbind_and_error_codes():
     lc.close()
 
 
+def _gemm_operands(M, N, K, fp16, seed):
+    """Seeded operands that both formats represent exactly (bf16-rounded values inside the fp16 normal range)."""
+    rng = np.random.default_rng(seed)
+    a = cases.round_bf16(rng.standard_normal((M, K), dtype=np.float32))
+    w = cases.round_bf16(rng.standard_normal((N, K), dtype=np.float32) * 0.05)
+    w[np.abs(w) < 2.0 ** -14] = 0.0                      # below the fp16 normal range: not exact in fp16
+    if fp16:
+        A = torch.from_numpy(a.astype(np.float16).view(np.int16)).cuda()
+        W = torch.from_numpy(w.astype(np.float16).view(np.int16)).cuda()
+    else:
+        A = torch.from_numpy(cases.f32_to_bf16_bits(a).view(np.int16)).cuda()
+        W = torch.from_numpy(cases.f32_to_bf16_bits(w).view(np.int16)).cuda()
+    return a, w, A, W
+
+
 @pytest.mark.parametrize("M,N,K", [(1, 64, 64), (127, 128, 192), (129, 256, 1024), (400, 2560, 1024),
                                    (3200, 1024, 4096), (333, 8192, 1024), (3200, 1024, 2048)])
 def test_tcgen05_gemm_unit(M, N, K):
-    """C = A W^T through the tcgen05/TMA kernel against numpy fp64 on the same bf16 operand values."""
-    rng = np.random.default_rng(M * 7 + N + K)
-    a = cases.round_bf16(rng.standard_normal((M, K), dtype=np.float32))
-    w = cases.round_bf16(rng.standard_normal((N, K), dtype=np.float32) * 0.05)
-    A = torch.from_numpy(cases.f32_to_bf16_bits(a).view(np.int16)).cuda()
-    W = torch.from_numpy(cases.f32_to_bf16_bits(w).view(np.int16)).cuda()
+    """C = A W^T through the tcgen05/TMA kernel the library picks, against numpy fp64 on the same bf16 operand values."""
+    a, w, A, W = _gemm_operands(M, N, K, 0, M * 7 + N + K)
     C = torch.zeros((M, N), dtype=torch.float32, device="cuda")
     rosa.rosa_debug_gemm(1, M, N, K, A, W, C)
     torch.cuda.synchronize()
     want = a.astype(np.float64) @ w.astype(np.float64).T
     got = C.cpu().numpy()
     assert np.abs(got - want).max() <= 2e-5 * K ** 0.5 * 4 + 1e-6, np.abs(got - want).max()
+
+
+PAIR_WIDTHS = (256, 224, 192, 160, 128, 96, 64)
+
+
+@pytest.mark.parametrize("epi", [rosa.EPI_STORE_F32, rosa.EPI_BIAS_F32, rosa.EPI_RESID])
+@pytest.mark.parametrize("pair,bn", [(1, b) for b in PAIR_WIDTHS] + [(0, 256), (0, 128), (0, 64)])
+def test_tcgen05_gemm_every_width_and_epilogue(epi, pair, bn):
+    """Every N-tile width of the CTA-pair kernel (and the three of the single-CTA kernel) x every fp32 epilogue of
+    the path (plain store, + bias, + residual), against numpy fp64 on the same 16-bit operands: the fp32 result,
+    the 16-bit copy of it (A operand of the next GEMM) and the per-32-column sums of squares (fused RMSNorm, a2).
+    M has a ragged last row block; N = 1024, so the widths 224 / 192 / 160 / 96 end in a masked column tile."""
+    M, N, K = (333 if pair else 100), 1024, 512
+    fp16 = 1 if epi != rosa.EPI_STORE_F32 else 0          # the path's operand format (R19'); the plain store runs bf16
+    a, w, A, W = _gemm_operands(M, N, K, fp16, 1000 + bn + 7 * epi + pair)
+    rng = np.random.default_rng(bn + epi)
+    c0 = rng.standard_normal((M, N), dtype=np.float32)
+    bias = rng.standard_normal(N, dtype=np.float32)
+    C = torch.from_numpy(c0.copy()).cuda()
+    kw = {}
+    if epi != rosa.EPI_STORE_F32:
+        h16 = torch.zeros((M, N), dtype=torch.int16, device="cuda")
+        ssq = torch.full((M, N // 32), -1.0, dtype=torch.float32, device="cuda")
+        kw = dict(h16=h16, ssq=ssq, bias=torch.from_numpy(bias).cuda() if epi == rosa.EPI_BIAS_F32 else None)
+    rosa.rosa_debug_gemm(1, M, N, K, A, W, C, epi=epi, pair=pair, bn=bn, fp16=fp16, **kw)
+    torch.cuda.synchronize()
+    want = a.astype(np.float64) @ w.astype(np.float64).T
+    if epi == rosa.EPI_BIAS_F32:
+        want = want + bias.astype(np.float64)
+    if epi == rosa.EPI_RESID:
+        want = want + c0.astype(np.float64)
+    got = C.cpu().numpy()
+    err = float(np.abs(got - want).max())
+    print(f"[gemm pair={pair} bn={bn} epi={epi}] max-abs {err:.3e}")
+    assert err <= 2e-5 * K ** 0.5 * 4 + 1e-6 + 4e-7 * np.abs(want).max(), err
+    if epi != rosa.EPI_STORE_F32:
+        got16 = h16.cpu().numpy().view(np.float16).astype(np.float32)
+        assert np.array_equal(got16, got.astype(np.float16).astype(np.float32))        # RNE of the fp32 value written
+        want_ssq = (got.astype(np.float64) ** 2).reshape(M, N // 32, 32).sum(-1)
+        got_ssq = ssq.cpu().numpy()
+        assert np.abs(got_ssq - want_ssq).max() <= 1e-5 * want_ssq.max()
 
 
 def test_bf16_operand_mode_measured(monkeypatch):
@@ -325,44 +377,6 @@ def test_bf16_operand_mode_measured(monkeypatch):
     assert res["bf16"][0] <= TOL_ACT_ABS and res["bf16"][1] <= TOL_ACT_REL
     assert res["fp16"][2] <= TOL_VEL_REL
     assert res["fp16"][2] < res["bf16"][2]
-
-
-def test_fused_dependent_gemm_kernel_opt_in(monkeypatch):
-    """ROSA_FUSED=1: O projection, gate/up and down GEMMs of a layer in ONE persistent kernel with a static
-    host-computed list schedule and per-row-block dependency counters (both priority orders)."""
-    case = edge_case([70, 150, 33, 90, 64, 200, 10, 129, 300, 17, 64, 65], n_steps=2)   # M = 600: three 256-row blocks
-    want_x, want_v = O.denoise_case(case, return_velocity=True)
-    for order in ("0", "1"):
-        monkeypatch.setenv("ROSA_FUSED", "1")
-        monkeypatch.setenv("ROSA_FUSED_ORDER", order)
-        lc = LoadedCase(case)
-        got_x, got_v = lc.run(want_velocity=True)
-        again, _ = lc.run()
-        n_launch = rosa.rosa_last_launch_count(lc.expert)
-        lc.close()
-        compare(f"fused-order{order}", got_x, got_v, want_x, want_v)
-        assert np.array_equal(got_x, again)                       # deterministic
-        assert n_launch == 3 + 2 * (2 + 2 * 3 + 1) + 1            # gather, tau, time GEMM; per step 2 + 3 per layer (not 5) + 1; scatter
-
-
-def test_two_lane_opt_in(monkeypatch):
-    """ROSA_LANES=2: a batch cut into two sub-batches whose kernel chains run as two branches of the captured graph
-    (measured slower at B=64 and left opt-in).  Mixed step counts, so each lane has its own shrinking
-    active set; the split 5 + 7 robots puts lane 1 on its own 256-row block of every workspace."""
-    case = edge_case([70, 150, 33, 90, 64, 200, 10, 129, 300, 17, 64, 65], n_steps=3)
-    case.n_steps[:] = np.array([3, 1, 2, 3, 1, 1, 2, 3, 3, 2, 1, 3], dtype=case.n_steps.dtype)
-    case.dt[:] = (-case.t_start / case.n_steps).astype(case.dt.dtype)
-    want_x, want_v = O.denoise_case(case, return_velocity=True)
-    monkeypatch.setenv("ROSA_LANES", "2")
-    monkeypatch.setenv("ROSA_LANE_MIN_BATCH", "4")
-    lc = LoadedCase(case)
-    got_x, got_v = lc.run(want_velocity=True)
-    again, _ = lc.run()
-    n_launch = rosa.rosa_last_launch_count(lc.expert)
-    lc.close()
-    compare("two-lane", got_x, got_v, want_x, want_v)
-    assert np.array_equal(got_x, again)                           # deterministic
-    assert n_launch == 3 + 2 * 3 * (2 + 5 * MINI.layers + 1) + 1  # both lanes run every kernel of the three steps
 
 
 # ------------------------------------------------------------------ adaptive-norm variant (reading R25, SURVEY 8(f) item 4)
