@@ -5,9 +5,9 @@
 // [prefix K/V (L_p rows, from the bound cache) ; own k/v (H rows, from the qkv buffer)], walked in blocks of
 // 64 keys:
 //     S = Q K_blk^T           tcgen05.mma  M=128 N=64  K=256   Q is the A operand FROM TENSOR MEMORY
-//     P = exp2(S*c - m_ref)   8 softmax warps, two per query row (32 keys each; both read all 64 scores for
-//                             the row maximum), running (m_ref, partial l) in registers; P (bf16) is written
-//                             back into tensor memory over S
+//     P = exp2(S*c - m_ref)   8 softmax warps, two per query row (32 keys each; the row maximum of the block is
+//                             exchanged through shared memory), running (m_ref, partial l) in registers; P (bf16)
+//                             is written back into tensor memory over the warp's own scores
 //     O += P V_blk            tcgen05.mma  M=128 N=256 K=64    P is the A operand from tensor memory,
 //                             V the MN-major B operand from shared memory
 // Tensor memory (512 columns): O [0,256) | S/P double buffer [256,384) | Q [384,512).
@@ -40,19 +40,22 @@ constexpr int AT_HD = 256;        // head_dim
 constexpr int AT_ROWS = 128;      // query rows per item = AT_TOK tokens x 8 heads
 constexpr int AT_TOK = 16;
 constexpr int AT_KV = 64;         // keys per block
-constexpr int AT_RING = 6;        // ring stages: Q (2 entries per segment), K and V blocks in MMA issue order
+constexpr int AT_RING = 5;        // ring stages: Q (2 entries per segment), K and V blocks in MMA issue order
 constexpr int AT_PF = 6;          // L2 prefetch distance in blocks
 constexpr int AT_THREADS = 320;   // warp 0 TMA, warp 1 MMA, warps 2..9 softmax/drain (two per TMEM lane quarter)
 constexpr int AT_STAGE_BYTES = AT_KV * AT_HD * 2;   // 32 KB: 4 chunks [64 x 64] SW128 (K/V) or 2 chunks [128 x 64] (Q)
-constexpr int AT_SCR_PITCH = 40;                    // 16-bit elements per scratch row (80 B: 16-byte aligned rows)
-constexpr int AT_SCR_BYTES = 8 * 32 * AT_SCR_PITCH * 2;  // per softmax warp: a 32 x 32 chunk of 16-bit outputs
-constexpr int AT_XCH_BYTES = 2 * AT_ROWS * 4;       // row-sum exchange between the two warps of a row
-constexpr int AT_SMEM = AT_RING * AT_STAGE_BYTES + AT_SCR_BYTES + AT_XCH_BYTES + 256;
+// Output staging: the segment's 128 x 256 result as 16-bit values, four SWIZZLE_128B boxes [128 rows x 64 columns],
+// followed by the row statistics (m[128], l[128], fp32) of a partial result.  The drain only moves O from tensor
+// memory into this tile (thread = row, 16-byte shared-memory stores); from there a head segment stores its rows
+// to o with coalesced 16-byte accesses, a continuation hands the whole tile to the copy engine (one bulk copy into
+// the CTA's scratch slot).  (TMA tensor stores into o were measured at ~1k cycles of issue time each.)
+constexpr int AT_STG_BYTES = AT_ROWS * AT_HD * 2;   // 64 KB
+constexpr int AT_ML_BYTES = 2 * AT_ROWS * 4;
+constexpr int AT_MX_BYTES = 2 * 2 * AT_ROWS * 2;    // row-maximum exchange per block (16-bit, rounded up), double-buffered by block parity
+constexpr int AT_SMEM = AT_RING * AT_STAGE_BYTES + AT_STG_BYTES + AT_ML_BYTES + AT_MX_BYTES + 192;
+static_assert(AT_SMEM <= 232448, "shared memory of one CTA");
 constexpr float AT_RESCALE_THR = 8.0f;              // log2 units
-// partial results of cut items: per CTA slot O [256 cols][128 rows] fp32 (row-contiguous per column: coalesced for
-// thread = row), then m[2][128], l[2][128] (one copy per column half), and 8 ready flags (one per softmax warp)
-constexpr size_t AT_PART_O = (size_t)AT_HD * AT_ROWS;          // floats
-constexpr size_t AT_PART_FLOATS = AT_PART_O + 4 * AT_ROWS;
+constexpr size_t AT_PART_BYTES = AT_STG_BYTES + AT_ML_BYTES;   // scratch slot of a CTA: a copy of staging + statistics
 
 // exp2 on the SFU without the denormal-range fix-up sequence of exp2f (inputs here are <= 2^8)
 __device__ __forceinline__ float ex2_approx(float x) {
@@ -65,14 +68,50 @@ __device__ __forceinline__ int ld_acquire_gpu(const int* p) {
   asm volatile("ld.acquire.gpu.global.b32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
+__device__ __forceinline__ int ld_relaxed_gpu(const int* p) {
+  int v;
+  asm volatile("ld.relaxed.gpu.global.b32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
 __device__ __forceinline__ void st_release_gpu(int* p, int v) {
   asm volatile("st.release.gpu.global.b32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
-__device__ __forceinline__ float ld_cg(const float* p) {  // L2 only: written by another SM during this launch
-  float v;
-  asm volatile("ld.global.cg.f32 %0, [%1];" : "=f"(v) : "l"(p));
-  return v;
+// generic <-> async proxy ordering for global and shared memory alike
+__device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
+// asynchronous copies out of / into shared memory (bulk groups are per thread: the issuing thread also waits)
+__device__ __forceinline__ void tma_store_4d(const CUtensorMap* tm, uint32_t src, int c0, int c1, int c2, int c3) {
+  asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.bulk_group [%0, {%2, %3, %4, %5}], [%1];"
+               ::"l"(tm), "r"(src), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
 }
+__device__ __forceinline__ void bulk_store(void* dst, uint32_t src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+
+__device__ __forceinline__ AttnSeg ld_seg(const AttnSeg* p) {   // read-only table: two 16-byte loads
+  union { AttnSeg s; uint4 u[2]; } v;
+  v.u[0] = __ldg(reinterpret_cast<const uint4*>(p));
+  v.u[1] = __ldg(reinterpret_cast<const uint4*>(p) + 1);
+  return v.s;
+}
+
+// Measurement aid, compiled in only with -DROSA_TRACE: clock64 of pipeline events per CTA, [cta][64]:
+// 0 entry, 1 after the dependency wait, 2 exit; per segment j < 6 at 8 + 8 j: +0 softmax: first S block ready,
+// +1 softmax loop done, +2 next Q copied, +7 last PV done, +3 O out of tensor memory, +4 drain done;
+// +5 MMA: segment start (Q ready), +6 last PV issued
+#ifdef ROSA_TRACE
+__device__ long long g_attn_trace[160 * 64];
+#define AT_TRACE(slot) do { if (lane == 0 && (slot) < 64) g_attn_trace[blockIdx.x * 64 + (slot)] = clock64(); } while (0)
+extern "C" int rosa_trace_attn(long long* host) { return (int)cudaMemcpyFromSymbol(host, g_attn_trace, sizeof(g_attn_trace)); }
+#else
+#define AT_TRACE(slot) do { } while (0)
+#endif
 
 struct AttnMaps {
   CUtensorMap q;    // qkv buffer as [M tokens][8 heads][256]   box {64, 8, 16}
@@ -81,7 +120,7 @@ struct AttnMaps {
 
 __global__ void __launch_bounds__(AT_THREADS, 1)
 k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__ kv_maps, Dims dm, Tables tb,
-          int layer, op16* __restrict__ o, int k_iter, float* __restrict__ part, int* __restrict__ part_flag) {
+          int layer, op16* __restrict__ o, int k_iter, uint8_t* __restrict__ part, int* __restrict__ part_flag) {
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   // this CTA's run of segments in the list of iteration k_iter
   const int* offs = tb.attn_offs + tb.attn_iter[k_iter];
@@ -91,8 +130,8 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
 
   const uint32_t base = smem_u32(smem_raw);  // 1024-byte aligned (SWIZZLE_128B tiles)
   auto stage = [&](int s) { return base + (uint32_t)s * AT_STAGE_BYTES; };
-  const uint32_t scr_base = base + AT_RING * AT_STAGE_BYTES;
-  const uint32_t bars = scr_base + AT_SCR_BYTES + AT_XCH_BYTES;
+  const uint32_t stg = base + AT_RING * AT_STAGE_BYTES;   // output staging (+ statistics right behind it)
+  const uint32_t bars = stg + AT_STG_BYTES + AT_ML_BYTES + AT_MX_BYTES;
   auto full = [&](int s) { return bars + 8u * s; };
   auto empty = [&](int s) { return bars + 8u * (AT_RING + s); };
   auto s_full = [&](int b) { return bars + 8u * (2 * AT_RING + b); };
@@ -101,10 +140,12 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
   auto p_full = [&](int b) { return bars + 8u * (2 * AT_RING + 2 + b); };
   const uint32_t pv_done = bars + 8u * (2 * AT_RING + 4);
   const uint32_t q_ready = bars + 8u * (2 * AT_RING + 5), o_empty = bars + 8u * (2 * AT_RING + 6);
-  const uint32_t tmem_slot = bars + 8u * (2 * AT_RING + 7);
+  const uint32_t part_full = bars + 8u * (2 * AT_RING + 7);   // the partner's partial result has landed in staging
+  const uint32_t tmem_slot = bars + 8u * (2 * AT_RING + 8);
   volatile uint32_t* tmem_slot_ptr = reinterpret_cast<volatile uint32_t*>(smem_raw + (tmem_slot - base));
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (warp == 2) AT_TRACE(0);
 
   if (warp == 0 && lane == 0) {
     prefetch_tensormap(&maps.q);
@@ -115,6 +156,7 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
     mbar_init(pv_done, 1);
     mbar_init(q_ready, 8);
     mbar_init(o_empty, 8);
+    mbar_init(part_full, 1);
     fence_barrier_init();
   }
   if (warp == 1) {
@@ -129,31 +171,63 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
   const uint32_t tmem_s = tmem_base + 256;      // columns [256, 384): S (fp32) / P (bf16 pairs), 2 x 64
   const uint32_t tmem_q = tmem_base + 384;      // columns [384, 512): Q, 256 bf16 per row
 
-  pdl_wait();     // everything above overlapped the previous kernel's tail
-  pdl_trigger();
-
   if (warp == 0) {
     // ------------------------------------------------ TMA producer (whole warp; one lane issues)
     // Ring entries in MMA consumption order: Q (2 entries), K(0), then K(i+1), V(i) for every block.
     uint32_t rp = 0;  // entries issued so far
-    auto acquire = [&]() {
+    AttnSeg nxt = ld_seg(segs + seg_beg);
+    if (lane == 0) {
+      const CUtensorMap* km = kv_maps + ((size_t)nxt.robot * dm.layers + layer) * 2;
+      prefetch_tensormap(km); prefetch_tensormap(km + 1);
+    }
+    // The prefix cache does not depend on the previous kernel: the first segment's K(kb0), K(kb0+1), V(kb0) go out
+    // BEFORE the dependency wait, straight into the ring entries they will be consumed from (2, 3, 4); Q and the
+    // block of the robot's own tokens (written by the QKV GEMM) follow after it.
+    uint32_t pre_mask = 0;
+    {
+      const int nbp = (nxt.len + AT_KV - 1) / AT_KV, n = nxt.kb1 - nxt.kb0;
+      const CUtensorMap* km = kv_maps + ((size_t)nxt.robot * dm.layers + layer) * 2;
+      const int blk[3] = {nxt.kb0, n > 1 ? nxt.kb0 + 1 : nxt.kb0, nxt.kb0};
+      const bool isv[3] = {false, n > 1 ? false : true, true};
+      const int cnt = n > 1 ? 3 : 2;
+      for (int x = 0; x < cnt; ++x)
+        if (blk[x] < nbp) {
+          if (elect_one()) {
+            mbar_expect_tx(full(2 + x), AT_STAGE_BYTES);
+            tma_load_3d(stage(2 + x), isv[x] ? km + 1 : km, full(2 + x), 0, blk[x] * AT_KV, 0);
+          }
+          __syncwarp();
+          pre_mask |= 1u << (2 + x);
+        }
+    }
+    pdl_wait();     // everything above overlapped the previous kernel's tail
+    pdl_trigger();
+    auto acquire = [&](bool& issue) {   // next ring entry; issue = false if it was filled before the wait
       const int s = (int)(rp % AT_RING);
-      mbar_wait_idle(empty(s), ((rp / AT_RING) & 1) ^ 1);
+      issue = !(rp < AT_RING && ((pre_mask >> rp) & 1u));
+      if (issue) mbar_wait_idle(empty(s), ((rp / AT_RING) & 1) ^ 1);
       ++rp;
       return s;
     };
     for (int si = seg_beg; si < seg_end; ++si) {
-      const AttnSeg sg = segs[si];
-      const int p = sg.p, robot = tb.ids[p], L = tb.rlen[robot];
+      const AttnSeg sg = nxt;
+      if (si + 1 < seg_end) {   // the next record and its robot's tensor maps are fetched a whole segment ahead
+        nxt = ld_seg(segs + si + 1);
+        if (lane == 0 && nxt.robot != sg.robot) {
+          const CUtensorMap* km = kv_maps + ((size_t)nxt.robot * dm.layers + layer) * 2;
+          prefetch_tensormap(km); prefetch_tensormap(km + 1);
+        }
+      }
+      const int p = sg.p, L = sg.len;
       const int nbp = (L + AT_KV - 1) / AT_KV;  // prefix blocks; block nbp = the robot's own tokens
-      const CUtensorMap* kmap = kv_maps + ((size_t)robot * dm.layers + layer) * 2;
+      const CUtensorMap* kmap = kv_maps + ((size_t)sg.robot * dm.layers + layer) * 2;
       const CUtensorMap* vmap = kmap + 1;
       const int tok0 = p * dm.H + sg.tt * AT_TOK;
-      if (lane == 0) { prefetch_tensormap(kmap); prefetch_tensormap(vmap); }
       // one TMA per 64-key block: 3-D maps (64 columns, rows, 4 column chunks) land as [chunk][row][128 B]
       auto load_kv = [&](int i, bool is_v) {
-        const int s = acquire();
-        if (elect_one()) {
+        bool issue;
+        const int s = acquire(issue);
+        if (issue && elect_one()) {
           mbar_expect_tx(full(s), AT_STAGE_BYTES);
           if (i == nbp) tma_load_3d(stage(s), &maps.own, full(s), 0, p * dm.H, (dm.q_n + (is_v ? AT_HD : 0)) / 64);
           else tma_load_3d(stage(s), is_v ? vmap : kmap, full(s), 0, i * AT_KV, 0);
@@ -161,7 +235,8 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
         __syncwarp();
       };
       for (int e = 0; e < 2; ++e) {
-        const int s = acquire();
+        bool issue;
+        const int s = acquire(issue);
         if (elect_one()) {
           mbar_expect_tx(full(s), AT_STAGE_BYTES);
           for (int c = 0; c < 2; ++c) tma_load_3d(stage(s) + c * (AT_ROWS * 128), &maps.q, full(s), (2 * e + c) * 64, 0, tok0);
@@ -185,17 +260,27 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
     }
   } else if (warp == 1) {
     // ------------------------------------------------ MMA issuer (whole warp; one lane issues)
+    pdl_wait();
+    pdl_trigger();
     constexpr uint32_t idesc_s = make_idesc_bf16(AT_ROWS, AT_KV);
     constexpr uint32_t idesc_o = make_idesc_bf16(AT_ROWS, AT_HD, /*b_mn_major=*/true);
     uint32_t rp = 0;  // ring entries consumed
     uint32_t g = 0;   // key blocks issued so far in this CTA (selects the S/P buffer and the barrier parities)
     uint32_t j = 0;   // segments started
+#ifdef ROSA_TRACE
+    long long w_full = 0, w_p = 0;   // cycles this warp waited for ring data / for the softmax warps
+#define AT_WAIT(acc, stmt) do { const long long t_ = clock64(); stmt; acc += clock64() - t_; } while (0)
+#else
+#define AT_WAIT(acc, stmt) do { stmt; } while (0)
+#endif
+    AttnSeg nxt = ld_seg(segs + seg_beg);
     for (int si = seg_beg; si < seg_end; ++si, ++j) {
-      const AttnSeg sg = segs[si];
+      const AttnSeg sg = nxt;
+      if (si + 1 < seg_end) nxt = ld_seg(segs + si + 1);
       const int n = sg.kb1 - sg.kb0;
       auto issue_s = [&](uint32_t gi) {  // S(gi) = Q K^T into S buffer gi&1 (overwrites P(gi-2), consumed by PV(gi-2))
         const int s = (int)(rp % AT_RING);
-        mbar_wait(full(s), (rp / AT_RING) & 1);
+        AT_WAIT(w_full, mbar_wait(full(s), (rp / AT_RING) & 1));
         ++rp;
         tc_fence_after();
         if (elect_one()) {
@@ -212,6 +297,7 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
       // Q of this segment is in tensor memory (softmax warps); its two ring entries are free again
       mbar_wait(q_ready, j & 1);
       tc_fence_after();
+      AT_TRACE(8 + 8 * j + 5);
       if (elect_one()) {
         mbar_arrive(empty((int)(rp % AT_RING)));
         mbar_arrive(empty((int)((rp + 1) % AT_RING)));
@@ -223,10 +309,10 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
         const uint32_t gi = g + i;
         if (i + 1 < n) issue_s(gi + 1);
         const int s = (int)(rp % AT_RING);
-        mbar_wait(full(s), (rp / AT_RING) & 1);
+        AT_WAIT(w_full, mbar_wait(full(s), (rp / AT_RING) & 1));
         ++rp;
-        if (i == 0 && j > 0) mbar_wait(o_empty, (j - 1) & 1);  // the previous segment's O has been drained
-        mbar_wait(p_full(gi & 1), (gi >> 1) & 1);
+        if (i == 0 && j > 0) mbar_wait(o_empty, (j - 1) & 1);  // the previous segment's O has left tensor memory
+        AT_WAIT(w_p, mbar_wait(p_full(gi & 1), (gi >> 1) & 1));
         tc_fence_after();
         if (elect_one()) {
 #pragma unroll
@@ -234,30 +320,43 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
             // A = P [128 x 64] bf16 in TMEM (8 columns per 16 keys); B = V block, MN-major: 4 hd chunks
             // 8192 B apart (LBO), 8-key groups 1024 B apart (SBO); 16 keys per MMA = 2048 B
             const uint64_t b_desc = make_sdesc_mn128(stage(s) + kk * 2048, AT_KV * 128, 1024);
-            umma_bf16_ts(tmem_o, tmem_s + (gi & 1) * AT_KV + kk * 8, b_desc, idesc_o, (i | kk) != 0);
+            // P of keys 16 kk .. 16 kk + 15: columns 8 (kk & 1) of the half (kk >> 1) that wrote it (32 columns apart)
+            umma_bf16_ts(tmem_o, tmem_s + (gi & 1) * AT_KV + (kk >> 1) * 32 + (kk & 1) * 8, b_desc, idesc_o, (i | kk) != 0);
           }
           umma_commit(empty(s));
           umma_commit(pv_done);
         }
         __syncwarp();
       }
+      AT_TRACE(8 + 8 * j + 6);
       g += n;
     }
+#ifdef ROSA_TRACE
+    if (lane == 0) { g_attn_trace[blockIdx.x * 64 + 3] = w_full; g_attn_trace[blockIdx.x * 64 + 4] = w_p; }
+#endif
   } else {
     // ---------------------------------------------------------- softmax + drain warps (2..9)
     // Two warps per TMEM lane quarter: a query row's 64 scores of a block are split 32 / 32 between
     // warp w (half 0) and warp w + 4 (half 1).  Both read all 64 scores for the row maximum
     // (so both take the same rescale decision) and keep separate partial row sums until the end.
-    const int q = warp & 3, half = (warp - 2) >> 2, sw = warp - 2;
+    pdl_wait();
+    pdl_trigger();
+    if (warp == 2) AT_TRACE(1);
+    const int q = warp & 3, half = (warp - 2) >> 2;
     const int r = q * 32 + lane;                       // query row of this thread
     const uint32_t lane_off = (uint32_t)(q * 32) << 16;
-    float* xch = reinterpret_cast<float*>(smem_raw + (AT_RING * AT_STAGE_BYTES + AT_SCR_BYTES));  // [2 halves][128]
-    const uint32_t scr = scr_base + (uint32_t)sw * (32 * AT_SCR_PITCH * 2);
+    float* ml = reinterpret_cast<float*>(smem_raw + (AT_RING * AT_STAGE_BYTES + AT_STG_BYTES));   // m[128], l[128]
+    float* xch = ml;   // the drain's row-sum exchange [2 halves][128] uses the same kilobyte (see the drain)
+    uint16_t* mx = reinterpret_cast<uint16_t*>(ml + 2 * AT_ROWS);                              // [2 parities][2 halves][128]
     const float c_log2 = rsqrtf((float)AT_HD) * 1.4426950408889634f;  // (1/sqrt(hd)) * log2(e)
-    const int lr = lane >> 3, lc = (lane & 7) * 4;
+    const bool issuer = warp == 2 && lane == 0;        // the thread that owns this CTA's bulk-copy groups
     // Q of a segment: shared memory (SW128 chunks of [128 rows x 128 B]) -> tensor memory, thread = row; this half's
     // two chunks are one ring entry (rq = ring position of the segment's first entry).  Called when every S MMA of
     // the previous segment has completed (its last s_full was waited on), so tmem_q is free.
+    auto q_landed = [&](uint32_t rq) {   // warp-uniform: has this half's ring entry of the segment's Q arrived?
+      const uint32_t e = rq + half;
+      return __all_sync(0xffffffffu, mbar_try_wait(full((int)(e % AT_RING)), (e / AT_RING) & 1)) != 0;
+    };
     auto copy_q = [&](uint32_t rq) {
       const uint32_t e = rq + half;
       const int s = (int)(e % AT_RING);
@@ -279,53 +378,84 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
       if (lane == 0) mbar_arrive(q_ready);
     };
     uint32_t rp = 0, g = 0;
+    bool flag_owed = false;     // issuer: a continuation's bulk copy is in flight; its ready flag is still to be set
+    auto settle = [&]() {       // issuer: staging is no longer being read; a pending partial result gets published
+      if (flag_owed) {
+        bulk_wait_all();
+        fence_proxy_async_all();
+        st_release_gpu(part_flag + blockIdx.x, 1);
+        flag_owed = false;
+      } else {
+        bulk_wait_read();
+      }
+    };
+    auto fetch_partial = [&](int cta) {   // issuer: the partial result CTA `cta` has published -> staging
+      settle();
+      (void)ld_acquire_gpu(part_flag + cta);
+      fence_proxy_async_all();
+      mbar_expect_tx(part_full, (uint32_t)AT_PART_BYTES);
+      bulk_load(stg, part + (size_t)cta * AT_PART_BYTES, (uint32_t)AT_PART_BYTES, part_full);
+    };
+    AttnSeg nxt = ld_seg(segs + seg_beg);
     copy_q(0);
     for (int si = seg_beg; si < seg_end; ++si) {
-      const AttnSeg sg = segs[si];
-      const int p = sg.p, L = tb.rlen[tb.ids[p]], nbp = (L + AT_KV - 1) / AT_KV;
+      const AttnSeg sg = nxt;
+      if (si + 1 < seg_end) nxt = ld_seg(segs + si + 1);
+      const int p = sg.p, L = sg.len, nbp = (L + AT_KV - 1) / AT_KV;
       const int n = sg.kb1 - sg.kb0;
+      const bool merge = sg.n_part > 0;   // head segment of a cut item: always the last entry of the list
       rp += 2 + 2 * n;   // ring position of the next segment's Q
+      bool part_issued = false;           // issuer: the partner's partial result is on its way into staging
       float m_ref = -INFINITY, l_sum = 0.f;            // m_ref in log2 units; l_sum: this half's part
       for (int i = 0; i < n; ++i) {
         const uint32_t gi = g + i;
         const int sb = gi & 1, kb = sg.kb0 + i;
         const int n_tot = kb == nbp ? dm.H : min(AT_KV, L - kb * AT_KV);
-        const int n_valid = n_tot - half * 32, n_other = n_tot - (half ^ 1) * 32;  // valid columns of this / the other half
+        const int n_valid = n_tot - half * 32;  // valid columns of this half
+        // Housekeeping of the asynchronous copies by the issuing thread, off the critical path.
+        //  * second block (or the last one): the previous drain's copy out of staging is (almost certainly) complete,
+        //    so a continuation's partial result is in global memory: publish it;
+        //  * last block: staging may be overwritten by this segment's drain (every warp's drain follows this thread's
+        //    p_full arrival of this block through pv_done);
+        //  * head of a cut item: as soon as the other CTA has published its partial, pull it into staging (the drain
+        //    merges it in place).  The flag is polled with a relaxed load issued here and looked at after the block.
+        int flag_seen = 0;
+        if (issuer) {
+          if (i == n - 1 || i == 1) settle();
+          if (merge && !part_issued) flag_seen = ld_relaxed_gpu(part_flag + sg.part0);
+        }
+        __syncwarp();
         mbar_wait(s_full(sb), (gi >> 1) & 1);
         tc_fence_after();
-        // Both warps of a row read all 64 scores for the row maximum (so they take the same rescale
-        // decision without an exchange); each exponentiates only its own 32.
+        if (warp == 2 && i == 0) AT_TRACE(8 + 8 * (si - seg_beg) + 0);
+        // Each warp of a row's pair reads only its own 32 scores; the row maximum of the block is exchanged through
+        // shared memory (so both take the same rescale decision).  P is stored over this warp's OWN score columns
+        // (P of half h at columns 32 h .. 32 h + 15 of the S buffer), so neither warp ever reads a column the other
+        // overwrites, however far apart the two run.
         float sc[32];
         float m_blk;
         {
-          uint32_t r0[32], r1[32];
+          uint32_t r0[32];
           tmem_ld32(tmem_s + lane_off + sb * AT_KV + half * 32, r0);
-          tmem_ld32(tmem_s + lane_off + sb * AT_KV + (half ^ 1) * 32, r1);
           tmem_ld_wait();
-          // P(gi) is written IN PLACE over S(gi), and each warp of a row's pair has just read the other's scores
-          // too: neither may store its P before both have read (the two were released by the same s_full, so
-          // this barrier costs little; without it a warp held up for more than a block - by a merge wait, say -
-          // reads scores its partner has already overwritten)
-          named_bar_sync(5 + q, 64);
 #pragma unroll
           for (int c = 0; c < 32; ++c) sc[c] = __uint_as_float(r0[c]);
-          float mo = -INFINITY;
-          // warp-uniform branches; only the last prefix block and the own-token block are ragged
-          if (n_valid < 32) {
+          if (n_valid < 32) {  // warp-uniform; only the last prefix block and the own-token block are ragged
 #pragma unroll
             for (int c = 0; c < 32; ++c) sc[c] = c < n_valid ? sc[c] : -INFINITY;
           }
-          if (n_other < 32) {
+          float mo = sc[0];
 #pragma unroll
-            for (int c = 0; c < 32; ++c) mo = fmaxf(mo, c < n_other ? __uint_as_float(r1[c]) : -INFINITY);
-          } else {
-#pragma unroll
-            for (int c = 0; c < 32; ++c) mo = fmaxf(mo, __uint_as_float(r1[c]));
-          }
-          m_blk = mo;
+          for (int c = 1; c < 32; ++c) mo = fmaxf(mo, sc[c]);
+          // exchanged as the smallest bf16 >= mo (both warps use the rounded values, their own included, so they
+          // agree exactly; a reference maximum slightly above the true one is harmless)
+          const uint32_t mb = __float_as_uint(mo);
+          const uint16_t up = (uint16_t)((mo >= 0.f ? mb + 0xffffu : mb) >> 16);
+          mx[(gi & 1) * (2 * AT_ROWS) + half * AT_ROWS + r] = up;
+          named_bar_sync(5 + q, 64);
+          const uint16_t other = mx[(gi & 1) * (2 * AT_ROWS) + (half ^ 1) * AT_ROWS + r];
+          m_blk = fmaxf(__uint_as_float((uint32_t)up << 16), __uint_as_float((uint32_t)other << 16));
         }
-#pragma unroll
-        for (int c = 0; c < 32; ++c) m_blk = fmaxf(m_blk, sc[c]);
         m_blk *= c_log2;
         float factor = 1.f;
         if (m_blk > m_ref + AT_RESCALE_THR) {            // first block always lands here
@@ -361,125 +491,147 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
             tmem_st32(tmem_o + lane_off + c * 32, rr);
           }
         }
-        // P row r, this half's 32 keys (16 columns of bf16 pairs) over the start of S(gi): the A operand of PV(gi)
-        tmem_st16(tmem_s + lane_off + sb * AT_KV + half * 16, pk);
+        // P row r, this half's 32 keys (16 columns of bf16 pairs) over this warp's own scores: the A operand of PV(gi)
+        tmem_st16(tmem_s + lane_off + sb * AT_KV + half * 32, pk);
         tmem_st_wait();
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(p_full(sb));  // 256 arrivals on one barrier would serialise on the critical path
+        if (issuer && flag_seen != 0) { fetch_partial(sg.part0); part_issued = true; }
+        __syncwarp();
       }
       g += n;
-      // The next segment's Q goes into tensor memory BEFORE this segment's O is drained: its first two S blocks then
-      // run on the tensor pipe while these warps drain.
-      if (si + 1 < seg_end) copy_q(rp);
-      // ------------------------------------------------ drain: O (+ partials of the item's other segments) -> o,
-      // or this segment's partial -> scratch.  Row r = (token jj, head a) with r = jj * 8 + a; each half owns 128
-      // of the 256 columns.
+      if (warp == 2) AT_TRACE(8 + 8 * (si - seg_beg) + 1);
+      // The next segment's Q goes into tensor memory BEFORE this segment's O is drained (if it has landed): its first
+      // two S blocks then run on the tensor pipe while these warps drain.
+      bool q_pending = si + 1 < seg_end;
+      if (q_pending && q_landed(rp)) { copy_q(rp); q_pending = false; }
+      if (warp == 2) AT_TRACE(8 + 8 * (si - seg_beg) + 2);
+      // ------------------------------------------------ drain.  Row r = (token jj, head a) with r = jj * 8 + a; each
+      // half owns 128 of the 256 columns.  O leaves tensor memory as 16-bit values into the staging tile (normalised
+      // by the row sum; a head segment first adds the other CTA's partial result, which is already in staging, in
+      // place), O is released, and one thread hands the tile to the copy engine.
+      if (merge && issuer && !part_issued) {   // the other CTA has not published yet: wait for it here
+        for (uint32_t spin = 0; ld_acquire_gpu(part_flag + sg.part0) == 0; ++spin) {
+          __nanosleep(64);
+          if (spin > (1u << 24)) __trap();
+        }
+        fetch_partial(sg.part0);
+      }
+      __syncwarp();
       mbar_wait(pv_done, (g - 1) & 1);
       tc_fence_after();
+      if (warp == 2) AT_TRACE(8 + 8 * (si - seg_beg) + 7);
+      // The statistics kilobyte behind the staging tile serves three purposes in turn: a merge reads the other
+      // segment's (m, l) from it, then the two warps of a row exchange their partial row sums through it, then a
+      // continuation leaves its own (m, l) there for the bulk copy.  The pair barriers keep the three apart.
+      float m_c = 0.f, l_c = 0.f;
+      if (merge) {
+        mbar_wait(part_full, 0);   // at most one merge per CTA (the last entry of its list)
+        m_c = ml[r];
+        l_c = ml[AT_ROWS + r];
+        named_bar_sync(1 + q, 64);
+      }
       xch[half * AT_ROWS + r] = l_sum;
       named_bar_sync(1 + q, 64);
       float l_tot = l_sum + xch[(half ^ 1) * AT_ROWS + r];
-      named_bar_sync(1 + q, 64);   // xch is reused by the next segment
-
-      if (sg.n_part < 0) {
-        // not the head segment: leave (O, m, l) for the CTA that holds the head
-        float* slot = part + (size_t)blockIdx.x * AT_PART_FLOATS;
-#pragma unroll 1
+      named_bar_sync(1 + q, 64);
+      float w_own = 1.f / l_tot, w_part = 0.f;
+      if (merge) {
+        const float m_new = fmaxf(m_ref, m_c);
+        const float f_own = ex2_approx(m_ref - m_new), f_c = ex2_approx(m_c - m_new);
+        const float l_new = l_tot * f_own + l_c * f_c;
+        w_own = f_own / l_new;           // applied to this segment's unnormalised O
+        w_part = l_c * f_c / l_new;      // applied to the other segment's normalised O
+      } else if (sg.n_part < 0 && half == 0) {
+        ml[r] = m_ref;                   // a continuation leaves its statistics behind the staging tile
+        ml[AT_ROWS + r] = l_tot;
+      }
+      {
+        uint32_t rbuf[2][32];  // the next chunk's TMEM load is in flight while this one is converted and stored
+        tmem_ld32(tmem_o + lane_off + (half * 4) * 32, rbuf[0]);
+#pragma unroll
         for (int cc = 0; cc < 4; ++cc) {
-          const int c = half * 4 + cc;
-          uint32_t rr[32];
-          tmem_ld32(tmem_o + lane_off + c * 32, rr);
+          const int c = half * 4 + cc;     // 32-column chunk; box c >> 1, 16-byte units (c & 1) * 4 .. + 3 of row r
+          const uint32_t rowaddr = stg + (uint32_t)(c >> 1) * (AT_ROWS * 128) + (uint32_t)r * 128;
+          uint32_t (&rr)[32] = rbuf[cc & 1];
           tmem_ld_wait();
-#pragma unroll
-          for (int e = 0; e < 32; ++e) slot[(size_t)(c * 32 + e) * AT_ROWS + r] = __uint_as_float(rr[e]);
-        }
-        slot[AT_PART_O + half * AT_ROWS + r] = m_ref;
-        slot[AT_PART_O + (2 + half) * AT_ROWS + r] = l_tot;
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(o_empty);
-        __threadfence();
-        __syncwarp();
-        if (lane == 0) st_release_gpu(part_flag + blockIdx.x * 8 + sw, 1);
-        __syncwarp();
-      } else {
-        float f_own = 1.f;
-        float fc[3] = {0.f, 0.f, 0.f};   // at most 3 other segments are merged per pass (attn_build_list guarantees <= 3)
-        const int np = sg.n_part;
-        if (np > 0) {
-          float mc[3] = {-INFINITY, -INFINITY, -INFINITY}, lcs[3] = {0.f, 0.f, 0.f};
-          float m_new = m_ref;
-          for (int t = 0; t < np; ++t) {
-            const int c_id = sg.part0 + t;
-            const int* fl = part_flag + c_id * 8 + sw;
-            for (uint32_t spin = 0; ld_acquire_gpu(fl) == 0; ++spin) {
-              __nanosleep(64);
-              if (spin > (1u << 24)) __trap();
-            }
-            __syncwarp();   // the lanes leave the spin at different polls; the TMEM loads below are .sync.aligned
-            const float* slot = part + (size_t)c_id * AT_PART_FLOATS;
-            mc[t] = ld_cg(slot + AT_PART_O + half * AT_ROWS + r);
-            lcs[t] = ld_cg(slot + AT_PART_O + (2 + half) * AT_ROWS + r);
-            m_new = fmaxf(m_new, mc[t]);
-          }
-          f_own = ex2_approx(m_ref - m_new);
-          l_tot *= f_own;
-          for (int t = 0; t < np; ++t) { fc[t] = ex2_approx(mc[t] - m_new); l_tot += lcs[t] * fc[t]; }
-        }
-        const float inv = 1.f / l_tot;
-        size_t orow[8];   // output row offsets of the 8 rows this lane stores per chunk; -1 = padding row
-#pragma unroll
-        for (int x = 0; x < 8; ++x) {
-          const int row = q * 32 + x * 4 + lr, jj = sg.tt * AT_TOK + (row >> 3);
-          orow[x] = jj < dm.H ? (size_t)(p * dm.H + jj) * dm.q_n + (row & 7) * AT_HD + lc : (size_t)-1;
-        }
-#pragma unroll 1
-        for (int cc = 0; cc < 4; ++cc) {
-          const int c = half * 4 + cc;
+          if (cc + 1 < 4) tmem_ld32(tmem_o + lane_off + (c + 1) * 32, rbuf[(cc + 1) & 1]);
           float v[32];
-          {
-            uint32_t rr[32];
-            tmem_ld32(tmem_o + lane_off + c * 32, rr);
-            tmem_ld_wait();
 #pragma unroll
-            for (int e = 0; e < 32; ++e) v[e] = __uint_as_float(rr[e]) * f_own;
-          }
+          for (int e = 0; e < 32; ++e) v[e] = __uint_as_float(rr[e]) * w_own;
           if (cc == 3) {  // this warp has read all of its part of O
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(o_empty);
           }
-          for (int t = 0; t < np; ++t) {
-            const float* src = part + (size_t)(sg.part0 + t) * AT_PART_FLOATS + (size_t)(c * 32) * AT_ROWS + r;
-            const float f = fc[t];
-#pragma unroll
-            for (int e = 0; e < 32; ++e) v[e] = fmaf(ld_cg(src + (size_t)e * AT_ROWS), f, v[e]);
-          }
-          // 16-bit outputs transposed through the warp's scratch: thread = row writes 64 B, then 8 lanes x 4 columns per row
 #pragma unroll
           for (int x = 0; x < 4; ++x) {
-            const uint32_t a0 = pack_op2(v[8 * x + 0] * inv, v[8 * x + 1] * inv, dm.fp16), a1 = pack_op2(v[8 * x + 2] * inv, v[8 * x + 3] * inv, dm.fp16);
-            const uint32_t a2 = pack_op2(v[8 * x + 4] * inv, v[8 * x + 5] * inv, dm.fp16), a3 = pack_op2(v[8 * x + 6] * inv, v[8 * x + 7] * inv, dm.fp16);
-            asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(scr + lane * (AT_SCR_PITCH * 2) + x * 16), "r"(a0), "r"(a1), "r"(a2), "r"(a3) : "memory");
+            const uint32_t addr = rowaddr + (uint32_t)((((c & 1) * 4 + x) ^ (r & 7)) << 4);
+            if (merge) {
+              uint32_t u[4];
+              asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(u[0]), "=r"(u[1]), "=r"(u[2]), "=r"(u[3]) : "r"(addr));
+#pragma unroll
+              for (int y = 0; y < 4; ++y) {
+                const uint16_t lo = (uint16_t)(u[y] & 0xffffu), hi = (uint16_t)(u[y] >> 16);
+                v[8 * x + 2 * y] = fmaf(op2f(lo, dm.fp16), w_part, v[8 * x + 2 * y]);
+                v[8 * x + 2 * y + 1] = fmaf(op2f(hi, dm.fp16), w_part, v[8 * x + 2 * y + 1]);
+              }
+            }
+            const uint32_t a0 = pack_op2(v[8 * x + 0], v[8 * x + 1], dm.fp16), a1 = pack_op2(v[8 * x + 2], v[8 * x + 3], dm.fp16);
+            const uint32_t a2 = pack_op2(v[8 * x + 4], v[8 * x + 5], dm.fp16), a3 = pack_op2(v[8 * x + 6], v[8 * x + 7], dm.fp16);
+            asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a0), "r"(a1), "r"(a2), "r"(a3) : "memory");
           }
-          __syncwarp();
-          uint2 ov[8];
-#pragma unroll
-          for (int x = 0; x < 8; ++x)
-            asm volatile("ld.shared.v2.b32 {%0, %1}, [%2];" : "=r"(ov[x].x), "=r"(ov[x].y) : "r"(scr + (x * 4 + lr) * (AT_SCR_PITCH * 2) + lc * 2));
-#pragma unroll
-          for (int x = 0; x < 8; ++x)
-            if (orow[x] != (size_t)-1) *reinterpret_cast<uint2*>(o + orow[x] + c * 32) = ov[x];
-          __syncwarp();
-        }
-        if (np > 0) {  // the slots are free for the next launch
-          __syncwarp();
-          if (lane == 0)
-            for (int t = 0; t < np; ++t) part_flag[(sg.part0 + t) * 8 + sw] = 0;
         }
       }
+      if (warp == 2) AT_TRACE(8 + 8 * (si - seg_beg) + 3);
+      if (sg.n_part < 0) {
+        // continuation: the tile and its statistics go, verbatim, into this CTA's scratch slot: one bulk copy
+        fence_proxy_async();              // this thread's staging writes -> visible to the copy engine
+        named_bar_sync(9, 256);           // all eight warps have written their part of the tile
+        if (issuer) {
+          bulk_store(part + (size_t)blockIdx.x * AT_PART_BYTES, stg, (uint32_t)AT_PART_BYTES);
+          bulk_commit();
+          flag_owed = true;
+        }
+      } else {
+        // head: this warp's 32 rows x 128 columns back out of staging, 8 lanes x 16 bytes per row (one 128-byte row
+        // segment of o per 8 lanes, 4 rows per instruction); rows of tokens >= H are padding and are not stored
+        __syncwarp();
+        const int lr = lane >> 3, lu = lane & 7;
+#pragma unroll
+        for (int bb = 0; bb < 2; ++bb) {
+          const int b = half * 2 + bb;
+          uint4 ov[8];
+#pragma unroll
+          for (int x = 0; x < 8; ++x) {
+            const int row = q * 32 + x * 4 + lr;
+            const uint32_t addr = stg + (uint32_t)b * (AT_ROWS * 128) + (uint32_t)row * 128 + (uint32_t)((lu ^ (row & 7)) << 4);
+            asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(ov[x].x), "=r"(ov[x].y), "=r"(ov[x].z), "=r"(ov[x].w) : "r"(addr));
+          }
+#pragma unroll
+          for (int x = 0; x < 8; ++x) {
+            const int row = q * 32 + x * 4 + lr, jj = sg.tt * AT_TOK + (row >> 3);
+            if (jj < dm.H)
+              *reinterpret_cast<uint4*>(o + (size_t)(p * dm.H + jj) * dm.q_n + (row & 7) * AT_HD + b * 64 + lu * 8) = ov[x];
+          }
+        }
+        if (merge) {   // every warp is done with the partner's data once it has left the drain loop: free the slot
+          named_bar_sync(9, 256);
+          if (issuer) st_release_gpu(part_flag + sg.part0, 0);
+        }
+      }
+      if (q_pending) copy_q(rp);
+      if (warp == 2) AT_TRACE(8 + 8 * (si - seg_beg) + 4);
     }
+    if (issuer) {   // nothing of this CTA's may be in flight when it exits
+      bulk_wait_all();
+      if (flag_owed) {
+        fence_proxy_async_all();
+        st_release_gpu(part_flag + blockIdx.x, 1);
+      }
+    }
+    if (warp == 2) AT_TRACE(2);
   }
   tc_fence_before();
   __syncthreads();
@@ -492,16 +644,16 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
 // ------------------------------------------------------------------ host side
 bool tc_attn_supported(const Dims& dm) { return dm.hd == AT_HD && dm.nq == 8 && dm.nkv == 1; }
 size_t tc_attn_map_bytes() { return sizeof(CUtensorMap); }
-size_t tc_attn_part_bytes(int n_cta) { return (size_t)n_cta * AT_PART_FLOATS * sizeof(float); }
+size_t tc_attn_part_bytes(int n_cta) { return (size_t)n_cta * AT_PART_BYTES; }
 int tc_attn_tiles(const Dims& dm) { return (dm.H + AT_TOK - 1) / AT_TOK; }
 
 // Stream-K work list of one Euler iteration: the first `n_active` robots (internal order) with prefix lengths
 // len[p]; item (p, tt) has ceil(len/64) + 1 key blocks; every segment costs its blocks + kSegOvh units (Q load,
 // drain).  The concatenated items are cut into equal shares for `n_cta` CTAs (fewer when there is little work:
-// a share is at least kMinShare units); no segment is shorter than kMinSeg blocks and no item has more than 4
-// segments.  offs[c] .. offs[c+1] = segments of CTA c (offs has n_cta + 1 entries; CTAs without work get none).
+// a share is at least kMinShare units); no segment is shorter than kMinSeg blocks and no item has more than 2
+// segments (the head merges at most one partial result).  offs[c] .. offs[c+1] = segments of CTA c (offs has n_cta + 1 entries; CTAs without work get none).
 int attn_build_list(const Dims& dm, int n_active, const int* len, int n_cta, std::vector<AttnSeg>& segs, int* offs) {
-  constexpr double kSegOvh = 2.0, kMinShare = 6.0;
+  constexpr double kSegOvh = 4.0, kMinShare = 8.0;
   constexpr int kMinSeg = 2;
   const int tpr = tc_attn_tiles(dm);
   const size_t seg0 = segs.size();
@@ -530,7 +682,7 @@ int attn_build_list(const Dims& dm, int n_active, const int* len, int n_cta, std
         const int rem = nb - kb;
         const double room = target - acc;
         int take = rem;
-        if (cta + 1 < used && rem + kSegOvh > room + 0.5 && n_seg < 3) {
+        if (cta + 1 < used && rem + kSegOvh > room + 0.5 && n_seg < 1) {
           take = (int)std::floor(room - kSegOvh + 0.5);
           if (take < kMinSeg) {            // not worth starting here: the next CTA takes it
             if (acc > 0.0) { next_cta(kb > 0); continue; }
@@ -538,9 +690,9 @@ int attn_build_list(const Dims& dm, int n_active, const int* len, int n_cta, std
           }
           if (rem - take < kMinSeg) take = rem;   // no crumbs at the end either
         }
-        AttnSeg sg;
-        sg.p = p; sg.tt = (int16_t)tt; sg.kb0 = (int16_t)kb; sg.kb1 = (int16_t)(kb + take);
-        sg.n_part = kb == 0 ? 0 : -1; sg.part0 = -1; sg.pad = 0;
+        AttnSeg sg{};
+        sg.p = p; sg.robot = p; sg.len = len[p]; sg.tt = (int16_t)tt; sg.kb0 = (int16_t)kb; sg.kb1 = (int16_t)(kb + take);
+        sg.n_part = kb == 0 ? 0 : -1; sg.part0 = -1;
         if (kb > 0) {  // a continuation is the first entry of a CTA's list; the head segment collects it
           segs[head].n_part += 1;
           if (segs[head].part0 < 0) segs[head].part0 = (int16_t)cta;
@@ -569,7 +721,7 @@ bool tc_attn_make_prefix_maps(void* out2, const bf16* k, const bf16* v, int len,
 }
 
 cudaError_t launch_attn_tc(const Dims& dm, const Tables& tb, int layer, const bf16* qkv, op16* o, int k_iter,
-                           int M, const void* d_kv_maps, float* part, int* part_flag, int n_cta, cudaStream_t s) {
+                           int M, const void* d_kv_maps, void* part, int* part_flag, int n_cta, cudaStream_t s) {
   static bool configured = false;
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(k_attn_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, AT_SMEM);
@@ -590,7 +742,7 @@ cudaError_t launch_attn_tc(const Dims& dm, const Tables& tb, int layer, const bf
     if (!encode_tmap(&maps.own, qkv, 3, dims, strides, box)) return cudaErrorInvalidValue;
   }
   return launch_k(k_attn_tc, dim3(n_cta), dim3(AT_THREADS), AT_SMEM, s, maps, (const CUtensorMap*)d_kv_maps, dm,
-                  tb, layer, o, k_iter, part, part_flag);
+                  tb, layer, o, k_iter, (uint8_t*)part, part_flag);
 }
 
 }  // namespace rosa

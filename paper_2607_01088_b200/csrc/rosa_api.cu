@@ -101,8 +101,8 @@ struct rosa_expert {
   size_t off_ids, off_src, off_t0, off_dt, off_ns, off_mact, off_ptrs, off_aiter, off_aoffs, off_asegs;
   size_t seg_cap = 0;              // capacity of the attention segment table (entries)
   int n_cta = 0;                   // CTAs of the persistent attention kernel (= SMs of the device)
-  float* attn_part = nullptr;      // per-CTA partial (O, m, l) of items cut between CTAs
-  int* attn_flag = nullptr;        // [n_cta][8] ready flags of those partials
+  void* attn_part = nullptr;       // per-CTA partial (O, m, l) of items cut between CTAs
+  int* attn_flag = nullptr;        // [n_cta] ready flags of those partials
   int64_t graph_captures = 0;      // graphs captured so far (rosa_debug_graph_captures)
   std::map<GraphKey, cudaGraphExec_t> graphs;
   std::map<GraphKey, int64_t> graph_launches;
@@ -706,6 +706,7 @@ static rosa_status_t denoise_impl(rosa_expert* e, int batch, const int32_t* ids,
       ++n_lists;
     }
     for (int k = nmax; k < e->cfg.max_steps; ++k) h_iter[k] = 0;
+    for (AttnSeg& sg : segs) sg.robot = h_ids[sg.p];
     if (segs.size() > e->seg_cap) { set_error("attention work list overflow"); return ROSA_ERR_CAPACITY; }
     memcpy(hs + e->off_asegs, segs.data(), segs.size() * sizeof(AttnSeg));
     copy_bytes = e->off_asegs + segs.size() * sizeof(AttnSeg);

@@ -50,11 +50,14 @@ struct Tables {
 // One entry of a CTA's attention work list: key blocks [kb0, kb1) of item (robot position p, token tile tt).
 // n_part >= 0: head segment (kb0 = 0): writes the output after merging the partials of CTAs part0 .. part0 + n_part - 1;
 // n_part < 0: continuation: leaves its partial (O, m, l) in the scratch slot of its CTA.
+// The record carries everything a role needs about the item (robot id, prefix length), so that walking the list
+// costs one 32-byte load per segment, issued a segment ahead, instead of a chain of dependent table lookups.
 struct AttnSeg {
-  int32_t p;
-  int16_t tt, kb0, kb1, n_part, part0, pad;
+  int32_t p, robot, len;
+  int16_t tt, kb0, kb1, n_part, part0, pad0;
+  int32_t pad1, pad2;
 };
-static_assert(sizeof(AttnSeg) == 16, "AttnSeg is copied to the device as 16-byte records");
+static_assert(sizeof(AttnSeg) == 32, "AttnSeg is copied to the device as 32-byte records");
 
 // Caller pointers of the current call live in device memory so that a captured graph can be
 // replayed for a different call (the kernels read them through this struct).
@@ -156,7 +159,7 @@ size_t tc_attn_part_bytes(int n_cta);  // scratch for the partial results of ite
 int tc_attn_tiles(const Dims& dm);     // token tiles (items) per robot
 int attn_build_list(const Dims& dm, int n_active, const int* len, int n_cta, std::vector<AttnSeg>& segs, int* offs);
 cudaError_t launch_attn_tc(const Dims& dm, const Tables& tb, int layer, const bf16* qkv, op16* o, int k_iter,
-                           int M, const void* d_kv_maps, float* part, int* part_flag, int n_cta, cudaStream_t s);
+                           int M, const void* d_kv_maps, void* part, int* part_flag, int n_cta, cudaStream_t s);
 
 void set_error(const std::string& msg);
 

@@ -81,7 +81,7 @@ def check_attn_plan(H, lens, n_cta):
         for a, b in zip(parts, parts[1:]):
             assert a[1] == b[0]                                   # contiguous, no overlap
         head = parts[0]
-        assert head[2] == len(parts) - 1 and len(parts) <= 4       # n_part of the head = number of continuations
+        assert head[2] == len(parts) - 1 and len(parts) <= 2       # n_part of the head = number of continuations (at most one)
         if len(parts) > 1:
             assert head[5] == offs[head[4] + 1] - 1               # the head ends its CTA's list
             assert head[3] == head[4] + 1                         # the continuations follow on the next CTAs
@@ -89,7 +89,7 @@ def check_attn_plan(H, lens, n_cta):
                 assert c[2] == -1 and c[4] == head[4] + 1 + k and c[5] == offs[c[4]]   # first entry of that CTA
             assert all(b - a >= 2 for a, b, *_ in parts)
         for a, b, _, _, cta, _ in parts:
-            loads[cta] += b - a + 2.0
+            loads[cta] += b - a + 4.0
     return loads
 
 
@@ -104,7 +104,7 @@ def test_attn_plan_host_logic(lib):
     assert loads.max() <= loads.sum() / 148 + 4.0, (loads.max(), loads.sum() / 148)
     # one robot: the four items are cut so that several CTAs share each key stream
     loads = check_attn_plan(50, [816], 148)
-    assert np.count_nonzero(loads) >= 8
+    assert np.count_nonzero(loads) >= 6
     # degenerate and ragged cases, few CTAs, L = 0
     for lens, n_cta, H in (([0], 148, 50), ([0, 1, 63, 64, 65], 7, 50), ([5000], 3, 8), (list(rng.integers(0, 1300, size=256)), 148, 50),
                            ([816] * 512, 148, 50), ([100, 100], 1, 50), ([1200] * 3, 148, 64)):
