@@ -11,9 +11,8 @@
 //   warps 2..9  epilogue, two warps per TMEM lane quarter (half of the tile's columns each): tcgen05.ld,
 //               fused epilogue (epilogue_tile below), coalesced global stores, release ("tmem empty")
 // The accumulator is double-buffered in TMEM (2 x BN columns) so the epilogue of tile i overlaps the
-// MMAs of tile i+1.  Three kernels share the pipeline: k_gemm_tc2 (CTA pairs, cta_group::2, 256-row tiles:
-// the workhorse for M > 128), k_gemm_tc (single CTA, 128-row tiles: small batches) and the opt-in
-// k_fused_tc2 (O -> gate/up -> down of a layer in one launch with dependency counters).
+// MMAs of tile i+1.  Two kernels share the pipeline: k_gemm_tc2 (CTA pairs, cta_group::2, 256-row tiles:
+// the workhorse for M > 128) and k_gemm_tc (single CTA, 128-row tiles: small batches).
 #include <algorithm>
 #include <cstdlib>
 #include <map>
@@ -81,11 +80,133 @@ __device__ __forceinline__ void ld_acc32(uint32_t taddr, float (&v)[32]) {
 // Fused RMSNorm (a2, R5): the A operand was the un-normalised residual h (16-bit copy) and the gain
 // is folded into W, so the accumulator row only needs the scale r = rsqrt(mean(h^2) + eps); the
 // producing GEMM left n_part partial sums of squares per row, added here in a fixed order.
+// The partials are one per 32 consecutive columns of h (n_part = d / 32), whatever tile width produced them, and are
+// added left to right: a row's statistics do not depend on the batch it was computed in (pin P2).
 __device__ __forceinline__ float row_rscale(const EpiArgs& ea, int row) {
   if (!ea.ssq_in) return 1.f;
   float ss = 0.f;
-  for (int i = 0; i < ea.n_part; ++i) ss += ea.ssq_in[(size_t)row * ea.n_part + i];
+  const float* p = ea.ssq_in + (size_t)row * ea.n_part;
+  if ((ea.n_part & 3) == 0) {
+    for (int i = 0; i < ea.n_part; i += 4) {
+      const float4 v = *reinterpret_cast<const float4*>(p + i);
+      ss += v.x; ss += v.y; ss += v.z; ss += v.w;
+    }
+  } else {
+    for (int i = 0; i < ea.n_part; ++i) ss += p[i];
+  }
   return rsqrtf(ss * ea.inv_d + ea.eps);
+}
+
+// ---------------------------------------------------------------- residual / bias tiles (a6, a8, a1)
+// h <- h + acc (or acc + bias), its 16-bit copy (A operand of the next GEMM) and the sum of squares of each
+// 32-column group of the new row (fused RMSNorm, a2).  One warp = 32 rows (its TMEM lane quarter) x half of the
+// tile's columns, in 32-column chunks: TMEM gives thread = row, global memory wants lanes along columns, so a chunk
+// is transposed through the warp's scratch and then handled 8 lanes x 4 columns per row, 4 rows per instruction.
+// Interior rows take no masks; the 16-bit format is fixed at compile time; row offsets live in registers (the clock
+// trace of round 1 showed this epilogue bound by instruction issue before that).
+// Tried in round 2 and dropped: starting the accumulator as h (written into tensor memory by these warps before the
+// tile's first MMA, for the first tiles before the dependency wait) so that the epilogue only writes.  The clock trace
+// (profiles/r2_gemm_trace.md) shows why it does not pay: the ~10k cycles after the last MMA are the 130 CTAs of the
+// single-round launch storing 22 MB at the same time, not the residual loads; the preload delayed the first MMA and
+// pulled 13 MB through L2 under the previous kernel's tail: +1 ms per call.
+// 16-bit copy of h: fp16 saturates at the largest finite value instead of becoming inf (include/rosa.h: range of the
+// residual stream in the default operand format; bf16 has the range of fp32).
+template <bool FP16>
+__device__ __forceinline__ uint32_t pack_h16(float lo, float hi) {
+  if constexpr (FP16) {
+    uint32_t r;
+    asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+    return r;
+  } else {
+    return pack_op2_t<false>(lo, hi);
+  }
+}
+
+template <int BN, int EPI, typename Release>
+__device__ __forceinline__ void epilogue_tile_resid(const EpiArgs& ea, float* scr, uint32_t t_acc, int r0, int n0, int m_lim,
+                                                    int N, int lane, int half, Release release) {
+  constexpr int P = 36;
+  constexpr int NCT = (BN + 31) / 32, NC0 = (NCT + 1) / 2;
+  const int c_beg = half ? NC0 : 0, c_end = half ? NCT : NC0;
+  const int lr = lane >> 3, lc = (lane & 7) * 4;
+  const int n32 = N >> 5;
+  int c_last = c_end - 1;   // last chunk of this warp that lies inside N (the last column tile may hang over)
+  while (c_last >= c_beg && n0 + c_last * 32 >= N) --c_last;
+  if (c_last < c_beg) { release(); return; }
+  // FULL: all 32 rows live, 16-bit copy and statistics wanted (every tile of the path but the ragged last row block):
+  // no predicates in the loop
+  auto run = [&](auto fp16_tag, auto full_tag) {
+    constexpr bool FP16 = decltype(fp16_tag)::value;
+    constexpr bool FULL = decltype(full_tag)::value;
+    uint32_t off[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) off[i] = (uint32_t)(i * 4 + lr) * (uint32_t)ea.ld_out;
+    const bool b0 = lane & 1, b1 = lane & 2, b2 = lane & 4;
+    const int srow = r0 + ((b0 ? 4 : 0) + (b1 ? 2 : 0) + (b2 ? 1 : 0)) * 4 + lr;   // the row whose statistics this lane ends up with
+#pragma unroll 1
+    for (int c = c_beg; c <= c_last; ++c) {
+      const int col0 = n0 + c * 32;
+      float* const gc = ea.out_f32 + (size_t)r0 * ea.ld_out + col0 + lc;
+      uint16_t* const hc = (uint16_t*)ea.h16 + (size_t)r0 * ea.ld_out + col0 + lc;
+      float4 hres[8];
+      if constexpr (EPI == EPI_RESID) {  // requested first: the latency overlaps the accumulator load and the transpose
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+          hres[i] = FULL || r0 + i * 4 + lr < m_lim ? *reinterpret_cast<const float4*>(gc + off[i]) : make_float4(0.f, 0.f, 0.f, 0.f);
+      } else {
+        const float4 b = *reinterpret_cast<const float4*>(ea.bias + col0 + lc);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) hres[i] = b;
+      }
+      {
+        float v[32];
+        ld_acc32(t_acc + c * 32, v);
+        if (c == c_last) release();
+#pragma unroll
+        for (int i = 0; i < 32; i += 4)
+          *reinterpret_cast<float4*>(&scr[lane * P + i]) = make_float4(v[i], v[i + 1], v[i + 2], v[i + 3]);
+      }
+      __syncwarp();
+      float4 o[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) o[i] = *reinterpret_cast<const float4*>(&scr[(i * 4 + lr) * P + lc]);
+      float sq[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        o[i].x += hres[i].x; o[i].y += hres[i].y; o[i].z += hres[i].z; o[i].w += hres[i].w;
+        if (FULL || r0 + i * 4 + lr < m_lim) {
+          *reinterpret_cast<float4*>(gc + off[i]) = o[i];
+          if (FULL || ea.h16)
+            *reinterpret_cast<uint2*>(hc + off[i]) = make_uint2(pack_h16<FP16>(o[i].x, o[i].y), pack_h16<FP16>(o[i].z, o[i].w));
+        }
+        sq[i] = o[i].x * o[i].x + o[i].y * o[i].y + o[i].z * o[i].z + o[i].w * o[i].w;
+      }
+      if (FULL || ea.ssq_out) {
+        // One partial per 32-column group of the row: the 8 lanes of a row group hold 4 columns each of 8 rows;
+        // a transposing butterfly (4 + 2 + 1 shuffles) leaves each lane with the group's sum for ONE row, added
+        // in a fixed order whatever the tile width: the row statistics, and with them the whole result, do not
+        // depend on the batch a robot is served in (pin P2).
+        float w[4], u[2];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const float send = b0 ? sq[j] : sq[j + 4], keep = b0 ? sq[j + 4] : sq[j];
+          w[j] = keep + __shfl_xor_sync(0xffffffffu, send, 1);
+        }
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+          const float send = b1 ? w[j] : w[j + 2], keep = b1 ? w[j + 2] : w[j];
+          u[j] = keep + __shfl_xor_sync(0xffffffffu, send, 2);
+        }
+        const float send = b2 ? u[0] : u[1], keep = b2 ? u[1] : u[0];
+        const float tot = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+        if (FULL || srow < m_lim) ea.ssq_out[(size_t)srow * n32 + (col0 >> 5)] = tot;
+      }
+      __syncwarp();
+    }
+  };
+  const bool full = r0 + 32 <= m_lim && ea.h16 && ea.ssq_out;
+  if (ea.out_fp16) { if (full) run(std::true_type{}, std::true_type{}); else run(std::true_type{}, std::false_type{}); }
+  else { if (full) run(std::false_type{}, std::true_type{}); else run(std::false_type{}, std::false_type{}); }
 }
 
 // What an epilogue warp fetches BEFORE it waits for its accumulator, so that the latency sits under the main
@@ -158,76 +279,24 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, EpiPre& pre, fl
     for (int i = 0; i < 8; ++i) o[i] = *reinterpret_cast<const float4*>(&scr[(i * 4 + lr) * P + lc]);
   };
   if constexpr (EPI == EPI_STORE_F32 || EPI == EPI_BIAS_F32 || EPI == EPI_RESID) {
-    // h (fp32) = acc [+ h] [+ bias]; optionally also the 16-bit copy of the new h (A operand of
-    // the next GEMM) and this half-tile's partial sum of squares of each row (fused RMSNorm, a2)
-    // 32-column chunks: half 0 takes the first NC0, half 1 the rest.  BN need not divide N (nor be a
-    // multiple of 32): columns at or beyond min(n0 + BN, N) are masked, in groups of 4.
+    // Read-modify-write form, used where the accumulator cannot start as h: the plain store of the GEMM unit
+    // test, and the adaptive-norm variant's gated residual h += gate * acc (R25).  Everything else goes through
+    // epilogue_tile_resid above.  32-column chunks: half 0 takes the first NC0, half 1 the rest;
+    // BN need not divide N: chunks at or beyond N are skipped (N is a multiple of 32).
     constexpr int NCT = (BN + 31) / 32, NC0 = (NCT + 1) / 2;
     const int c_beg = half ? NC0 : 0, c_end = half ? NCT : NC0;
-    const int n_end = min(n0 + BN, N);
-    float rowss[8];
-#pragma unroll
-    for (int i = 0; i < 8; ++i) rowss[i] = 0.f;
+    const int n32 = N >> 5;
     const bool want_h16 = EPI != EPI_STORE_F32 && ea.h16 != nullptr;
-    // Fast path (every interior tile): no row or column masks, the 16-bit format fixed at compile time, row
-    // offsets kept in registers.  The clock trace showed this epilogue bound by instruction issue (about 600
-    // SASS instructions per 32 x 32 chunk, most of them 64-bit address arithmetic, mask predicates and the
-    // per-value format branch), not by memory.
-    const bool fast = EPI != EPI_STORE_F32 && BN % 32 == 0 && want_h16 && ea.ssq_out && !ea.gate && r0 + 32 <= m_lim && n0 + BN <= N;
-    if (fast) {
-      auto run = [&](auto fp16_tag) {
-        constexpr bool FP16 = decltype(fp16_tag)::value;
-        float* const gbase = ea.out_f32 + (size_t)r0 * ea.ld_out + n0 + lc;
-        uint16_t* const hbase = (uint16_t*)ea.h16 + (size_t)r0 * ea.ld_out + n0 + lc;
-        uint32_t off[8];
-#pragma unroll
-        for (int i = 0; i < 8; ++i) off[i] = (uint32_t)(i * 4 + lr) * (uint32_t)ea.ld_out;
-#pragma unroll 1
-        for (int c = c_beg; c < c_end; ++c) {
-          float* const gc = gbase + c * 32;
-          uint16_t* const hc = hbase + c * 32;
-          float4 hres[8];
-          if constexpr (EPI == EPI_RESID) {  // requested first: the latency overlaps the accumulator load and the transpose
-#pragma unroll
-            for (int i = 0; i < 8; ++i) hres[i] = *reinterpret_cast<const float4*>(gc + off[i]);
-          } else {
-            const float4 b = *reinterpret_cast<const float4*>(ea.bias + n0 + c * 32 + lc);
-#pragma unroll
-            for (int i = 0; i < 8; ++i) hres[i] = b;
-          }
-          {
-            float v[32];
-            ld_acc32(t_acc + c * 32, v);
-            if (c == c_end - 1) release();
-            to_scratch(v);
-          }
-          __syncwarp();
-          float4 o[8];
-          from_scratch(o);
-#pragma unroll
-          for (int i = 0; i < 8; ++i) {
-            o[i].x += hres[i].x; o[i].y += hres[i].y; o[i].z += hres[i].z; o[i].w += hres[i].w;
-            *reinterpret_cast<float4*>(gc + off[i]) = o[i];
-            *reinterpret_cast<uint2*>(hc + off[i]) = make_uint2(pack_op2_t<FP16>(o[i].x, o[i].y), pack_op2_t<FP16>(o[i].z, o[i].w));
-            rowss[i] += o[i].x * o[i].x + o[i].y * o[i].y + o[i].z * o[i].z + o[i].w * o[i].w;
-          }
-          __syncwarp();
-        }
-      };
-      if (ea.out_fp16) run(std::true_type{});
-      else run(std::false_type{});
-    } else
 #pragma unroll 1
     for (int c = c_beg; c < c_end; ++c) {
       const int col = n0 + c * 32 + lc;
-      const bool colok = col < n_end;
+      const bool colok = n0 + c * 32 < N;
       float4 add = make_float4(0.f, 0.f, 0.f, 0.f);
       if constexpr (EPI == EPI_BIAS_F32) { if (colok) add = *reinterpret_cast<const float4*>(ea.bias + col); }
       float* gp = ea.out_f32 + (size_t)(r0 + lr) * ea.ld_out + col;
       uint16_t* hp = (uint16_t*)ea.h16 + (size_t)(r0 + lr) * ea.ld_out + col;
       const size_t step = (size_t)4 * ea.ld_out;
-      // the residual rows are requested first: their latency (L2, after epilogue_prefetch) overlaps the
-      // accumulator load and the transpose
+      // the residual rows are requested first: their latency overlaps the accumulator load and the transpose
       float4 hres[8];
       if constexpr (EPI == EPI_RESID) {
 #pragma unroll
@@ -263,31 +332,24 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, EpiPre& pre, fl
 #pragma unroll
       for (int i = 0; i < 8; ++i) {
         o[i].x += add.x; o[i].y += add.y; o[i].z += add.z; o[i].w += add.w;
-        if (colok && r0 + i * 4 + lr < m_lim) {
+        const bool ok = colok && r0 + i * 4 + lr < m_lim;
+        if (ok) {
           *reinterpret_cast<float4*>(gp + i * step) = o[i];
-          if constexpr (EPI != EPI_STORE_F32) {
-            if (want_h16)
-              *reinterpret_cast<uint2*>(hp + i * step) =
-                  make_uint2(pack_op2(o[i].x, o[i].y, ea.out_fp16), pack_op2(o[i].z, o[i].w, ea.out_fp16));
-            rowss[i] += o[i].x * o[i].x + o[i].y * o[i].y + o[i].z * o[i].z + o[i].w * o[i].w;
+          if (want_h16)
+            *reinterpret_cast<uint2*>(hp + i * step) =
+                make_uint2(pack_op2(o[i].x, o[i].y, ea.out_fp16), pack_op2(o[i].z, o[i].w, ea.out_fp16));
+        }
+        if constexpr (EPI != EPI_STORE_F32) {
+          if (ea.ssq_out) {  // one partial per 32-column group: the layout row_rscale reads
+            float v = o[i].x * o[i].x + o[i].y * o[i].y + o[i].z * o[i].z + o[i].w * o[i].w;
+            v += __shfl_xor_sync(0xffffffffu, v, 1);
+            v += __shfl_xor_sync(0xffffffffu, v, 2);
+            v += __shfl_xor_sync(0xffffffffu, v, 4);
+            if ((lane & 7) == 0 && ok) ea.ssq_out[(size_t)(r0 + i * 4 + lr) * n32 + ((n0 >> 5) + c)] = v;
           }
         }
       }
       __syncwarp();
-    }
-    if constexpr (EPI != EPI_STORE_F32) {
-      if (ea.ssq_out) {
-#pragma unroll
-        for (int i = 0; i < 8; ++i) {
-          float v = rowss[i];
-          v += __shfl_xor_sync(0xffffffffu, v, 1);
-          v += __shfl_xor_sync(0xffffffffu, v, 2);
-          v += __shfl_xor_sync(0xffffffffu, v, 4);
-          const int rw = r0 + i * 4 + lr;
-          if ((lane & 7) == 0 && rw < m_lim)
-            ea.ssq_out[(size_t)rw * (2 * ((N + BN - 1) / BN)) + 2 * (n0 / BN) + half] = v;
-        }
-      }
     }
   } else if constexpr (EPI == EPI_FINAL) {
     // a9 + a10: columns are action dimensions (N = 64 covers A <= 64): v = r acc + b_out, x += dt_p v
@@ -542,6 +604,12 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         __syncwarp();
         if (lane == 0) mbar_arrive(tempty_bar(acc));
       };
+      if constexpr (EPI == EPI_RESID || EPI == EPI_BIAS_F32) {
+        if (!ea.gate) {  // the adaptive-norm variant's gated residual takes the general form in epilogue_tile
+          epilogue_tile_resid<BN, EPI>(ea, scr, t_acc, r0, n0, m_lim, N, lane, half, release);
+          continue;
+        }
+      }
       epilogue_tile<BN, EPI>(ea, pre, scr, t_acc, r0, n0, m_lim, N, lane, half, release);
     }
   }
@@ -559,6 +627,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
 __device__ long long g_gemm_trace[16 * 2 * 16];
 #define GT_TRACE(slot) do { if ((blockIdx.x == 0 || blockIdx.x == 64) && lane == 0) \
   g_gemm_trace[((2 * EPI + (K > 2048)) * 2 + (blockIdx.x != 0)) * 16 + (slot)] = clock64(); } while (0)
+extern "C" int rosa_trace_gemm(long long* host) { return (int)cudaMemcpyFromSymbol(host, g_gemm_trace, sizeof(g_gemm_trace)); }
 #else
 #define GT_TRACE(slot) do { } while (0)
 #endif
@@ -710,6 +779,12 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
       };
       if (warp == 2) GT_TRACE(5);
       if (warp == 2 && it == 0) GT_TRACE(11);
+      if constexpr (EPI == EPI_RESID || EPI == EPI_BIAS_F32) {
+        if (!ea.gate) {  // the adaptive-norm variant's gated residual takes the general form in epilogue_tile
+          epilogue_tile_resid<BN, EPI>(ea, scr, t_acc, r0, n0, m_lim, N, lane, half, release);
+          continue;
+        }
+      }
       epilogue_tile<BN, EPI>(ea, pre, scr, t_acc, r0, n0, m_lim, N, lane, half, release);
       if (warp == 2) GT_TRACE(6);
       if (warp == 2 && it == 0) GT_TRACE(12);
@@ -815,11 +890,8 @@ static int resid_bn(int N, int M) {
   }
   return best;
 }
-// sum-of-squares partials per row written by those launches: one per half N tile (two epilogue warps per row)
-int tc_ssq_parts(int N, int M) {
-  const int bn = resid_bn(N, M);
-  return 2 * ((N + bn - 1) / bn);
-}
+// sum-of-squares partials per row written by the residual / bias launches: one per 32 columns, whatever the tile width
+int tc_ssq_parts(int N) { return N / 32; }
 int tc_resid_bn(int N, int M) { return resid_bn(N, M); }
 
 template <int BN, int EPI>

@@ -568,7 +568,7 @@ static cudaError_t enqueue_steps(rosa_expert* e, const Tables& tb, int nmax, cud
     EpiArgs ea{};
     ea.m_active = tb.m_active + k;
     ea.H = dm.H; ea.hd = dm.hd; ea.gu_blk = dm.gu_blk; ea.in_fp16 = dm.fp16; ea.out_fp16 = dm.fp16;
-    ea.inv_d = 1.f / (float)d; ea.eps = dm.eps; ea.n_part = tc_ssq_parts(d, M);
+    ea.inv_d = 1.f / (float)d; ea.eps = dm.eps; ea.n_part = tc_ssq_parts(d);
     if (fused_norm) { ea.h16 = nrm; ea.ssq_out = ssq; ea.ssq_in = ssq; }
     // a1: h0 = W2 swish(W1 [tau ; W_in x + b_in] + b1) + b2
     mark(e, ROSA_KC_INPROJ, s);

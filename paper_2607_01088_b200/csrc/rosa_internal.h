@@ -144,7 +144,7 @@ void launch_f32_to_bf16(bf16* dst, const float* src, size_t n, cudaStream_t s);
 // tcgen05 family (gemm_tcgen05.cu)
 bool tc_gemm_supported(int N, int K);
 int tc_resid_bn(int N, int M);  // N tile of the BIAS_F32 / RESID launches
-int tc_ssq_parts(int N, int M);  // sum-of-squares partials per row written by the BIAS_F32 / RESID launches (two per N tile)
+int tc_ssq_parts(int N);       // sum-of-squares partials per row written by the BIAS_F32 / RESID launches (one per 32 columns)
 // A [M,K] row-major, W [N,K] row-major, both fp16 or both bf16 (EpiArgs::in_fp16)
 cudaError_t launch_gemm_tc(Epi epi, const op16* A, const op16* W, int M, int N, int K,
                            const EpiArgs& a, cudaStream_t s);
