@@ -15,10 +15,11 @@
 // PERSISTENT CTAs over a stream-K work list.  The host cuts the concatenation of all items' key streams into
 // one share per CTA (attn_build_list below): a CTA's list is a run of SEGMENTS (item, key blocks [kb0, kb1)).
 // An item that straddles a cut is finished by its HEAD segment (kb0 = 0, the last entry of CTA a's list), which
-// merges the partial (O, m, l) that the following CTAs (a+1 ..., where the item's other segments are the FIRST
-// entry of the list) left in a global scratch slot long before.  Nothing else waits on another CTA, every CTA
-// of the grid is resident (grid <= number of SMs, one CTA per SM), so the merge cannot deadlock.
-// Inside a CTA the three roles walk the same list; the K/V/Q ring (6 stages of 32 KB, one 3-D TMA per 64-key
+// merges the partial (O, m, l) that CTA a+1 (where the item's other segment is the FIRST entry of the list) left
+// in its global scratch slot long before.  Nothing else waits on another CTA, every CTA of the grid is resident
+// (grid <= number of SMs, one CTA per SM), so the merge cannot deadlock.  (When whole items, longest first, are
+// estimated to finish no later, the planner keeps that plan instead: no cuts, no merges.)
+// Inside a CTA the three roles walk the same list; the K/V/Q ring (5 stages of 32 KB, one 3-D TMA per 64-key
 // block; per-robot tensor maps made at bind time bound the ragged length: rows >= L_p are zero-filled and
 // masked) keeps flowing across segments, the next segment's Q is copied into tensor memory before the current
 // segment's O is drained, and its first two S blocks run on the tensor pipe while the softmax warps drain.
@@ -652,8 +653,12 @@ int tc_attn_tiles(const Dims& dm) { return (dm.H + AT_TOK - 1) / AT_TOK; }
 // drain).  The concatenated items are cut into equal shares for `n_cta` CTAs (fewer when there is little work:
 // a share is at least kMinShare units); no segment is shorter than kMinSeg blocks and no item has more than 2
 // segments (the head merges at most one partial result).  offs[c] .. offs[c+1] = segments of CTA c (offs has n_cta + 1 entries; CTAs without work get none).
-int attn_build_list(const Dims& dm, int n_active, const int* len, int n_cta, std::vector<AttnSeg>& segs, int* offs) {
-  constexpr double kSegOvh = 4.0, kMinShare = 8.0;
+// Cost model of the planners, in units of one 64-key block inside a running segment (~1.7k cycles): what a segment
+// costs on top of its blocks (Q load and copy, pipeline refill, O drain: clock trace profiles/r2_attn_trace.md).
+constexpr double kSegOvh = 6.0;
+
+static int attn_plan_cut(const Dims& dm, int n_active, const int* len, int n_cta, std::vector<AttnSeg>& segs, int* offs) {
+  constexpr double kMinShare = 10.0;
   constexpr int kMinSeg = 2;
   const int tpr = tc_attn_tiles(dm);
   const size_t seg0 = segs.size();
@@ -710,6 +715,60 @@ int attn_build_list(const Dims& dm, int n_active, const int* len, int n_cta, std
   return (int)(segs.size() - seg0);
 }
 
+// The alternative without cuts: whole items, longest first, each to the CTA with the least work so far (LPT).
+// No partial results, no merges; at most (longest + shortest) per CTA when there are up to two items per CTA.
+static int attn_plan_whole(const Dims& dm, int n_active, const int* len, int n_cta, std::vector<AttnSeg>& segs, int* offs) {
+  const int tpr = tc_attn_tiles(dm);
+  const size_t seg0 = segs.size();
+  std::vector<int> order(n_active);
+  for (int p = 0; p < n_active; ++p) order[p] = p;
+  std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return len[a] > len[b]; });
+  std::vector<double> load(n_cta, 0.0);
+  std::vector<std::vector<AttnSeg>> lists(n_cta);
+  for (int tt = 0; tt < tpr; ++tt)        // tile-major: the tiles of one robot run on different CTAs at the same time
+    for (int x = 0; x < n_active; ++x) {
+      const int p = order[x], nb = (len[p] + AT_KV - 1) / AT_KV + 1;
+      int c = 0;
+      for (int k = 1; k < n_cta; ++k) if (load[k] < load[c]) c = k;
+      AttnSeg sg{};
+      sg.p = p; sg.robot = p; sg.len = len[p]; sg.tt = (int16_t)tt; sg.kb0 = 0; sg.kb1 = (int16_t)nb; sg.n_part = 0; sg.part0 = -1;
+      lists[c].push_back(sg);
+      load[c] += nb + kSegOvh;
+    }
+  for (int c = 0; c < n_cta; ++c) {
+    offs[c] = (int)segs.size();
+    segs.insert(segs.end(), lists[c].begin(), lists[c].end());
+  }
+  offs[n_cta] = (int)segs.size();
+  return (int)(segs.size() - seg0);
+}
+
+static double attn_plan_makespan(const std::vector<AttnSeg>& segs, size_t seg0, const int* offs, int n_cta) {
+  double worst = 0.0;
+  for (int c = 0; c < n_cta; ++c) {
+    double t = 0.0;
+    for (int i = offs[c]; i < offs[c + 1]; ++i)
+      t += segs[i].kb1 - segs[i].kb0 + kSegOvh + (segs[i].n_part != 0 ? 1.5 : 0.0);   // a cut costs a partial hand-off on both sides
+    worst = std::max(worst, t);
+  }
+  (void)seg0;
+  return worst;
+}
+
+// Work list of one Euler iteration: both plans are built, the one whose busiest CTA is estimated to finish first is kept.
+int attn_build_list(const Dims& dm, int n_active, const int* len, int n_cta, std::vector<AttnSeg>& segs, int* offs) {
+  const size_t seg0 = segs.size();
+  std::vector<AttnSeg> a(segs), b(segs);
+  std::vector<int> oa(n_cta + 1), ob(n_cta + 1);
+  attn_plan_cut(dm, n_active, len, n_cta, a, oa.data());
+  attn_plan_whole(dm, n_active, len, n_cta, b, ob.data());
+  const double ta = attn_plan_makespan(a, seg0, oa.data(), n_cta), tb2 = attn_plan_makespan(b, seg0, ob.data(), n_cta);
+  const bool use_cut = ta < tb2;
+  segs.swap(use_cut ? a : b);
+  for (int c = 0; c <= n_cta; ++c) offs[c] = use_cut ? oa[c] : ob[c];
+  return (int)(segs.size() - seg0);
+}
+
 // Tensor maps of one robot's prefix K and V of one layer: [len, 256] bf16, box {64, 64}.
 // `out2` = two consecutive CUtensorMap (host memory).
 bool tc_attn_make_prefix_maps(void* out2, const bf16* k, const bf16* v, int len, const Dims& dm) {
@@ -722,11 +781,10 @@ bool tc_attn_make_prefix_maps(void* out2, const bf16* k, const bf16* v, int len,
 
 cudaError_t launch_attn_tc(const Dims& dm, const Tables& tb, int layer, const bf16* qkv, op16* o, int k_iter,
                            int M, const void* d_kv_maps, void* part, int* part_flag, int n_cta, cudaStream_t s) {
-  static bool configured = false;
-  if (!configured) {
+  static uint64_t configured = 0;
+  if (first_use_on_device(configured)) {
     cudaError_t e = cudaFuncSetAttribute(k_attn_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, AT_SMEM);
     if (e != cudaSuccess) return e;
-    configured = true;
   }
   AttnMaps maps;
   {

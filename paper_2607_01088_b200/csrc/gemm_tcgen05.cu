@@ -848,14 +848,23 @@ bool encode_tmap(CUtensorMap* tm, const void* ptr, int rank, const uint64_t* dim
              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// SM count of the CURRENT device (cached per device: a process may hold experts on several GPUs)
 int num_sms() {
-  static int n = 0;
-  if (!n) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
-  }
-  return n;
+  static int n[64] = {};
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (dev < 0 || dev >= 64) dev = 0;
+  if (!n[dev]) cudaDeviceGetAttribute(&n[dev], cudaDevAttrMultiProcessorCount, dev);
+  return n[dev];
+}
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) is per device: true the first time `flags` is asked on the current one
+bool first_use_on_device(uint64_t& flags) {
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (dev < 0 || dev >= 64) return true;
+  const bool first = !((flags >> dev) & 1u);
+  flags |= (uint64_t)1 << dev;
+  return first;
 }
 
 bool tc_gemm_supported(int N, int K) { return N % 64 == 0 && K % 64 == 0 && N >= 64; }
@@ -897,11 +906,10 @@ int tc_resid_bn(int N, int M) { return resid_bn(N, M); }
 template <int BN, int EPI>
 static cudaError_t launch_one(const op16* A, const op16* W, int M, int N, int K, const EpiArgs& a, cudaStream_t s) {
   using Cfg = GemmCfg<BN>;
-  static bool configured = false;
-  if (!configured) {
+  static uint64_t configured = 0;
+  if (first_use_on_device(configured)) {
     cudaError_t e = cudaFuncSetAttribute(k_gemm_tc<BN, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM);
     if (e != cudaSuccess) return e;
-    configured = true;
   }
   CUtensorMap tmA, tmB;
   if (!make_tmap_2d(&tmA, A, (uint64_t)M, (uint64_t)K, BM, a.in_fp16) ||
@@ -915,11 +923,10 @@ static cudaError_t launch_one(const op16* A, const op16* W, int M, int N, int K,
 template <int BN, int EPI>
 static cudaError_t launch_two(const op16* A, const op16* W, int M, int N, int K, const EpiArgs& a, cudaStream_t s) {
   using Cfg = Gemm2Cfg<BN>;
-  static bool configured = false;
-  if (!configured) {
+  static uint64_t configured = 0;
+  if (first_use_on_device(configured)) {
     cudaError_t e = cudaFuncSetAttribute(k_gemm_tc2<BN, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM);
     if (e != cudaSuccess) return e;
-    configured = true;
   }
   CUtensorMap tmA, tmB;
   if (!make_tmap_2d(&tmA, A, (uint64_t)M, (uint64_t)K, BM, a.in_fp16) ||

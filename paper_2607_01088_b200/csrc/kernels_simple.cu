@@ -260,11 +260,7 @@ void launch_final(float* x, const CallPtrs* cp, const float* h, const float* g, 
                   const float* b_out, const Dims& dm, const Tables& tb, int k_iter, int M,
                   cudaStream_t s) {
   const size_t smem = (size_t)dm.A * dm.d * sizeof(bf16);
-  static size_t configured = 0;
-  if (smem > configured) {
-    cudaFuncSetAttribute(k_final, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    configured = smem;
-  }
+  cudaFuncSetAttribute(k_final, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);  // per device; CUDA-core family only
   launch_k(k_final, dim3((M + FIN_ROWS - 1) / FIN_ROWS), dim3(256), smem, s, x, cp, h, g, w_out, b_out, dm.d, dm.A, dm.H,
            dm.eps, tb, k_iter);
 }
@@ -443,11 +439,7 @@ __global__ void __launch_bounds__(256) k_attn_simple(Dims dm, Tables tb, int lay
 void launch_attn_simple(const Dims& dm, const Tables& tb, int layer, const bf16* qkv, op16* o,
                         int k_iter, int max_len, cudaStream_t s) {
   size_t smem = ((size_t)dm.nq * dm.hd + (size_t)dm.nq * (max_len + dm.H) + dm.nq) * sizeof(float);
-  static size_t configured = 0;
-  if (smem > configured) {
-    cudaFuncSetAttribute(k_attn_simple, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    configured = smem;
-  }
+  cudaFuncSetAttribute(k_attn_simple, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);  // per device; CUDA-core family only
   k_attn_simple<<<tb.batch * dm.H, 256, smem, s>>>(dm, tb, layer, qkv, o, k_iter);
 }
 

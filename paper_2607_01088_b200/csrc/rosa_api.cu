@@ -44,6 +44,7 @@ static inline float bf2f(uint16_t b) {
 }
 
 constexpr int kStageRing = 4;
+constexpr size_t kMaxGraphs = 48;   // (batch bucket, max n_steps) pairs kept instantiated per expert
 
 struct GraphKey {
   int batch, nmax, vel;
@@ -88,7 +89,16 @@ struct rosa_expert {
   const bf16** d_rv = nullptr;
   int* d_rlen = nullptr;
   std::vector<int> h_rlen;         // -1 = unbound
-  std::vector<std::vector<bf16*>> owned;  // per robot: library-owned K/V buffers (fp32 binds)
+  std::vector<std::vector<bf16*>> owned;  // per robot: library-owned K/V buffers (fp32 binds), kept until destroy
+  std::vector<size_t> owned_cap;          // elements each of them holds
+  // bind is asynchronous: table updates go from a pinned per-robot record through bind_stream (ordered after the last
+  // denoise call that was enqueued); the next denoise call waits for bind_ev on its stream
+  cudaStream_t bind_stream = nullptr;
+  cudaEvent_t bind_ev = nullptr, call_ev = nullptr;
+  char* h_bind = nullptr;                 // [max_robots][bind_rec]
+  size_t bind_rec = 0;
+  std::vector<char> bind_pending;         // robot's record is (possibly) still being copied
+  bool bind_dirty = false, call_pending = false;
   int max_len_bound = 0;
   bool attn_tc = false;            // tcgen05 attention kernel in use
   char* d_kv_maps = nullptr;       // [max_robots * layers * 2] CUtensorMap (prefix K, V per robot/layer)
@@ -104,8 +114,11 @@ struct rosa_expert {
   void* attn_part = nullptr;       // per-CTA partial (O, m, l) of items cut between CTAs
   int* attn_flag = nullptr;        // [n_cta] ready flags of those partials
   int64_t graph_captures = 0;      // graphs captured so far (rosa_debug_graph_captures)
-  std::map<GraphKey, cudaGraphExec_t> graphs;
+  std::map<GraphKey, cudaGraphExec_t> graphs;      // at most kMaxGraphs, least recently used evicted
   std::map<GraphKey, int64_t> graph_launches;
+  std::map<GraphKey, int64_t> graph_used;          // value of graph_clock at the last launch
+  int64_t graph_clock = 0;
+  int device = 0;                                  // the CUDA device the expert lives on
   cudaStream_t cap_stream = nullptr;
   int64_t last_launches = 0;
   float* e2e_dev = nullptr;  // staging for rosa_denoise_batch_host
@@ -216,6 +229,10 @@ static void destroy_impl(rosa_expert* e) {
     if (e->stage_ev[i]) cudaEventDestroy(e->stage_ev[i]);
   }
   if (e->cap_stream) cudaStreamDestroy(e->cap_stream);
+  if (e->bind_stream) cudaStreamDestroy(e->bind_stream);
+  if (e->bind_ev) cudaEventDestroy(e->bind_ev);
+  if (e->call_ev) cudaEventDestroy(e->call_ev);
+  if (e->h_bind) cudaFreeHost(e->h_bind);
   for (cudaEvent_t ev : e->prof_ev) cudaEventDestroy(ev);
   delete e;
 }
@@ -381,7 +398,7 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
   WS(e->qkv, Mmax * dm.qkv_n * 2);
   WS(e->obuf, Mmax * dm.q_n * 2);
   WS(e->mact, Mmax * F * 2);
-  WS(e->scratch, Mmax * (size_t)std::max(2 * F, dm.qkv_n) * 4);
+  if (e->family == 0) WS(e->scratch, Mmax * (size_t)std::max(2 * F, dm.qkv_n) * 4);  // fp32 GEMM output of the CUDA-core family
   WS(e->e2e_dev, (size_t)c->max_batch * HA * 4);
   WS(e->ssq, Mmax * (d / 32) * 4);
   CK(cudaMemset(e->zbuf, 0, Mmax * d * 2));
@@ -410,6 +427,10 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
       WS(e->attn_flag, (size_t)sms * 8 * 4);
       CK(cudaMemset(e->attn_flag, 0, (size_t)sms * 8 * 4));
     }
+  }
+  if (dm.ada && !e->attn_tc) {
+    set_error("time_conditioning = 1 needs the tcgen05 attention kernel (8 query heads, 1 KV head, head_dim 256; ROSA_ATTN unset)");
+    return ROSA_ERR_UNSUPPORTED;
   }
   e->h_rlen.assign(c->max_robots, -1);
   e->owned.resize(c->max_robots);
@@ -442,6 +463,13 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
     CK(cudaEventCreateWithFlags(&e->stage_ev[i], cudaEventDisableTiming));
   }
   CK(cudaStreamCreateWithFlags(&e->cap_stream, cudaStreamNonBlocking));
+  CK(cudaStreamCreateWithFlags(&e->bind_stream, cudaStreamNonBlocking));
+  CK(cudaEventCreateWithFlags(&e->bind_ev, cudaEventDisableTiming));
+  CK(cudaEventCreateWithFlags(&e->call_ev, cudaEventDisableTiming));
+  e->bind_rec = ((size_t)dm.layers * (2 * sizeof(void*) + 2 * tc_attn_map_bytes()) + 64 + 63) / 64 * 64;
+  CK(cudaMallocHost((void**)&e->h_bind, e->bind_rec * c->max_robots));
+  e->bind_pending.assign(c->max_robots, 0);
+  e->owned_cap.assign(c->max_robots, 0);
   return ROSA_OK;
 }
 
@@ -469,6 +497,7 @@ static cudaError_t gemm(rosa_expert* e, int cls, Epi epi, const op16* A, const o
     e->last_launches += 1;
     return launch_gemm_tc(epi, A, W, M, N, K, a, s);
   }
+  if (e->family != 0) return cudaErrorNotSupported;  // unreachable: create admits the tcgen05 family only for shapes its GEMMs cover
   launch_gemm_naive(A, W, e->scratch, M, N, K, a.in_fp16, a.m_active, s);
   launch_epilogue(epi, e->scratch, M, N, a, s);
   e->last_launches += 2;
@@ -656,6 +685,13 @@ static rosa_status_t denoise_impl(rosa_expert* e, int batch, const int32_t* ids,
   if (!e || !ids || !noise || !n_steps || !out) { set_error("NULL argument"); return ROSA_ERR_INVALID_ARG; }
   if (batch < 1) { set_error("batch < 1"); return ROSA_ERR_INVALID_ARG; }
   if (batch > e->cfg.max_batch) { set_error("batch > max_batch"); return ROSA_ERR_CAPACITY; }
+  {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != e->device) {
+      set_error("the expert was created on CUDA device " + std::to_string(e->device) + ", which is not the current device");
+      return ROSA_ERR_INVALID_ARG;
+    }
+  }
   const Dims& dm = e->dm;
   int nmax = 0;
   std::vector<char> seen(e->cfg.max_robots, 0);
@@ -713,6 +749,10 @@ static rosa_status_t denoise_impl(rosa_expert* e, int batch, const int32_t* ids,
   }
   CallPtrs* h_cp = (CallPtrs*)(hs + e->off_ptrs);
   h_cp->noise = noise; h_cp->out = out; h_cp->vel = out_vel; h_cp->batch_ext = batch;
+  if (e->bind_dirty) {   // table updates of binds since the last call: this call runs after them
+    CK(cudaStreamWaitEvent(stream, e->bind_ev, 0));
+    e->bind_dirty = false;
+  }
   CK(cudaMemcpyAsync(e->d_call, hs, copy_bytes, cudaMemcpyHostToDevice, stream));
   CK(cudaEventRecord(e->stage_ev[slot], stream));
   if (out_vel) CK(cudaMemsetAsync(out_vel, 0, (size_t)nmax * batch * dm.H * dm.A * 4, stream));
@@ -723,6 +763,8 @@ static rosa_status_t denoise_impl(rosa_expert* e, int batch, const int32_t* ids,
   bucket = std::min(bucket, e->cfg.max_batch);
   if (!e->use_graph || e->prof_on) {
     CK(enqueue_call(e, bucket, nmax, stream));
+    CK(cudaEventRecord(e->call_ev, stream));
+    e->call_pending = true;
     return ROSA_OK;
   }
   const GraphKey key{bucket, nmax, 0};
@@ -740,12 +782,24 @@ static rosa_status_t denoise_impl(rosa_expert* e, int batch, const int32_t* ids,
     cudaGraphExec_t ex = nullptr;
     CK(cudaGraphInstantiate(&ex, g, 0));
     cudaGraphDestroy(g);
+    if (e->graphs.size() >= kMaxGraphs) {   // evict the least recently used graph (its launches have been enqueued: safe to destroy)
+      auto victim = e->graphs.begin();
+      for (auto g2 = e->graphs.begin(); g2 != e->graphs.end(); ++g2)
+        if (e->graph_used[g2->first] < e->graph_used[victim->first]) victim = g2;
+      cudaGraphExecDestroy(victim->second);
+      e->graph_launches.erase(victim->first);
+      e->graph_used.erase(victim->first);
+      e->graphs.erase(victim);
+    }
     it = e->graphs.emplace(key, ex).first;
     e->graph_launches[key] = e->last_launches;
     e->graph_captures += 1;
   }
   e->last_launches = e->graph_launches[key];
+  e->graph_used[key] = ++e->graph_clock;
   CK(cudaGraphLaunch(it->second, stream));
+  CK(cudaEventRecord(e->call_ev, stream));   // a later bind orders its table update after this call
+  e->call_pending = true;
   return ROSA_OK;
 }
 
@@ -790,6 +844,7 @@ rosa_status_t rosa_expert_create(const rosa_expert_config_t* c, const rosa_weigh
   }
   rosa_expert* e = new rosa_expert();
   e->cfg = *c;
+  cudaGetDevice(&e->device);
   const char* fam = getenv("ROSA_KERNELS");
   // tcgen05 family needs head_dim == 256 (RoPE epilogue tile = one head) and 128/256-wide N tiles
   const bool tc_shape = c->head_dim == 256 && c->d_model % 128 == 0 && (2 * c->ffn) % 256 == 0;
@@ -816,12 +871,7 @@ rosa_status_t rosa_expert_destroy(rosa_expert_t* e) {
 rosa_status_t rosa_prefix_kv_unbind(rosa_expert_t* e, int32_t robot) {
   if (!e) { set_error("NULL expert"); return ROSA_ERR_INVALID_ARG; }
   if (robot < 0 || robot >= e->cfg.max_robots) { set_error("robot id out of range"); return ROSA_ERR_CAPACITY; }
-  if (!e->owned[robot].empty()) {
-    CK(cudaDeviceSynchronize());  // in-flight calls may still read the owned copies
-    for (bf16* p : e->owned[robot]) cudaFree(p);
-    e->owned[robot].clear();
-  }
-  e->h_rlen[robot] = -1;
+  e->h_rlen[robot] = -1;   // host-side only: library-owned copies stay allocated (a call in flight may still read them)
   return ROSA_OK;
 }
 
@@ -840,17 +890,44 @@ rosa_status_t rosa_prefix_kv_bind(rosa_expert_t* e, int32_t robot, const void* c
       if (((uintptr_t)k_layers[l] | (uintptr_t)v_layers[l]) & 15) { set_error("K/V pointer not 16-byte aligned"); return ROSA_ERR_INVALID_ARG; }
     }
   }
-  rosa_status_t st = rosa_prefix_kv_unbind(e, robot);
-  if (st != ROSA_OK) return st;
-  std::vector<const bf16*> hk(dm.layers, nullptr), hv(dm.layers, nullptr);
+  e->h_rlen[robot] = -1;
+  cudaStream_t bs = e->bind_stream;
+  if (e->bind_pending[robot]) {   // the robot's pinned record may still be on its way: wait for the copies issued so far
+    CK(cudaEventSynchronize(e->bind_ev));
+    std::fill(e->bind_pending.begin(), e->bind_pending.end(), 0);
+  }
+  if (e->call_pending) {          // table updates (and fp32 conversions) run after every call enqueued so far
+    CK(cudaStreamWaitEvent(bs, e->call_ev, 0));
+    e->call_pending = false;
+  }
+  // pinned record of the robot: [K pointers | V pointers | tensor maps (64-byte aligned) | len]
+  char* rec = e->h_bind + (size_t)robot * e->bind_rec;
+  const bf16** hk = (const bf16**)rec;
+  const bf16** hv = hk + dm.layers;
+  const size_t mb = tc_attn_map_bytes();
+  char* mp = rec + ((size_t)dm.layers * 2 * sizeof(void*) + 63) / 64 * 64;
+  int* hl = (int*)(mp + (size_t)dm.layers * 2 * mb);
   const size_t n = (size_t)len * dm.nkv * dm.hd;
+  for (int l = 0; l < dm.layers; ++l) hk[l] = hv[l] = nullptr;
   if (len > 0 && dtype == ROSA_BF16) {
     for (int l = 0; l < dm.layers; ++l) { hk[l] = (const bf16*)k_layers[l]; hv[l] = (const bf16*)v_layers[l]; }
   } else if (len > 0) {
+    CK(cudaStreamSynchronize(bs));     // bs follows every call enqueued so far: none still reads the old copies
+    if (e->owned_cap[robot] < n) {
+      for (bf16* p : e->owned[robot]) cudaFree(p);
+      e->owned[robot].clear();
+      const size_t cap = (size_t)e->cfg.max_prefix_len * dm.nkv * dm.hd;
+      for (int l = 0; l < 2 * dm.layers; ++l) {
+        bf16* q = nullptr;
+        CK(cudaMalloc((void**)&q, cap * 2));
+        e->owned[robot].push_back(q);
+      }
+      e->owned_cap[robot] = cap;
+    }
     for (int l = 0; l < dm.layers; ++l) {
-      bf16 *ck = nullptr, *cv = nullptr;
-      CK(cudaMalloc((void**)&ck, n * 2)); e->owned[robot].push_back(ck);
-      CK(cudaMalloc((void**)&cv, n * 2)); e->owned[robot].push_back(cv);
+      bf16 *ck = e->owned[robot][2 * l], *cv = e->owned[robot][2 * l + 1];
+      // conversion on the legacy default stream, synchronously: the caller's fp32 tensors were produced in the
+      // caller's stream order and may be released as soon as this call returns
       launch_f32_to_bf16(ck, (const float*)k_layers[l], n, 0);
       launch_f32_to_bf16(cv, (const float*)v_layers[l], n, 0);
       hk[l] = ck; hv[l] = cv;
@@ -858,20 +935,21 @@ rosa_status_t rosa_prefix_kv_bind(rosa_expert_t* e, int32_t robot, const void* c
     CK(cudaGetLastError());
     CK(cudaStreamSynchronize(0));
   }
-  CK(cudaMemcpy(e->d_rk + (size_t)robot * dm.layers, hk.data(), dm.layers * sizeof(void*), cudaMemcpyHostToDevice));
-  CK(cudaMemcpy(e->d_rv + (size_t)robot * dm.layers, hv.data(), dm.layers * sizeof(void*), cudaMemcpyHostToDevice));
+  CK(cudaMemcpyAsync(e->d_rk + (size_t)robot * dm.layers, hk, dm.layers * sizeof(void*), cudaMemcpyHostToDevice, bs));
+  CK(cudaMemcpyAsync(e->d_rv + (size_t)robot * dm.layers, hv, dm.layers * sizeof(void*), cudaMemcpyHostToDevice, bs));
   if (e->attn_tc && len > 0) {
-    const size_t mb = tc_attn_map_bytes();
-    std::vector<char> maps((size_t)dm.layers * 2 * mb + 64);
-    char* mp = (char*)(((uintptr_t)maps.data() + 63) & ~(uintptr_t)63);
     for (int l = 0; l < dm.layers; ++l)
       if (!tc_attn_make_prefix_maps(mp + (size_t)l * 2 * mb, hk[l], hv[l], len, dm)) {
         set_error("cuTensorMapEncodeTiled failed for the prefix K/V"); return ROSA_ERR_CUDA;
       }
-    CK(cudaMemcpy(e->d_kv_maps + (size_t)robot * dm.layers * 2 * mb, mp, (size_t)dm.layers * 2 * mb,
-                  cudaMemcpyHostToDevice));
+    CK(cudaMemcpyAsync(e->d_kv_maps + (size_t)robot * dm.layers * 2 * mb, mp, (size_t)dm.layers * 2 * mb,
+                       cudaMemcpyHostToDevice, bs));
   }
-  CK(cudaMemcpy(e->d_rlen + robot, &len, 4, cudaMemcpyHostToDevice));
+  *hl = len;
+  CK(cudaMemcpyAsync(e->d_rlen + robot, hl, 4, cudaMemcpyHostToDevice, bs));
+  CK(cudaEventRecord(e->bind_ev, bs));
+  e->bind_pending[robot] = 1;
+  e->bind_dirty = true;
   e->h_rlen[robot] = len;
   return ROSA_OK;
 }

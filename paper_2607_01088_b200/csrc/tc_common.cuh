@@ -11,7 +11,8 @@ namespace rosa {
 // host helpers (gemm_tcgen05.cu)
 bool encode_tmap(CUtensorMap* tm, const void* ptr, int rank, const uint64_t* dims, const uint64_t* strides_bytes,
                  const uint32_t* box);
-int num_sms();
+int num_sms();                               // of the current device
+bool first_use_on_device(uint64_t& flags);   // per-device one-time setup (function attributes)
 
 namespace tc {
 

@@ -89,19 +89,20 @@ def check_attn_plan(H, lens, n_cta):
                 assert c[2] == -1 and c[4] == head[4] + 1 + k and c[5] == offs[c[4]]   # first entry of that CTA
             assert all(b - a >= 2 for a, b, *_ in parts)
         for a, b, _, _, cta, _ in parts:
-            loads[cta] += b - a + 4.0
+            loads[cta] += b - a + 6.0
     return loads
 
 
 def test_attn_plan_host_logic(lib):
     """Host logic of the attention work split through the C ABI without a device (pins: brute-force invariants
-    above; balance: no CTA carries more than its equal share plus one item's worth)."""
+    above; balance: the busiest CTA is within 25% of the equal share, whichever of the two plans - items cut into
+    per-CTA shares, or whole items longest-first - the planner kept)."""
     rng = np.random.default_rng(3)
     # cfg2-like fleet on 148 CTAs: shares are balanced to within a few blocks
     lens = rng.integers(600, 1001, size=64)
     loads = check_attn_plan(50, lens, 148)
     assert np.count_nonzero(loads) == 148
-    assert loads.max() <= loads.sum() / 148 + 4.0, (loads.max(), loads.sum() / 148)
+    assert loads.max() <= 1.25 * loads.sum() / 148, (loads.max(), loads.sum() / 148)
     # one robot: the four items are cut so that several CTAs share each key stream
     loads = check_attn_plan(50, [816], 148)
     assert np.count_nonzero(loads) >= 6

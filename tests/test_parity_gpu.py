@@ -69,12 +69,13 @@ def test_cfg1_pi0_b8():
     lc.close()
 
 
-def test_cfg2_fleet_b64_ragged_sampled():
+def test_cfg2_fleet_b64_ragged_full():
+    """The headline workload, ALL 64 robots against the oracle (full tensors on cfg0-3): every ragged
+    prefix length, every attention work-list segment and every GEMM row block of the launch bench.py times."""
     case = cases.make_case(2)
     assert case.batch == 64 and case.prefix_lens.min() >= 600 and case.prefix_lens.max() <= 1000
     lc = LoadedCase(case)
-    # robot 2 (rows 100..149) and robot 5 (rows 250..299) straddle 128-row GEMM tile boundaries
-    check_against_oracle(case, lc, list(range(64)), "cfg2", sample=[0, 2, 5, 33, 63])
+    check_against_oracle(case, lc, list(range(64)), "cfg2-full")
     lc.close()
 
 
@@ -82,8 +83,15 @@ def test_cfg3_continuous_batching_b256_sampled():
     case = cases.make_case(3)
     assert case.batch == 256
     ns = case.n_steps
-    # one robot per remaining-step count that occurs, plus the first and last robots
-    sample = sorted({int(np.nonzero(ns == n)[0][0]) for n in np.unique(ns)} | {0, 255})
+    # stratified over the remaining-step counts (three robots of each count that occurs: first, middle, last), plus
+    # the first and last robots and the robots whose 50 token rows straddle a 256-row tile boundary after the
+    # library's own ordering is unknown here, so simply every 16th robot as well: 40+ of the 256
+    sample = {0, 255} | set(range(7, 256, 16))
+    for n in np.unique(ns):
+        idx = np.nonzero(ns == n)[0]
+        sample |= {int(idx[0]), int(idx[len(idx) // 2]), int(idx[-1])}
+    sample = sorted(sample)
+    assert len(sample) >= 32
     lc = LoadedCase(case)
     got_x, got_v = check_against_oracle(case, lc, list(range(256)), "cfg3", sample=sample)
     # R16: velocity rows of a robot are zero once it is inactive
@@ -105,8 +113,11 @@ def test_cfg3_parity_variant_per_robot_dt():
     lc.close()
 
 
-@pytest.mark.parametrize("B,sample", [(1, [0]), (3, [0, 2]), (128, [0, 127])])
+@pytest.mark.parametrize("B,sample", [(1, [0]), (2, [0, 1]), (3, [0, 2]), (4, [1, 3]), (16, [0, 15]), (25, [3, 24]),
+                                      (32, [7, 31]), (49, [11, 48]), (56, [30, 55]), (128, [0, 127])])
 def test_cfg4_sweep_points(B, sample):
+    """Every batch size of the sweep up to 128 (8 and 64 are cfg1 / cfg2's sizes), plus one B inside each range in
+    which the residual GEMMs pick another N-tile width (21-30, 47-51, 52-61: gemm_tcgen05.cu resid_bn)."""
     case = cases.make_case(4, batch=B)
     lc = LoadedCase(case)
     check_against_oracle(case, lc, list(range(B)), f"cfg4-B{B}", sample=sample)
@@ -134,9 +145,11 @@ def test_cfg4_max_batch_512_property_and_sample():
                                small_out, vel, None)
     torch.cuda.synchronize()
     small = small_out.cpu().numpy()
-    # not bitwise: the residual GEMMs pick narrower N tiles at small batch (more CTAs), which changes the summation
-    # order of the fused RMSNorm statistics; a last-bit difference there flips a few fp16 operand roundings downstream
-    assert np.abs(big[pick] - small).max() <= 5e-3
+    # P2 on the GPU.  The RMSNorm statistics no longer depend on the tile width; what is left is the attention
+    # work split: at B = 3 the planner cuts items between CTAs (a segment starts its own running maximum, so P is
+    # rounded to bf16 against another reference, and the partial result is handed over in 16 bits), at B = 512 it
+    # does not.  Measured 2.2e-3 over 18 layers x 10 steps here; 1e-3 holds wherever the plans agree (tests below).
+    assert np.abs(big[pick] - small).max() <= 3e-3
     # robot 511 against the oracle
     row = cfg.n_kv_heads * cfg.head_dim
     sl = slice(511 * 816, 512 * 816)
@@ -391,9 +404,9 @@ def test_adarms_variant_pi0_shapes():
     assert np.array_equal(got_x, again)                                   # P13
     # M = 100 rows: the single-CTA GEMM kernels; batch invariance against the batched run (P2)
     sub, _ = check_against_oracle(case, lc, [4, 1], "adarms-pi0-b2")
-    assert np.abs(sub - got_x[[4, 1]]).max() <= 5e-3
+    assert np.abs(sub - got_x[[4, 1]]).max() <= 1e-3
     one, _ = check_against_oracle(case, lc, [3], "adarms-pi0-b1")         # one robot: one row of cond / modulation
-    assert np.abs(one[0] - got_x[3]).max() <= 5e-3
+    assert np.abs(one[0] - got_x[3]).max() <= 1e-3
     lc.close()
 
 
@@ -487,9 +500,92 @@ def test_soak_random_batch_compositions_are_reproducible():
         a = o1.cpu().numpy()
         assert np.all(np.isfinite(a)) and np.array_equal(a, o2.cpu().numpy()), (b, idx[:4], ns[:4])
         for j, r in enumerate(idx):
-            if int(r) in single and ns[j] == 10:
-                assert np.abs(a[j] - single[int(r)]).max() <= 5e-3
+            if int(r) in single and ns[j] == 10:   # 3e-3: the attention work split differs between a lone robot and a batch
+                assert np.abs(a[j] - single[int(r)]).max() <= 3e-3
         calls += 2
-    print(f"[soak] {calls} calls")
+    print(f"[soak] {calls} calls, {rosa.rosa_debug_graph_captures(lc.expert)} graphs captured")
     assert calls >= 100
     lc.close()
+
+
+def test_bucketed_graphs_no_capture_after_warmup():
+    """Graphs are keyed by (batch bucket, max n_steps): after one call per key, 200 random (batch, n) pairs replay
+    captured graphs only (no capture + instantiate on the request path), and a smaller batch run through its
+    bucket's graph gives each robot the result of its own run."""
+    case = edge_case([70, 150, 33, 90, 64, 200, 10, 129, 300, 17, 64, 65, 5], n_steps=3)
+    lc = LoadedCase(case, max_steps=4)
+    B = case.batch
+    solo = {r: lc.run(robots=[r])[0][0] for r in (0, 7, 12)}
+    noise_all = torch.from_numpy(case.noise).to(lc.device)
+
+    def call(idx, ns):
+        idx = np.asarray(idx, dtype=np.int32)
+        ns = np.asarray(ns, dtype=np.int32)
+        t0 = np.ones(len(idx), np.float32)
+        out = torch.empty((len(idx),) + tuple(noise_all.shape[1:]), dtype=torch.float32, device=lc.device)
+        rosa.rosa_denoise_batch_ex(lc.expert, idx, noise_all[idx.tolist()].contiguous(), t0, (-t0 / ns).astype(np.float32), ns, out)
+        torch.cuda.synchronize()
+        return out.cpu().numpy()
+
+    for bucket in (1, 2, 4, 8, 13):                     # warm-up: one call per (bucket, n)
+        for n in (1, 2, 3, 4):
+            call(list(range(bucket)), [n] * bucket)
+    warm = rosa.rosa_debug_graph_captures(lc.expert)
+    assert warm <= 5 * 4
+    rng = np.random.default_rng(11)
+    for _ in range(200):
+        b = int(rng.integers(1, B + 1))
+        idx = rng.permutation(B)[:b]
+        ns = rng.integers(1, 5, size=b)
+        out = call(idx, ns)
+        assert np.all(np.isfinite(out))
+        for j, r in enumerate(idx):
+            if int(r) in solo and ns[j] == 3:
+                assert np.abs(out[j] - solo[int(r)]).max() <= 1e-3
+    assert rosa.rosa_debug_graph_captures(lc.expert) == warm
+    lc.close()
+
+
+def test_fp16_range_of_the_residual_stream():
+    """The default operand format keeps a 16-bit fp16 copy of the UN-normalised residual h as the A operand of the
+    QKV / gate-up GEMMs (R23); fp16 ends at 65504.  The library's contract (include/rosa.h): the copy
+    SATURATES at +-65504, so an out-of-range residual gives finite, clipped results, never inf / NaN; with
+    ROSA_GEMM_DTYPE=bf16 the operand has the range of fp32 and the same model stays within the bf16-mode accuracy.
+    Here b_t2 (the bias of the embedding MLP's second layer, which enters h0 directly) is scaled so that |h| reaches
+    ~1e5 on some channels while everything downstream is scale-invariant (RMSNorm)."""
+    import os
+    case = edge_case([40, 90], n_steps=2)
+    b = case.weights["b_t2"].copy()
+    b[::7] = cases.round_bf16(np.full_like(b[::7], 1.0e5))
+    case.weights["b_t2"] = b
+    want_x, want_v = O.denoise_case(case, return_velocity=True)
+    lc = LoadedCase(case)
+    got_x, got_v = lc.run(want_velocity=True)
+    lc.close()
+    assert np.all(np.isfinite(got_x)) and np.all(np.isfinite(got_v))          # saturated, not inf / NaN
+    print(f"[fp16-range fp16 operands] actions rel-L2 {rel_l2(got_x, want_x):.3e} (clipped channels)")
+    old = os.environ.get("ROSA_GEMM_DTYPE")
+    os.environ["ROSA_GEMM_DTYPE"] = "bf16"
+    try:
+        lc = LoadedCase(case)
+        got_x, got_v = lc.run(want_velocity=True)
+        lc.close()
+    finally:
+        if old is None:
+            del os.environ["ROSA_GEMM_DTYPE"]
+        else:
+            os.environ["ROSA_GEMM_DTYPE"] = old
+    err = rel_l2(got_x, want_x)
+    print(f"[fp16-range bf16 operands] actions rel-L2 {err:.3e}")
+    assert np.all(np.isfinite(got_x)) and err <= TOL_ACT_REL
+
+
+def test_adarms_variant_needs_the_tcgen05_attention_shape():
+    """time_conditioning = 1 with a head layout the tcgen05 attention kernel does not cover (16 query heads, 2 KV
+    heads) is refused at create, not run through null tensor maps."""
+    from dataclasses import replace
+    cfg = replace(MINI, n_q_heads=16, n_kv_heads=2, time_conditioning=1)
+    case = cases.build_case("adarms-bad-heads", 3, cfg, bf16=True, prefix_lens=[20], n_steps=1)
+    with pytest.raises(rosa.RosaError) as ei:
+        LoadedCase(case)
+    assert ei.value.status == rosa.ROSA_ERR_UNSUPPORTED
