@@ -3,7 +3,7 @@
 
   python bench.py [--gpus N] [--steps K] [--warmup W]            # our arm (CUDA library)
   python bench.py --impl reference ...                           # the CPU oracle, as it stands
-  python bench.py --sweep                                        # cfg4 batch sweep -> gpurun_out/sweep.json
+  python bench.py --sweep                                        # cfg4 batch sweep, long form -> gpurun_out/sweep.json
 
 A *step* is one `rosa_denoise_batch` call: the whole hot path (a1..a11) over one batch of
 synthetic robots — 10 Euler steps of the pi0-scale action expert for B=64 robots with ragged
@@ -15,7 +15,8 @@ at B=64" is quoted on; seeds and recipe in DESIGN.md section 3).  One chunk = on
 Printed JSON keys beyond the base contract: `roofline` (dominant kernel class, event-timed in a
 separate un-graphed profiling pass via rosa_profile_batch), `whole_path` (all algorithmic FLOPs
 of a call / call time against the three peaks), `classes` (per kernel class ms per call),
-`latency_ms` (p50/p99 per call = per chunk), `cpu_baseline`.
+`latency_ms` (p50/p99 per call = per chunk), `cpu_baseline`, `sweep` (BASELINE.json configs[4]: chunks/s, p50 / p99
+and roofline fraction at B = 1..512, a few timed calls each; N = 1 only), `e2e.with_rebind_of_every_robot`.
 """
 from __future__ import annotations
 
@@ -35,9 +36,27 @@ if ROOT not in sys.path:
 
 METRIC = "action_chunks_per_sec_B64_10step"
 UNIT = "chunks/s"
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel class, from the
-# `ncu --set full` capture summarised in profiles/ (None until captured for the current kernel).
-NCU_TRAFFIC_BYTES = {"gemm_gateup_geglu": 24475392}  # profiles/r1_ncu_summary.md: 23.47 MB read + 1.01 MB written
+
+
+def ncu_traffic(kernel_class):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel_class` from the `ncu --set full` capture
+    recorded in profiles/r2_ncu_traffic.json, or (None, why): the record names the sha256 of the kernel source it was
+    captured with, and a number taken from another build of the kernel is not reported."""
+    import hashlib
+    rec = os.path.join(ROOT, "profiles", "r2_ncu_traffic.json")
+    if not os.path.exists(rec):
+        return None, "no capture recorded"
+    with open(rec) as f:
+        d = json.load(f)
+    ent = d.get(kernel_class)
+    if not ent:
+        return None, "no capture of this kernel class"
+    src = os.path.join(ROOT, "paper_2607_01088_b200", "csrc", ent["source"])
+    with open(src, "rb") as f:
+        sha = hashlib.sha256(f.read()).hexdigest()
+    if sha != ent["source_sha256"]:
+        return None, f"capture is of another build of {ent['source']} (profiles/r2_ncu_traffic.json)"
+    return int(ent["dram_bytes_per_launch"]), ent.get("capture", "")
 
 
 def load_peaks():
@@ -299,6 +318,25 @@ def run_ours(args, rank, world, local_rank):
             dist.destroy_process_group()
         return
 
+    # ---- the paper's per-request pattern (every request carries a new observation, so its prefix
+    # K/V is new): rosa_prefix_kv_bind of every robot before every call.  Host time of a bind, and the end-to-end
+    # rate with the 64 re-binds inside the timed region.
+    t_b = time.perf_counter()
+    for _ in range(5):
+        lc.rebind_all()
+    bind_us = (time.perf_counter() - t_b) / (5 * B) * 1e6
+    torch.cuda.synchronize()
+    n_rb = max(3, args.steps // 2)
+    for _ in range(2):
+        lc.rebind_all()
+        rosa.rosa_denoise_batch_host(lc.expert, ids, noise_h, case.t_start, case.dt, case.n_steps, out_h, stream)
+    t_e = time.perf_counter()
+    for _ in range(n_rb):
+        lc.rebind_all()
+        rosa.rosa_denoise_batch_host(lc.expert, ids, noise_h, case.t_start, case.dt, case.n_steps, out_h, stream)
+    torch.cuda.synchronize()
+    e2e_rebind_value = B * n_rb / (time.perf_counter() - t_e)
+
     # ---- per kernel class (separate un-graphed pass with an event between launches)
     n_prof = 3
     cls_ms, cls_n = {}, {}
@@ -310,20 +348,30 @@ def run_ours(args, rank, world, local_rank):
     flops = class_flops(cfg, case.prefix_lens, case.n_steps)
     tot_flops = sum(flops.values())
     tot_bytes = call_bytes(cfg, case.prefix_lens, case.n_steps)
+    # The event-timed pass runs the launches un-graphed (an event between launches defeats the overlap of a kernel's
+    # prologue with its predecessor's tail), so its classes sum to more than the graphed call: `ms_per_call` is the
+    # share of the graphed call (scaled so that the classes sum to ms_per_step), `ms_ungraphed` the raw event time.
+    ungraphed_sum = sum(cls_ms.values())
+    scale = (total_ms / args.steps) / ungraphed_sum if ungraphed_sum > 0 else 1.0
     classes = {}
     for k, ms in cls_ms.items():
-        ent = {"ms_per_call": round(ms, 4), "launches": cls_n[k]}
+        if cls_n[k] == 0:
+            continue
+        ent = {"ms_per_call": round(ms * scale, 4), "ms_ungraphed": round(ms, 4), "launches": cls_n[k]}
         if k in flops and ms > 0:
-            ent["tflops"] = round(flops[k] / (ms * 1e-3) / 1e12, 1)
+            ent["tflops"] = round(flops[k] / (ms * scale * 1e-3) / 1e12, 1)
         classes[k] = ent
     dom = max((k for k in cls_ms if k in flops), key=lambda k: cls_ms[k])
     dom_tf = flops[dom] / (cls_ms[dom] * 1e-3) / 1e12
-    peak = peaks["bf16_tflops_sustained"]
-    roofline = {"bound": "tensor", "kernel": dom, "achieved": round(dom_tf, 1), "peak": peak, "unit": "TFLOP/s",
-                "frac": round(dom_tf / peak, 4), "traffic": NCU_TRAFFIC_BYTES.get(dom),
-                "peak_source": f"{peaks['source']} bf16_tflops_sustained (kernel timed inside a long step)",
+    traffic, traffic_note = ncu_traffic(dom)
+    # SURVEY 8(d) / BASELINE.md 3: the measured BURST peak is the primary denominator; the sustained one beside it
+    roofline = {"bound": "tensor", "kernel": dom, "achieved": round(dom_tf, 1), "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
+                "frac": round(dom_tf / peaks["bf16_tflops"], 4), "traffic": traffic, "traffic_note": traffic_note,
+                "peak_source": f"{peaks['source']} bf16_tflops (burst)",
+                "peak_sustained": peaks["bf16_tflops_sustained"], "frac_sustained": round(dom_tf / peaks["bf16_tflops_sustained"], 4),
                 "launches_per_call": cls_n[dom], "avg_launch_us": round(1e3 * cls_ms[dom] / cls_n[dom], 2),
-                "flops_per_launch": flops[dom] / cls_n[dom]}
+                "flops_per_launch": flops[dom] / cls_n[dom],
+                "timing": "CUDA events between un-graphed launches (rosa_profile_batch), averaged over the call's launches of the class"}
     ms_call = total_ms / args.steps
     t_roof = {name: max(tot_flops / (pk * 1e12), tot_bytes / (peaks["hbm_gbs"] * 1e9)) * 1e3
               for name, pk in (("burst", peaks["bf16_tflops"]), ("sustained", peaks["bf16_tflops_sustained"]),
@@ -359,58 +407,78 @@ def run_ours(args, rank, world, local_rank):
                        "parallelism": f"replicas x{world}, robots sharded, no collective"},
             "latency_ms": {"p50": pct(per_call, 0.5), "p99": pct(per_call, 0.99), "min": min(per_call)},
             "clocks": clocks,
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": io_bytes, "d2h_bytes_per_step": io_bytes},
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": io_bytes, "d2h_bytes_per_step": io_bytes,
+                    "with_rebind_of_every_robot": {"value": e2e_rebind_value, "unit": UNIT, "calls": n_rb,
+                                                   "bind_us_per_robot": round(bind_us, 2),
+                                                   "what": "rosa_prefix_kv_bind of all robots before every call (borrowed bf16 K/V, "
+                                                           "asynchronous table update), host wall clock, this rank"}},
             "gpu_launches": int(launches_per_call * args.steps),
-            "roofline": roofline, "whole_path": whole, "classes": classes}
+            "roofline": roofline, "whole_path": whole, "classes": classes,
+            "classes_ungraphed_sum_ms": round(ungraphed_sum, 3)}
     if cpu:
         line["cpu_baseline"] = cpu
-    print(json.dumps(line), flush=True)
     lc.close()
+    del lc
+    torch.cuda.empty_cache()
+    if world == 1 and not args.no_sweep:
+        line["sweep"] = sweep_rows(torch, rosa, cases, peaks, stream, compact=True)
+    print(json.dumps(line), flush=True)
     if dist:
         dist.destroy_process_group()
 
 
-def run_sweep(args):
-    """cfg4: B in {1..512}, L=816, 10 steps; chunks/s, p50/p99, roofline fraction per B."""
-    import torch
-    from paper_2607_01088_b200 import binding as rosa
-    from paper_2607_01088_b200 import build as rosa_build
-    from paper_2607_01088_b200 import cases
+def sweep_rows(torch, rosa, cases, peaks, stream, compact, sweep_max=512):
+    """BASELINE.json configs[4]: B in {1..512}, prefix length 816, 10 Euler steps, ONE expert (max_batch 512) with 512
+    robots bound; batch size B = its first B robots.  Per B: chunks/s, p50 / p99 per call (= per chunk), roofline
+    fraction against the measured burst peak.  compact = the few-second version that rides in the default line."""
     from paper_2607_01088_b200.runner import DeviceFleet
-    rosa_build.build()
-    rosa.load()
-    peaks = load_peaks()
     base = cases.make_case(4, batch=1, with_prefix=False)
     cfg = base.cfg
-    stream = torch.cuda.Stream()
+    n_rob = min(512, sweep_max)
+    fl = DeviceFleet(base, [816] * n_rob, seed=4)
     rows = []
     for B in cases.SWEEP_BATCHES:
-        if B > args.sweep_max:
+        if B > n_rob:
             break
-        fl = DeviceFleet(base, [816] * B, seed=4)
         ids = np.arange(B, dtype=np.int32)
         t0 = np.ones(B, dtype=np.float32)
         ns = np.full(B, 10, dtype=np.int32)
         dt = (-t0 / 10).astype(np.float32)
-        out = torch.empty_like(fl.noise)
-        steps = max(10, min(200, int(2000 / max(1.0, B * 0.4))))
+        noise = fl.noise[:B].contiguous()
+        out = torch.empty_like(noise)
+        if compact:
+            steps = 20 if B <= 64 else (10 if B <= 128 else 6)
+        else:
+            steps = max(10, min(200, int(2000 / max(1.0, B * 0.4))))
         with torch.cuda.stream(stream):
-            total_ms, per_call = measure(torch, rosa, fl.expert, ids, fl.noise, t0, dt, ns, out, stream, steps, 5)
+            total_ms, per_call = measure(torch, rosa, fl.expert, ids, noise, t0, dt, ns, out, stream, steps, 3)
         ms = total_ms / steps
         fl_tot = sum(class_flops(cfg, [816] * B, ns).values())
         by = call_bytes(cfg, [816] * B, ns)
         t_c, t_m = fl_tot / (peaks["bf16_tflops"] * 1e12) * 1e3, by / (peaks["hbm_gbs"] * 1e9) * 1e3
-        row = {"B": B, "chunks_per_s": B / (ms * 1e-3), "ms_per_call": ms, "p50_ms": pct(per_call, 0.5),
-               "p99_ms": pct(per_call, 0.99), "bound": "tensor" if t_c > t_m else "hbm",
-               "roofline_ms": max(t_c, t_m), "roofline_frac": max(t_c, t_m) / ms,
-               # SURVEY 8(d): also against the sustained measured peak and the nominal 2250 TFLOP/s / 8 TB/s
-               "roofline_frac_sustained": max(fl_tot / (peaks["bf16_tflops_sustained"] * 1e12) * 1e3, t_m) / ms,
-               "roofline_frac_nominal": max(fl_tot / 2250e12, by / 8000e9) * 1e3 / ms, "steps": steps}
+        row = {"B": B, "chunks_per_s": round(B / (ms * 1e-3), 1), "ms_per_call": round(ms, 3), "p50_ms": round(pct(per_call, 0.5), 3),
+               "p99_ms": round(pct(per_call, 0.99), 3), "bound": "tensor" if t_c > t_m else "hbm",
+               "roofline_ms": round(max(t_c, t_m), 3), "roofline_frac": round(max(t_c, t_m) / ms, 4), "calls": steps}
+        if not compact:  # SURVEY 8(d): also against the sustained measured peak and the nominal 2250 TFLOP/s / 8 TB/s
+            row["roofline_frac_sustained"] = max(fl_tot / (peaks["bf16_tflops_sustained"] * 1e12) * 1e3, t_m) / ms
+            row["roofline_frac_nominal"] = max(fl_tot / 2250e12, by / 8000e9) * 1e3 / ms
         rows.append(row)
+    fl.close()
+    return rows
+
+
+def run_sweep(args):
+    """cfg4 on its own: more timed calls per batch size; rows printed and written to gpurun_out/sweep.json."""
+    import torch
+    from paper_2607_01088_b200 import binding as rosa
+    from paper_2607_01088_b200 import build as rosa_build
+    from paper_2607_01088_b200 import cases
+    rosa_build.build()
+    rosa.load()
+    peaks = load_peaks()
+    rows = sweep_rows(torch, rosa, cases, peaks, torch.cuda.Stream(), compact=False, sweep_max=args.sweep_max)
+    for row in rows:
         print(json.dumps(row), flush=True)
-        fl.close()
-        del fl
-        torch.cuda.empty_cache()
     os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
     with open(os.path.join(ROOT, "gpurun_out", "sweep.json"), "w") as f:
         json.dump({"peaks": peaks, "rows": rows}, f, indent=1)
@@ -428,6 +496,7 @@ def main():
                     help="concat = the contract workload (pi0-style); adarms = the adaptive-RMSNorm variant (extra line)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true")
+    ap.add_argument("--no-sweep", action="store_true", help="leave the compact cfg4 sweep out of the default line")
     ap.add_argument("--sweep-max", type=int, default=512)
     args = ap.parse_args()
     if args.batch is None:

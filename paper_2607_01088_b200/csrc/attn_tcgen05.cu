@@ -426,8 +426,15 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
           if (merge && !part_issued) flag_seen = ld_relaxed_gpu(part_flag + sg.part0);
         }
         __syncwarp();
+#ifdef ROSA_TRACE
+#define AT_BLK(k) do { if ((warp == 2 || warp == 6) && i == 4 && si == seg_beg) AT_TRACE((warp == 2 ? 40 : 48) + (k)); } while (0)
+#else
+#define AT_BLK(k) do { } while (0)
+#endif
+        AT_BLK(0);
         mbar_wait(s_full(sb), (gi >> 1) & 1);
         tc_fence_after();
+        AT_BLK(1);
         if (warp == 2 && i == 0) AT_TRACE(8 + 8 * (si - seg_beg) + 0);
         // Each warp of a row's pair reads only its own 32 scores; the row maximum of the block is exchanged through
         // shared memory (so both take the same rescale decision).  P is stored over this warp's OWN score columns
@@ -453,7 +460,9 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
           const uint32_t mb = __float_as_uint(mo);
           const uint16_t up = (uint16_t)((mo >= 0.f ? mb + 0xffffu : mb) >> 16);
           mx[(gi & 1) * (2 * AT_ROWS) + half * AT_ROWS + r] = up;
+          AT_BLK(2);
           named_bar_sync(5 + q, 64);
+          AT_BLK(3);
           const uint16_t other = mx[(gi & 1) * (2 * AT_ROWS) + (half ^ 1) * AT_ROWS + r];
           m_blk = fmaxf(__uint_as_float((uint32_t)up << 16), __uint_as_float((uint32_t)other << 16));
         }
@@ -477,9 +486,11 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
           }
         }
         l_sum = l_sum * factor + (s0 + s1);
+        AT_BLK(4);
         // Every block, not only when rescaling: a parity wait is only meaningful while the waiter is at
         // most one phase behind the barrier (PV(gi-1) was issued ~a softmax block ago, so this is free).
         if (gi > 0) mbar_wait(pv_done, (gi - 1) & 1);
+        AT_BLK(5);
         if (i > 0 && __any_sync(0xffffffffu, factor != 1.f)) {  // rare: rescale this warp's rows, its half of O's columns
           tc_fence_after();                                     // O quiescent: PV(gi-1) done, PV(gi) needs this P
 #pragma unroll 1
@@ -498,6 +509,7 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(p_full(sb));  // 256 arrivals on one barrier would serialise on the critical path
+        AT_BLK(6);
         if (issuer && flag_seen != 0) { fetch_partial(sg.part0); part_issued = true; }
         __syncwarp();
       }
@@ -657,61 +669,76 @@ int tc_attn_tiles(const Dims& dm) { return (dm.H + AT_TOK - 1) / AT_TOK; }
 // costs on top of its blocks (Q load and copy, pipeline refill, O drain: clock trace profiles/r2_attn_trace.md).
 constexpr double kSegOvh = 6.0;
 
+// Stream-K over ROBOTS on GROUPS of tpr CTAs: CTA tpr g + t of group g handles tile t of the robots (and parts of
+// robots) assigned to the group, so the tpr tiles of a robot run side by side, in lockstep (they cost the same),
+// and the robot's K/V stream is read from HBM once and from L2 by the other tiles - whatever the batch size (a
+// layer's prefix K/V stops fitting in L2 at B >= 128).  The concatenated key streams of the robots are cut into
+// equal shares per group; a robot that straddles a cut is cut at the same key block for all its tiles: tile t's
+// head segment ends the list of CTA tpr g + t, its continuation starts the list of CTA tpr (g + 1) + t.
 static int attn_plan_cut(const Dims& dm, int n_active, const int* len, int n_cta, std::vector<AttnSeg>& segs, int* offs) {
   constexpr double kMinShare = 10.0;
   constexpr int kMinSeg = 2;
   const int tpr = tc_attn_tiles(dm);
   const size_t seg0 = segs.size();
-  double total = 0.0;
-  for (int p = 0; p < n_active; ++p) total += tpr * ((len[p] + AT_KV - 1) / AT_KV + 1 + kSegOvh);
-  const int used = (int)std::min<double>(n_cta, std::max(1.0, std::floor(total / kMinShare)));
-  // units not yet assigned, counting one extra segment overhead for each of the used - 1 CTA boundaries still ahead
-  // (most of them cut an item in two); a boundary that falls between two items gives its overhead back
-  double left = total + kSegOvh * (used - 1);
-  double target = left / used;  // share of the current CTA: re-derived at every CTA from what is left
-  int cta = 0;
-  double acc = 0.0;
-  offs[0] = (int)seg0;
-  auto next_cta = [&](bool cut) {
-    if (cta + 1 < used) {
-      if (!cut) left -= kSegOvh;
-      ++cta; offs[cta] = (int)segs.size(); acc = 0.0; target = left / (used - cta);
-    }
-  };
-  for (int p = 0; p < n_active; ++p) {
-    const int nb = (len[p] + AT_KV - 1) / AT_KV + 1;
-    for (int tt = 0; tt < tpr; ++tt) {
+  const int groups = n_cta / tpr;
+  std::vector<std::vector<AttnSeg>> lists(n_cta);
+  if (groups >= 1) {
+    double total = 0.0;
+    for (int p = 0; p < n_active; ++p) total += (len[p] + AT_KV - 1) / AT_KV + 1 + kSegOvh;
+    const int used = (int)std::min<double>(groups, std::max(1.0, std::floor(total / kMinShare)));
+    // units not yet assigned, counting one extra segment overhead for each of the used - 1 group boundaries still
+    // ahead (most of them cut a robot in two); a boundary that falls between two robots gives its overhead back
+    double left = total + kSegOvh * (used - 1);
+    double target = left / used;  // share of the current group: re-derived at every group from what is left
+    int g = 0;
+    double acc = 0.0;
+    auto next_group = [&](bool cut) {
+      if (g + 1 < used) {
+        if (!cut) left -= kSegOvh;
+        ++g; acc = 0.0; target = left / (used - g);
+      }
+    };
+    for (int p = 0; p < n_active; ++p) {
+      const int nb = (len[p] + AT_KV - 1) / AT_KV + 1;
       int kb = 0, n_seg = 0;
-      const size_t head = segs.size();
+      int head_g = -1;
       while (kb < nb) {
         const int rem = nb - kb;
         const double room = target - acc;
         int take = rem;
-        if (cta + 1 < used && rem + kSegOvh > room + 0.5 && n_seg < 1) {
+        if (g + 1 < used && rem + kSegOvh > room + 0.5 && n_seg < 1) {
           take = (int)std::floor(room - kSegOvh + 0.5);
-          if (take < kMinSeg) {            // not worth starting here: the next CTA takes it
-            if (acc > 0.0) { next_cta(kb > 0); continue; }
+          if (take < kMinSeg) {            // not worth starting here: the next group takes it
+            if (acc > 0.0) { next_group(false); continue; }
             take = std::min(rem, kMinSeg);
           }
           if (rem - take < kMinSeg) take = rem;   // no crumbs at the end either
         }
-        AttnSeg sg{};
-        sg.p = p; sg.robot = p; sg.len = len[p]; sg.tt = (int16_t)tt; sg.kb0 = (int16_t)kb; sg.kb1 = (int16_t)(kb + take);
-        sg.n_part = kb == 0 ? 0 : -1; sg.part0 = -1;
-        if (kb > 0) {  // a continuation is the first entry of a CTA's list; the head segment collects it
-          segs[head].n_part += 1;
-          if (segs[head].part0 < 0) segs[head].part0 = (int16_t)cta;
+        for (int tt = 0; tt < tpr; ++tt) {
+          AttnSeg sg{};
+          sg.p = p; sg.robot = p; sg.len = len[p]; sg.tt = (int16_t)tt; sg.kb0 = (int16_t)kb; sg.kb1 = (int16_t)(kb + take);
+          sg.n_part = kb == 0 ? 0 : -1; sg.part0 = -1;
+          if (kb > 0) {  // a continuation is the first entry of its CTA's list; the head segment of the same tile collects it
+            AttnSeg& head = lists[head_g * tpr + tt].back();
+            head.n_part = 1;
+            head.part0 = (int16_t)(g * tpr + tt);
+          }
+          lists[g * tpr + tt].push_back(sg);
         }
-        segs.push_back(sg);
+        if (kb == 0) head_g = g;
         ++n_seg;
         kb += take;
         acc += take + kSegOvh;
         left -= take + kSegOvh;
-        if (kb < nb || acc >= target - 0.5) next_cta(kb < nb);
+        if (kb < nb || acc >= target - 0.5) next_group(kb < nb);
       }
     }
   }
-  for (int c = cta + 1; c <= n_cta; ++c) offs[c] = (int)segs.size();
+  for (int c = 0; c < n_cta; ++c) {
+    offs[c] = (int)segs.size();
+    segs.insert(segs.end(), lists[c].begin(), lists[c].end());
+  }
+  offs[n_cta] = (int)segs.size();
   return (int)(segs.size() - seg0);
 }
 
@@ -725,8 +752,11 @@ static int attn_plan_whole(const Dims& dm, int n_active, const int* len, int n_c
   std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return len[a] > len[b]; });
   std::vector<double> load(n_cta, 0.0);
   std::vector<std::vector<AttnSeg>> lists(n_cta);
-  for (int tt = 0; tt < tpr; ++tt)        // tile-major: the tiles of one robot run on different CTAs at the same time
-    for (int x = 0; x < n_active; ++x) {
+  // Robot-major: the tiles of one robot go to the (then) least loaded CTAs one after the other, i.e. to CTAs that
+  // reach them at about the same time, so the robot's K/V is read from HBM once and from L2 by the other tiles
+  // (at B >= 128 a layer's prefix K/V no longer fits in L2: tile-major order re-read it from HBM for every tile).
+  for (int x = 0; x < n_active; ++x)
+    for (int tt = 0; tt < tpr; ++tt) {
       const int p = order[x], nb = (len[p] + AT_KV - 1) / AT_KV + 1;
       int c = 0;
       for (int k = 1; k < n_cta; ++k) if (load[k] < load[c]) c = k;
@@ -763,7 +793,7 @@ int attn_build_list(const Dims& dm, int n_active, const int* len, int n_cta, std
   attn_plan_cut(dm, n_active, len, n_cta, a, oa.data());
   attn_plan_whole(dm, n_active, len, n_cta, b, ob.data());
   const double ta = attn_plan_makespan(a, seg0, oa.data(), n_cta), tb2 = attn_plan_makespan(b, seg0, ob.data(), n_cta);
-  const bool use_cut = ta < tb2;
+  const bool use_cut = a.size() > seg0 && ta < tb2;
   segs.swap(use_cut ? a : b);
   for (int c = 0; c <= n_cta; ++c) offs[c] = use_cut ? oa[c] : ob[c];
   return (int)(segs.size() - seg0);

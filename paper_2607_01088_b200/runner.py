@@ -41,11 +41,11 @@ class LoadedCase:
                     kl.append(torch.from_numpy(k.view(np.int16)).to(self.device).view(torch.bfloat16))
                     vl.append(torch.from_numpy(v.view(np.int16)).to(self.device).view(torch.bfloat16))
                 self.kv_buffers = kl + vl
-                for i in range(B):
-                    off = int(cu[i]) * row * 2
-                    rosa.rosa_prefix_kv_bind(self.expert, i, [t.data_ptr() + off for t in kl],
-                                             [t.data_ptr() + off for t in vl], int(case.prefix_lens[i]),
-                                             rosa.ROSA_BF16)
+                # per robot: (K pointers per layer, V pointers per layer, length) into the packed buffers
+                self.bind_args = [([t.data_ptr() + int(cu[i]) * row * 2 for t in kl],
+                                   [t.data_ptr() + int(cu[i]) * row * 2 for t in vl], int(case.prefix_lens[i]))
+                                  for i in range(B)]
+                self.rebind_all()
             else:
                 for i in range(B):
                     ks = [torch.from_numpy(np.ascontiguousarray(case.prefix_k[i][l])).to(self.device)
@@ -54,6 +54,12 @@ class LoadedCase:
                           for l in range(cfg.layers)]
                     rosa.rosa_prefix_kv_bind(self.expert, i, ks, vs, int(case.prefix_lens[i]), rosa.ROSA_F32)
             torch.cuda.synchronize(self.device)
+
+    def rebind_all(self):
+        """rosa_prefix_kv_bind for every robot of a bf16 case (what a serving loop does when each request carries a
+        new observation): borrowed pointers, no copy."""
+        for i, (kp, vp, length) in enumerate(self.bind_args):
+            rosa.rosa_prefix_kv_bind(self.expert, i, kp, vp, length, rosa.ROSA_BF16)
 
     def kv_bytes(self) -> int:
         return sum(t.numel() * t.element_size() for t in self.kv_buffers)

@@ -60,9 +60,10 @@ def test_argument_validation_without_gpu(lib):
 
 def check_attn_plan(H, lens, n_cta):
     """Invariants of the stream-K split of the attention step (attn_tcgen05.cu): every key block of every item is
-    covered exactly once; a head segment (kb0 = 0) is the last entry of its CTA's list unless the item is whole;
-    a continuation is the FIRST entry of its CTA's list and sits on the CTAs part0 .. part0 + n_part - 1 right
-    after the head's CTA; nothing is shorter than 2 blocks unless the item is."""
+    covered exactly once; an item is whole or cut in two; the head segment (kb0 = 0) of a cut item is the LAST entry
+    of its CTA's list and names the CTA of the continuation (the same tile's CTA of the next group: + tiles), where
+    the continuation is the FIRST entry of the list (a CTA never waits for work queued behind something that
+    waits); the tiles of a robot are cut at the same key block; nothing is shorter than 2 blocks unless the item is."""
     offs, segs = rosa.rosa_debug_attn_plan(H, lens, n_cta)
     tiles = (H + 15) // 16
     assert offs[0] == 0 and offs[-1] == len(segs) and np.all(np.diff(offs) >= 0)
@@ -84,9 +85,10 @@ def check_attn_plan(H, lens, n_cta):
         assert head[2] == len(parts) - 1 and len(parts) <= 2       # n_part of the head = number of continuations (at most one)
         if len(parts) > 1:
             assert head[5] == offs[head[4] + 1] - 1               # the head ends its CTA's list
-            assert head[3] == head[4] + 1                         # the continuations follow on the next CTAs
-            for k, c in enumerate(parts[1:]):
-                assert c[2] == -1 and c[4] == head[4] + 1 + k and c[5] == offs[c[4]]   # first entry of that CTA
+            assert head[3] == head[4] + tiles                     # the continuation: same tile, next group of CTAs
+            c = parts[1]
+            assert c[2] == -1 and c[4] == head[3] and c[5] == offs[c[4]]              # first entry of that CTA
+            assert parts[0][1] == cover[(p, 0)][0][1]             # every tile of the robot is cut at the same block
             assert all(b - a >= 2 for a, b, *_ in parts)
         for a, b, _, _, cta, _ in parts:
             loads[cta] += b - a + 6.0
