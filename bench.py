@@ -250,6 +250,7 @@ def run_ours(args, rank, world, local_rank):
     from paper_2607_01088_b200 import build as rosa_build
     from paper_2607_01088_b200 import cases
     from paper_2607_01088_b200.runner import LoadedCase
+    from paper_2607_01088_b200.sharding import assign_robots, max_over_ranks, whole_job_rate
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
@@ -266,7 +267,14 @@ def run_ours(args, rank, world, local_rank):
     B = args.batch
     # same weights on every rank, different robots; --config 3 = the continuous-batching mix (extra line, not the contract metric)
     ada = args.time_conditioning == "adarms"
-    case = cases.make_case(args.config, batch=B, robot_stream=rank, time_conditioning=1 if ada else 0)
+    if args.scaling == "strong" and world > 1:
+        # ONE fleet of B robots, partitioned over the ranks by prefix length (KV bytes and attention work, LPT);
+        # every rank draws the same fleet and takes its shard: no communication
+        fleet = cases.make_case(args.config, batch=B, time_conditioning=1 if ada else 0)
+        case = fleet.subset(assign_robots(fleet.prefix_lens, fleet.cfg.horizon, world)[rank])
+        B = case.batch
+    else:   # weak: B robots per rank; same weights on every rank, different robots
+        case = cases.make_case(args.config, batch=B, robot_stream=rank, time_conditioning=1 if ada else 0)
     cfg = case.cfg
     lc = LoadedCase(case, device=dev)
     stream = torch.cuda.Stream(device=dev)
@@ -286,11 +294,13 @@ def run_ours(args, rank, world, local_rank):
         clocks = sampler.stop()
     launches_per_call = rosa.rosa_last_launch_count(lc.expert)
     family = rosa.rosa_kernel_family(lc.expert)
-    if dist:
-        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
-    value = world * B * args.steps / (total_ms * 1e-3)
+    total_ms = max_over_ranks(total_ms, dist, dev)          # device time of the slowest rank
+    units = [B] * world
+    if dist and args.scaling == "strong":
+        got = [None] * world
+        dist.all_gather_object(got, B)
+        units = [int(u) for u in got]
+    value = whole_job_rate(units, args.steps, total_ms)     # chunks of all ranks / that time
 
     # ---- end to end: host buffers, H2D + D2H inside the timed region, through the C ABI
     noise_h = torch.from_numpy(case.noise).pin_memory()
@@ -305,11 +315,8 @@ def run_ours(args, rank, world, local_rank):
         rosa.rosa_denoise_batch_host(lc.expert, ids, noise_h, case.t_start, case.dt, case.n_steps, out_h, stream)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t_e
-    if dist:
-        t = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
-    e2e_value = world * B * args.steps / e2e_s
+    e2e_s = max_over_ranks(e2e_s, dist, dev)
+    e2e_value = whole_job_rate(units, args.steps, e2e_s * 1e3)
     io_bytes = int(noise_h.numel() * 4)
 
     if rank != 0:
@@ -393,7 +400,7 @@ def run_ours(args, rank, world, local_rank):
                          f"{t_cpu:.1f} s wall"}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_call, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": ms_call, "higher_is_better": True, "scaling": args.scaling if world > 1 else "weak",
             "vs_baseline": None, "dtype": "fp16 operands / fp32 accumulate" if os.environ.get("ROSA_GEMM_DTYPE") != "bf16"
             else "bf16 operands / fp32 accumulate", "data": "synthetic",
             "config": {"workload": f"cfg{args.config} " + ("fleet batch" if args.config == 2 else "continuous-batching mix (t_i in {1.0..0.1}, n_i = 10 t_i)") + (", adaptive-RMSNorm time conditioning (pi0.5-style variant, DESIGN.md R25; not the contract workload)" if ada else "") + f": B={B} robots/GPU, pi0-scale expert (18L d1024 8q/1kv hd256 "
@@ -494,6 +501,8 @@ def main():
     ap.add_argument("--config", type=int, default=2, choices=[2, 3], help="2 = fleet batch (the metric), 3 = continuous-batching mix")
     ap.add_argument("--time-conditioning", default="concat", choices=["concat", "adarms"],
                     help="concat = the contract workload (pi0-style); adarms = the adaptive-RMSNorm variant (extra line)")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = --batch robots per GPU (default); strong = one fleet of --batch robots sharded by prefix length")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true")
     ap.add_argument("--no-sweep", action="store_true", help="leave the compact cfg4 sweep out of the default line")

@@ -8,6 +8,8 @@
 #include <numeric>
 #include <tuple>
 
+#include <nvtx3/nvToolsExt.h>   // header-only NVTX: host ranges around a call, its capture and each Euler step
+
 #include "rosa_internal.h"
 
 namespace rosa {
@@ -594,6 +596,8 @@ static cudaError_t enqueue_steps(rosa_expert* e, const Tables& tb, int nmax, cud
   cudaError_t err;
   const bool fused_norm = e->family == 1;  // RMSNorm fused into the GEMM epilogues (tcgen05 family)
   for (int k = 0; k < nmax; ++k) {
+    struct StepRange { StepRange(int k) { char nm[32]; snprintf(nm, sizeof(nm), "rosa euler step %d", k); nvtxRangePushA(nm); }
+                       ~StepRange() { nvtxRangePop(); } } step_range(k);
     EpiArgs ea{};
     ea.m_active = tb.m_active + k;
     ea.H = dm.H; ea.hd = dm.hd; ea.gu_blk = dm.gu_blk; ea.in_fp16 = dm.fp16; ea.out_fp16 = dm.fp16;
@@ -771,9 +775,11 @@ static rosa_status_t denoise_impl(rosa_expert* e, int batch, const int32_t* ids,
   auto it = e->graphs.find(key);
   if (it == e->graphs.end()) {
     cudaGraph_t g = nullptr;
+    nvtxRangePushA("rosa graph capture");
     CK(cudaStreamBeginCapture(e->cap_stream, cudaStreamCaptureModeThreadLocal));
     cudaError_t err = enqueue_call(e, bucket, nmax, e->cap_stream);
     cudaError_t err2 = cudaStreamEndCapture(e->cap_stream, &g);
+    nvtxRangePop();
     if (err != cudaSuccess || err2 != cudaSuccess) {
       if (g) cudaGraphDestroy(g);
       set_error(std::string("graph capture failed: ") + cudaGetErrorString(err != cudaSuccess ? err : err2));

@@ -103,7 +103,13 @@ def profile(batch_sizes: Sequence[int], service_pool: Dict[int, Sequence[float]]
 def feasible_configs(prof: Dict[int, dict], freq_hz: float, slo_ms: float, percentile: str = "p99_ms") -> List[dict]:
     """P(f) for one model: (b, k) with aggregate load k f under the worker's maximum
     throughput and the SLO percentile of L(b, k f) (linear interpolation between profiled rates) below
-    the deadline.  For each b the largest feasible k is marked `best`."""
+    the deadline.  For each b the largest feasible k is marked `best`.
+
+    Below the lowest profiled rate nothing is extrapolated flat: a discrete-batch worker waits for
+    b requests, so at low load the batch-fill wait grows as 1 / lambda - the first request of a batch waits for
+    b - 1 more arrivals, (b - 1) / lambda, before the service time even starts (mean: half of that).  That lower
+    bound (and never less than the lowest profiled point) is what is compared with the deadline there
+    ("valid only if it satisfies the SLO under the corresponding load", PAPER.md:352)."""
     out = []
     for b, p in sorted(prof.items()):
         rates = np.array([r["rate_per_s"] for r in p["rates"]])
@@ -113,9 +119,10 @@ def feasible_configs(prof: Dict[int, dict], freq_hz: float, slo_ms: float, perce
         k = b
         while k * freq_hz <= rates[-1]:
             lam = k * freq_hz
-            l = float(np.interp(lam, rates, lats)) if lam >= rates[0] else float(lats[0])
+            fill_ms = 1e3 * (b - 1) / lam
+            l = float(np.interp(lam, rates, lats)) if lam >= rates[0] else max(float(lats[0]), p["service_ms_mean"] + fill_ms)
             if l <= slo_ms:
-                mean = float(np.interp(lam, rates, means)) if lam >= rates[0] else float(means[0])
+                mean = float(np.interp(lam, rates, means)) if lam >= rates[0] else max(float(means[0]), p["service_ms_mean"] + 0.5 * fill_ms)
                 best = {"batch": int(b), "robots": int(k), "load_per_s": lam, percentile: l, "mean_ms": mean}
                 out.append(dict(best))
             k += 1

@@ -92,3 +92,25 @@ def test_bench_work_accounting_for_both_time_conditionings():
     extra = bench.call_bytes(ada, lens, ns) - bench.call_bytes(cases.PI0, lens, ns)
     # parameters per step (2 B each): + 37 modulation matrices and biases, - the action half of W_1, - the 37 gain vectors
     assert abs(extra / 10 / 2 - (37 * (3 * 1024 ** 2 + 3 * 1024) - 1024 ** 2 - 37 * 1024)) < 1
+
+
+def test_feasible_configs_does_not_extrapolate_flat_below_the_profiled_rates():
+    """b = 16, 13.5 ms service, 16 robots at 1 Hz sits below the lowest profiled rate (10% of the maximum
+    throughput); the discrete-batch worker's first request of a batch waits ~15 inter-arrival times there.  The
+    feasible set must agree with the simulator on the same load: not feasible under a 200 ms deadline."""
+    from paper_2607_01088_b200 import latency_profile as lp
+    b, service = 16, 13.5e-3
+    prof = lp.profile([b], {b: [service] * 8}, n_requests=1500, seed=1)
+    lam = 16 * 1.0
+    assert lam < prof[b]["rates"][0]["rate_per_s"]
+    rng = np.random.default_rng(0)
+    arr = lp.periodic_arrivals(16, 1.0, 1600, rng)
+    lat = lp.simulate_discrete_batching(arr, b, lambda m: service)
+    lat = lat[~np.isnan(lat)][200:]
+    p99_sim = 1e3 * float(np.percentile(lat, 99))
+    assert p99_sim > 200.0                                          # the simulator says: deadline missed
+    conf = lp.feasible_configs(prof, 1.0, 200.0)
+    assert not any(c["batch"] == b and c["robots"] == 16 for c in conf)
+    # and where the bound applies it is within the simulator's percentile (a lower bound, not a guess)
+    bound = prof[b]["service_ms_mean"] + 1e3 * (b - 1) / lam
+    assert bound <= p99_sim * 1.05
