@@ -117,12 +117,14 @@ def feasible_configs(prof: Dict[int, dict], freq_hz: float, slo_ms: float, perce
         means = np.array([r.get("mean_ms", r[percentile]) for r in p["rates"]])
         best = None
         k = b
+        # service time of a batch: recorded by profile(); a hand-built profile without it: b / the highest profiled rate
+        service_ms = float(p.get("service_ms_mean", 1e3 * b / rates[-1]))
         while k * freq_hz <= rates[-1]:
             lam = k * freq_hz
             fill_ms = 1e3 * (b - 1) / lam
-            l = float(np.interp(lam, rates, lats)) if lam >= rates[0] else max(float(lats[0]), p["service_ms_mean"] + fill_ms)
+            l = float(np.interp(lam, rates, lats)) if lam >= rates[0] else max(float(lats[0]), service_ms + fill_ms)
             if l <= slo_ms:
-                mean = float(np.interp(lam, rates, means)) if lam >= rates[0] else max(float(means[0]), p["service_ms_mean"] + 0.5 * fill_ms)
+                mean = float(np.interp(lam, rates, means)) if lam >= rates[0] else max(float(means[0]), service_ms + 0.5 * fill_ms)
                 best = {"batch": int(b), "robots": int(k), "load_per_s": lam, percentile: l, "mean_ms": mean}
                 out.append(dict(best))
             k += 1
