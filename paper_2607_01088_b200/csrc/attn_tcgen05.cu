@@ -666,7 +666,7 @@ int tc_attn_tiles(const Dims& dm) { return (dm.H + AT_TOK - 1) / AT_TOK; }
 // a share is at least kMinShare units); no segment is shorter than kMinSeg blocks and no item has more than 2
 // segments (the head merges at most one partial result).  offs[c] .. offs[c+1] = segments of CTA c (offs has n_cta + 1 entries; CTAs without work get none).
 // Cost model of the planners, in units of one 64-key block inside a running segment (~1.7k cycles): what a segment
-// costs on top of its blocks (Q load and copy, pipeline refill, O drain: clock trace profiles/r2_attn_trace.md).
+// costs on top of its blocks (Q load and copy, pipeline refill, O drain: clock trace DESIGN.md section 5d).
 constexpr double kSegOvh = 6.0;
 
 // Stream-K over ROBOTS on GROUPS of tpr CTAs: CTA tpr g + t of group g handles tile t of the robots (and parts of

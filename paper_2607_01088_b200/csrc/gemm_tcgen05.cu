@@ -106,7 +106,7 @@ __device__ __forceinline__ float row_rscale(const EpiArgs& ea, int row) {
 // trace of round 1 showed this epilogue bound by instruction issue before that).
 // Tried in round 2 and dropped: starting the accumulator as h (written into tensor memory by these warps before the
 // tile's first MMA, for the first tiles before the dependency wait) so that the epilogue only writes.  The clock trace
-// (profiles/r2_gemm_trace.md) shows why it does not pay: the ~10k cycles after the last MMA are the 130 CTAs of the
+// shows why it does not pay: the ~10k cycles after the last MMA are the 130 CTAs of the
 // single-round launch storing 22 MB at the same time, not the residual loads; the preload delayed the first MMA and
 // pulled 13 MB through L2 under the previous kernel's tail: +1 ms per call.
 // 16-bit copy of h: fp16 saturates at the largest finite value instead of becoming inf (include/rosa.h: range of the
