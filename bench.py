@@ -40,10 +40,10 @@ UNIT = "chunks/s"
 
 def ncu_traffic(kernel_class):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel_class` from the `ncu --set full` capture
-    recorded in profiles/r2_ncu_traffic.json, or (None, why): the record names the sha256 of the kernel source it was
+    recorded in profiles/r2_ncu_traffic.txt, or (None, why): the record names the sha256 of the kernel source it was
     captured with, and a number taken from another build of the kernel is not reported."""
     import hashlib
-    rec = os.path.join(ROOT, "profiles", "r2_ncu_traffic.json")
+    rec = os.path.join(ROOT, "profiles", "r2_ncu_traffic.txt")
     if not os.path.exists(rec):
         return None, "no capture recorded"
     with open(rec) as f:
@@ -55,7 +55,7 @@ def ncu_traffic(kernel_class):
     with open(src, "rb") as f:
         sha = hashlib.sha256(f.read()).hexdigest()
     if sha != ent["source_sha256"]:
-        return None, f"capture is of another build of {ent['source']} (profiles/r2_ncu_traffic.json)"
+        return None, f"capture is of another build of {ent['source']} (profiles/r2_ncu_traffic.txt)"
     return int(ent["dram_bytes_per_launch"]), ent.get("capture", "")
 
 

@@ -466,10 +466,15 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
           const uint16_t other = mx[(gi & 1) * (2 * AT_ROWS) + (half ^ 1) * AT_ROWS + r];
           m_blk = fmaxf(__uint_as_float((uint32_t)up << 16), __uint_as_float((uint32_t)other << 16));
         }
-        m_blk *= c_log2;
+        // The reference is an INTEGER in the log2 domain: a different reference (another lazy-rescale history,
+        // another cut of the key stream between CTAs: R27) then scales P, l and O by an exact power of two, so the
+        // bf16 rounding of P - the dominant rounding of the whole attention step - is the same whichever way the
+        // item was planned.  What is left between two plans is fp32 summation order and the 16-bit hand-over.
+        m_blk = ceilf(m_blk * c_log2);
         float factor = 1.f;
         if (m_blk > m_ref + AT_RESCALE_THR) {            // first block always lands here
-          factor = ex2_approx(m_ref - m_blk);            // 0 on the first block (m_ref = -inf)
+          const float dref = m_ref - m_blk;              // an integer <= -8, or -inf on the first block
+          factor = dref < -126.f ? 0.f : __int_as_float(((int)dref + 127) << 23);   // 2^dref, exactly
           m_ref = m_blk;
         }
         uint32_t pk[16];
