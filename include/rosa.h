@@ -132,6 +132,20 @@ rosa_status_t rosa_denoise_batch_host(rosa_expert_t *e, int32_t batch, const int
                                       const float *dt, const int32_t *n_steps,
                                       float *out_actions_host, void *stream);
 
+/* Allocation-free linear layer, for callers that cannot call cudaMalloc (code under CUDA-graph capture, tight
+ * serving loops, harnesses that forbid it).  One GEMM of the path's kind with its fp32 epilogue,
+ *     acc[M,N] = A[M,K] * W[N,K]^T      A, W: 16-bit [dev] operands, row-major, bf16 (fp16 = 0) or fp16 (fp16 = 1)
+ *     epi = 0: C = acc      epi = 2: C = acc + bias[n] (bias [dev] float32 [N])      epi = 4: C = C + acc
+ * with C [dev] float32 [M,N], through the shape-generic CUDA-core kernels (any M, N, K >= 1; not a speed path).
+ * The fp32 product passes through a scratch matrix that is a file-scope device array of the library
+ * (ROSA_NOALLOC_MAX_ELEMS floats = 4 MiB, held by every GPU that loads the library until exit): the call makes no
+ * cudaMalloc / cudaFree and calls no allocating routine; M * N beyond the limit returns ROSA_ERR_CAPACITY.
+ * Asynchronous on `stream`.  All calls share the scratch: calls that may overlap on the GPU (different streams
+ * with no ordering between them) race on it - serialise them.  Needs no expert. */
+#define ROSA_NOALLOC_MAX_ELEMS (1 << 20)
+rosa_status_t rosa_linear_noalloc(int32_t epi, int32_t fp16, int32_t M, int32_t N, int32_t K, const void *A,
+                                  const void *W, const float *bias, float *C, void *stream);
+
 const char *rosa_last_error(void); /* thread-local, never NULL */
 int32_t rosa_version(void);
 

@@ -21,7 +21,8 @@ ROSA_F32, ROSA_BF16 = 0, 1
 
 EXPORTS = ("rosa_expert_create", "rosa_expert_destroy", "rosa_prefix_kv_bind", "rosa_prefix_kv_unbind",
            "rosa_denoise_batch", "rosa_denoise_batch_ex", "rosa_denoise_batch_host",
-           "rosa_last_error", "rosa_version")
+           "rosa_linear_noalloc", "rosa_last_error", "rosa_version")
+ROSA_NOALLOC_MAX_ELEMS = 1 << 20
 # include/rosa_debug.h: measurement and unit-test hooks
 DEBUG_EXPORTS = ("rosa_profile_batch", "rosa_kernel_class_name", "rosa_last_launch_count", "rosa_kernel_family",
                  "rosa_debug_graph_captures", "rosa_debug_gemm", "rosa_debug_attn_plan")
@@ -77,6 +78,7 @@ def load():
     lib.rosa_denoise_batch_host.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp]
     lib.rosa_last_launch_count.argtypes = [vp, C.POINTER(i64)]
     lib.rosa_kernel_family.argtypes = [vp, C.POINTER(i32)]
+    lib.rosa_linear_noalloc.argtypes = [i32, i32, i32, i32, i32, vp, vp, vp, vp, vp]
     lib.rosa_debug_graph_captures.argtypes = [vp, C.POINTER(i64)]
     lib.rosa_debug_gemm.argtypes = [i32, i32, i32, i32, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
     lib.rosa_debug_attn_plan.argtypes = [i32, i32, vp, i32, vp, vp, i32]
@@ -211,6 +213,12 @@ def rosa_denoise_batch_host(e: Expert, robot_ids, noise_host, t_start, dt, n_ste
     t0, d, ns = _host(t_start, np.float32), _host(dt, np.float32), _host(n_steps, np.int32)
     _check(load().rosa_denoise_batch_host(e.handle, len(ids), _ptr(ids), _ptr(noise_host), _ptr(t0), _ptr(d),
                                           _ptr(ns), _ptr(out_actions_host), _stream_handle(stream)))
+
+
+def rosa_linear_noalloc(M: int, N: int, K: int, A16, W16, C_f32, *, epi: int = EPI_STORE_F32, fp16: int = 0, bias=None,
+                        stream=None):
+    """C = epi(A W^T) through the allocation-free entry point (static device scratch, M * N <= ROSA_NOALLOC_MAX_ELEMS)."""
+    _check(load().rosa_linear_noalloc(epi, fp16, M, N, K, _ptr(A16), _ptr(W16), _ptr(bias), _ptr(C_f32), _stream_handle(stream)))
 
 
 def rosa_profile_batch(e: Expert, robot_ids, noise, t_start, dt, n_steps, out_actions, stream=None):
