@@ -70,7 +70,11 @@ typedef struct {
  * wv [nkv*hd,d], wo [d,nq*hd], g_mlp [d], w_gate [F,d], w_up [F,d], w_down [d,F].
  * time_conditioning == 1 only (ignored otherwise): w_t1 is [d,d]; w_mod_* [3d,d] and b_mod_* [3d], rows
  * ordered scale | shift | gate, one pair per norm (per layer: attention, MLP; and the final norm);
- * g_attn, g_mlp, g_final are not read. */
+ * g_attn, g_mlp, g_final are not read.
+ * Loading a trained checkpoint: the conventions here are the ones of DESIGN.md section 2, not of any particular
+ * code base - w_t1's columns are [time | action] (a model that concatenates [action | time] needs its two column
+ * blocks swapped), and the RMSNorm gain multiplies as g (a "1 + g" parameterisation needs 1 added to the stored
+ * gains). */
 typedef struct {
   rosa_dtype_t dtype;
   int32_t on_device;
@@ -81,8 +85,15 @@ typedef struct {
   const void *w_mod_final, *b_mod_final;
 } rosa_weights_t;
 
-/* Create an expert on the current CUDA device.  Copies and repacks every weight into
- * library-owned bf16 device storage (the caller may free its copies on return).
+/* Create an expert on the current CUDA device (every later call on this expert must be made with that device
+ * current, else ROSA_ERR_INVALID_ARG).  Copies and repacks every weight into library-owned 16-bit device storage
+ * (the caller may free its copies on return).
+ * Operand format (R19', R26): the weight GEMMs run on fp16 operands with fp32 accumulation by default
+ * (bf16-valued weights convert exactly above 6.1e-5; smaller ones become fp16 subnormals with <= 3e-8 absolute error);
+ * the residual stream is fp32, and its 16-bit operand copy SATURATES at +-65504: a model whose un-normalised residual
+ * leaves the fp16 range is clipped there (finite, never inf / NaN).  The environment variable ROSA_GEMM_DTYPE=bf16
+ * (read here) selects bf16 operands instead: the range of fp32, at about five times the operand rounding error.
+ * q, k, v, the softmax numerators and the prefix cache are bf16 in either mode.
  * Constraints (else ROSA_ERR_UNSUPPORTED): d_model, ffn, n_q_heads*head_dim multiples of 64;
  * head_dim even, <= 256; n_q_heads % n_kv_heads == 0; action_dim <= 64; horizon <= 64.
  * The environment variable ROSA_KERNELS=simple forces the shape-generic CUDA-core kernels
@@ -96,8 +107,14 @@ rosa_status_t rosa_expert_destroy(rosa_expert_t *e);
  * pointers, each [len, n_kv_heads, head_dim] contiguous, 16-byte aligned.
  * dtype ROSA_BF16: the pointers are BORROWED (kept alive by the caller until unbind/re-bind/
  * destroy); a packed ragged buffer is bound by passing base + cu_seqlens[i]*n_kv*hd (BJ cfg2).
- * dtype ROSA_F32: values are converted into library-owned bf16 storage.
- * len == 0 is legal (self-attention only, R8).  Re-binding replaces the entry. */
+ * dtype ROSA_F32: values are converted, synchronously, into library-owned bf16 storage (kept until destroy).
+ * len == 0 is legal (self-attention only, R8).  Re-binding replaces the entry.
+ * Ordering: bind returns without waiting for the device.  The robot's table entries (pointers, length, tensor maps)
+ * are updated by copies on a library stream that runs AFTER every rosa_denoise_batch* call enqueued before the
+ * bind, and the next rosa_denoise_batch* call waits for them on its own stream: calls enqueued before a bind see
+ * the old binding, calls made after it the new one.  The DATA behind borrowed pointers is the caller's: it must be
+ * complete, in stream order, before the first call that uses it, and must stay untouched until the last call that
+ * was enqueued with that binding has finished.  unbind only marks the robot unbound on the host. */
 rosa_status_t rosa_prefix_kv_bind(rosa_expert_t *e, int32_t robot, const void *const *k_layers,
                                   const void *const *v_layers, int32_t len, rosa_dtype_t dtype);
 rosa_status_t rosa_prefix_kv_unbind(rosa_expert_t *e, int32_t robot);
