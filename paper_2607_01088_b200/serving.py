@@ -271,3 +271,97 @@ def continuous_worker(fleet, max_inflight: int, n_steps: int = 10, **kw) -> Work
             return len(cb)
 
     return Worker(max_inflight, stepper=_Stepper(), sync=stream.synchronize, noise_of=lambda r: fleet.noise[r], **kw)
+
+
+# ------------------------------------------------------------------ measurements on the GPU
+def measure_latency_profile(fleet, batch_sizes: Sequence[int], slo_s: float, seconds_per_point: float = 2.5,
+                            fractions: Sequence[float] = tuple(j / 10 for j in range(1, 11)), seed: int = 0) -> Dict[int, dict]:
+    """L(b, lambda) MEASURED: per batch size, Poisson arrivals paced in real time at ten rates from
+    10% to 100% of the measured maximum throughput mu_b = b / (mean duration of a back-to-back call), against a
+    discrete-batch `Worker` making real `rosa_denoise_batch_ex` calls.  Next to every measured row: the virtual-time
+    simulator of latency_profile.py on the SAME arrivals with the measured mean service time (the cross-check)."""
+    from . import latency_profile as lp
+    run = gpu_batch_call(fleet)
+    n_robots = int(fleet.noise.shape[0])
+    out: Dict[int, dict] = {}
+    for b in batch_sizes:
+        robots = list(range(b))
+        for _ in range(3):
+            run(robots)                                           # warm-up: graph capture for this bucket
+        t0 = time.perf_counter()
+        reps = 8
+        for _ in range(reps):
+            run(robots)
+        service = (time.perf_counter() - t0) / reps               # host-to-host, synchronised: what a request sees
+        mu = b / service
+        rows = []
+        for frac in fractions:
+            rng = np.random.default_rng([seed, b, int(round(frac * 1000))])
+            lam = frac * mu
+            n = max(int(lam * seconds_per_point), 4 * b)
+            n -= n % b                                            # whole batches (no flush: the paper's worker)
+            arr = lp.poisson_arrivals(lam, n, rng)
+            w = Worker(b, run).start()
+            res = open_loop(w, arr, n_robots=max(n_robots, b), slo_s=slo_s, drain_s=10.0)
+            w.stop()
+            sim = lp.simulate_discrete_batching(arr, b, lambda m: service)
+            sim = sim[~np.isnan(sim)][len(arr) // 10:]
+            rows.append({"fraction": frac, "rate_per_s": lam, **{k: res[k] for k in ("requests", "p50_ms", "p99_ms", "mean_ms",
+                         "slo_meet_rate", "actions_per_s", "unserved")},
+                         "sim_p50_ms": 1e3 * float(np.percentile(sim, 50)), "sim_p99_ms": 1e3 * float(np.percentile(sim, 99)),
+                         "sim_mean_ms": 1e3 * float(sim.mean()), "worker_busy_frac": w.busy_s / max(arr[-1], 1e-9)})
+        out[int(b)] = {"service_ms_mean": 1e3 * service, "max_throughput_per_s": mu, "rates": rows}
+    return out
+
+
+def main():
+    import argparse
+    import json
+    import os
+    from . import build as rosa_build, cases
+    from . import latency_profile as lp
+    from .runner import DeviceFleet
+    ap = argparse.ArgumentParser(description="real-time latency profile L(b, lambda) and closed-loop fleets against one B200")
+    ap.add_argument("--batches", type=int, nargs="+", default=[1, 4, 16, 64])
+    ap.add_argument("--robots", type=int, nargs="+", default=[16, 64, 256])
+    ap.add_argument("--t-act", type=float, default=0.2)
+    ap.add_argument("--slo-ms", type=float, default=200.0, help="p99 deadline (Table 1 of the paper: 200 ms)")
+    ap.add_argument("--freq", type=float, default=3.9, help="scheduled per-robot request rate f (Hz): the rate cap")
+    ap.add_argument("--seconds", type=float, default=2.5, help="real time per (b, rate) point; closed loops run twice as long")
+    ap.add_argument("--out", default=os.path.join("gpurun_out", "serving.json"))
+    args = ap.parse_args()
+    rosa_build.build()
+    base = cases.make_case(4, batch=1, with_prefix=False)
+    n_fleet = max(max(args.robots), max(args.batches))
+    fleet = DeviceFleet(base, [816] * n_fleet, seed=4)
+    slo = args.slo_ms * 1e-3
+    prof = measure_latency_profile(fleet, args.batches, slo, args.seconds)
+    for b, p in prof.items():
+        print(f"b={b}: service {p['service_ms_mean']:.2f} ms, max {p['max_throughput_per_s']:.0f} req/s; measured p99 (ms) at 10%..100%: "
+              + " ".join(f"{r['p99_ms']:.0f}" for r in p["rates"]) + " | simulated: " + " ".join(f"{r['sim_p99_ms']:.0f}" for r in p["rates"]), flush=True)
+    feas = [c for c in lp.feasible_configs(prof, args.freq, args.slo_ms) if c.get("best")]
+    print("feasible (best k per b) at f = %.1f Hz, p99 <= %.0f ms:" % (args.freq, args.slo_ms), feas, flush=True)
+    rows = []
+    for robots in args.robots:
+        for mode, b in (("discrete", 1), ("discrete", 16), ("discrete", 64), ("continuous", 64)):
+            if mode == "discrete" and b > robots:
+                continue
+            for cap in (None, args.freq):
+                if mode == "discrete":
+                    w = Worker(b, gpu_batch_call(fleet), n_clients=robots).start()
+                else:
+                    w = continuous_worker(fleet, min(b, robots)).start()
+                r = closed_loop(w, robots, args.t_act, cap, 2 * args.seconds, slo)
+                w.stop()
+                rows.append({"robots": robots, "mode": mode, "batch": b, "rate_cap_hz": cap, "launches": w.calls, **r})
+                print(rows[-1], flush=True)
+    fleet.close()
+    os.makedirs(os.path.dirname(args.out) or ".", exist_ok=True)
+    with open(args.out, "w") as f:
+        json.dump({"workload": "pi0-scale expert, prefix 816, 10 Euler steps (BASELINE.json configs[4]); real-time pacing, host clocks",
+                   "slo_ms": args.slo_ms, "t_act": args.t_act, "freq_hz": args.freq, "profile": prof, "feasible": feas,
+                   "closed_loop": rows}, f, indent=1)
+
+
+if __name__ == "__main__":
+    main()
