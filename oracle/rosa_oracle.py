@@ -234,6 +234,19 @@ def denoise_batch(cfg, W: Dict, prefix_k: Sequence[np.ndarray], prefix_v: Sequen
     return x, (vel if return_velocity else None)
 
 
+def prefix_kv(cfg, hidden: np.ndarray, w_pk: np.ndarray, w_pv: np.ndarray, dtype=F):
+    """The step before the loop (PAPER.md:78: the VLM backbone processes the observation; SURVEY 8(f) item 4;
+    reading R29 of DESIGN.md): one layer's prefix K/V of a robot from the backbone's NORMALISED hidden states of its
+    L prefix tokens,  K = RoPE(n W_pk^T, positions 0..L-1)  ("K pre-rotated", BASELINE.json configs[1]; R7),
+    V = n W_pv^T.   hidden [L, d_p]; w_pk, w_pv [n_kv * hd, d_p]  ->  K, V [L, n_kv, hd].
+    (The backbone that produces `hidden` is out of scope: its weights are not public.)"""
+    n = np.asarray(hidden, dtype=dtype)
+    L = n.shape[0]
+    k = (n @ _as(w_pk, dtype).T).reshape(L, cfg.n_kv_heads, cfg.head_dim)
+    v = (n @ _as(w_pv, dtype).T).reshape(L, cfg.n_kv_heads, cfg.head_dim)
+    return rope(k, np.arange(L), cfg.rope_base), v
+
+
 def denoise_case(case, robots: Optional[Sequence[int]] = None, return_velocity: bool = False, dtype=F):
     """Run ``denoise_batch`` on a ``cases.Case`` (optionally only some robots — exact,
     because robots are independent units)."""

@@ -550,3 +550,43 @@ def test_adarms_batch_invariance_and_generator_contract():
     # the modulation weights come from their own generator: the first draw of the main stream is the base one's
     base = cases.build_case("b", 5, cases.TINY, bf16=False, prefix_lens=[48, 64], n_steps=4)
     np.testing.assert_array_equal(base.weights["w_in"], c.weights["w_in"])
+
+
+# ------------------------------------------------------------------ prefix K/V production (reading R29)
+def test_prefix_kv_brute_force_and_closed_forms():
+    """O.prefix_kv against a scalar loop written from the definition (math only): K[t, c] of head g pairs channel c
+    with c + hd/2 and rotates by t * base^(-2c/hd); V is the plain projection.  Closed forms: token 0 is not rotated;
+    with W_pk = identity the result is the rotation of the hidden state itself; rows keep their norm; and the K it
+    produces is what P8 expects (an action-token query scores the same against it wherever the prefix starts)."""
+    cfg = cases.TINY
+    hd, nkv = cfg.head_dim, cfg.n_kv_heads
+    rng = np.random.default_rng(61)
+    L, dp = 5, 12
+    n = rng.standard_normal((L, dp))
+    wk = rng.standard_normal((nkv * hd, dp)) * 0.3
+    wv = rng.standard_normal((nkv * hd, dp)) * 0.3
+    K, V = O.prefix_kv(cfg, n, wk, wv)
+    assert K.shape == V.shape == (L, nkv, hd)
+    half = hd // 2
+    for t in range(L):
+        for g in range(nkv):
+            proj_k = [sum(n[t, j] * wk[g * hd + c, j] for j in range(dp)) for c in range(hd)]
+            proj_v = [sum(n[t, j] * wv[g * hd + c, j] for j in range(dp)) for c in range(hd)]
+            for c in range(half):
+                phi = t * cfg.rope_base ** (-2.0 * c / hd)
+                lo = proj_k[c] * math.cos(phi) - proj_k[c + half] * math.sin(phi)
+                hi = proj_k[c + half] * math.cos(phi) + proj_k[c] * math.sin(phi)
+                assert abs(K[t, g, c] - lo) < 1e-12 and abs(K[t, g, c + half] - hi) < 1e-12
+            for c in range(hd):
+                assert abs(V[t, g, c] - proj_v[c]) < 1e-12
+    np.testing.assert_allclose(K[0].ravel(), n[0] @ wk.T, rtol=1e-13)                       # position 0: no rotation
+    np.testing.assert_allclose(np.linalg.norm(K, axis=-1), np.linalg.norm((n @ wk.T).reshape(L, nkv, hd), axis=-1), rtol=1e-13)
+    eye = np.eye(nkv * hd)
+    Ki, Vi = O.prefix_kv(cfg, n[:, :1].repeat(nkv * hd, axis=1) * 0 + rng.standard_normal((L, nkv * hd)), eye, eye)
+    np.testing.assert_allclose(Ki, O.rope(Vi, np.arange(L), cfg.rope_base), rtol=1e-13)     # W = I: K is the rotated input, V the input
+    # relative positions: <rope(q, L + j), K[t]> equals the unrotated <q, k_t> rotated by (L + j - t) only
+    q = rng.standard_normal((1, nkv, hd))
+    s1 = np.sum(O.rope(q, np.array([L + 2.0]), cfg.rope_base)[0] * K[3])
+    k3 = (n[3] @ wk.T).reshape(1, nkv, hd)
+    s2 = np.sum(O.rope(q, np.array([L + 2.0 - 3.0]), cfg.rope_base)[0] * k3[0])
+    assert abs(s1 - s2) < 1e-12
