@@ -119,6 +119,20 @@ rosa_status_t rosa_prefix_kv_bind(rosa_expert_t *e, int32_t robot, const void *c
                                   const void *const *v_layers, int32_t len, rosa_dtype_t dtype);
 rosa_status_t rosa_prefix_kv_unbind(rosa_expert_t *e, int32_t robot);
 
+/* The step before the loop (the VLM backbone processes the observation before the action head runs;
+ * SURVEY.md 8(f) item 4; reading R29): produce one robot's prefix K/V cache from the backbone's NORMALISED
+ * hidden states of its `len` prefix tokens, per layer l:
+ *     K_l = RoPE(n_l W_pk,l^T, positions 0..len-1)   ("K pre-rotated", BJ cfg1; R7),     V_l = n_l W_pv,l^T
+ * hidden_layers / wk_layers / wv_layers / k_out_layers / v_out_layers: [host] arrays of `layers` [dev] pointers,
+ * 16-byte aligned, all bf16: hidden [len, d_prefix], wk / wv [n_kv_heads*head_dim, d_prefix] row-major, outputs
+ * [len, n_kv_heads, head_dim] contiguous - exactly what rosa_prefix_kv_bind(..., ROSA_BF16) borrows.  Nothing is
+ * bound: bind the outputs afterwards (in stream order before the first call that uses them).  The backbone that
+ * produces the hidden states is outside this library.  Asynchronous on `stream`; needs the tcgen05 kernels
+ * (head_dim 256) and d_prefix % 64 == 0, else ROSA_ERR_UNSUPPORTED; len <= max_prefix_len, else ROSA_ERR_CAPACITY. */
+rosa_status_t rosa_prefix_kv_produce(rosa_expert_t *e, int32_t d_prefix, const void *const *hidden_layers,
+                                     const void *const *wk_layers, const void *const *wv_layers, int32_t len,
+                                     void *const *k_out_layers, void *const *v_out_layers, void *stream);
+
 /* One batched denoise call (BJ north_star (1); PAPER.md:293/:527 discrete batch).
  * Robot i is integrated from t_start[i] (NULL = 1.0 for all) to 0 in n_steps[i] uniform Euler
  * steps, dt_i = -t_start[i]/n_steps[i] (R1).  The call runs max_i n_steps[i] iterations;

@@ -19,7 +19,7 @@ ROSA_OK, ROSA_ERR_INVALID_ARG, ROSA_ERR_UNBOUND_ROBOT = 0, -1, -2
 ROSA_ERR_CAPACITY, ROSA_ERR_CUDA, ROSA_ERR_UNSUPPORTED = -3, -4, -5
 ROSA_F32, ROSA_BF16 = 0, 1
 
-EXPORTS = ("rosa_expert_create", "rosa_expert_destroy", "rosa_prefix_kv_bind", "rosa_prefix_kv_unbind",
+EXPORTS = ("rosa_expert_create", "rosa_expert_destroy", "rosa_prefix_kv_bind", "rosa_prefix_kv_unbind", "rosa_prefix_kv_produce",
            "rosa_denoise_batch", "rosa_denoise_batch_ex", "rosa_denoise_batch_host",
            "rosa_linear_noalloc", "rosa_last_error", "rosa_version")
 ROSA_NOALLOC_MAX_ELEMS = 1 << 20
@@ -73,6 +73,7 @@ def load():
     lib.rosa_expert_destroy.argtypes = [vp]
     lib.rosa_prefix_kv_bind.argtypes = [vp, i32, C.POINTER(vp), C.POINTER(vp), i32, C.c_int]
     lib.rosa_prefix_kv_unbind.argtypes = [vp, i32]
+    lib.rosa_prefix_kv_produce.argtypes = [vp, i32, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), i32, C.POINTER(vp), C.POINTER(vp), vp]
     lib.rosa_denoise_batch.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp]
     lib.rosa_denoise_batch_ex.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.rosa_denoise_batch_host.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp]
@@ -185,6 +186,16 @@ def rosa_prefix_kv_bind(e: Expert, robot: int, k_layers: Sequence, v_layers: Seq
     va = (C.c_void_p * n)(*[_ptr(t) for t in v_layers]) if length > 0 else None
     _check(load().rosa_prefix_kv_bind(e.handle, robot, ka, va, length, dtype))
     e._keep[robot] = (list(k_layers), list(v_layers))
+
+
+def rosa_prefix_kv_produce(e: Expert, d_prefix: int, hidden_layers: Sequence, wk_layers: Sequence, wv_layers: Sequence,
+                           length: int, k_out_layers: Sequence, v_out_layers: Sequence, stream=None):
+    """Per-layer device tensors (or raw device addresses), all bf16: hidden [len, d_prefix], wk / wv [n_kv*hd, d_prefix],
+    outputs [len, n_kv, hd]."""
+    n = e.cfg.layers
+    arr = lambda ts: (C.c_void_p * n)(*[_ptr(t) for t in ts])
+    _check(load().rosa_prefix_kv_produce(e.handle, d_prefix, arr(hidden_layers), arr(wk_layers), arr(wv_layers), length,
+                                         arr(k_out_layers), arr(v_out_layers), _stream_handle(stream)))
 
 
 def rosa_prefix_kv_unbind(e: Expert, robot: int):

@@ -90,6 +90,7 @@ struct rosa_expert {
   const bf16** d_rk = nullptr;
   const bf16** d_rv = nullptr;
   int* d_rlen = nullptr;
+  int* d_zero = nullptr;           // two device zeros: the (ids, rlen) tables of rosa_prefix_kv_produce (positions = row index)
   std::vector<int> h_rlen;         // -1 = unbound
   std::vector<std::vector<bf16*>> owned;  // per robot: library-owned K/V buffers (fp32 binds), kept until destroy
   std::vector<size_t> owned_cap;          // elements each of them holds
@@ -415,6 +416,8 @@ static rosa_status_t create_impl(const rosa_expert_config_t* c, const rosa_weigh
   CK(cudaMemset(e->d_rk, 0, (size_t)c->max_robots * dm.layers * sizeof(void*)));
   CK(cudaMemset(e->d_rv, 0, (size_t)c->max_robots * dm.layers * sizeof(void*)));
   CK(cudaMemset(e->d_rlen, 0, (size_t)c->max_robots * 4));
+  WS(e->d_zero, 16);
+  CK(cudaMemset(e->d_zero, 0, 16));
   {
     const char* at = getenv("ROSA_ATTN");
     e->attn_tc = e->family == 1 && tc_attn_supported(dm) && !(at && !strcmp(at, "simple"));
@@ -957,6 +960,48 @@ rosa_status_t rosa_prefix_kv_bind(rosa_expert_t* e, int32_t robot, const void* c
   e->bind_pending[robot] = 1;
   e->bind_dirty = true;
   e->h_rlen[robot] = len;
+  return ROSA_OK;
+}
+
+rosa_status_t rosa_prefix_kv_produce(rosa_expert_t* e, int32_t d_prefix, const void* const* hidden_layers,
+                                     const void* const* wk_layers, const void* const* wv_layers, int32_t len,
+                                     void* const* k_out_layers, void* const* v_out_layers, void* stream) {
+  if (!e || !hidden_layers || !wk_layers || !wv_layers || !k_out_layers || !v_out_layers) { set_error("NULL argument"); return ROSA_ERR_INVALID_ARG; }
+  if (len < 0 || d_prefix < 1) { set_error("len < 0 or d_prefix < 1"); return ROSA_ERR_INVALID_ARG; }
+  if (len > e->cfg.max_prefix_len) { set_error("len > max_prefix_len (the RoPE table ends there)"); return ROSA_ERR_CAPACITY; }
+  const Dims& dm = e->dm;
+  const int N = dm.nkv * dm.hd;
+  if (e->family != 1 || dm.hd != 256 || d_prefix % 64) {
+    set_error("rosa_prefix_kv_produce needs the tcgen05 kernels (head_dim 256) and d_prefix % 64 == 0"); return ROSA_ERR_UNSUPPORTED;
+  }
+  {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != e->device) { set_error("the expert lives on another CUDA device"); return ROSA_ERR_INVALID_ARG; }
+  }
+  if (len == 0) return ROSA_OK;
+  for (int l = 0; l < dm.layers; ++l) {
+    const void* ptrs[5] = {hidden_layers[l], wk_layers[l], wv_layers[l], k_out_layers[l], v_out_layers[l]};
+    for (const void* q : ptrs) {
+      if (!q) { set_error("NULL layer pointer"); return ROSA_ERR_INVALID_ARG; }
+      if ((uintptr_t)q & 15) { set_error("layer pointer not 16-byte aligned"); return ROSA_ERR_INVALID_ARG; }
+    }
+  }
+  cudaStream_t s = (cudaStream_t)stream;
+  // K = RoPE(n W_pk^T) at positions 0..len-1, V = n W_pv^T: the QKV GEMM's kernel with its RoPE epilogue (a3 + a4),
+  // bf16 operands (the backbone's hidden states and the cache are bf16), one head per 256-column tile.  The epilogue
+  // takes a row's position from (ids, rlen, H) as rlen[ids[row / H]] + row % H: two device zeros and an H beyond
+  // any row count make that the row index itself.
+  EpiArgs ea{};
+  ea.in_fp16 = 0; ea.out_fp16 = 0;
+  ea.H = 1 << 30; ea.hd = dm.hd; ea.ld_out = N;
+  ea.rope_tab = e->rope_tab; ea.ids = e->d_zero; ea.rlen = e->d_zero + 1;
+  ea.inv_d = 1.f; ea.eps = 0.f;
+  for (int l = 0; l < dm.layers; ++l) {
+    ea.out16 = k_out_layers[l]; ea.rope_cols = N;
+    CK(launch_gemm_tc(EPI_ROPE, (const op16*)hidden_layers[l], (const op16*)wk_layers[l], len, N, d_prefix, ea, s));
+    ea.out16 = v_out_layers[l]; ea.rope_cols = 0;
+    CK(launch_gemm_tc(EPI_ROPE, (const op16*)hidden_layers[l], (const op16*)wv_layers[l], len, N, d_prefix, ea, s));
+  }
   return ROSA_OK;
 }
 

@@ -589,3 +589,47 @@ def test_adarms_variant_needs_the_tcgen05_attention_shape():
     with pytest.raises(rosa.RosaError) as ei:
         LoadedCase(case)
     assert ei.value.status == rosa.ROSA_ERR_UNSUPPORTED
+
+
+# ------------------------------------------------------------------ the step before: prefix K/V production (R29)
+def test_prefix_kv_produce_matches_oracle_and_feeds_the_loop():
+    """rosa_prefix_kv_produce against O.prefix_kv element by element (ragged lengths: one token, a full 64-key block,
+    rows that straddle the 128- and 256-row GEMM tiles), then the produced cache is bound and the whole denoise loop is
+    compared with the oracle running on the oracle's own K/V."""
+    lens = [1, 64, 200, 333]
+    case = edge_case(lens, seed=29, n_steps=3)
+    cfg = case.cfg
+    d_p, row = 320, cfg.n_kv_heads * cfg.head_dim
+    rng = np.random.default_rng(290)
+    wk = [cases.round_bf16(rng.standard_normal((row, d_p), dtype=np.float32) / np.sqrt(d_p)) for _ in range(cfg.layers)]
+    wv = [cases.round_bf16(rng.standard_normal((row, d_p), dtype=np.float32) / np.sqrt(d_p)) for _ in range(cfg.layers)]
+    hidden = [[cases.round_bf16(rng.standard_normal((L, d_p), dtype=np.float32)) for _ in range(cfg.layers)] for L in lens]
+    want = [[O.prefix_kv(cfg, hidden[i][l], wk[l], wv[l]) for l in range(cfg.layers)] for i in range(len(lens))]
+    for i in range(len(lens)):   # what an exact producer would store: the oracle's K/V rounded to the cache's bf16
+        case.prefix_k[i] = cases.f32_to_bf16_bits(np.stack([want[i][l][0] for l in range(cfg.layers)]).astype(np.float32))
+        case.prefix_v[i] = cases.f32_to_bf16_bits(np.stack([want[i][l][1] for l in range(cfg.layers)]).astype(np.float32))
+    lc = LoadedCase(case)
+    dev = lc.device
+    to_dev = lambda a: torch.from_numpy(cases.f32_to_bf16_bits(a).view(np.int16)).to(dev)
+    wk_d, wv_d = [to_dev(w) for w in wk], [to_dev(w) for w in wv]
+    keep = []
+    for i, L in enumerate(lens):
+        h_d = [to_dev(hidden[i][l]) for l in range(cfg.layers)]
+        k_d = [torch.zeros((L, row), dtype=torch.int16, device=dev) for _ in range(cfg.layers)]
+        v_d = [torch.zeros((L, row), dtype=torch.int16, device=dev) for _ in range(cfg.layers)]
+        rosa.rosa_prefix_kv_produce(lc.expert, d_p, h_d, wk_d, wv_d, L, k_d, v_d)
+        torch.cuda.synchronize()
+        for l in range(cfg.layers):
+            for got_t, ref, name in ((k_d[l], want[i][l][0], "K"), (v_d[l], want[i][l][1], "V")):
+                got = cases.bf16_bits_to_f32(got_t.cpu().numpy().view(np.uint16)).reshape(L, cfg.n_kv_heads, cfg.head_dim)
+                err, big = rel_l2(got, ref), float(np.abs(got - ref).max())
+                # one bf16 rounding of the stored value (2^-9 relative per element) on top of fp32 accumulation
+                assert err <= 3e-3 and big <= 2.0 ** -8 * float(np.abs(ref).max()) + 1e-6, (i, l, name, err, big)
+        rosa.rosa_prefix_kv_bind(lc.expert, i, k_d, v_d, L, rosa.ROSA_BF16)
+        keep.append((h_d, k_d, v_d))
+    print(f"[prefix-kv-produce] lens {lens}: K/V within one bf16 rounding of the oracle")
+    check_against_oracle(case, lc, list(range(len(lens))), "prefix-kv-produce -> denoise")
+    with pytest.raises(rosa.RosaError) as ei:
+        rosa.rosa_prefix_kv_produce(lc.expert, 100, keep[0][0], wk_d, wv_d, 1, keep[0][1], keep[0][2])   # d_prefix % 64 != 0
+    assert ei.value.status == rosa.ROSA_ERR_UNSUPPORTED
+    lc.close()
