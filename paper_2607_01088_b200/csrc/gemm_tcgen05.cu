@@ -5,9 +5,11 @@
 // Persistent, warp-specialised, one CTA per SM, 10 warps:
 //   warp 0      TMA producer: A tile [128 x 64] + W tile per k-block into a ring of SWIZZLE_128B
 //               stages, completion on "full" mbarriers
-//   warp 1      MMA issuer: the elected lane issues 4 x tcgen05.mma per stage into a TMEM accumulator;
-//               tcgen05.commit frees the stage ("empty") and, after the last k-block, publishes the
-//               accumulator ("tmem full")
+//   warp 1      MMA issuer: 4 x tcgen05.mma per k-block into a TMEM accumulator; tcgen05.commit frees the
+//               stage ("empty") and, after the last k-block, publishes the accumulator ("tmem full")
+//               Both run on ONE elected lane from start to end: each is a chain of dependent instructions, and what
+//               it executes per k-block (not the tensor pipe, not the feed) bounded every tile narrower than 256
+//               columns while the loops were warp-wide with an elect and a warp sync per k-block (DESIGN 5d).
 //   warps 2..9  epilogue, two warps per TMEM lane quarter (half of the tile's columns each): tcgen05.ld,
 //               fused epilogue (epilogue_tile below), coalesced global stores, release ("tmem empty")
 // The accumulator is double-buffered in TMEM (2 x BN columns) so the epilogue of tile i overlaps the
@@ -38,11 +40,16 @@ constexpr int kScrFloats = 32 * 36;    // per epilogue warp: a 32 x 32 fp32 chun
 
 template <int BN>
 struct GemmCfg {
-  static constexpr int STAGES = BN == 256 ? 3 : (BN == 128 ? 5 : 7);
+  // The operand ring takes whatever the fixed parts leave of the 227 KB; the number of stages is a launch-time
+  // value: a stage is [a_rows x 64] of A (a_rows = the launch's live rows rounded up to 8, at most 128; the TMA box
+  // is that high) and [BN x 64] of W, so a launch with few rows gets more, shorter stages.
+  static constexpr int MAX_STAGES = 16;
   static constexpr int A_BYTES = BM * BK * 2;
   static constexpr int B_BYTES = BN * BK * 2;
-  static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
-  static constexpr int SMEM = STAGES * STAGE_BYTES + 1024 /*align slack*/ + 256 /*barriers*/ + kEpiWarps * kScrFloats * 4;
+  static constexpr int FIXED = 1024 /*align slack*/ + 512 /*barriers*/ + kEpiWarps * kScrFloats * 4;
+  static constexpr int RING = ((232448 - FIXED) / 1024) * 1024;
+  static constexpr int SMEM = RING + FIXED;
+  static_assert(RING >= 3 * (A_BYTES + B_BYTES), "three full stages");
   static constexpr int TMEM_COLS = 2 * BN < 32 ? 32 : 2 * BN;
 };
 
@@ -483,31 +490,107 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, EpiPre& pre, fl
   }
 }
 
+// Role loops of the single-CTA kernel.  A stage of the ring holds KC consecutive k-blocks (64 columns each) of A and
+// of W behind ONE full / empty barrier pair: the MMA issuer is one thread running dependent instructions, and what it
+// spends per barrier round trip (wait, fence, commit, ring bookkeeping: ~200 cycles, measured) is amortised over KC
+// times the MMAs.  Barrier slots: full[s] at 8 s, empty[s] at 8 (MAX_STAGES + s), then the two accumulator pairs.
+template <int BN, int KC>
+__device__ __forceinline__ void gemm1_producer(const CUtensorMap* tmA, const CUtensorMap* tmB, uint32_t smem_base,
+                                               uint32_t bar_base, uint32_t a_chunk, int n_stages, int n_tiles, int n_m,
+                                               int n_kb) {
+  using Cfg = GemmCfg<BN>;
+  const uint32_t a_span = a_chunk * KC, stage_bytes = a_span + Cfg::B_BYTES * KC;
+  if (elect_one()) {
+    int s = 0;
+    uint32_t ph = 0;
+    for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+      const int m0 = (t % n_m) * BM, n0 = (t / n_m) * BN;
+      for (int kb = 0; kb < n_kb; ++kb) {
+        const uint32_t full = bar_base + 8u * s;
+        mbar_wait_idle(bar_base + 8u * (Cfg::MAX_STAGES + s), ph ^ 1);
+        mbar_expect_tx(full, stage_bytes);
+        const uint32_t a_dst = smem_base + s * stage_bytes;
+#pragma unroll
+        for (int c = 0; c < KC; ++c) {
+          tma_load_2d(a_dst + c * a_chunk, tmA, full, (kb * KC + c) * BK, m0);
+          tma_load_2d(a_dst + a_span + c * Cfg::B_BYTES, tmB, full, (kb * KC + c) * BK, n0);
+        }
+        if (++s == n_stages) { s = 0; ph ^= 1; }
+      }
+    }
+  }
+  __syncwarp();
+}
+
+template <int BN, int KC>
+__device__ __forceinline__ void gemm1_mma(uint32_t smem_base, uint32_t bar_base, uint32_t tmem_base, uint32_t idesc,
+                                          uint32_t a_chunk, int n_stages, int n_tiles, int n_kb) {
+  using Cfg = GemmCfg<BN>;
+  const uint32_t tfull0 = bar_base + 8u * (2 * Cfg::MAX_STAGES), tempty0 = tfull0 + 16u;
+  if (elect_one()) {
+    // shared-memory descriptors (make_sdesc_k128): everything but the 14-bit start address is constant
+    const uint64_t desc_hi = make_sdesc_k128(0);
+    const uint32_t a_chunk16 = a_chunk >> 4, stage16 = (a_chunk * KC + Cfg::B_BYTES * KC) >> 4;
+    const uint32_t base16 = (smem_base >> 4) & 0x3FFF;
+    int s = 0, it = 0;
+    uint32_t ph = 0;
+    for (int t = blockIdx.x; t < n_tiles; t += gridDim.x, ++it) {
+      const int acc = it & 1;
+      mbar_wait(tempty0 + 8u * acc, ((it >> 1) & 1) ^ 1);
+      tc_fence_after();
+      const uint32_t d_tmem = tmem_base + acc * BN;
+      for (int kb = 0; kb < n_kb; ++kb) {
+        mbar_wait(bar_base + 8u * s, ph);
+        tc_fence_after();
+        const uint32_t a16 = base16 + s * stage16, b16 = a16 + KC * a_chunk16;
+#pragma unroll
+        for (int c = 0; c < KC; ++c) {
+#pragma unroll
+          for (int kk = 0; kk < BK / 16; ++kk) {
+            umma_bf16(d_tmem, desc_hi | (uint64_t)(a16 + c * a_chunk16 + kk * 2),
+                      desc_hi | (uint64_t)(b16 + c * (Cfg::B_BYTES >> 4) + kk * 2), idesc, (c | kk) ? 1u : (uint32_t)(kb != 0));
+          }
+        }
+        umma_commit(bar_base + 8u * (Cfg::MAX_STAGES + s));
+        if (kb == n_kb - 1) umma_commit(tfull0 + 8u * acc);
+        if (++s == n_stages) { s = 0; ph ^= 1; }
+      }
+    }
+  }
+  __syncwarp();
+}
+
 template <int BN, int EPI>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, int M, int N, int K,
-          EpiArgs ea) {
+          int a_rows, int kc, EpiArgs ea) {
   using Cfg = GemmCfg<BN>;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t bar_base = smem_base + Cfg::STAGES * Cfg::STAGE_BYTES;
+  // a_rows < 128: the MMA still reads 128 rows from a_addr; rows a_rows.. are whatever follows in shared memory (this
+  // stage's W, the next stage).  They feed accumulator rows >= m_lim only, which no epilogue stores.
+  // kc consecutive k-blocks of A and of W per stage (gemm1_producer)
+  const uint32_t a_chunk = (uint32_t)a_rows * (BK * 2);        // a_rows % 8 == 0: a multiple of the swizzle atom
+  const uint32_t stage_bytes = (a_chunk + Cfg::B_BYTES) * kc;
+  const int n_stages = min(Cfg::MAX_STAGES, Cfg::RING / (int)stage_bytes);
+  const uint32_t bar_base = smem_base + Cfg::RING;
   auto full_bar = [&](int s) { return bar_base + 8u * s; };
-  auto empty_bar = [&](int s) { return bar_base + 8u * (Cfg::STAGES + s); };
-  auto tfull_bar = [&](int a) { return bar_base + 8u * (2 * Cfg::STAGES + a); };
-  auto tempty_bar = [&](int a) { return bar_base + 8u * (2 * Cfg::STAGES + 2 + a); };
-  const uint32_t tmem_slot = bar_base + 8u * (2 * Cfg::STAGES + 4);
+  auto empty_bar = [&](int s) { return bar_base + 8u * (Cfg::MAX_STAGES + s); };
+  auto tfull_bar = [&](int a) { return bar_base + 8u * (2 * Cfg::MAX_STAGES + a); };
+  auto tempty_bar = [&](int a) { return bar_base + 8u * (2 * Cfg::MAX_STAGES + 2 + a); };
+  const uint32_t tmem_slot = bar_base + 8u * (2 * Cfg::MAX_STAGES + 4);
   volatile uint32_t* tmem_slot_ptr =
       reinterpret_cast<volatile uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int m_lim = ea.m_active ? min(M, *ea.m_active) : M;
   const int n_m = (m_lim + BM - 1) / BM, n_n = N / BN;
-  const int n_tiles = n_m * n_n, n_kb = K / BK;
+  const int n_tiles = n_m * n_n, n_kb = K / (BK * kc);
 
   if (warp == 0 && lane == 0) {
     prefetch_tensormap(&tmA);
     prefetch_tensormap(&tmB);
-    for (int s = 0; s < Cfg::STAGES; ++s) {
+    for (int s = 0; s < n_stages; ++s) {
       mbar_init(full_bar(s), 1);
       mbar_init(empty_bar(s), 1);
     }
@@ -525,69 +608,23 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
-  // The weights do not depend on the previous kernel: pull this CTA's first tile of W towards L2 before waiting
-  // for it (small batches: the K loop is bound by TMA round trips, and an L2 hit is a shorter trip than HBM;
-  // the previous kernel leaves HBM mostly idle there).  Measured: B=1 14.04 -> 13.64 ms per call; in the pair
-  // kernel it is neutral at B = 8..32 and costs 3% at B = 64, so only this kernel does it.
-  if (warp == 0 && (int)blockIdx.x < n_tiles && elect_one()) {
-    const int n0 = ((int)blockIdx.x / n_m) * BN;
-    for (int kb = 0; kb < n_kb; ++kb) tma_prefetch_2d(&tmB, kb * BK, n0);
-  }
   pdl_wait();     // everything above overlapped the previous kernel's tail
   pdl_trigger();
 
-  // Role loops run with whole warps (warp-uniform state stays in uniform registers); only the
-  // TMA / tcgen05 issue is fenced to one elected lane.
   if (warp == 0) {  // ---------------- TMA producer
-    int s = 0;
-    uint32_t ph = 0;
-    for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
-      const int m0 = (t % n_m) * BM, n0 = (t / n_m) * BN;
-      for (int kb = 0; kb < n_kb; ++kb) {
-        mbar_wait_idle(empty_bar(s), ph ^ 1);
-        if (elect_one()) {
-          mbar_expect_tx(full_bar(s), Cfg::STAGE_BYTES);
-          const uint32_t a_dst = smem_base + s * Cfg::STAGE_BYTES;
-          tma_load_2d(a_dst, &tmA, full_bar(s), kb * BK, m0);
-          tma_load_2d(a_dst + Cfg::A_BYTES, &tmB, full_bar(s), kb * BK, n0);
-        }
-        __syncwarp();
-        if (++s == Cfg::STAGES) { s = 0; ph ^= 1; }
-      }
-    }
+    if (kc == 4) gemm1_producer<BN, 4>(&tmA, &tmB, smem_base, bar_base, a_chunk, n_stages, n_tiles, n_m, n_kb);
+    else if (kc == 2) gemm1_producer<BN, 2>(&tmA, &tmB, smem_base, bar_base, a_chunk, n_stages, n_tiles, n_m, n_kb);
+    else gemm1_producer<BN, 1>(&tmA, &tmB, smem_base, bar_base, a_chunk, n_stages, n_tiles, n_m, n_kb);
   } else if (warp == 1) {  // ---------------- MMA issuer
     // fp16 operands: A/B format bits 0 instead of 1 (bf16)
     const uint32_t idesc = ea.in_fp16 ? (make_idesc_bf16(BM, BN) & ~((1u << 7) | (1u << 10))) : make_idesc_bf16(BM, BN);
-    int s = 0, it = 0;
-    uint32_t ph = 0;
-    for (int t = blockIdx.x; t < n_tiles; t += gridDim.x, ++it) {
-      const int acc = it & 1;
-      const uint32_t acc_ph = (it >> 1) & 1;
-      mbar_wait(tempty_bar(acc), acc_ph ^ 1);
-      tc_fence_after();
-      const uint32_t d_tmem = tmem_base + acc * BN;
-      for (int kb = 0; kb < n_kb; ++kb) {
-        mbar_wait(full_bar(s), ph);
-        tc_fence_after();
-        if (elect_one()) {
-          const uint32_t a_addr = smem_base + s * Cfg::STAGE_BYTES;
-          const uint32_t b_addr = a_addr + Cfg::A_BYTES;
-#pragma unroll
-          for (int kk = 0; kk < BK / 16; ++kk) {
-            umma_bf16(d_tmem, make_sdesc_k128(a_addr + kk * 32), make_sdesc_k128(b_addr + kk * 32), idesc,
-                      (kb | kk) != 0);
-          }
-          umma_commit(empty_bar(s));
-          if (kb == n_kb - 1) umma_commit(tfull_bar(acc));
-        }
-        __syncwarp();
-        if (++s == Cfg::STAGES) { s = 0; ph ^= 1; }
-      }
-    }
+    if (kc == 4) gemm1_mma<BN, 4>(smem_base, bar_base, tmem_base, idesc, a_chunk, n_stages, n_tiles, n_kb);
+    else if (kc == 2) gemm1_mma<BN, 2>(smem_base, bar_base, tmem_base, idesc, a_chunk, n_stages, n_tiles, n_kb);
+    else gemm1_mma<BN, 1>(smem_base, bar_base, tmem_base, idesc, a_chunk, n_stages, n_tiles, n_kb);
   } else {  // ---------------- epilogue warps 2..9
     const int q = warp & 3;            // TMEM lane quarter this warp may access
     const int half = (warp - 2) >> 2;  // which half of the tile's columns
-    float* scr = reinterpret_cast<float*>(smem_raw + (bar_base + 256u - smem_u32(smem_raw))) + (warp - 2) * kScrFloats;
+    float* scr = reinterpret_cast<float*>(smem_raw + (bar_base + 512u - smem_u32(smem_raw))) + (warp - 2) * kScrFloats;
     int it = 0;
     for (int t = blockIdx.x; t < n_tiles; t += gridDim.x, ++it) {
       const int acc = it & 1;
@@ -703,29 +740,39 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
   pdl_trigger();
   if (warp == 0) GT_TRACE(2);
 
+  // The two issue loops are each ONE thread's dependent instruction stream: what they execute per k-block bounds the
+  // K loop of every tile narrower than the tensor pipe's 2 BN cycles, so they run on one elected lane from start to
+  // end (no per-k-block elect / warp sync) with the descriptors' constant parts hoisted.
   if (warp == 0) {  // ---------------- TMA producer (both CTAs; completion counted in the leader)
-    int s = 0;
-    uint32_t ph = 0;
-    for (int t = pair; t < n_tiles; t += n_pairs) {
-      const int m0 = (t % n_m) * (2 * BM) + (int)rank * BM, n0 = (t / n_m) * BN + (int)rank * (BN / 2);
-      for (int kb = 0; kb < n_kb; ++kb) {
-        mbar_wait_idle(empty_bar(s), ph ^ 1);
-        if (t == pair && kb == 0) GT_TRACE(10);
-        if (elect_one()) {
-          const uint32_t lfull = mapa_shared(full_bar(s), 0);
+    if (elect_one()) {
+      const int lane = 0;  // GT_TRACE
+      (void)lane;
+      const uint32_t lfull0 = mapa_shared(full_bar(0), 0);
+      int s = 0;
+      uint32_t ph = 0;
+      for (int t = pair; t < n_tiles; t += n_pairs) {
+        const int m0 = (t % n_m) * (2 * BM) + (int)rank * BM, n0 = (t / n_m) * BN + (int)rank * (BN / 2);
+        for (int kb = 0; kb < n_kb; ++kb) {
+          mbar_wait_idle(empty_bar(s), ph ^ 1);
+          if (t == pair && kb == 0) GT_TRACE(10);
+          const uint32_t lfull = lfull0 + 8u * s;
           mbar_expect_tx_cluster(lfull, Cfg::STAGE_BYTES);
           const uint32_t a_dst = smem_base + s * Cfg::STAGE_BYTES;
           tma_load_2d_cg2(a_dst, &tmA, lfull, kb * BK, m0);
           tma_load_2d_cg2(a_dst + Cfg::A_BYTES, &tmB, lfull, kb * BK, n0);
+          if (++s == Cfg::STAGES) { s = 0; ph ^= 1; }
         }
-        __syncwarp();
-        if (++s == Cfg::STAGES) { s = 0; ph ^= 1; }
       }
     }
+    __syncwarp();
   } else if (warp == 1) {
-    if (rank == 0) {  // ---------------- MMA issuer (leader CTA only)
+    if (rank == 0 && elect_one()) {  // ---------------- MMA issuer (leader CTA only)
+      const int lane = 0;  // GT_TRACE
+      (void)lane;
       const uint32_t idesc =
           ea.in_fp16 ? (make_idesc_bf16(2 * BM, BN) & ~((1u << 7) | (1u << 10))) : make_idesc_bf16(2 * BM, BN);
+      const uint64_t desc_hi = make_sdesc_k128(0);   // all but the 14-bit start address
+      const uint32_t base16 = (smem_base >> 4) & 0x3FFF;
       int s = 0, it = 0;
       uint32_t ph = 0;
       for (int t = pair; t < n_tiles; t += n_pairs, ++it) {
@@ -741,22 +788,19 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
           if (kb == n_kb - 1) GT_TRACE(4);
           if (it == 0 && kb == n_kb - 1) GT_TRACE(9);
           if (it == 0 && kb == 8) GT_TRACE(13);
-          if (elect_one()) {
-            const uint32_t a_addr = smem_base + s * Cfg::STAGE_BYTES;
-            const uint32_t b_addr = a_addr + Cfg::A_BYTES;
+          const uint32_t a16 = base16 + s * (Cfg::STAGE_BYTES >> 4), b16 = a16 + (Cfg::A_BYTES >> 4);
 #pragma unroll
-            for (int kk = 0; kk < BK / 16; ++kk) {
-              umma_bf16_cg2(d_tmem, make_sdesc_k128(a_addr + kk * 32), make_sdesc_k128(b_addr + kk * 32), idesc,
-                            (kb | kk) != 0);
-            }
-            umma_commit_cg2(empty_bar(s));
-            if (kb == n_kb - 1) umma_commit_cg2(tfull_bar(acc));
+          for (int kk = 0; kk < BK / 16; ++kk) {
+            umma_bf16_cg2(d_tmem, desc_hi | (uint64_t)(a16 + kk * 2), desc_hi | (uint64_t)(b16 + kk * 2), idesc,
+                          kk ? 1u : (uint32_t)(kb != 0));
           }
-          __syncwarp();
+          umma_commit_cg2(empty_bar(s));
+          if (kb == n_kb - 1) umma_commit_cg2(tfull_bar(acc));
           if (++s == Cfg::STAGES) { s = 0; ph ^= 1; }
         }
       }
     }
+    __syncwarp();
   } else {  // ---------------- epilogue warps 2..9 (both CTAs, each on its own 128 rows)
     const int q = warp & 3;
     const int half = (warp - 2) >> 2;
@@ -912,12 +956,17 @@ static cudaError_t launch_one(const op16* A, const op16* W, int M, int N, int K,
     if (e != cudaSuccess) return e;
   }
   CUtensorMap tmA, tmB;
-  if (!make_tmap_2d(&tmA, A, (uint64_t)M, (uint64_t)K, BM, a.in_fp16) ||
+  // one row block of fewer than 128 rows: load only those rows (rounded up to the swizzle's 8-row period)
+  const int a_rows = M < BM ? (M + 7) / 8 * 8 : BM;
+  // k-blocks per stage (gemm1_mma): 4, 2 or 1, as many as divide K and still leave three stages in the ring
+  int kc = 1;
+  while (kc < 4 && K % (BK * kc * 2) == 0 && Cfg::RING / ((a_rows * BK * 2 + Cfg::B_BYTES) * kc * 2) >= 3) kc *= 2;
+  if (!make_tmap_2d(&tmA, A, (uint64_t)M, (uint64_t)K, (uint32_t)a_rows, a.in_fp16) ||
       !make_tmap_2d(&tmB, W, (uint64_t)N, (uint64_t)K, BN, a.in_fp16))
     return cudaErrorInvalidValue;
   const int tiles = ((M + BM - 1) / BM) * (N / BN);
   const int grid = tiles < num_sms() ? tiles : num_sms();
-  return launch_k(k_gemm_tc<BN, EPI>, dim3(grid), dim3(kGemmThreads), Cfg::SMEM, s, tmA, tmB, M, N, K, a);
+  return launch_k(k_gemm_tc<BN, EPI>, dim3(grid), dim3(kGemmThreads), Cfg::SMEM, s, tmA, tmB, M, N, K, a_rows, kc, a);
 }
 
 template <int BN, int EPI>
