@@ -500,20 +500,38 @@ __device__ __forceinline__ void gemm1_producer(const CUtensorMap* tmA, const CUt
                                                int n_kb) {
   using Cfg = GemmCfg<BN>;
   const uint32_t a_span = a_chunk * KC, stage_bytes = a_span + Cfg::B_BYTES * KC;
-  if (elect_one()) {
+  const bool issuer = elect_one();
+  // weights do not depend on the previous kernel: the W tiles of the first ring-full of stages go out before the
+  // dependency wait, the A tiles of the same stages after it (they complete the same barriers)
+  const int pre = (int)blockIdx.x < n_tiles ? min(n_stages, n_kb) : 0;
+  if (issuer) {
+    const int n0 = ((int)blockIdx.x / n_m) * BN;
+    for (int kb = 0; kb < pre; ++kb) {
+      mbar_expect_tx(bar_base + 8u * kb, stage_bytes);
+#pragma unroll
+      for (int c = 0; c < KC; ++c)
+        tma_load_2d(smem_base + kb * stage_bytes + a_span + c * Cfg::B_BYTES, tmB, bar_base + 8u * kb, (kb * KC + c) * BK, n0);
+    }
+  }
+  pdl_wait();
+  pdl_trigger();
+  if (issuer) {
     int s = 0;
     uint32_t ph = 0;
     for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
       const int m0 = (t % n_m) * BM, n0 = (t / n_m) * BN;
       for (int kb = 0; kb < n_kb; ++kb) {
         const uint32_t full = bar_base + 8u * s;
-        mbar_wait_idle(bar_base + 8u * (Cfg::MAX_STAGES + s), ph ^ 1);
-        mbar_expect_tx(full, stage_bytes);
         const uint32_t a_dst = smem_base + s * stage_bytes;
+        const bool first_pass = t == (int)blockIdx.x && kb < pre;
+        if (!first_pass) {
+          mbar_wait_idle(bar_base + 8u * (Cfg::MAX_STAGES + s), ph ^ 1);
+          mbar_expect_tx(full, stage_bytes);
+        }
 #pragma unroll
         for (int c = 0; c < KC; ++c) {
           tma_load_2d(a_dst + c * a_chunk, tmA, full, (kb * KC + c) * BK, m0);
-          tma_load_2d(a_dst + a_span + c * Cfg::B_BYTES, tmB, full, (kb * KC + c) * BK, n0);
+          if (!first_pass) tma_load_2d(a_dst + a_span + c * Cfg::B_BYTES, tmB, full, (kb * KC + c) * BK, n0);
         }
         if (++s == n_stages) { s = 0; ph ^= 1; }
       }
@@ -608,8 +626,9 @@ k_gemm_tc(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
-  pdl_wait();     // everything above overlapped the previous kernel's tail
-  pdl_trigger();
+  // dependency wait: per role (the producer sends out its first W tiles before it, gemm1_producer); everything
+  // above overlapped the previous kernel's tail
+  if (warp != 0) { pdl_wait(); pdl_trigger(); }
 
   if (warp == 0) {  // ---------------- TMA producer
     if (kc == 4) gemm1_producer<BN, 4>(&tmA, &tmB, smem_base, bar_base, a_chunk, n_stages, n_tiles, n_m, n_kb);
@@ -736,30 +755,47 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
   if (warp == 0) GT_TRACE(1);
-  pdl_wait();     // everything above overlapped the previous kernel's tail
-  pdl_trigger();
-  if (warp == 0) GT_TRACE(2);
+  // Dependency wait: per role.  The producer first sends out the W tiles of its first ring-full of stages (weights do
+  // not depend on the previous kernel; the A tiles of the same stages follow after the wait and complete the same
+  // barriers); everyone else waits here.  Everything above overlapped the previous kernel's tail.
+  if (warp != 0) { pdl_wait(); pdl_trigger(); }
 
   // The two issue loops are each ONE thread's dependent instruction stream: what they execute per k-block bounds the
   // K loop of every tile narrower than the tensor pipe's 2 BN cycles, so they run on one elected lane from start to
   // end (no per-k-block elect / warp sync) with the descriptors' constant parts hoisted.
   if (warp == 0) {  // ---------------- TMA producer (both CTAs; completion counted in the leader)
-    if (elect_one()) {
+    const bool issuer = elect_one();
+    const uint32_t lfull0 = mapa_shared(full_bar(0), 0);
+    const int pre = pair < n_tiles ? min(Cfg::STAGES, n_kb) : 0;   // stages whose W tile goes out before the wait
+    if (issuer) {
+      const int n0 = (pair / n_m) * BN + (int)rank * (BN / 2);
+      for (int kb = 0; kb < pre; ++kb) {
+        mbar_expect_tx_cluster(lfull0 + 8u * kb, Cfg::STAGE_BYTES);
+        tma_load_2d_cg2(smem_base + kb * Cfg::STAGE_BYTES + Cfg::A_BYTES, &tmB, lfull0 + 8u * kb, kb * BK, n0);
+      }
+    }
+    pdl_wait();
+    pdl_trigger();
+    GT_TRACE(2);
+    if (issuer) {
       const int lane = 0;  // GT_TRACE
       (void)lane;
-      const uint32_t lfull0 = mapa_shared(full_bar(0), 0);
       int s = 0;
       uint32_t ph = 0;
       for (int t = pair; t < n_tiles; t += n_pairs) {
         const int m0 = (t % n_m) * (2 * BM) + (int)rank * BM, n0 = (t / n_m) * BN + (int)rank * (BN / 2);
         for (int kb = 0; kb < n_kb; ++kb) {
-          mbar_wait_idle(empty_bar(s), ph ^ 1);
-          if (t == pair && kb == 0) GT_TRACE(10);
           const uint32_t lfull = lfull0 + 8u * s;
-          mbar_expect_tx_cluster(lfull, Cfg::STAGE_BYTES);
           const uint32_t a_dst = smem_base + s * Cfg::STAGE_BYTES;
-          tma_load_2d_cg2(a_dst, &tmA, lfull, kb * BK, m0);
-          tma_load_2d_cg2(a_dst + Cfg::A_BYTES, &tmB, lfull, kb * BK, n0);
+          if (t == pair && kb < pre) {   // first pass over the ring: stage free, W already on its way
+            if (kb == 0) GT_TRACE(10);
+            tma_load_2d_cg2(a_dst, &tmA, lfull, kb * BK, m0);
+          } else {
+            mbar_wait_idle(empty_bar(s), ph ^ 1);
+            mbar_expect_tx_cluster(lfull, Cfg::STAGE_BYTES);
+            tma_load_2d_cg2(a_dst, &tmA, lfull, kb * BK, m0);
+            tma_load_2d_cg2(a_dst + Cfg::A_BYTES, &tmB, lfull, kb * BK, n0);
+          }
           if (++s == Cfg::STAGES) { s = 0; ph ^= 1; }
         }
       }
