@@ -173,36 +173,32 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
   const uint32_t tmem_q = tmem_base + 384;      // columns [384, 512): Q, 256 bf16 per row
 
   if (warp == 0) {
-    // ------------------------------------------------ TMA producer (whole warp; one lane issues)
+    // ------------------------------------------------ TMA producer: ONE thread from start to end
     // Ring entries in MMA consumption order: Q (2 entries), K(0), then K(i+1), V(i) for every block.
+    const bool issuer = elect_one();
     uint32_t rp = 0;  // entries issued so far
     AttnSeg nxt = ld_seg(segs + seg_beg);
-    if (lane == 0) {
-      const CUtensorMap* km = kv_maps + ((size_t)nxt.robot * dm.layers + layer) * 2;
-      prefetch_tensormap(km); prefetch_tensormap(km + 1);
-    }
     // The prefix cache does not depend on the previous kernel: the first segment's K(kb0), K(kb0+1), V(kb0) go out
     // BEFORE the dependency wait, straight into the ring entries they will be consumed from (2, 3, 4); Q and the
     // block of the robot's own tokens (written by the QKV GEMM) follow after it.
     uint32_t pre_mask = 0;
-    {
-      const int nbp = (nxt.len + AT_KV - 1) / AT_KV, n = nxt.kb1 - nxt.kb0;
+    if (issuer) {
       const CUtensorMap* km = kv_maps + ((size_t)nxt.robot * dm.layers + layer) * 2;
+      prefetch_tensormap(km); prefetch_tensormap(km + 1);
+      const int nbp = (nxt.len + AT_KV - 1) / AT_KV, n = nxt.kb1 - nxt.kb0;
       const int blk[3] = {nxt.kb0, n > 1 ? nxt.kb0 + 1 : nxt.kb0, nxt.kb0};
       const bool isv[3] = {false, n > 1 ? false : true, true};
       const int cnt = n > 1 ? 3 : 2;
       for (int x = 0; x < cnt; ++x)
         if (blk[x] < nbp) {
-          if (elect_one()) {
-            mbar_expect_tx(full(2 + x), AT_STAGE_BYTES);
-            tma_load_3d(stage(2 + x), isv[x] ? km + 1 : km, full(2 + x), 0, blk[x] * AT_KV, 0);
-          }
-          __syncwarp();
+          mbar_expect_tx(full(2 + x), AT_STAGE_BYTES);
+          tma_load_3d(stage(2 + x), isv[x] ? km + 1 : km, full(2 + x), 0, blk[x] * AT_KV, 0);
           pre_mask |= 1u << (2 + x);
         }
     }
     pdl_wait();     // everything above overlapped the previous kernel's tail
     pdl_trigger();
+    if (issuer) {
     auto acquire = [&](bool& issue) {   // next ring entry; issue = false if it was filled before the wait
       const int s = (int)(rp % AT_RING);
       issue = !(rp < AT_RING && ((pre_mask >> rp) & 1u));
@@ -214,7 +210,7 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
       const AttnSeg sg = nxt;
       if (si + 1 < seg_end) {   // the next record and its robot's tensor maps are fetched a whole segment ahead
         nxt = ld_seg(segs + si + 1);
-        if (lane == 0 && nxt.robot != sg.robot) {
+        if (nxt.robot != sg.robot) {
           const CUtensorMap* km = kv_maps + ((size_t)nxt.robot * dm.layers + layer) * 2;
           prefetch_tensormap(km); prefetch_tensormap(km + 1);
         }
@@ -228,48 +224,52 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
       auto load_kv = [&](int i, bool is_v) {
         bool issue;
         const int s = acquire(issue);
-        if (issue && elect_one()) {
+        if (issue) {
           mbar_expect_tx(full(s), AT_STAGE_BYTES);
           if (i == nbp) tma_load_3d(stage(s), &maps.own, full(s), 0, p * dm.H, (dm.q_n + (is_v ? AT_HD : 0)) / 64);
           else tma_load_3d(stage(s), is_v ? vmap : kmap, full(s), 0, i * AT_KV, 0);
         }
-        __syncwarp();
       };
       for (int e = 0; e < 2; ++e) {
         bool issue;
         const int s = acquire(issue);
-        if (elect_one()) {
-          mbar_expect_tx(full(s), AT_STAGE_BYTES);
-          for (int c = 0; c < 2; ++c) tma_load_3d(stage(s) + c * (AT_ROWS * 128), &maps.q, full(s), (2 * e + c) * 64, 0, tok0);
-        }
-        __syncwarp();
+        mbar_expect_tx(full(s), AT_STAGE_BYTES);
+        for (int c = 0; c < 2; ++c) tma_load_3d(stage(s) + c * (AT_ROWS * 128), &maps.q, full(s), (2 * e + c) * 64, 0, tok0);
       }
       load_kv(sg.kb0, false);
       for (int i = sg.kb0; i < sg.kb1; ++i) {  // K runs one block ahead of V: it is needed a whole softmax earlier
         if (i + 1 < sg.kb1) load_kv(i + 1, false);
         load_kv(i, true);
-        if (elect_one()) {
-          // L2 prefetches go out only after everything the first MMAs wait for (Q, K0, K1, V0) is in flight
-          const int lim = min(sg.kb1, nbp);
-          if (i == sg.kb0)
-            for (int j = sg.kb0 + 2; j < sg.kb0 + AT_PF; ++j)
-              if (j < lim) { tma_prefetch_3d(kmap, 0, j * AT_KV, 0); tma_prefetch_3d(vmap, 0, j * AT_KV, 0); }
-          if (i + AT_PF < lim) { tma_prefetch_3d(kmap, 0, (i + AT_PF) * AT_KV, 0); tma_prefetch_3d(vmap, 0, (i + AT_PF) * AT_KV, 0); }
-        }
-        __syncwarp();
+        // L2 prefetches go out only after everything the first MMAs wait for (Q, K0, K1, V0) is in flight
+        const int lim = min(sg.kb1, nbp);
+        if (i == sg.kb0)
+          for (int j = sg.kb0 + 2; j < sg.kb0 + AT_PF; ++j)
+            if (j < lim) { tma_prefetch_3d(kmap, 0, j * AT_KV, 0); tma_prefetch_3d(vmap, 0, j * AT_KV, 0); }
+        if (i + AT_PF < lim) { tma_prefetch_3d(kmap, 0, (i + AT_PF) * AT_KV, 0); tma_prefetch_3d(vmap, 0, (i + AT_PF) * AT_KV, 0); }
       }
     }
+    }
+    __syncwarp();
   } else if (warp == 1) {
-    // ------------------------------------------------ MMA issuer (whole warp; one lane issues)
+    // ------------------------------------------------ MMA issuer: ONE thread from start to end.  Its instruction
+    // stream is a chain of dependent instructions on the path P ready -> PV issued -> O / next S; as a warp-wide
+    // loop with an elect and a warp sync per step and a descriptor built per MMA it took longer to ISSUE the 16 MMAs
+    // of an S block than the tensor pipe takes to run them (the GEMM issue loops).
     pdl_wait();
     pdl_trigger();
+    if (elect_one()) {
     constexpr uint32_t idesc_s = make_idesc_bf16(AT_ROWS, AT_KV);
     constexpr uint32_t idesc_o = make_idesc_bf16(AT_ROWS, AT_HD, /*b_mn_major=*/true);
+    // shared-memory descriptors: everything but the 14-bit start address is constant
+    const uint64_t kdesc_hi = make_sdesc_k128(0);                       // K block, K-major
+    const uint64_t vdesc_hi = make_sdesc_mn128(0, AT_KV * 128, 1024);   // V block, MN-major: 4 hd chunks 8192 B apart (LBO), 8-key groups 1024 B apart (SBO)
+    const uint32_t base16 = (base >> 4) & 0x3FFF;
     uint32_t rp = 0;  // ring entries consumed
     uint32_t g = 0;   // key blocks issued so far in this CTA (selects the S/P buffer and the barrier parities)
     uint32_t j = 0;   // segments started
 #ifdef ROSA_TRACE
-    long long w_full = 0, w_p = 0;   // cycles this warp waited for ring data / for the softmax warps
+    const int lane = 0;   // AT_TRACE
+    long long w_full = 0, w_p = 0;   // cycles this thread waited for ring data / for the softmax warps
 #define AT_WAIT(acc, stmt) do { const long long t_ = clock64(); stmt; acc += clock64() - t_; } while (0)
 #else
 #define AT_WAIT(acc, stmt) do { stmt; } while (0)
@@ -284,26 +284,20 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
         AT_WAIT(w_full, mbar_wait(full(s), (rp / AT_RING) & 1));
         ++rp;
         tc_fence_after();
-        if (elect_one()) {
+        const uint32_t k16 = base16 + (uint32_t)s * (AT_STAGE_BYTES >> 4);
+        const uint32_t d_s = tmem_s + (gi & 1) * AT_KV;
 #pragma unroll
-          for (int kk = 0; kk < AT_HD / 16; ++kk) {
-            const uint32_t ka = stage(s) + (kk >> 2) * (AT_KV * 128) + (kk & 3) * 32;
-            umma_bf16_ts(tmem_s + (gi & 1) * AT_KV, tmem_q + kk * 8, make_sdesc_k128(ka), idesc_s, kk != 0);
-          }
-          umma_commit(empty(s));
-          umma_commit(s_full(gi & 1));
-        }
-        __syncwarp();
+        for (int kk = 0; kk < AT_HD / 16; ++kk)   // 64-column chunk kk >> 2 of the block (AT_KV * 128 B apart), 32 B per 16 columns
+          umma_bf16_ts(d_s, tmem_q + kk * 8, kdesc_hi | (uint64_t)(k16 + (kk >> 2) * ((AT_KV * 128) >> 4) + (kk & 3) * 2), idesc_s, kk != 0);
+        umma_commit(empty(s));
+        umma_commit(s_full(gi & 1));
       };
       // Q of this segment is in tensor memory (softmax warps); its two ring entries are free again
       mbar_wait(q_ready, j & 1);
       tc_fence_after();
       AT_TRACE(8 + 8 * j + 5);
-      if (elect_one()) {
-        mbar_arrive(empty((int)(rp % AT_RING)));
-        mbar_arrive(empty((int)((rp + 1) % AT_RING)));
-      }
-      __syncwarp();
+      mbar_arrive(empty((int)(rp % AT_RING)));
+      mbar_arrive(empty((int)((rp + 1) % AT_RING)));
       rp += 2;
       issue_s(g);
       for (int i = 0; i < n; ++i) {
@@ -315,26 +309,26 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
         if (i == 0 && j > 0) mbar_wait(o_empty, (j - 1) & 1);  // the previous segment's O has left tensor memory
         AT_WAIT(w_p, mbar_wait(p_full(gi & 1), (gi >> 1) & 1));
         tc_fence_after();
-        if (elect_one()) {
+        const uint32_t v16 = base16 + (uint32_t)s * (AT_STAGE_BYTES >> 4);
+        const uint32_t a_p = tmem_s + (gi & 1) * AT_KV;
 #pragma unroll
-          for (int kk = 0; kk < AT_KV / 16; ++kk) {
-            // A = P [128 x 64] bf16 in TMEM (8 columns per 16 keys); B = V block, MN-major: 4 hd chunks
-            // 8192 B apart (LBO), 8-key groups 1024 B apart (SBO); 16 keys per MMA = 2048 B
-            const uint64_t b_desc = make_sdesc_mn128(stage(s) + kk * 2048, AT_KV * 128, 1024);
-            // P of keys 16 kk .. 16 kk + 15: columns 8 (kk & 1) of the half (kk >> 1) that wrote it (32 columns apart)
-            umma_bf16_ts(tmem_o, tmem_s + (gi & 1) * AT_KV + (kk >> 1) * 32 + (kk & 1) * 8, b_desc, idesc_o, (i | kk) != 0);
-          }
-          umma_commit(empty(s));
-          umma_commit(pv_done);
+        for (int kk = 0; kk < AT_KV / 16; ++kk) {
+          // A = P [128 x 64] bf16 in TMEM (8 columns per 16 keys): keys 16 kk .. 16 kk + 15 are columns 8 (kk & 1) of the
+          // half (kk >> 1) that wrote them (32 columns apart); B = V block, 16 keys per MMA = 2048 B
+          umma_bf16_ts(tmem_o, a_p + (kk >> 1) * 32 + (kk & 1) * 8, vdesc_hi | (uint64_t)(v16 + kk * (2048 >> 4)), idesc_o,
+                       kk ? 1u : (uint32_t)(i != 0));
         }
-        __syncwarp();
+        umma_commit(empty(s));
+        umma_commit(pv_done);
       }
       AT_TRACE(8 + 8 * j + 6);
       g += n;
     }
 #ifdef ROSA_TRACE
-    if (lane == 0) { g_attn_trace[blockIdx.x * 64 + 3] = w_full; g_attn_trace[blockIdx.x * 64 + 4] = w_p; }
+    g_attn_trace[blockIdx.x * 64 + 3] = w_full; g_attn_trace[blockIdx.x * 64 + 4] = w_p;
 #endif
+    }
+    __syncwarp();
   } else {
     // ---------------------------------------------------------- softmax + drain warps (2..9)
     // Two warps per TMEM lane quarter: a query row's 64 scores of a block are split 32 / 32 between
