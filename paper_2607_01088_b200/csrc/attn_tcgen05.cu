@@ -5,9 +5,10 @@
 // [prefix K/V (L_p rows, from the bound cache) ; own k/v (H rows, from the qkv buffer)], walked in blocks of
 // 64 keys:
 //     S = Q K_blk^T           tcgen05.mma  M=128 N=64  K=256   Q is the A operand FROM TENSOR MEMORY
-//     P = exp2(S*c - m_ref)   8 softmax warps, two per query row (32 keys each; the row maximum of the block is
-//                             exchanged through shared memory), running (m_ref, partial l) in registers; P (bf16)
-//                             is written back into tensor memory over the warp's own scores
+//     P = exp2(S*c - m_ref)   8 softmax warps, two per query row: one takes the even key blocks, the other the odd ones
+//                             (whole rows of 64 scores; the row's reference m_ref is handed from block to block
+//                             through shared memory), each with its own partial l in registers; P (bf16) is
+//                             written back into tensor memory over the scores
 //     O += P V_blk            tcgen05.mma  M=128 N=256 K=64    P is the A operand from tensor memory,
 //                             V the MN-major B operand from shared memory
 // Tensor memory (512 columns): O [0,256) | S/P double buffer [256,384) | Q [384,512).
@@ -52,8 +53,8 @@ constexpr int AT_STAGE_BYTES = AT_KV * AT_HD * 2;   // 32 KB: 4 chunks [64 x 64]
 // the CTA's scratch slot).  (TMA tensor stores into o were measured at ~1k cycles of issue time each.)
 constexpr int AT_STG_BYTES = AT_ROWS * AT_HD * 2;   // 64 KB
 constexpr int AT_ML_BYTES = 2 * AT_ROWS * 4;
-constexpr int AT_MX_BYTES = 2 * 2 * AT_ROWS * 2;    // row-maximum exchange per block (16-bit, rounded up), double-buffered by block parity
-constexpr int AT_SMEM = AT_RING * AT_STAGE_BYTES + AT_STG_BYTES + AT_ML_BYTES + AT_MX_BYTES + 192;
+constexpr int AT_MX_BYTES = AT_ROWS * 4;            // the row's softmax reference, handed from the warp of block i to the warp of block i + 1
+constexpr int AT_SMEM = AT_RING * AT_STAGE_BYTES + AT_STG_BYTES + AT_ML_BYTES + AT_MX_BYTES + 256;
 static_assert(AT_SMEM <= 232448, "shared memory of one CTA");
 constexpr float AT_RESCALE_THR = 8.0f;              // log2 units
 constexpr size_t AT_PART_BYTES = AT_STG_BYTES + AT_ML_BYTES;   // scratch slot of a CTA: a copy of staging + statistics
@@ -139,10 +140,16 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
   // p_full is double-buffered like S/P: the softmax warps may finish block i+1 before the MMA thread
   // has looked at block i's barrier, and a single barrier two phases ahead reads as "not yet"
   auto p_full = [&](int b) { return bars + 8u * (2 * AT_RING + 2 + b); };
-  const uint32_t pv_done = bars + 8u * (2 * AT_RING + 4);
-  const uint32_t q_ready = bars + 8u * (2 * AT_RING + 5), o_empty = bars + 8u * (2 * AT_RING + 6);
-  const uint32_t part_full = bars + 8u * (2 * AT_RING + 7);   // the partner's partial result has landed in staging
-  const uint32_t tmem_slot = bars + 8u * (2 * AT_RING + 8);
+  // PV(x) completes pv_done(x & 3), phase x >> 2.  A parity wait is only meaningful while the barrier is at most one
+  // phase ahead of the waiter; the softmax warps look at these barriers rarely (an O rescale, the drain) and with four
+  // of them "PV(x - 4) is known to be complete, PV(x + 4) cannot have been issued" is all a waiter for PV(x) needs -
+  // both hold wherever PV(x) is waited for (the MMA thread issues PV(x + 1) only after this warp's or its partner's P).
+  auto pv_done = [&](uint32_t x) { return bars + 8u * (2 * AT_RING + 4 + (x & 3u)); };
+  const uint32_t q_ready = bars + 8u * (2 * AT_RING + 8), o_empty = bars + 8u * (2 * AT_RING + 9);
+  const uint32_t part_full = bars + 8u * (2 * AT_RING + 10);   // the partner's partial result has landed in staging
+  const uint32_t tmem_slot = bars + 8u * (2 * AT_RING + 11);
+  // hand(q, b): the warp of lane quarter q that did block gi (b = gi & 1) has left the rows' reference in shared memory
+  auto hand = [&](int qq, int b) { return bars + 8u * (2 * AT_RING + 12 + qq * 2 + b); };
   volatile uint32_t* tmem_slot_ptr = reinterpret_cast<volatile uint32_t*>(smem_raw + (tmem_slot - base));
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -153,8 +160,9 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
     prefetch_tensormap(&maps.own);
     for (int s = 0; s < AT_RING; ++s) { mbar_init(full(s), 1); mbar_init(empty(s), 1); }
     mbar_init(s_full(0), 1); mbar_init(s_full(1), 1);
-    mbar_init(p_full(0), 8); mbar_init(p_full(1), 8);  // one arrival per softmax warp
-    mbar_init(pv_done, 1);
+    mbar_init(p_full(0), 4); mbar_init(p_full(1), 4);  // one arrival per softmax warp of the block's set
+    for (uint32_t x = 0; x < 4; ++x) mbar_init(pv_done(x), 1);
+    for (int x = 0; x < 8; ++x) mbar_init(hand(x >> 1, x & 1), 1);
     mbar_init(q_ready, 8);
     mbar_init(o_empty, 8);
     mbar_init(part_full, 1);
@@ -319,7 +327,7 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
                        kk ? 1u : (uint32_t)(i != 0));
         }
         umma_commit(empty(s));
-        umma_commit(pv_done);
+        umma_commit(pv_done(gi));
       }
       AT_TRACE(8 + 8 * j + 6);
       g += n;
@@ -337,12 +345,17 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
     pdl_wait();
     pdl_trigger();
     if (warp == 2) AT_TRACE(1);
-    const int q = warp & 3, half = (warp - 2) >> 2;
+    const int q = warp & 3, set = (warp - 2) >> 2;     // set: does the softmax of the key blocks with (CTA-wide count) & 1 == set
+    const int half = set;                              // which half of O's columns / of Q's chunks this warp moves
     const int r = q * 32 + lane;                       // query row of this thread
     const uint32_t lane_off = (uint32_t)(q * 32) << 16;
     float* ml = reinterpret_cast<float*>(smem_raw + (AT_RING * AT_STAGE_BYTES + AT_STG_BYTES));   // m[128], l[128]
     float* xch = ml;   // the drain's row-sum exchange [2 halves][128] uses the same kilobyte (see the drain)
-    uint16_t* mx = reinterpret_cast<uint16_t*>(ml + 2 * AT_ROWS);                              // [2 parities][2 halves][128]
+    float* mref_sm = ml + 2 * AT_ROWS;                 // [128] the rows' reference after the latest block
+    auto pv_wait = [&](uint32_t x) { mbar_wait(pv_done(x), (x >> 2) & 1); };   // PV(x) has completed
+    auto exp2_int = [](float d) {   // 2^d for an integer d <= 0 (or -inf), exactly; 0 below the normal range
+      return d < -126.f ? 0.f : __int_as_float(((int)d + 127) << 23);
+    };
     const float c_log2 = rsqrtf((float)AT_HD) * 1.4426950408889634f;  // (1/sqrt(hd)) * log2(e)
     const bool issuer = warp == 2 && lane == 0;        // the thread that owns this CTA's bulk-copy groups
     // Q of a segment: shared memory (SW128 chunks of [128 rows x 128 B]) -> tensor memory, thread = row; this half's
@@ -401,27 +414,29 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
       const bool merge = sg.n_part > 0;   // head segment of a cut item: always the last entry of the list
       rp += 2 + 2 * n;   // ring position of the next segment's Q
       bool part_issued = false;           // issuer: the partner's partial result is on its way into staging
-      float m_ref = -INFINITY, l_sum = 0.f;            // m_ref in log2 units; l_sum: this half's part
-      for (int i = 0; i < n; ++i) {
+      // Reference m (log2 units, an integer) and this warp's part of the row sum, relative to the reference at this
+      // warp's last own block (m_own); the row's current reference travels through mref_sm from block to block.
+      float m_own = -INFINITY, l_own = 0.f;
+      for (int i = (int)((g ^ (uint32_t)set) & 1u); i < n; i += 2) {   // the blocks with (g + i) & 1 == set
         const uint32_t gi = g + i;
-        const int sb = gi & 1, kb = sg.kb0 + i;
-        const int n_tot = kb == nbp ? dm.H : min(AT_KV, L - kb * AT_KV);
-        const int n_valid = n_tot - half * 32;  // valid columns of this half
+        const int sb = set, kb = sg.kb0 + i;
+        const int n_tot = kb == nbp ? dm.H : min(AT_KV, L - kb * AT_KV);   // valid keys of the block
         // Housekeeping of the asynchronous copies by the issuing thread, off the critical path.
-        //  * second block (or the last one): the previous drain's copy out of staging is (almost certainly) complete,
-        //    so a continuation's partial result is in global memory: publish it;
-        //  * last block: staging may be overwritten by this segment's drain (every warp's drain follows this thread's
-        //    p_full arrival of this block through pv_done);
+        //  * from the segment's second block on: the previous drain's copy out of staging is (almost certainly)
+        //    complete, so a continuation's partial result is in global memory: publish it;
+        //  * this thread's last block of the segment: staging may be overwritten by this segment's drain (every warp's
+        //    drain follows the last PV, whose P needs this block's reference or P: both come after this point);
         //  * head of a cut item: as soon as the other CTA has published its partial, pull it into staging (the drain
         //    merges it in place).  The flag is polled with a relaxed load issued here and looked at after the block.
         int flag_seen = 0;
         if (issuer) {
-          if (i == n - 1 || i == 1) settle();
+          if (i >= 1 || i + 2 >= n) settle();
           if (merge && !part_issued) flag_seen = ld_relaxed_gpu(part_flag + sg.part0);
         }
         __syncwarp();
 #ifdef ROSA_TRACE
-#define AT_BLK(k) do { if ((warp == 2 || warp == 6) && i == 4 && si == seg_beg) AT_TRACE((warp == 2 ? 40 : 48) + (k)); } while (0)
+#define AT_BLK(k) do { if ((warp == 2 || warp == 6) && (i == 4 || i == 5) && si == seg_beg) AT_TRACE((warp == 2 ? 40 : 48) + (k)); \
+                       if ((warp == 2 || warp == 6) && (i == 6 || i == 7) && si == seg_beg && (k) == 0) AT_TRACE((warp == 2 ? 47 : 55)); } while (0)
 #else
 #define AT_BLK(k) do { } while (0)
 #endif
@@ -429,71 +444,57 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
         mbar_wait(s_full(sb), (gi >> 1) & 1);
         tc_fence_after();
         AT_BLK(1);
-        if (warp == 2 && i == 0) AT_TRACE(8 + 8 * (si - seg_beg) + 0);
-        // Each warp of a row's pair reads only its own 32 scores; the row maximum of the block is exchanged through
-        // shared memory (so both take the same rescale decision).  P is stored over this warp's OWN score columns
-        // (P of half h at columns 32 h .. 32 h + 15 of the S buffer), so neither warp ever reads a column the other
-        // overwrites, however far apart the two run.
-        float sc[32];
-        float m_blk;
+        if (warp == 2 + 4 * (int)(g & 1) && i < 2) AT_TRACE(8 + 8 * (si - seg_beg) + 0);
+        // The warp takes the block's whole rows (64 scores per thread): no exchange of the maximum, and the two
+        // warps of a scheduler are in different phases of different blocks - one in its 64 ex2 per thread while the
+        // other loads, reduces or stores - instead of both queueing on the SFU at the same moment.
+        float sc[64];
         {
-          uint32_t r0[32];
-          tmem_ld32(tmem_s + lane_off + sb * AT_KV + half * 32, r0);
+          uint32_t r0[32], r1[32];
+          tmem_ld32(tmem_s + lane_off + sb * AT_KV, r0);
+          tmem_ld32(tmem_s + lane_off + sb * AT_KV + 32, r1);
           tmem_ld_wait();
 #pragma unroll
-          for (int c = 0; c < 32; ++c) sc[c] = __uint_as_float(r0[c]);
-          if (n_valid < 32) {  // warp-uniform; only the last prefix block and the own-token block are ragged
+          for (int c = 0; c < 32; ++c) { sc[c] = __uint_as_float(r0[c]); sc[32 + c] = __uint_as_float(r1[c]); }
+        }
+        if (n_tot < AT_KV) {  // warp-uniform; only the last prefix block and the own-token block are ragged
 #pragma unroll
-            for (int c = 0; c < 32; ++c) sc[c] = c < n_valid ? sc[c] : -INFINITY;
+          for (int c = 0; c < 64; ++c) sc[c] = c < n_tot ? sc[c] : -INFINITY;
+        }
+        float mo;
+        {   // four independent chains (the serial one is 32 dependent 3-input maxima on the critical path)
+          float m4[4] = {sc[0], sc[1], sc[2], sc[3]};
+#pragma unroll
+          for (int c = 4; c < 64; c += 4) {
+#pragma unroll
+            for (int x = 0; x < 4; ++x) m4[x] = fmaxf(m4[x], sc[c + x]);
           }
-          float mo = sc[0];
-#pragma unroll
-          for (int c = 1; c < 32; ++c) mo = fmaxf(mo, sc[c]);
-          // exchanged as the smallest bf16 >= mo (both warps use the rounded values, their own included, so they
-          // agree exactly; a reference maximum slightly above the true one is harmless)
-          const uint32_t mb = __float_as_uint(mo);
-          const uint16_t up = (uint16_t)((mo >= 0.f ? mb + 0xffffu : mb) >> 16);
-          mx[(gi & 1) * (2 * AT_ROWS) + half * AT_ROWS + r] = up;
-          AT_BLK(2);
-          named_bar_sync(5 + q, 64);
-          AT_BLK(3);
-          const uint16_t other = mx[(gi & 1) * (2 * AT_ROWS) + (half ^ 1) * AT_ROWS + r];
-          m_blk = fmaxf(__uint_as_float((uint32_t)up << 16), __uint_as_float((uint32_t)other << 16));
+          mo = fmaxf(fmaxf(m4[0], m4[1]), fmaxf(m4[2], m4[3]));
         }
         // The reference is an INTEGER in the log2 domain: a different reference (another lazy-rescale history,
         // another cut of the key stream between CTAs: R27) then scales P, l and O by an exact power of two, so the
         // bf16 rounding of P - the dominant rounding of the whole attention step - is the same whichever way the
         // item was planned.  What is left between two plans is fp32 summation order and the 16-bit hand-over.
-        m_blk = ceilf(m_blk * c_log2);
+        const float m_blk = ceilf(mo * c_log2);
+        AT_BLK(2);
+        // the row's reference after block gi - 1, from the other set's warp of this lane quarter (waited for at every
+        // block but the CTA's first, so that nobody is ever more than one phase behind these barriers)
+        if (gi > 0) mbar_wait(hand(q, (int)((gi - 1) & 1)), ((gi - 1) >> 1) & 1);
+        AT_BLK(3);
+        float m_ref = i > 0 ? mref_sm[r] : -INFINITY;
         float factor = 1.f;
-        if (m_blk > m_ref + AT_RESCALE_THR) {            // first block always lands here
-          const float dref = m_ref - m_blk;              // an integer <= -8, or -inf on the first block
-          factor = dref < -126.f ? 0.f : __int_as_float(((int)dref + 127) << 23);   // 2^dref, exactly
+        if (m_blk > m_ref + AT_RESCALE_THR) {            // the segment's first block always lands here
+          factor = exp2_int(m_ref - m_blk);              // 2^(an integer <= -8), exactly; 0 on the first block
           m_ref = m_blk;
         }
-        uint32_t pk[16];
-        float s0 = 0.f, s1 = 0.f;
-        {
-          const float neg_m = -m_ref;
-#pragma unroll
-          for (int c = 0; c < 32; c += 2) {
-            const float a = ex2_approx(fmaf(sc[c], c_log2, neg_m)), b = ex2_approx(fmaf(sc[c + 1], c_log2, neg_m));
-            s0 += a;
-            s1 += b;
-            __nv_bfloat162 v2 = __floats2bfloat162_rn(a, b);
-            pk[c >> 1] = *reinterpret_cast<uint32_t*>(&v2);
-          }
-        }
-        l_sum = l_sum * factor + (s0 + s1);
-        AT_BLK(4);
-        // Every block, not only when rescaling: a parity wait is only meaningful while the waiter is at
-        // most one phase behind the barrier (PV(gi-1) was issued ~a softmax block ago, so this is free).
-        if (gi > 0) mbar_wait(pv_done, (gi - 1) & 1);
-        AT_BLK(5);
-        if (i > 0 && __any_sync(0xffffffffu, factor != 1.f)) {  // rare: rescale this warp's rows, its half of O's columns
+        mref_sm[r] = m_ref;
+        __syncwarp();
+        if (lane == 0) mbar_arrive(hand(q, (int)(gi & 1)));
+        if (i > 0 && __any_sync(0xffffffffu, factor != 1.f)) {  // rare: rescale this warp's rows of O (all 256 columns)
+          pv_wait(gi - 1);
           tc_fence_after();                                     // O quiescent: PV(gi-1) done, PV(gi) needs this P
 #pragma unroll 1
-          for (int c = half * 4; c < half * 4 + 4; ++c) {
+          for (int c = 0; c < 8; ++c) {
             uint32_t rr[32];
             tmem_ld32(tmem_o + lane_off + c * 32, rr);
             tmem_ld_wait();
@@ -502,13 +503,30 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
             tmem_st32(tmem_o + lane_off + c * 32, rr);
           }
         }
-        // P row r, this half's 32 keys (16 columns of bf16 pairs) over this warp's own scores: the A operand of PV(gi)
-        tmem_st16(tmem_s + lane_off + sb * AT_KV + half * 32, pk);
+        float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+        const float neg_m = -m_ref;
+        // P row r: keys 32 h .. 32 h + 31 as 16 columns of bf16 pairs at columns 32 h of the S buffer (over scores this
+        // thread already holds in registers): the A operand of PV(gi)
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          uint32_t pk[16];
+#pragma unroll
+          for (int c = 0; c < 32; c += 2) {
+            const float a = ex2_approx(fmaf(sc[32 * h + c], c_log2, neg_m)), b = ex2_approx(fmaf(sc[32 * h + c + 1], c_log2, neg_m));
+            if (c & 2) { s2 += a; s3 += b; } else { s0 += a; s1 += b; }   // fixed order: four partial sums per thread
+            __nv_bfloat162 v2 = __floats2bfloat162_rn(a, b);
+            pk[c >> 1] = *reinterpret_cast<uint32_t*>(&v2);
+          }
+          tmem_st16(tmem_s + lane_off + sb * AT_KV + h * 32, pk);
+        }
+        AT_BLK(4);
+        l_own = l_own * exp2_int(m_own - m_ref) + ((s0 + s1) + (s2 + s3));   // m_own = -inf on the first own block: 0 * 0
+        m_own = m_ref;
         tmem_st_wait();
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(p_full(sb));  // 256 arrivals on one barrier would serialise on the critical path
-        AT_BLK(6);
+        if (lane == 0) mbar_arrive(p_full(sb));  // 128 arrivals on one barrier would serialise on the critical path
+        AT_BLK(5);
         if (issuer && flag_seen != 0) { fetch_partial(sg.part0); part_issued = true; }
         __syncwarp();
       }
@@ -517,6 +535,12 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
       // The next segment's Q goes into tensor memory BEFORE this segment's O is drained (if it has landed): its first
       // two S blocks then run on the tensor pipe while these warps drain.
       bool q_pending = si + 1 < seg_end;
+      // tmem_q is free once every S MMA of this segment has completed: the warps of the set that did not take the last
+      // block have not seen its s_full yet (one phase behind at most: they saw the hand-over that followed S(g - 2))
+      if (q_pending && ((g - 1) & 1u) != (uint32_t)set) {
+        mbar_wait(s_full((int)((g - 1) & 1u)), ((g - 1) >> 1) & 1);
+        tc_fence_after();
+      }
       if (q_pending && q_landed(rp)) { copy_q(rp); q_pending = false; }
       if (warp == 2) AT_TRACE(8 + 8 * (si - seg_beg) + 2);
       // ------------------------------------------------ drain.  Row r = (token jj, head a) with r = jj * 8 + a; each
@@ -531,7 +555,13 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
         fetch_partial(sg.part0);
       }
       __syncwarp();
-      mbar_wait(pv_done, (g - 1) & 1);
+      if (n == 1 && ((g - 1) & 1u) != 0u) {
+        // the issuing thread's set had no block in this one-block segment: its settle (staging free) comes here, ahead
+        // of everybody's staging writes
+        if (issuer) settle();
+        named_bar_sync(9, 256);
+      }
+      pv_wait(g - 1);   // the segment's last PV, hence all of them, has completed
       tc_fence_after();
       if (warp == 2) AT_TRACE(8 + 8 * (si - seg_beg) + 7);
       // The statistics kilobyte behind the staging tile serves three purposes in turn: a merge reads the other
@@ -542,8 +572,10 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
         mbar_wait(part_full, 0);   // at most one merge per CTA (the last entry of its list)
         m_c = ml[r];
         l_c = ml[AT_ROWS + r];
-        named_bar_sync(1 + q, 64);
       }
+      named_bar_sync(1 + q, 64);   // both warps of the row are through their blocks: mref_sm holds the final reference
+      const float m_ref = mref_sm[r];
+      const float l_sum = l_own * exp2_int(m_own - m_ref);   // this set's part, brought to the final reference (0 if it had no block)
       xch[half * AT_ROWS + r] = l_sum;
       named_bar_sync(1 + q, 64);
       float l_tot = l_sum + xch[(half ^ 1) * AT_ROWS + r];
