@@ -104,9 +104,11 @@ __device__ __forceinline__ AttnSeg ld_seg(const AttnSeg* p) {   // read-only tab
 }
 
 // Measurement aid, compiled in only with -DROSA_TRACE: clock64 of pipeline events per CTA, [cta][64]:
-// 0 entry, 1 after the dependency wait, 2 exit; per segment j < 6 at 8 + 8 j: +0 softmax: first S block ready,
-// +1 softmax loop done, +2 next Q copied, +7 last PV done, +3 O out of tensor memory, +4 drain done;
-// +5 MMA: segment start (Q ready), +6 last PV issued
+// 0 entry, 1 after the dependency wait, 2 exit, 3 / 4 cycles the MMA thread waited for ring data / for P; per segment
+// j < 4 at 8 + 8 j: +0 softmax: first S block ready, +1 softmax loop done, +2 next Q copied, +7 last PV done, +3 O out of
+// tensor memory, +4 drain done; +5 MMA: segment start (Q ready), +6 last PV issued.  Blocks 4 (warp 2, slots 40..45) and 5
+// (warp 6, 48..53) of the CTA's first segment: block start, S ready, maximum done, reference received, P stored, arrived;
+// 47 / 55 = start of blocks 6 / 7.  MMA thread, same blocks (56..59, 60..63): waiting for P from, P seen, PV issued, S(i+2) issued.
 #ifdef ROSA_TRACE
 __device__ long long g_attn_trace[160 * 64];
 #define AT_TRACE(slot) do { if (lane == 0 && (slot) < 64) g_attn_trace[blockIdx.x * 64 + (slot)] = clock64(); } while (0)
@@ -299,6 +301,9 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
           umma_bf16_ts(d_s, tmem_q + kk * 8, kdesc_hi | (uint64_t)(k16 + (kk >> 2) * ((AT_KV * 128) >> 4) + (kk & 3) * 2), idesc_s, kk != 0);
         umma_commit(empty(s));
         umma_commit(s_full(gi & 1));
+#ifdef ROSA_TRACE
+        if (si == seg_beg && (gi - g == 6 || gi - g == 7)) g_attn_trace[blockIdx.x * 64 + 56 + (gi - g - 6) * 4 + 3] = clock64();   // S(i + 2) issued
+#endif
       };
       // Q of this segment is in tensor memory (softmax warps); its two ring entries are free again
       mbar_wait(q_ready, j & 1);
@@ -315,7 +320,13 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
         AT_WAIT(w_full, mbar_wait(full(s), (rp / AT_RING) & 1));
         ++rp;
         if (i == 0 && j > 0) mbar_wait(o_empty, (j - 1) & 1);  // the previous segment's O has left tensor memory
+#ifdef ROSA_TRACE
+        if (si == seg_beg && (i == 4 || i == 5)) g_attn_trace[blockIdx.x * 64 + 56 + (i - 4) * 4 + 0] = clock64();   // about to wait for P(i)
+#endif
         AT_WAIT(w_p, mbar_wait(p_full(gi & 1), (gi >> 1) & 1));
+#ifdef ROSA_TRACE
+        if (si == seg_beg && (i == 4 || i == 5)) g_attn_trace[blockIdx.x * 64 + 56 + (i - 4) * 4 + 1] = clock64();   // P(i) seen
+#endif
         tc_fence_after();
         const uint32_t v16 = base16 + (uint32_t)s * (AT_STAGE_BYTES >> 4);
         const uint32_t a_p = tmem_s + (gi & 1) * AT_KV;
@@ -328,6 +339,9 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
         }
         umma_commit(empty(s));
         umma_commit(pv_done(gi));
+#ifdef ROSA_TRACE
+        if (si == seg_beg && (i == 4 || i == 5)) g_attn_trace[blockIdx.x * 64 + 56 + (i - 4) * 4 + 2] = clock64();   // PV(i) issued
+#endif
       }
       AT_TRACE(8 + 8 * j + 6);
       g += n;
