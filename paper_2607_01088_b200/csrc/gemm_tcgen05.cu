@@ -458,35 +458,40 @@ __device__ __forceinline__ void epilogue_tile(const EpiArgs& ea, EpiPre& pre, fl
     uint16_t* outp = (uint16_t*)ea.out16;
     const int blk = BN == 256 ? half : 0;
     const int hh_beg = BN == 256 ? 0 : half, hh_end = BN == 256 ? 2 : half + 1;
+    // The 32 x 32 chunk goes through the scratch as PACKED 16-bit pairs (pitch 20 words: conflict-free 16-byte writes): half the
+    // shared-memory traffic of an fp32 transpose, and the main loop of the next tile is running on the same 128 B/clk
+    uint32_t* scr16 = reinterpret_cast<uint32_t*>(scr);
+    constexpr int P16 = 20;
+    auto run = [&](auto fp16_tag) {
+      constexpr bool FP16 = decltype(fp16_tag)::value;
 #pragma unroll 1
-    for (int hh = hh_beg; hh < hh_end; ++hh) {
-      {
-        float g[32], u[32];
-        ld_acc32(t_acc + blk * 128 + hh * 32, g);
-        ld_acc32(t_acc + blk * 128 + 64 + hh * 32, u);
-        if (hh == hh_end - 1) release();
+      for (int hh = hh_beg; hh < hh_end; ++hh) {
+        {
+          float g[32], u[32];
+          ld_acc32(t_acc + blk * 128 + hh * 32, g);
+          ld_acc32(t_acc + blk * 128 + 64 + hh * 32, u);
+          if (hh == hh_end - 1) release();
 #pragma unroll
-        for (int i = 0; i < 32; ++i) g[i] = gelu_tanh_f(g[i] * rs) * (u[i] * rs);
-        to_scratch(g);
-      }
-      __syncwarp();
-      float4 o[8];
-      from_scratch(o);
-      uint16_t* dst = outp + (size_t)(r0 + lr) * ea.ld_out + n0 / 2 + blk * 64 + hh * 32 + lc;
-      const size_t step = (size_t)4 * ea.ld_out;
-      if (ea.out_fp16) {  // warp-uniform: one branch per chunk, not one per value
+          for (int i = 0; i < 32; ++i) g[i] = gelu_tanh_f(g[i] * rs) * (u[i] * rs);
+#pragma unroll
+          for (int i = 0; i < 32; i += 8)
+            *reinterpret_cast<uint4*>(&scr16[lane * P16 + (i >> 1)]) =
+                make_uint4(pack_op2_t<FP16>(g[i], g[i + 1]), pack_op2_t<FP16>(g[i + 2], g[i + 3]),
+                           pack_op2_t<FP16>(g[i + 4], g[i + 5]), pack_op2_t<FP16>(g[i + 6], g[i + 7]));
+        }
+        __syncwarp();
+        uint2 o[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) o[i] = *reinterpret_cast<const uint2*>(&scr16[(i * 4 + lr) * P16 + (lc >> 1)]);
+        uint16_t* dst = outp + (size_t)(r0 + lr) * ea.ld_out + n0 / 2 + blk * 64 + hh * 32 + lc;
+        const size_t step = (size_t)4 * ea.ld_out;
 #pragma unroll
         for (int i = 0; i < 8; ++i)
-          if (r0 + i * 4 + lr < m_lim)
-            *reinterpret_cast<uint2*>(dst + i * step) = make_uint2(pack_op2_t<true>(o[i].x, o[i].y), pack_op2_t<true>(o[i].z, o[i].w));
-      } else {
-#pragma unroll
-        for (int i = 0; i < 8; ++i)
-          if (r0 + i * 4 + lr < m_lim)
-            *reinterpret_cast<uint2*>(dst + i * step) = make_uint2(pack_op2_t<false>(o[i].x, o[i].y), pack_op2_t<false>(o[i].z, o[i].w));
+          if (r0 + i * 4 + lr < m_lim) *reinterpret_cast<uint2*>(dst + i * step) = o[i];
+        __syncwarp();
       }
-      __syncwarp();
-    }
+    };
+    if (ea.out_fp16) run(std::true_type{}); else run(std::false_type{});   // warp-uniform
   }
 }
 
