@@ -174,6 +174,28 @@ def test_edge_prefix_lengths():
     lc.close()
 
 
+def test_edge_one_block_segment_after_an_odd_block_count():
+    """Attention work lists in which a one-block item (L = 0: the robot's own tokens only) follows a three-block item
+    on EVERY CTA: the softmax warps split the key blocks by parity of the CTA-wide block count, so here the set that
+    owns the thread issuing the bulk copies has no block in the second segment: the kernel then settles the staging
+    tile ahead of the drain, behind a barrier of all eight warps, and that set's row sums are empty (0 at reference
+    -inf).  The plan is checked on the host first so that the test keeps meaning what it says if the planner changes."""
+    lens = [100] * 37 + [0] * 37            # 4 tiles per robot (H = 50): 148 + 148 items on 148 CTAs
+    offs, segs = rosa.rosa_debug_attn_plan(MINI.horizon, lens, 148)
+    special = 0
+    for c in range(148):
+        g = 0
+        for i in range(offs[c], offs[c + 1]):
+            n = int(segs[i][3] - segs[i][2])
+            special += n == 1 and (g & 1) == 1
+            g += n
+    assert special >= 100, special
+    case = edge_case(lens, seed=29, n_steps=2)
+    lc = LoadedCase(case)
+    check_against_oracle(case, lc, list(range(case.batch)), "edge-one-block-after-odd", sample=[0, 17, 36, 37, 55, 73])
+    lc.close()
+
+
 def test_edge_single_step_and_single_robot():
     case = edge_case([100], n_steps=1)
     lc = LoadedCase(case)
