@@ -455,6 +455,12 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
 #define AT_BLK(k) do { } while (0)
 #endif
         AT_BLK(0);
+        // The row's reference after block gi - 1, from the other set's warp of this lane quarter.  It was published right
+        // after that warp's row maximum, i.e. about when S(gi - 1) arrived: long before S(gi) does, so waiting for it and
+        // reading it HERE takes the hand-over off the chain S ready -> P ready.  (Waited for at every block but the CTA's
+        // first, so that nobody is ever more than one phase behind these barriers.)
+        if (gi > 0) mbar_wait(hand(q, (int)((gi - 1) & 1)), ((gi - 1) >> 1) & 1);
+        float m_ref = i > 0 ? mref_sm[r] : -INFINITY;
         mbar_wait(s_full(sb), (gi >> 1) & 1);
         tc_fence_after();
         AT_BLK(1);
@@ -491,11 +497,7 @@ k_attn_tc(const __grid_constant__ AttnMaps maps, const CUtensorMap* __restrict__
         // item was planned.  What is left between two plans is fp32 summation order and the 16-bit hand-over.
         const float m_blk = ceilf(mo * c_log2);
         AT_BLK(2);
-        // the row's reference after block gi - 1, from the other set's warp of this lane quarter (waited for at every
-        // block but the CTA's first, so that nobody is ever more than one phase behind these barriers)
-        if (gi > 0) mbar_wait(hand(q, (int)((gi - 1) & 1)), ((gi - 1) >> 1) & 1);
         AT_BLK(3);
-        float m_ref = i > 0 ? mref_sm[r] : -INFINITY;
         float factor = 1.f;
         if (m_blk > m_ref + AT_RESCALE_THR) {            // the segment's first block always lands here
           factor = exp2_int(m_ref - m_blk);              // 2^(an integer <= -8), exactly; 0 on the first block
