@@ -237,7 +237,8 @@ __device__ __forceinline__ void rope_load_cs(const EpiArgs& ea, int posr, int c,
   }
 }
 template <int BN, int EPI>
-__device__ __forceinline__ void epilogue_pre(EpiPre& pre, const EpiArgs& ea, int r0, int n0, int m_lim, int N, int lane, int half) {
+__device__ __forceinline__ void epilogue_pre(EpiPre& pre, const EpiArgs& ea, int r0, int n0, int m_lim, int N, int lane, int half,
+                                             bool same_rows = false) {   // same_rows: pre.rs / pre.posr are those of the previous tile's rows
   const int row = r0 + lane;
   const bool ok = row < m_lim;
   if constexpr (EPI == EPI_RESID) {
@@ -251,16 +252,17 @@ __device__ __forceinline__ void epilogue_pre(EpiPre& pre, const EpiArgs& ea, int
         asm volatile("prefetch.global.L2 [%0];" ::"l"(hp + col));
     }
   }
-  if constexpr (EPI == EPI_ROPE || EPI == EPI_GEGLU || EPI == EPI_FINAL) pre.rs = row_rscale(ea, ok ? row : 0);
+  if constexpr (EPI == EPI_ROPE || EPI == EPI_GEGLU || EPI == EPI_FINAL) { if (!same_rows) pre.rs = row_rscale(ea, ok ? row : 0); }
   if constexpr (EPI == EPI_ROPE) {
-    pre.posr = 0;
-    if (n0 < ea.rope_cols) {  // warp-uniform (one head per tile)
+    if (!same_rows) {   // the position does not depend on the head: kept across the heads of a row block
+      pre.posr = 0;
       if (ok) {
         const int p = row / ea.H;
         pre.posr = ea.rlen[ea.ids[p]] + (row - p * ea.H);
       }
-      rope_load_cs<BN, EPI>(ea, pre.posr, half * 2, lane, pre.cs0, pre.cs1);
     }
+    if (n0 < ea.rope_cols)   // warp-uniform (one head per tile)
+      rope_load_cs<BN, EPI>(ea, pre.posr, half * 2, lane, pre.cs0, pre.cs1);
   }
 }
 
@@ -736,6 +738,16 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
   const int m_lim = ea.m_active ? min(M, *ea.m_active) : M;
   const int n_m = (m_lim + 2 * BM - 1) / (2 * BM), n_n = (N + BN - 1) / BN;  // the last column tile may hang over N
   const int n_tiles = n_m * n_n, n_kb = K / BK;
+  // Tile order.  Default: the k-th tile of a pair is pair + k n_pairs with the ROW block running fastest, so the pairs that
+  // run side by side share a W tile.  RoPE launches (QKV: two tiles per pair at B = 64, the second tile's epilogue is
+  // exposed): a pair takes CONSECUTIVE tiles with the COLUMN tile (head) running fastest, i.e. heads of the same row block,
+  // so the second tile's epilogue reuses the rows' norm scale and position instead of waiting for three dependent loads
+  // (robot id -> prefix length -> cos / sin rows) after the first tile's epilogue.
+  constexpr bool kHeadFastest = EPI == EPI_ROPE;
+  const int tpp = (n_tiles + n_pairs - 1) / n_pairs;   // tiles per pair (the last pairs may get fewer, or none)
+  auto tile_of = [&](int k) { return kHeadFastest ? (k < tpp ? pair * tpp + k : n_tiles) : pair + k * n_pairs; };
+  auto tile_mb = [&](int t) { return kHeadFastest ? t / n_n : t % n_m; };
+  auto tile_nb = [&](int t) { return kHeadFastest ? t % n_n : t / n_m; };
 
   if (warp == 0 && lane == 0) {
     prefetch_tensormap(&tmA);
@@ -771,9 +783,9 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
   if (warp == 0) {  // ---------------- TMA producer (both CTAs; completion counted in the leader)
     const bool issuer = elect_one();
     const uint32_t lfull0 = mapa_shared(full_bar(0), 0);
-    const int pre = pair < n_tiles ? min(Cfg::STAGES, n_kb) : 0;   // stages whose W tile goes out before the wait
+    const int pre = tile_of(0) < n_tiles ? min(Cfg::STAGES, n_kb) : 0;   // stages whose W tile goes out before the wait
     if (issuer) {
-      const int n0 = (pair / n_m) * BN + (int)rank * (BN / 2);
+      const int n0 = tile_nb(tile_of(0)) * BN + (int)rank * (BN / 2);
       for (int kb = 0; kb < pre; ++kb) {
         mbar_expect_tx_cluster(lfull0 + 8u * kb, Cfg::STAGE_BYTES);
         tma_load_2d_cg2(smem_base + kb * Cfg::STAGE_BYTES + Cfg::A_BYTES, &tmB, lfull0 + 8u * kb, kb * BK, n0);
@@ -787,12 +799,12 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
       (void)lane;
       int s = 0;
       uint32_t ph = 0;
-      for (int t = pair; t < n_tiles; t += n_pairs) {
-        const int m0 = (t % n_m) * (2 * BM) + (int)rank * BM, n0 = (t / n_m) * BN + (int)rank * (BN / 2);
+      for (int k = 0, t; (t = tile_of(k)) < n_tiles; ++k) {
+        const int m0 = tile_mb(t) * (2 * BM) + (int)rank * BM, n0 = tile_nb(t) * BN + (int)rank * (BN / 2);
         for (int kb = 0; kb < n_kb; ++kb) {
           const uint32_t lfull = lfull0 + 8u * s;
           const uint32_t a_dst = smem_base + s * Cfg::STAGE_BYTES;
-          if (t == pair && kb < pre) {   // first pass over the ring: stage free, W already on its way
+          if (k == 0 && kb < pre) {   // first pass over the ring: stage free, W already on its way
             if (kb == 0) GT_TRACE(10);
             tma_load_2d_cg2(a_dst, &tmA, lfull, kb * BK, m0);
           } else {
@@ -816,7 +828,7 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
       const uint32_t base16 = (smem_base >> 4) & 0x3FFF;
       int s = 0, it = 0;
       uint32_t ph = 0;
-      for (int t = pair; t < n_tiles; t += n_pairs, ++it) {
+      for (; tile_of(it) < n_tiles; ++it) {
         const int acc = it & 1;
         const uint32_t acc_ph = (it >> 1) & 1;
         mbar_wait(tempty_bar(acc), acc_ph ^ 1);
@@ -846,14 +858,16 @@ k_gemm_tc2(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
     const int q = warp & 3;
     const int half = (warp - 2) >> 2;
     float* scr = reinterpret_cast<float*>(smem_raw + (bar_base + 256u - smem_u32(smem_raw))) + (warp - 2) * kScrFloats;
-    int it = 0;
-    for (int t = pair; t < n_tiles; t += n_pairs, ++it) {
+    int it = 0, mb_prev = -1;
+    EpiPre pre;
+    for (int t; (t = tile_of(it)) < n_tiles; ++it) {
       const int acc = it & 1;
       const uint32_t acc_ph = (it >> 1) & 1;
-      const int m0 = (t % n_m) * (2 * BM) + (int)rank * BM, n0 = (t / n_m) * BN;
+      const int mb = tile_mb(t);
+      const int m0 = mb * (2 * BM) + (int)rank * BM, n0 = tile_nb(t) * BN;
       const int r0 = m0 + q * 32;
-      EpiPre pre;
-      epilogue_pre<BN, EPI>(pre, ea, r0, n0, m_lim, N, lane, half);
+      epilogue_pre<BN, EPI>(pre, ea, r0, n0, m_lim, N, lane, half, /*same_rows=*/mb == mb_prev);
+      mb_prev = mb;
       mbar_wait_idle(tfull_bar(acc), acc_ph);
       tc_fence_after();
       const uint32_t t_acc = tmem_base + ((uint32_t)(q * 32) << 16) + acc * Cfg::ACC_STRIDE;
